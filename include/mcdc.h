@@ -1,0 +1,143 @@
+/* mcdc.h -- C ABI of the B200-native MC/DC hot path (libmcdc.so).
+ *
+ * The library runs, on one sm_100a GPU, the time-dependent multigroup Monte Carlo particle-history
+ * transport loop of arXiv 2409.04668: "a fixed source problem will loop over all the particles and
+ * transport them until the particle's history is terminated from a physical event (capture, fission,
+ * time or space boundary), a simulation event (time census) ..." (section 2), with the
+ * kernel set of PAPER.md:77 (move particle, tally, daughter particles from fission), full 3-D CSG and
+ * multigroup data and hash-based, schedule-independent random numbers.
+ * A problem is what the paper's input handler collects: materials and multigroup
+ * cross sections, CSG surfaces and cells, a source, a tally mesh and time bins.  The quantitative
+ * definition (draw order, tie-breaks, track-length estimator, batch statistics) is SURVEY.md
+ * Appendix A/B as fixed in DESIGN.md.
+ *
+ * Conventions
+ *  - Every pointer in mcdc_problem_desc and every result buffer is HOST memory owned by the caller.
+ *    mcdc_problem_create deep-copies the description; the caller may free it on return.
+ *  - The only DEVICE pointer crossing the boundary is the workspace handed to mcdc_workspace_bind
+ *    (e.g. the data_ptr of a torch uint8 CUDA tensor) together with a CUDA stream handle
+ *    (cudaStream_t as void*; NULL = default stream).  The library never frees the workspace; it
+ *    must outlive every run made with it.
+ *  - All real quantities are IEEE fp64; indices are int32; counters uint64.
+ *  - Every call returns MCDC_OK (0) or a negative MCDC_ERR_* code; nothing throws across the ABI.
+ *    A handle is not thread-safe; distinct handles are independent.
+ *  - There is no CPU fallback: without a CUDA device the compute calls return MCDC_ERR_CUDA.
+ */
+#ifndef MCDC_H
+#define MCDC_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mcdc_problem mcdc_problem; /* opaque */
+
+enum {
+  MCDC_OK = 0,
+  MCDC_ERR_ARG = -1,           /* null pointer, non-positive size, B does not divide N ...          */
+  MCDC_ERR_XS = -2,            /* cross sections inconsistent (Sigma_t != Sigma_c+Sigma_s+Sigma_f,
+                                  negative entries, chi not normalised where Sigma_f > 0)           */
+  MCDC_ERR_GEOM = -3,          /* surface / cell / material ids out of range, empty cell            */
+  MCDC_ERR_SIZE = -4,          /* result buffer size does not match the problem                     */
+  MCDC_ERR_NO_WORKSPACE = -5,  /* run without a bound workspace, or workspace too small             */
+  MCDC_ERR_BANK_OVERFLOW = -6, /* a particle bank overflowed; results of that run are invalid       */
+  MCDC_ERR_CUDA = -7,          /* CUDA runtime error (mcdc_last_cuda_error gives the text)          */
+  MCDC_ERR_NOMEM = -8,
+  MCDC_ERR_GRID = -9           /* mesh / time edges / census not increasing or empty                */
+};
+
+enum { MCDC_BC_TRANSMISSION = 0, MCDC_BC_VACUUM = 1, MCDC_BC_REFLECTIVE = 2 };
+enum { MCDC_DIR_ISOTROPIC = 0, MCDC_DIR_FIXED = 1 };
+
+/* Problem description.  Layouts are C row-major.
+ *  sigma_s[m][g][g2] is the transfer cross section FROM group g TO group g2.
+ *  A surface is the quadric f = A x^2+B y^2+C z^2+D xy+E xz+F yz+G x+H y+I z+J (surf_coef[s][0..9]).
+ *  A cell is the intersection of its half-spaces (hs_surface, hs_sense=+1 for f>0 / -1 for f<0),
+ *  listed in CSR form by cell_offset[n_cells+1].  Cells must not overlap.
+ *  The source is an axis-aligned box (lo==hi allowed per axis), a time interval and a group pdf.
+ *  The tally mesh has mesh_n[a] uniform bins on [mesh_lo[a], mesh_hi[a]] (+-INFINITY allowed when
+ *  mesh_n[a]==1), explicit time edges and all groups; bin index (((it*G+g)*nz+iz)*ny+iy)*nx+ix.
+ *  census_times[n_census] is increasing; the last entry is the final time (particles stop there). */
+typedef struct {
+  int32_t n_groups, n_materials, n_surfaces, n_cells;
+  const double *sigma_t, *sigma_c, *sigma_f, *nu, *chi; /* [M][G]                                  */
+  const double *sigma_s;                                /* [M][G][G]                               */
+  const double *speed;                                  /* [G] cm/s                                */
+  const double *surf_coef;                              /* [S][10]                                 */
+  const int32_t *surf_bc;                               /* [S] MCDC_BC_*                           */
+  const int32_t *cell_offset;                           /* [C+1]                                   */
+  const int32_t *hs_surface, *hs_sense;                 /* [cell_offset[C]]                        */
+  const int32_t *cell_material;                         /* [C]                                     */
+  double src_lo[3], src_hi[3], src_t0, src_t1;
+  const double *src_group_pdf;                          /* [G]                                     */
+  int32_t src_dir_mode;                                 /* MCDC_DIR_*                              */
+  double src_dir[3];                                    /* unit vector when MCDC_DIR_FIXED         */
+  double mesh_lo[3], mesh_hi[3];
+  int32_t mesh_n[3];                                    /* nx, ny, nz                              */
+  int32_t n_time_bins;
+  const double *time_edges;                             /* [n_time_bins+1]                         */
+  int32_t n_census;
+  const double *census_times;                           /* [n_census]                              */
+} mcdc_problem_desc;
+
+/* Options of one run.  Histories first_history_id .. first_history_id+N-1 are simulated in
+ * n_batches equal batches (n_batches must divide N); batch statistics per SURVEY.md A.9.        */
+typedef struct {
+  uint32_t n_batches;             /* >= 1                                                          */
+  uint64_t first_history_id;      /* global id of the first history (resumable / shardable runs)   */
+  int32_t record_history_events;  /* keep per-history event counts of this run (N x 4 uint32)      */
+} mcdc_run_opts;
+
+typedef struct {
+  /* weight ledger (A.9): source + production == capture + fission_abs + leak + census_final + lost */
+  double source, production, capture, fission_abs, leak, census_final, lost;
+  uint64_t histories, segments, collisions, surf_hits, census_events, children, lost_n, batches;
+  uint64_t kernel_launches;       /* launches of this library's kernels since create/reset          */
+  double ms_run;                  /* device time of the last mcdc_run (CUDA events on its stream)   */
+  double ms_transport;            /* of which: transport kernels of the last run                    */
+} mcdc_counters;
+
+/* Validates and deep-copies *d, classifies surfaces, builds cell-neighbour tables and uploads the
+ * problem to the current CUDA device.  *out is untouched on error.                                */
+int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out);
+void mcdc_problem_destroy(mcdc_problem *p);
+/* Zero tallies, ledger, census populations and counters (keeps problem and workspace).            */
+int mcdc_problem_reset(mcdc_problem *p);
+
+/* Bytes of device workspace needed to run sub-batches of up to max_histories_per_subbatch source
+ * histories with up to max_batches_in_flight statistical batches resident at once (particle,
+ * census and fission banks, per-batch tally accumulators).                                        */
+int mcdc_workspace_size(const mcdc_problem *p, uint64_t max_histories_per_subbatch,
+                        uint32_t max_batches_in_flight, size_t *bytes);
+/* dev_ptr: device memory of at least `bytes` (256-byte aligned); cuda_stream: cudaStream_t.       */
+int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes, uint64_t max_histories_per_subbatch,
+                        uint32_t max_batches_in_flight, void *cuda_stream);
+
+/* Simulate N source histories with the 64-bit seed; accumulates into the handle's tallies and
+ * ledger.  Synchronous: results are complete on return.  mcdc_run == mcdc_run_ex with one batch.  */
+int mcdc_run(mcdc_problem *p, uint64_t n_histories, uint64_t seed);
+int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts);
+
+/* mean[i] = sum_i / N (cm of track per source history, not divided by bin volume);
+ * sdev[i] = batch standard error of the mean (0 with a single batch).  n_bins must equal
+ * n_time_bins*G*nz*ny*nx.                                                                          */
+int mcdc_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
+/* Raw accumulators: sum over batches of S_b and of S_b^2.                                          */
+int mcdc_tally_sums_get(const mcdc_problem *p, double *sum, double *sumsq, size_t n_bins);
+int mcdc_counters_get(const mcdc_problem *p, mcdc_counters *c);
+/* Population bookkeeping at census: summed weight and number of particles that reached census k.  */
+int mcdc_census_get(const mcdc_problem *p, double *pop_w, uint64_t *pop_n, size_t n_census);
+/* ev[h][0..3] = collisions, surface events, fission children, census events of history
+ * first_history_id+h of the LAST run (needs record_history_events).                               */
+int mcdc_history_events_get(const mcdc_problem *p, uint32_t *ev, size_t n_histories);
+
+const char *mcdc_strerror(int code);
+const char *mcdc_last_cuda_error(const mcdc_problem *p);
+/* "major.minor sm_XX" of the build; never fails.                                                  */
+const char *mcdc_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MCDC_H */

@@ -1,0 +1,26 @@
+"""paper_2409_04668_b200 -- B200-native hot path of MC/DC (arXiv 2409.04668): the time-dependent
+multigroup Monte Carlo particle-history transport loop as a C-ABI CUDA library (libmcdc.so, sm_100a)
+plus this thin binding.  Every step of the path runs in the library's kernels; Python only marshals
+arguments and lends PyTorch device memory and a stream.  There is no CPU fallback.
+"""
+from .api import (  # noqa: F401
+    McdcError,
+    Problem,
+    lib,
+    lib_path,
+    mcdc_problem_create,
+    mcdc_problem_destroy,
+    mcdc_problem_reset,
+    mcdc_workspace_size,
+    mcdc_workspace_bind,
+    mcdc_run,
+    mcdc_run_ex,
+    mcdc_tallies_get,
+    mcdc_tally_sums_get,
+    mcdc_counters_get,
+    mcdc_census_get,
+    mcdc_history_events_get,
+    mcdc_strerror,
+    mcdc_version,
+    EXPORTED_SYMBOLS,
+)

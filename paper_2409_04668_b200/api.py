@@ -1,0 +1,296 @@
+"""Thin ctypes binding of libmcdc.so: same names as include/mcdc.h, argument marshalling only.
+
+PyTorch is used for exactly two things: the device workspace (a uint8 CUDA tensor whose data_ptr is
+handed to mcdc_workspace_bind) and the CUDA stream handle.  If libmcdc.so is missing this module
+raises at import of the first call -- there is no fallback path.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libmcdc.so")
+
+EXPORTED_SYMBOLS = [
+    "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size",
+    "mcdc_workspace_bind", "mcdc_run", "mcdc_run_ex", "mcdc_tallies_get", "mcdc_tally_sums_get",
+    "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
+    "mcdc_last_cuda_error", "mcdc_version",
+]
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+
+
+class McdcError(RuntimeError):
+    def __init__(self, code, where, detail=""):
+        self.code = code
+        msg = f"{where}: {mcdc_strerror(code)} ({code})"
+        if detail:
+            msg += f" [{detail}]"
+        super().__init__(msg)
+
+
+class ProblemDesc(C.Structure):
+    _fields_ = [
+        ("n_groups", C.c_int32), ("n_materials", C.c_int32), ("n_surfaces", C.c_int32), ("n_cells", C.c_int32),
+        ("sigma_t", _dp), ("sigma_c", _dp), ("sigma_f", _dp), ("nu", _dp), ("chi", _dp),
+        ("sigma_s", _dp), ("speed", _dp),
+        ("surf_coef", _dp), ("surf_bc", _ip),
+        ("cell_offset", _ip), ("hs_surface", _ip), ("hs_sense", _ip), ("cell_material", _ip),
+        ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3), ("src_t0", C.c_double), ("src_t1", C.c_double),
+        ("src_group_pdf", _dp), ("src_dir_mode", C.c_int32), ("src_dir", C.c_double * 3),
+        ("mesh_lo", C.c_double * 3), ("mesh_hi", C.c_double * 3), ("mesh_n", C.c_int32 * 3),
+        ("n_time_bins", C.c_int32), ("time_edges", _dp), ("n_census", C.c_int32), ("census_times", _dp),
+    ]
+
+
+class RunOpts(C.Structure):
+    _fields_ = [("n_batches", C.c_uint32), ("first_history_id", C.c_uint64), ("record_history_events", C.c_int32)]
+
+
+class Counters(C.Structure):
+    _fields_ = [(n, C.c_double) for n in
+                ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost")] + \
+               [(n, C.c_uint64) for n in ("histories", "segments", "collisions", "surf_hits", "census_events",
+                                          "children", "lost_n", "batches", "kernel_launches")] + \
+               [("ms_run", C.c_double), ("ms_transport", C.c_double)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def lib():
+    """Load libmcdc.so (once).  Raises if the CUDA extension has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(f"{_LIB_PATH} not found: build it with `python -m paper_2409_04668_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(_LIB_PATH)
+    vp = C.c_void_p
+    L.mcdc_problem_create.argtypes = [C.POINTER(ProblemDesc), C.POINTER(vp)]; L.mcdc_problem_create.restype = C.c_int
+    L.mcdc_problem_destroy.argtypes = [vp]; L.mcdc_problem_destroy.restype = None
+    L.mcdc_problem_reset.argtypes = [vp]; L.mcdc_problem_reset.restype = C.c_int
+    L.mcdc_workspace_size.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
+    L.mcdc_workspace_size.restype = C.c_int
+    L.mcdc_workspace_bind.argtypes = [vp, vp, C.c_size_t, C.c_uint64, C.c_uint32, vp]
+    L.mcdc_workspace_bind.restype = C.c_int
+    L.mcdc_run.argtypes = [vp, C.c_uint64, C.c_uint64]; L.mcdc_run.restype = C.c_int
+    L.mcdc_run_ex.argtypes = [vp, C.c_uint64, C.c_uint64, C.POINTER(RunOpts)]; L.mcdc_run_ex.restype = C.c_int
+    L.mcdc_tallies_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_tallies_get.restype = C.c_int
+    L.mcdc_tally_sums_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_tally_sums_get.restype = C.c_int
+    L.mcdc_counters_get.argtypes = [vp, C.POINTER(Counters)]; L.mcdc_counters_get.restype = C.c_int
+    L.mcdc_census_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.mcdc_census_get.restype = C.c_int
+    L.mcdc_history_events_get.argtypes = [vp, C.POINTER(C.c_uint32), C.c_size_t]
+    L.mcdc_history_events_get.restype = C.c_int
+    L.mcdc_strerror.argtypes = [C.c_int]; L.mcdc_strerror.restype = C.c_char_p
+    L.mcdc_last_cuda_error.argtypes = [vp]; L.mcdc_last_cuda_error.restype = C.c_char_p
+    L.mcdc_version.argtypes = []; L.mcdc_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def mcdc_strerror(code: int) -> str:
+    return lib().mcdc_strerror(int(code)).decode()
+
+
+def mcdc_version() -> str:
+    return lib().mcdc_version().decode()
+
+
+def _check(rc, where, handle=None):
+    if rc != 0:
+        detail = ""
+        if handle is not None and rc == -7:
+            detail = lib().mcdc_last_cuda_error(handle).decode()
+        raise McdcError(rc, where, detail)
+
+
+def _d(a):
+    return a.ctypes.data_as(_dp)
+
+
+def _i(a):
+    return a.ctypes.data_as(_ip)
+
+
+def _vec3(v):
+    return (C.c_double * 3)(*[float(x) for x in v])
+
+
+def _make_desc(prob):
+    """workloads.Problem (or any object with the same attributes) -> (ProblemDesc, keep-alive list)."""
+    d = ProblemDesc()
+    keep = []
+    d.n_groups, d.n_materials = int(prob.n_groups), int(prob.n_materials)
+    d.n_surfaces, d.n_cells = int(prob.n_surfaces), int(prob.n_cells)
+    for name in ("sigma_t", "sigma_c", "sigma_f", "nu", "chi", "sigma_s", "speed", "surf_coef"):
+        a = np.ascontiguousarray(getattr(prob, name), dtype=np.float64); keep.append(a)
+        setattr(d, name, _d(a))
+    for name in ("surf_bc", "cell_offset", "hs_surface", "hs_sense", "cell_material"):
+        a = np.ascontiguousarray(getattr(prob, name), dtype=np.int32); keep.append(a)
+        setattr(d, name, _i(a))
+    d.src_lo, d.src_hi = _vec3(prob.src_lo), _vec3(prob.src_hi)
+    d.src_t0, d.src_t1 = float(prob.src_t0), float(prob.src_t1)
+    pdf = np.ascontiguousarray(prob.src_group_pdf, dtype=np.float64); keep.append(pdf)
+    d.src_group_pdf = _d(pdf)
+    d.src_dir_mode = int(prob.src_dir_mode); d.src_dir = _vec3(prob.src_dir)
+    d.mesh_lo, d.mesh_hi = _vec3(prob.mesh_lo), _vec3(prob.mesh_hi)
+    d.mesh_n = (C.c_int32 * 3)(*[int(v) for v in prob.mesh_n])
+    te = np.ascontiguousarray(prob.time_edges, dtype=np.float64); keep.append(te)
+    ce = np.ascontiguousarray(prob.census_times, dtype=np.float64); keep.append(ce)
+    d.n_time_bins, d.time_edges = len(te) - 1, _d(te)
+    d.n_census, d.census_times = len(ce), _d(ce)
+    return d, keep
+
+
+# ---- functions with the names of include/mcdc.h ------------------------------------------------
+def mcdc_problem_create(prob):
+    d, keep = _make_desc(prob)
+    h = C.c_void_p()
+    _check(lib().mcdc_problem_create(C.byref(d), C.byref(h)), "mcdc_problem_create")
+    return h
+
+
+def mcdc_problem_destroy(h):
+    lib().mcdc_problem_destroy(h)
+
+
+def mcdc_problem_reset(h):
+    _check(lib().mcdc_problem_reset(h), "mcdc_problem_reset", h)
+
+
+def mcdc_workspace_size(h, max_histories_per_subbatch, max_batches_in_flight) -> int:
+    n = C.c_size_t()
+    _check(lib().mcdc_workspace_size(h, int(max_histories_per_subbatch), int(max_batches_in_flight), C.byref(n)),
+           "mcdc_workspace_size", h)
+    return int(n.value)
+
+
+def mcdc_workspace_bind(h, dev_ptr, nbytes, max_histories_per_subbatch, max_batches_in_flight, cuda_stream=0):
+    _check(lib().mcdc_workspace_bind(h, C.c_void_p(int(dev_ptr)), int(nbytes), int(max_histories_per_subbatch),
+                                     int(max_batches_in_flight), C.c_void_p(int(cuda_stream))),
+           "mcdc_workspace_bind", h)
+
+
+def mcdc_run(h, n_histories, seed):
+    _check(lib().mcdc_run(h, int(n_histories), int(seed)), "mcdc_run", h)
+
+
+def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False):
+    o = RunOpts(int(n_batches), int(first_history_id), int(bool(record_history_events)))
+    _check(lib().mcdc_run_ex(h, int(n_histories), int(seed), C.byref(o)), "mcdc_run_ex", h)
+
+
+def mcdc_tallies_get(h, n_bins):
+    mean = np.empty(n_bins); sdev = np.empty(n_bins)
+    _check(lib().mcdc_tallies_get(h, _d(mean), _d(sdev), n_bins), "mcdc_tallies_get", h)
+    return mean, sdev
+
+
+def mcdc_tally_sums_get(h, n_bins):
+    s = np.empty(n_bins); q = np.empty(n_bins)
+    _check(lib().mcdc_tally_sums_get(h, _d(s), _d(q), n_bins), "mcdc_tally_sums_get", h)
+    return s, q
+
+
+def mcdc_counters_get(h) -> dict:
+    c = Counters()
+    _check(lib().mcdc_counters_get(h, C.byref(c)), "mcdc_counters_get", h)
+    return c.as_dict()
+
+
+def mcdc_census_get(h, n_census):
+    w = np.empty(n_census); n = np.empty(n_census, dtype=np.uint64)
+    _check(lib().mcdc_census_get(h, _d(w), n.ctypes.data_as(C.POINTER(C.c_uint64)), n_census), "mcdc_census_get", h)
+    return w, n
+
+
+def mcdc_history_events_get(h, n_histories):
+    ev = np.empty((n_histories, 4), dtype=np.uint32)
+    _check(lib().mcdc_history_events_get(h, ev.ctypes.data_as(C.POINTER(C.c_uint32)), n_histories),
+           "mcdc_history_events_get", h)
+    return ev
+
+
+# ---- convenience wrapper: owns the handle and the torch workspace ------------------------------
+class Problem:
+    """Handle + PyTorch-owned workspace.  Marshalling only; all work happens in libmcdc.so."""
+
+    def __init__(self, prob, max_histories_per_subbatch=None, max_batches_in_flight=None, device="cuda:0",
+                 workspace_scale=1.0):
+        import torch  # device memory and stream only
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2409_04668_b200 needs a CUDA device (no CPU fallback)")
+        self.prob = prob
+        self.n_bins = int(prob.n_bins)
+        self.shape = prob.tally_shape()
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self._h = mcdc_problem_create(prob)
+        nb = int(max_batches_in_flight or max(1, getattr(prob, "n_batches", 1)))
+        nh = int(max_histories_per_subbatch or max(1, getattr(prob, "n_histories", 1)))
+        self._bind(nh, nb, workspace_scale)
+
+    def _bind(self, nh, nb, scale=1.0):
+        import torch
+
+        nbytes = int(mcdc_workspace_size(self._h, nh, nb) * scale)
+        self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        self._stream = torch.cuda.current_stream(self.device)
+        mcdc_workspace_bind(self._h, ptr, nbytes, nh, nb, self._stream.cuda_stream)
+        self.workspace_bytes = nbytes
+        self.max_hist, self.max_slots = nh, nb
+
+    def close(self):
+        if getattr(self, "_h", None):
+            mcdc_problem_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def reset(self):
+        mcdc_problem_reset(self._h)
+
+    def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False):
+        n = int(n_histories if n_histories is not None else self.prob.n_histories)
+        s = int(seed if seed is not None else self.prob.seed)
+        b = int(n_batches if n_batches is not None else self.prob.n_batches)
+        mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events)
+        self._last_n = n
+
+    def tallies(self):
+        m, s = mcdc_tallies_get(self._h, self.n_bins)
+        return m.reshape(self.shape), s.reshape(self.shape)
+
+    def tally_sums(self):
+        a, b = mcdc_tally_sums_get(self._h, self.n_bins)
+        return a.reshape(self.shape), b.reshape(self.shape)
+
+    def counters(self):
+        return mcdc_counters_get(self._h)
+
+    def census(self):
+        return mcdc_census_get(self._h, int(self.prob.n_census))
+
+    def history_events(self):
+        return mcdc_history_events_get(self._h, self._last_n)

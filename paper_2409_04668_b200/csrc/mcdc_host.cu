@@ -1,0 +1,799 @@
+// mcdc_host.cu -- C ABI (include/mcdc.h) of libmcdc.so: validation, problem upload, the census-step
+// driver loop and result read-back.  All transport arithmetic runs in the kernels of mcdc_kernels.cuh.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/mcdc.h"
+#include "mcdc_kernels.cuh"
+
+using namespace mcdc;
+
+namespace {
+
+const double HINF = std::numeric_limits<double>::infinity();
+
+struct DeviceArena {           // device allocations owned by the handle
+  std::vector<void *> ptrs;
+  cudaError_t err = cudaSuccess;
+  template <class V>
+  const V *upload(const std::vector<V> &h) {
+    void *d = nullptr;
+    size_t bytes = std::max<size_t>(h.size(), 1) * sizeof(V);
+    cudaError_t e = cudaMalloc(&d, bytes);
+    if (e != cudaSuccess) { err = e; return nullptr; }
+    ptrs.push_back(d);
+    if (!h.empty()) {
+      e = cudaMemcpy(d, h.data(), h.size() * sizeof(V), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) err = e;
+    }
+    return (const V *)d;
+  }
+  template <class V>
+  V *zeros(size_t n) {
+    void *d = nullptr;
+    size_t bytes = std::max<size_t>(n, 1) * sizeof(V);
+    cudaError_t e = cudaMalloc(&d, bytes);
+    if (e != cudaSuccess) { err = e; return nullptr; }
+    ptrs.push_back(d);
+    e = cudaMemset(d, 0, bytes);
+    if (e != cudaSuccess) err = e;
+    return (V *)d;
+  }
+  void release() {
+    for (void *p : ptrs) cudaFree(p);
+    ptrs.clear();
+  }
+};
+
+struct Box { double lo[3], hi[3]; };
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+}  // namespace
+
+struct mcdc_problem {
+  // host copy of the description (deep)
+  int G, M, S, C, K, Nt;
+  std::vector<double> sigma_t, sigma_c, sigma_f, nu, chi, sigma_s, speed, surf_coef, src_pdf, T, census;
+  std::vector<int> surf_bc, cell_off, hs_surface, hs_sense, cell_mat;
+  double src_lo[3], src_hi[3], src_t0, src_t1, src_dir[3];
+  int src_dir_mode;
+  double mesh_lo[3], mesh_hi[3];
+  int mesh_n[3];
+  size_t n_bins, n_spatial;
+  // device
+  DeviceArena arena;
+  Tables tab;
+  double *d_sum = nullptr, *d_sumsq = nullptr, *d_pop_w = nullptr;
+  unsigned long long *d_pop_n = nullptr;
+  DevCounters *d_cnt = nullptr;
+  uint32_t *d_ev = nullptr;      // [n][4] of the last run (cudaMalloc'ed on demand)
+  size_t ev_n = 0;
+  // workspace (caller-owned)
+  char *ws = nullptr;
+  size_t ws_bytes = 0;
+  uint64_t ws_hist = 0;
+  uint32_t ws_slots = 0;
+  uint32_t cap = 0;              // bank capacity per slot
+  cudaStream_t stream = nullptr;
+  Bank bankA, bankB, bankS1, bankS2;
+  double *x_acc = nullptr;
+  // bookkeeping
+  uint64_t histories = 0, batches = 0, batch_size = 0, launches = 0;
+  double ms_run = 0.0, ms_transport = 0.0;
+  int n_sm = 148, blocks_per_sm = 1;
+  std::string cuda_err;
+};
+
+namespace {
+
+int cuda_fail(mcdc_problem *p, cudaError_t e, const char *where) {
+  p->cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
+  return MCDC_ERR_CUDA;
+}
+#define CK(call)                                                     \
+  do {                                                               \
+    cudaError_t e__ = (call);                                        \
+    if (e__ != cudaSuccess) return cuda_fail(p, e__, #call);         \
+  } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// validation
+// ---------------------------------------------------------------------------------------------
+int validate(const mcdc_problem_desc *d) {
+  if (!d) return MCDC_ERR_ARG;
+  if (d->n_groups < 1 || d->n_materials < 1 || d->n_surfaces < 1 || d->n_cells < 1) return MCDC_ERR_ARG;
+  if (!d->sigma_t || !d->sigma_c || !d->sigma_f || !d->nu || !d->chi || !d->sigma_s || !d->speed) return MCDC_ERR_ARG;
+  if (!d->surf_coef || !d->surf_bc || !d->cell_offset || !d->hs_surface || !d->hs_sense || !d->cell_material)
+    return MCDC_ERR_ARG;
+  if (!d->src_group_pdf || !d->time_edges || !d->census_times) return MCDC_ERR_ARG;
+  if (d->n_time_bins < 1 || d->n_census < 1) return MCDC_ERR_GRID;
+  const int G = d->n_groups, M = d->n_materials;
+  for (int g = 0; g < G; ++g)
+    if (!(d->speed[g] > 0.0) || !std::isfinite(d->speed[g])) return MCDC_ERR_XS;
+  for (int m = 0; m < M; ++m) {
+    bool fissile = false;
+    double chi_sum = 0.0;
+    for (int g = 0; g < G; ++g) {
+      size_t mg = (size_t)m * G + g;
+      double st = d->sigma_t[mg], sc = d->sigma_c[mg], sf = d->sigma_f[mg], nu = d->nu[mg];
+      if (!(st >= 0.0) || !(sc >= 0.0) || !(sf >= 0.0) || !(nu >= 0.0) || !std::isfinite(st)) return MCDC_ERR_XS;
+      if (nu >= 254.0) return MCDC_ERR_XS;
+      double ss = 0.0;
+      for (int gp = 0; gp < G; ++gp) {
+        double v = d->sigma_s[mg * G + gp];
+        if (!(v >= 0.0)) return MCDC_ERR_XS;
+        ss += v;
+      }
+      if (std::fabs(st - (sc + ss + sf)) > 1e-12 * std::max(st, 1e-300) + 1e-300) return MCDC_ERR_XS;
+      if (sf > 0.0) fissile = true;
+      if (!(d->chi[mg] >= 0.0)) return MCDC_ERR_XS;
+      chi_sum += d->chi[mg];
+    }
+    if (fissile && std::fabs(chi_sum - 1.0) > 1e-9) return MCDC_ERR_XS;
+  }
+  for (int s = 0; s < d->n_surfaces; ++s) {
+    if (d->surf_bc[s] < 0 || d->surf_bc[s] > 2) return MCDC_ERR_GEOM;
+    bool any = false;
+    for (int i = 0; i < 9; ++i) {
+      if (!std::isfinite(d->surf_coef[10 * s + i])) return MCDC_ERR_GEOM;
+      if (d->surf_coef[10 * s + i] != 0.0) any = true;
+    }
+    if (!any || !std::isfinite(d->surf_coef[10 * s + 9])) return MCDC_ERR_GEOM;
+  }
+  if (d->cell_offset[0] != 0) return MCDC_ERR_GEOM;
+  for (int c = 0; c < d->n_cells; ++c) {
+    if (d->cell_offset[c + 1] <= d->cell_offset[c]) return MCDC_ERR_GEOM;
+    if (d->cell_material[c] < 0 || d->cell_material[c] >= M) return MCDC_ERR_GEOM;
+    for (int i = d->cell_offset[c]; i < d->cell_offset[c + 1]; ++i) {
+      if (d->hs_surface[i] < 0 || d->hs_surface[i] >= d->n_surfaces) return MCDC_ERR_GEOM;
+      if (d->hs_sense[i] != 1 && d->hs_sense[i] != -1) return MCDC_ERR_GEOM;
+    }
+  }
+  double pdf_sum = 0.0;
+  for (int g = 0; g < G; ++g) {
+    if (!(d->src_group_pdf[g] >= 0.0)) return MCDC_ERR_ARG;
+    pdf_sum += d->src_group_pdf[g];
+  }
+  if (std::fabs(pdf_sum - 1.0) > 1e-9) return MCDC_ERR_ARG;
+  for (int a = 0; a < 3; ++a) {
+    if (!(d->src_lo[a] <= d->src_hi[a]) || !std::isfinite(d->src_lo[a]) || !std::isfinite(d->src_hi[a])) return MCDC_ERR_ARG;
+    if (d->mesh_n[a] < 1 || !(d->mesh_lo[a] < d->mesh_hi[a])) return MCDC_ERR_GRID;
+    if (d->mesh_n[a] > 1 && (!std::isfinite(d->mesh_lo[a]) || !std::isfinite(d->mesh_hi[a]))) return MCDC_ERR_GRID;
+  }
+  if (d->src_dir_mode != MCDC_DIR_ISOTROPIC && d->src_dir_mode != MCDC_DIR_FIXED) return MCDC_ERR_ARG;
+  if (d->src_dir_mode == MCDC_DIR_FIXED) {
+    double n2 = d->src_dir[0] * d->src_dir[0] + d->src_dir[1] * d->src_dir[1] + d->src_dir[2] * d->src_dir[2];
+    if (std::fabs(n2 - 1.0) > 1e-12) return MCDC_ERR_ARG;
+  }
+  if (!(d->src_t0 <= d->src_t1)) return MCDC_ERR_ARG;
+  for (int i = 0; i < d->n_time_bins; ++i)
+    if (!(d->time_edges[i] < d->time_edges[i + 1])) return MCDC_ERR_GRID;
+  for (int k = 0; k < d->n_census; ++k) {
+    if (!std::isfinite(d->census_times[k])) return MCDC_ERR_GRID;
+    if (k > 0 && !(d->census_times[k - 1] < d->census_times[k])) return MCDC_ERR_GRID;
+  }
+  if (!(d->census_times[0] > d->src_t0) || !(d->src_t1 <= d->census_times[d->n_census - 1])) return MCDC_ERR_GRID;
+  return MCDC_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// surface classification, cell boxes, neighbour tables, source locator grid
+// ---------------------------------------------------------------------------------------------
+void classify_surface(const double *c, int &type, double4 &q) {
+  q = make_double4(0, 0, 0, 0);
+  const bool quad = c[0] != 0 || c[1] != 0 || c[2] != 0 || c[3] != 0 || c[4] != 0 || c[5] != 0;
+  if (!quad) {
+    int nz = 0, ax = -1;
+    for (int a = 0; a < 3; ++a)
+      if (c[6 + a] != 0.0) { nz++; ax = a; }
+    if (nz == 1) {
+      type = ST_PLANE_X + ax;
+      q.x = -c[9] / c[6 + ax];
+      q.y = c[6 + ax] > 0.0 ? 1.0 : -1.0;
+      return;
+    }
+    type = ST_QUADRIC;
+    return;
+  }
+  if (c[0] == c[1] && c[0] != 0.0 && c[2] == 0 && c[3] == 0 && c[4] == 0 && c[5] == 0 && c[8] == 0) {
+    double A = c[0];
+    double x0 = -c[6] / (2.0 * A), y0 = -c[7] / (2.0 * A);
+    double r2 = x0 * x0 + y0 * y0 - c[9] / A;
+    if (r2 > 0.0) {
+      type = ST_CYL_Z;
+      q.x = x0; q.y = y0; q.z = r2; q.w = A > 0.0 ? 1.0 : -1.0;
+      return;
+    }
+  }
+  type = ST_QUADRIC;
+}
+
+Box cell_box(const mcdc_problem &P, const std::vector<int> &type, const std::vector<double4> &q, int c) {
+  Box b;
+  for (int a = 0; a < 3; ++a) { b.lo[a] = -HINF; b.hi[a] = HINF; }
+  for (int i = P.cell_off[c]; i < P.cell_off[c + 1]; ++i) {
+    int s = P.hs_surface[i], sense = P.hs_sense[i];
+    if (type[s] <= ST_PLANE_Z) {
+      int a = type[s] - ST_PLANE_X;
+      bool below = (q[s].y > 0.0) == (sense < 0);          // coordinate < position
+      if (below) b.hi[a] = std::min(b.hi[a], q[s].x); else b.lo[a] = std::max(b.lo[a], q[s].x);
+    } else if (type[s] == ST_CYL_Z && (double)sense * q[s].w < 0.0) {   // inside the cylinder
+      double r = std::sqrt(q[s].z);
+      b.lo[0] = std::max(b.lo[0], q[s].x - r); b.hi[0] = std::min(b.hi[0], q[s].x + r);
+      b.lo[1] = std::max(b.lo[1], q[s].y - r); b.hi[1] = std::min(b.hi[1], q[s].y + r);
+    }
+  }
+  for (int a = 0; a < 3; ++a) {                            // pad: a point within rounding of a face stays inside
+    double ref = 1.0 + (std::isfinite(b.lo[a]) ? std::fabs(b.lo[a]) : 0.0) + (std::isfinite(b.hi[a]) ? std::fabs(b.hi[a]) : 0.0);
+    b.lo[a] -= 1e-6 * ref; b.hi[a] += 1e-6 * ref;
+  }
+  return b;
+}
+
+inline bool boxes_touch(const Box &a, const Box &b) {
+  for (int i = 0; i < 3; ++i)
+    if (a.hi[i] < b.lo[i] || b.hi[i] < a.lo[i]) return false;
+  return true;
+}
+
+}  // namespace
+
+// =============================================================================================
+// create / destroy / reset
+// =============================================================================================
+extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out) {
+  if (!out) return MCDC_ERR_ARG;
+  int rc = validate(d);
+  if (rc != MCDC_OK) return rc;
+  mcdc_problem *p = new (std::nothrow) mcdc_problem();
+  if (!p) return MCDC_ERR_NOMEM;
+  const int G = d->n_groups, M = d->n_materials, S = d->n_surfaces, C = d->n_cells;
+  p->G = G; p->M = M; p->S = S; p->C = C; p->K = d->n_census; p->Nt = d->n_time_bins;
+  const size_t MG = (size_t)M * G;
+  p->sigma_t.assign(d->sigma_t, d->sigma_t + MG); p->sigma_c.assign(d->sigma_c, d->sigma_c + MG);
+  p->sigma_f.assign(d->sigma_f, d->sigma_f + MG); p->nu.assign(d->nu, d->nu + MG);
+  p->chi.assign(d->chi, d->chi + MG); p->sigma_s.assign(d->sigma_s, d->sigma_s + MG * G);
+  p->speed.assign(d->speed, d->speed + G);
+  p->surf_coef.assign(d->surf_coef, d->surf_coef + (size_t)10 * S);
+  p->surf_bc.assign(d->surf_bc, d->surf_bc + S);
+  p->cell_off.assign(d->cell_offset, d->cell_offset + C + 1);
+  const int nhs = p->cell_off[C];
+  p->hs_surface.assign(d->hs_surface, d->hs_surface + nhs);
+  p->hs_sense.assign(d->hs_sense, d->hs_sense + nhs);
+  p->cell_mat.assign(d->cell_material, d->cell_material + C);
+  p->src_pdf.assign(d->src_group_pdf, d->src_group_pdf + G);
+  p->T.assign(d->time_edges, d->time_edges + d->n_time_bins + 1);
+  p->census.assign(d->census_times, d->census_times + d->n_census);
+  for (int a = 0; a < 3; ++a) {
+    p->src_lo[a] = d->src_lo[a]; p->src_hi[a] = d->src_hi[a]; p->src_dir[a] = d->src_dir[a];
+    p->mesh_lo[a] = d->mesh_lo[a]; p->mesh_hi[a] = d->mesh_hi[a]; p->mesh_n[a] = d->mesh_n[a];
+  }
+  p->src_t0 = d->src_t0; p->src_t1 = d->src_t1; p->src_dir_mode = d->src_dir_mode;
+  p->n_spatial = (size_t)d->mesh_n[0] * d->mesh_n[1] * d->mesh_n[2];
+  p->n_bins = (size_t)p->Nt * G * p->n_spatial;
+
+  // ---- derived cross-section tables (same summation order as the definition, A.1 / A.6) ----
+  std::vector<double> inv_sig_t(MG), s_tot(MG), s_sc(MG), cdf_s(MG * G), cdf_chi(MG), inv_speed(G), src_cdf(G);
+  std::vector<int> last_s(MG, 0), last_chi(M, 0);
+  for (size_t mg = 0; mg < MG; ++mg) {
+    double run = 0.0;
+    for (int gp = 0; gp < G; ++gp) {
+      double v = p->sigma_s[mg * G + gp];
+      run += v;
+      cdf_s[mg * G + gp] = run;
+      if (v != 0.0) last_s[mg] = gp;
+    }
+    s_tot[mg] = run;
+    s_sc[mg] = run + p->sigma_c[mg];
+    inv_sig_t[mg] = p->sigma_t[mg] > 0.0 ? 1.0 / p->sigma_t[mg] : 0.0;
+  }
+  for (int m = 0; m < M; ++m) {
+    double run = 0.0;
+    for (int g = 0; g < G; ++g) {
+      double v = p->chi[(size_t)m * G + g];
+      run += v;
+      cdf_chi[(size_t)m * G + g] = run;
+      if (v != 0.0) last_chi[m] = g;
+    }
+  }
+  int src_last = 0;
+  {
+    double run = 0.0;
+    for (int g = 0; g < G; ++g) {
+      run += p->src_pdf[g];
+      src_cdf[g] = run;
+      if (p->src_pdf[g] != 0.0) src_last = g;
+      inv_speed[g] = 1.0 / p->speed[g];
+    }
+  }
+  // ---- geometry tables ----
+  std::vector<int> type(S);
+  std::vector<double4> q(S);
+  for (int s = 0; s < S; ++s) classify_surface(&p->surf_coef[(size_t)10 * s], type[s], q[s]);
+  std::vector<int> hs(nhs);
+  for (int i = 0; i < nhs; ++i) hs[i] = (p->hs_surface[i] << 1) | (p->hs_sense[i] > 0 ? 1 : 0);
+  std::vector<Box> box(C);
+  for (int c = 0; c < C; ++c) box[c] = cell_box(*p, type, q, c);
+  // cells listing half-space (s, sense): index 2*s + (sense>0)
+  std::vector<std::vector<int>> users((size_t)2 * S);
+  for (int c = 0; c < C; ++c)
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) users[(size_t)hs[i]].push_back(c);
+  std::vector<int> nb_off(nhs + 1, 0), nb_cell;
+  for (int c = 0; c < C; ++c)
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
+      const std::vector<int> &cand = users[(size_t)(hs[i] ^ 1)];          // same surface, opposite sense
+      for (int c2 : cand)
+        if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);  // increasing id by construction
+      nb_off[i + 1] = (int)nb_cell.size();
+    }
+  // ---- source locator grid ----
+  int loc_n[3];
+  double loc_lo[3], loc_inv_d[3];
+  for (int a = 0; a < 3; ++a) {
+    double ext = p->src_hi[a] - p->src_lo[a];
+    loc_n[a] = ext > 0.0 ? 16 : 1;
+    loc_lo[a] = p->src_lo[a];
+    loc_inv_d[a] = ext > 0.0 ? loc_n[a] / ext : 0.0;
+  }
+  const int nvox = loc_n[0] * loc_n[1] * loc_n[2];
+  std::vector<int> loc_off(nvox + 1, 0), loc_cell;
+  for (int vz = 0; vz < loc_n[2]; ++vz)
+    for (int vy = 0; vy < loc_n[1]; ++vy)
+      for (int vx = 0; vx < loc_n[0]; ++vx) {
+        int v[3] = {vx, vy, vz};
+        Box vb;
+        for (int a = 0; a < 3; ++a) {
+          double ext = p->src_hi[a] - p->src_lo[a];
+          double dlt = ext / loc_n[a];
+          vb.lo[a] = p->src_lo[a] + v[a] * dlt - 1e-9 * (1.0 + std::fabs(p->src_lo[a]) + ext);
+          vb.hi[a] = p->src_lo[a] + (v[a] + 1) * dlt + 1e-9 * (1.0 + std::fabs(p->src_lo[a]) + ext);
+        }
+        for (int c = 0; c < C; ++c)
+          if (boxes_touch(vb, box[c])) loc_cell.push_back(c);
+        loc_off[(vz * loc_n[1] + vy) * loc_n[0] + vx + 1] = (int)loc_cell.size();
+      }
+
+  // ---- upload ----
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { delete p; return MCDC_ERR_CUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete p; return MCDC_ERR_CUDA; }
+  p->n_sm = prop.multiProcessorCount;
+  Tables &t = p->tab;
+  DeviceArena &ar = p->arena;
+  t.G = G; t.M = M; t.S = S; t.C = C; t.K = p->K; t.Nt = p->Nt;
+  t.sig_t = ar.upload(p->sigma_t); t.inv_sig_t = ar.upload(inv_sig_t); t.sig_s_tot = ar.upload(s_tot);
+  t.sig_sc = ar.upload(s_sc); t.sig_f = ar.upload(p->sigma_f); t.nu = ar.upload(p->nu);
+  t.cdf_s = ar.upload(cdf_s); t.last_s = ar.upload(last_s); t.cdf_chi = ar.upload(cdf_chi);
+  t.last_chi = ar.upload(last_chi); t.speed = ar.upload(p->speed); t.inv_speed = ar.upload(inv_speed);
+  t.surf_coef = ar.upload(p->surf_coef); t.surf_q = ar.upload(q); t.surf_type = ar.upload(type);
+  t.surf_bc = ar.upload(p->surf_bc); t.cell_off = ar.upload(p->cell_off); t.hs = ar.upload(hs);
+  t.cell_mat = ar.upload(p->cell_mat); t.nb_off = ar.upload(nb_off); t.nb_cell = ar.upload(nb_cell);
+  t.src_cdf = ar.upload(src_cdf); t.src_last = src_last; t.src_dir_mode = p->src_dir_mode;
+  t.src_t0 = p->src_t0; t.src_t1 = p->src_t1;
+  t.loc_off = ar.upload(loc_off); t.loc_cell = ar.upload(loc_cell);
+  t.T = ar.upload(p->T); t.census = ar.upload(p->census);
+  for (int a = 0; a < 3; ++a) {
+    t.src_lo[a] = p->src_lo[a]; t.src_hi[a] = p->src_hi[a]; t.src_dir[a] = p->src_dir[a];
+    t.loc_n[a] = loc_n[a]; t.loc_lo[a] = loc_lo[a]; t.loc_inv_d[a] = loc_inv_d[a];
+    t.mesh_lo[a] = p->mesh_lo[a]; t.mesh_hi[a] = p->mesh_hi[a]; t.mesh_n[a] = p->mesh_n[a];
+    t.mesh_d[a] = (p->mesh_hi[a] - p->mesh_lo[a]) / (double)p->mesh_n[a];
+    t.mesh_inv_d[a] = (p->mesh_n[a] > 1) ? 1.0 / t.mesh_d[a] : 0.0;
+  }
+  t.n_bins = p->n_bins;
+  p->d_sum = ar.zeros<double>(p->n_bins); p->d_sumsq = ar.zeros<double>(p->n_bins);
+  p->d_pop_w = ar.zeros<double>(p->K); p->d_pop_n = ar.zeros<unsigned long long>(p->K);
+  p->d_cnt = ar.zeros<DevCounters>(1);
+  if (ar.err != cudaSuccess) {
+    ar.release();
+    delete p;
+    return MCDC_ERR_CUDA;
+  }
+  int occ = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, 0) == cudaSuccess && occ > 0)
+    p->blocks_per_sm = occ;
+  *out = p;
+  return MCDC_OK;
+}
+
+extern "C" void mcdc_problem_destroy(mcdc_problem *p) {
+  if (!p) return;
+  p->arena.release();
+  if (p->d_ev) cudaFree(p->d_ev);
+  delete p;
+}
+
+extern "C" int mcdc_problem_reset(mcdc_problem *p) {
+  if (!p) return MCDC_ERR_ARG;
+  CK(cudaMemsetAsync(p->d_sum, 0, p->n_bins * sizeof(double), p->stream));
+  CK(cudaMemsetAsync(p->d_sumsq, 0, p->n_bins * sizeof(double), p->stream));
+  CK(cudaMemsetAsync(p->d_pop_w, 0, p->K * sizeof(double), p->stream));
+  CK(cudaMemsetAsync(p->d_pop_n, 0, p->K * sizeof(unsigned long long), p->stream));
+  CK(cudaMemsetAsync(p->d_cnt, 0, sizeof(DevCounters), p->stream));
+  if (p->x_acc) CK(cudaMemsetAsync(p->x_acc, 0, (size_t)p->ws_slots * p->n_bins * sizeof(double), p->stream));
+  CK(cudaStreamSynchronize(p->stream));
+  p->histories = p->batches = p->batch_size = p->launches = 0;
+  p->ms_run = p->ms_transport = 0.0;
+  p->ev_n = 0;
+  return MCDC_OK;
+}
+
+// =============================================================================================
+// workspace
+// =============================================================================================
+namespace {
+
+constexpr size_t FULL_BYTES = 8 * 8 + 8 + 16 + 4;    // x y z ux uy uz t w, key, meta, hid = 92
+constexpr size_t BIRTH_BYTES = 5 * 8 + 8 + 16 + 4;   // x y z t w, key, meta, hid         = 68 (meta kept whole)
+
+struct WsLayout {
+  size_t total = 0;
+  size_t x_acc = 0, counts = 0, bank[4] = {0, 0, 0, 0};
+  size_t fixed = 0;          // bytes that do not scale with the bank capacity
+};
+
+// slots * cap particles per bank; two full banks (live, census) and two birth banks (fission ping-pong)
+WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap) {
+  WsLayout L;
+  size_t off = 0;
+  L.x_acc = off; off += align_up((size_t)slots * p->n_bins * sizeof(double), 256);
+  L.counts = off; off += align_up((size_t)8 * slots * sizeof(uint32_t), 256);
+  L.fixed = off;
+  const size_t n = (size_t)slots * cap;
+  for (int b = 0; b < 4; ++b) {
+    L.bank[b] = off;
+    const int n_dbl = (b < 2) ? 8 : 5;
+    off += (size_t)n_dbl * align_up(n * 8, 256) + align_up(n * 8, 256) + align_up(n * 16, 256) + align_up(n * 4, 256);
+  }
+  L.total = off;
+  return L;
+}
+
+void carve_bank(Bank &B, char *base, size_t off, size_t n, bool full, uint32_t *count, uint32_t *cursor) {
+  char *q = base + off;
+  auto take = [&](size_t bytes) { char *r = q; q += align_up(bytes, 256); return r; };
+  B.x = (double *)take(n * 8); B.y = (double *)take(n * 8); B.z = (double *)take(n * 8);
+  if (full) { B.ux = (double *)take(n * 8); B.uy = (double *)take(n * 8); B.uz = (double *)take(n * 8); }
+  else B.ux = B.uy = B.uz = nullptr;
+  B.t = (double *)take(n * 8); B.w = (double *)take(n * 8);
+  B.key = (unsigned long long *)take(n * 8);
+  B.meta = (int4 *)take(n * 16);
+  B.hid = (uint32_t *)take(n * 4);
+  B.count = count; B.cursor = cursor;
+}
+
+uint64_t default_cap(uint64_t hist, uint32_t slots) {
+  uint64_t hb = (hist + slots - 1) / slots;
+  return align_up((size_t)(2 * hb + 1024), 32);
+}
+
+}  // namespace
+
+extern "C" int mcdc_workspace_size(const mcdc_problem *p, uint64_t max_hist, uint32_t max_slots, size_t *bytes) {
+  if (!p || !bytes || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
+  *bytes = layout(p, max_slots, default_cap(max_hist, max_slots)).total;
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes, uint64_t max_hist, uint32_t max_slots,
+                                   void *cuda_stream) {
+  if (!p || !dev_ptr || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
+  if (((uintptr_t)dev_ptr & 255u) != 0) return MCDC_ERR_ARG;
+  uint64_t cap = default_cap(max_hist, max_slots);
+  WsLayout L = layout(p, max_slots, cap);
+  if (bytes < L.total) return MCDC_ERR_NO_WORKSPACE;
+  // a larger workspace buys larger banks: grow cap while it fits
+  {
+    uint64_t lo = cap, hi = cap * 64;
+    while (lo + 32 <= hi) {
+      uint64_t mid = align_up((size_t)((lo + hi) / 2), 32);
+      if (mid * max_slots <= 0xFFFFFFF0ull && layout(p, max_slots, mid).total <= bytes) lo = mid; else hi = mid - 32;
+    }
+    cap = lo;
+    L = layout(p, max_slots, cap);
+  }
+  p->ws = (char *)dev_ptr; p->ws_bytes = bytes; p->ws_hist = max_hist; p->ws_slots = max_slots;
+  p->cap = (uint32_t)cap;
+  p->stream = (cudaStream_t)cuda_stream;
+  p->x_acc = (double *)(p->ws + L.x_acc);
+  uint32_t *cnt = (uint32_t *)(p->ws + L.counts);
+  const size_t n = (size_t)max_slots * cap;
+  carve_bank(p->bankA, p->ws, L.bank[0], n, true, cnt + 0 * max_slots, cnt + 1 * max_slots);
+  carve_bank(p->bankB, p->ws, L.bank[1], n, true, cnt + 2 * max_slots, cnt + 3 * max_slots);
+  carve_bank(p->bankS1, p->ws, L.bank[2], n, false, cnt + 4 * max_slots, cnt + 5 * max_slots);
+  carve_bank(p->bankS2, p->ws, L.bank[3], n, false, cnt + 6 * max_slots, cnt + 7 * max_slots);
+  CK(cudaMemsetAsync(p->ws, 0, L.fixed, p->stream));
+  CK(cudaStreamSynchronize(p->stream));
+  return MCDC_OK;
+}
+
+// =============================================================================================
+// run
+// =============================================================================================
+namespace {
+
+constexpr int SLAB_MAX_BINS = 8192;   // 64 KB of shared memory for the privatised tally slab
+
+int step_of(const mcdc_problem *p, double t) {          // smallest k with C[k] > t, else K-1
+  for (int k = 0; k < p->K; ++k)
+    if (p->census[k] > t) return k;
+  return p->K - 1;
+}
+
+struct SubBatch {
+  uint64_t first_local;   // index of its first history within the run
+  uint32_t n_hist;
+  uint32_t n_slots;
+  uint32_t hs;            // histories per slot
+  int closeout;           // 0 none, 1 per-slot batches, 2 all slots form one batch
+};
+
+int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
+                 cudaEvent_t ev0, cudaEvent_t ev1) {
+  const uint32_t ns = sb.n_slots;
+  const uint32_t ws_ns = p->ws_slots;
+  uint32_t *counts_dev = (uint32_t *)((char *)p->x_acc + align_up((size_t)ws_ns * p->n_bins * sizeof(double), 256));
+  std::vector<uint32_t> h_counts((size_t)8 * ws_ns);
+  CK(cudaMemsetAsync(counts_dev, 0, (size_t)8 * ws_ns * sizeof(uint32_t), p->stream));
+  Bank A = p->bankA, Bk = p->bankB, S1 = p->bankS1, S2 = p->bankS2;
+  const int k_first = step_of(p, p->src_t0), k_last = step_of(p, p->src_t1);
+  const size_t n_spatial_g = p->n_spatial * (size_t)p->G;
+  TransportArgs ta;
+  ta.x_acc = p->x_acc; ta.cnt = p->d_cnt; ta.pop_w = p->d_pop_w; ta.pop_n = p->d_pop_n;
+  ta.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
+  const int max_grid = p->n_sm * p->blocks_per_sm;
+  uint64_t live_total = 0;
+
+  for (int k = 0; k < p->K; ++k) {
+    if (k >= k_first && k <= k_last) {
+      SourceParams sp;
+      sp.seed_mixed = mix64(seed + MCDC_GAMMA);
+      sp.first_history = first_history_id + sb.first_local;
+      sp.n_hist = sb.n_hist; sp.hb = sb.hs; sp.cap = p->cap; sp.k = k; sp.single_step = (k_first == k_last);
+      k_source<<<(sb.n_hist + 255) / 256, 256, 0, p->stream>>>(p->tab, sp, A, p->d_cnt);
+      p->launches++;
+      live_total += sb.n_hist;          // upper bound, refined by the read-back below
+    } else if (live_total == 0) {
+      if (k > k_last) break;            // nothing alive and no source left
+      continue;
+    }
+    StepParams st;
+    st.k = k; st.is_last = (k == p->K - 1); st.t_census = p->census[k];
+    {
+      const double t_lo = (k == 0) ? p->src_t0 : p->census[k - 1];
+      int it_lo = 0, it_hi = 0;
+      for (int j = 0; j < p->Nt; ++j) {
+        if (p->T[j] <= t_lo) it_lo = j;
+        if (p->T[j] < p->census[k]) it_hi = j;
+      }
+      if (it_hi < it_lo) it_hi = it_lo;
+      st.it_lo = it_lo; st.it_n = it_hi - it_lo + 1;
+      size_t bins = (size_t)st.it_n * n_spatial_g;
+      st.slab_bins = bins <= (size_t)SLAB_MAX_BINS ? (int)bins : 0;
+    }
+    st.n_slots = (int)ns; st.cap = p->cap; st.hb = sb.hs; st.record_events = record ? 1 : 0;
+    const size_t smem = (size_t)st.slab_bins * sizeof(double);
+
+    // ---- generation 0: the live bank; then fission generations until the fission bank is empty ----
+    Bank in = A;
+    int gen = 0;
+    uint64_t n_in = live_total;
+    for (;;) {
+      st.in_is_birth = gen > 0 ? 1 : 0;
+      ta.in = in; ta.census_out = Bk; ta.sec_out = (gen & 1) ? S2 : S1;
+      Bank &sec = (gen & 1) ? S2 : S1;
+      CK(cudaMemsetAsync(in.cursor, 0, ns * sizeof(uint32_t), p->stream));
+      CK(cudaMemsetAsync(sec.count, 0, ns * sizeof(uint32_t), p->stream));
+      int grid = (int)std::min<uint64_t>((uint64_t)max_grid, std::max<uint64_t>(1, (n_in + TRANSPORT_THREADS - 1) / TRANSPORT_THREADS));
+      CK(cudaEventRecord(ev0, p->stream));
+      k_transport<<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, st, ta);
+      CK(cudaEventRecord(ev1, p->stream));
+      p->launches++;
+      CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+      CK(cudaStreamSynchronize(p->stream));
+      CK(cudaGetLastError());
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, ev0, ev1);
+      p->ms_transport += ms;
+      const uint32_t *hc = h_counts.data() + (sec.count - counts_dev);
+      uint64_t n_sec = 0;
+      for (uint32_t s = 0; s < ns; ++s) {
+        if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
+        n_sec += hc[s];
+      }
+      if (n_sec == 0) break;
+      in = sec; n_in = n_sec; gen++;
+    }
+    // census bank becomes the next step's live bank
+    {
+      const uint32_t *hc = h_counts.data() + (Bk.count - counts_dev);
+      live_total = 0;
+      for (uint32_t s = 0; s < ns; ++s) {
+        if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
+        live_total += hc[s];
+      }
+    }
+    std::swap(A, Bk);
+    CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));
+  }
+  if (sb.closeout) {
+    int grid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
+    k_closeout<<<grid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    p->launches++;
+  }
+  return MCDC_OK;
+}
+
+}  // namespace
+
+extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts) {
+  if (!p || n_histories == 0) return MCDC_ERR_ARG;
+  mcdc_run_opts def = {1u, 0ull, 0};
+  if (!opts) opts = &def;
+  const uint32_t B = opts->n_batches ? opts->n_batches : 1u;
+  if (n_histories % B != 0) return MCDC_ERR_ARG;
+  const uint64_t hb = n_histories / B;
+  if (p->batch_size != 0 && p->batch_size != hb) return MCDC_ERR_ARG;
+  if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
+  const bool record = opts->record_history_events != 0;
+  if (record) {
+    if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
+    CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
+    CK(cudaMemsetAsync(p->d_ev, 0, n_histories * 4 * sizeof(uint32_t), p->stream));
+    p->ev_n = n_histories;
+  } else p->ev_n = 0;
+
+  static bool attr_set = false;
+  if (!attr_set) {
+    CK(cudaFuncSetAttribute(k_transport, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_MAX_BINS * (int)sizeof(double)));
+    attr_set = true;
+  }
+  {
+    int occ = 1;   // occupancy with the largest slab this problem can ask for
+    size_t per_step = (size_t)p->G * p->n_spatial;
+    size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
+      p->blocks_per_sm = occ;
+  }
+  cudaEvent_t e_run0, e_run1, ev0, ev1;
+  CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1)); CK(cudaEventCreate(&ev0)); CK(cudaEventCreate(&ev1));
+  p->ms_transport = 0.0;
+  CK(cudaEventRecord(e_run0, p->stream));
+
+  // ---- plan sub-batches ----
+  const uint64_t slot_max = std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist));
+  int rc = MCDC_OK;
+  if (hb <= slot_max) {                                  // whole batches, one per slot
+    const uint32_t per_sub = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(p->ws_slots, p->ws_hist / hb));
+    for (uint32_t b = 0; b < B && rc == MCDC_OK; b += per_sub) {
+      SubBatch sb;
+      sb.n_slots = std::min<uint32_t>(per_sub, B - b);
+      sb.first_local = (uint64_t)b * hb; sb.n_hist = (uint32_t)(sb.n_slots * hb); sb.hs = (uint32_t)hb; sb.closeout = 1;
+      rc = run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+    }
+  } else {                                               // one batch = several pieces spread over the slots
+    const uint64_t per_sub = std::min<uint64_t>(p->ws_hist, slot_max * p->ws_slots);
+    for (uint32_t b = 0; b < B && rc == MCDC_OK; ++b) {
+      for (uint64_t off = 0; off < hb && rc == MCDC_OK; off += per_sub) {
+        SubBatch sb;
+        uint64_t n = std::min<uint64_t>(per_sub, hb - off);
+        sb.hs = (uint32_t)std::min<uint64_t>(slot_max, (n + p->ws_slots - 1) / p->ws_slots);
+        sb.n_slots = (uint32_t)((n + sb.hs - 1) / sb.hs);
+        sb.first_local = (uint64_t)b * hb + off; sb.n_hist = (uint32_t)n;
+        sb.closeout = (off + n >= hb) ? 2 : 0;
+        rc = run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+      }
+    }
+  }
+  cudaEventRecord(e_run1, p->stream);
+  cudaError_t se = cudaStreamSynchronize(p->stream);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e_run0, e_run1);
+  p->ms_run = ms;
+  cudaEventDestroy(e_run0); cudaEventDestroy(e_run1); cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+  if (rc != MCDC_OK) return rc;
+  if (se != cudaSuccess) return cuda_fail(p, se, "cudaStreamSynchronize");
+  int overflow = 0;
+  CK(cudaMemcpy(&overflow, &p->d_cnt->overflow, sizeof(int), cudaMemcpyDeviceToHost));
+  if (overflow) return MCDC_ERR_BANK_OVERFLOW;
+  p->histories += n_histories; p->batches += B; p->batch_size = hb;
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_run(mcdc_problem *p, uint64_t n_histories, uint64_t seed) {
+  return mcdc_run_ex(p, n_histories, seed, nullptr);
+}
+
+// =============================================================================================
+// results
+// =============================================================================================
+extern "C" int mcdc_tally_sums_get(const mcdc_problem *cp, double *sum, double *sumsq, size_t n_bins) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !sum || !sumsq) return MCDC_ERR_ARG;
+  if (n_bins != p->n_bins) return MCDC_ERR_SIZE;
+  CK(cudaMemcpy(sum, p->d_sum, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(sumsq, p->d_sumsq, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+// A.9: mean = sum / N; with m_b = S_b / (N/B): sdev = sqrt((sum m_b^2 / B - mean^2) / (B - 1)); B = 1 -> 0
+extern "C" int mcdc_tallies_get(const mcdc_problem *cp, double *mean, double *sdev, size_t n_bins) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !mean || !sdev) return MCDC_ERR_ARG;
+  if (n_bins != p->n_bins) return MCDC_ERR_SIZE;
+  if (p->histories == 0) return MCDC_ERR_ARG;
+  CK(cudaMemcpy(mean, p->d_sum, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(sdev, p->d_sumsq, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  const double N = (double)p->histories, B = (double)p->batches, hb = N / B;
+  for (size_t i = 0; i < n_bins; ++i) {
+    double mu = mean[i] / N;
+    double sd = 0.0;
+    if (B > 1.0) {
+      double m2 = sdev[i] / (hb * hb) / B;
+      double var = (m2 - mu * mu) / (B - 1.0);
+      sd = var > 0.0 ? std::sqrt(var) : 0.0;
+    }
+    mean[i] = mu; sdev[i] = sd;
+  }
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_counters_get(const mcdc_problem *cp, mcdc_counters *c) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !c) return MCDC_ERR_ARG;
+  DevCounters h;
+  CK(cudaMemcpy(&h, p->d_cnt, sizeof(h), cudaMemcpyDeviceToHost));
+  c->source = h.ledger[0]; c->production = h.ledger[1]; c->capture = h.ledger[2]; c->fission_abs = h.ledger[3];
+  c->leak = h.ledger[4]; c->census_final = h.ledger[5]; c->lost = h.ledger[6];
+  c->histories = h.n[0]; c->segments = h.n[1]; c->collisions = h.n[2]; c->surf_hits = h.n[3];
+  c->census_events = h.n[4]; c->children = h.n[5]; c->lost_n = h.n[6];
+  c->batches = p->batches; c->kernel_launches = p->launches;
+  c->ms_run = p->ms_run; c->ms_transport = p->ms_transport;
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_census_get(const mcdc_problem *cp, double *pop_w, uint64_t *pop_n, size_t K) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !pop_w || !pop_n) return MCDC_ERR_ARG;
+  if (K != (size_t)p->K) return MCDC_ERR_SIZE;
+  CK(cudaMemcpy(pop_w, p->d_pop_w, K * sizeof(double), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(pop_n, p->d_pop_n, K * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_history_events_get(const mcdc_problem *cp, uint32_t *ev, size_t n) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !ev) return MCDC_ERR_ARG;
+  if (n != p->ev_n || !p->d_ev) return MCDC_ERR_SIZE;
+  CK(cudaMemcpy(ev, p->d_ev, n * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+extern "C" const char *mcdc_strerror(int code) {
+  switch (code) {
+    case MCDC_OK: return "ok";
+    case MCDC_ERR_ARG: return "invalid argument";
+    case MCDC_ERR_XS: return "inconsistent cross sections";
+    case MCDC_ERR_GEOM: return "invalid geometry description";
+    case MCDC_ERR_SIZE: return "result buffer size mismatch";
+    case MCDC_ERR_NO_WORKSPACE: return "no workspace bound or workspace too small";
+    case MCDC_ERR_BANK_OVERFLOW: return "particle bank overflow (bind a larger workspace)";
+    case MCDC_ERR_CUDA: return "CUDA error";
+    case MCDC_ERR_NOMEM: return "out of host memory";
+    case MCDC_ERR_GRID: return "invalid mesh, time or census grid";
+    default: return "unknown error";
+  }
+}
+
+extern "C" const char *mcdc_last_cuda_error(const mcdc_problem *p) { return p ? p->cuda_err.c_str() : ""; }
+
+extern "C" const char *mcdc_version(void) { return "0.1 sm_100a"; }

@@ -1,0 +1,93 @@
+// mcdc_types.h -- plain structs shared by the host side and the kernels of libmcdc.so.
+// (Product code: nothing here is shared with oracle/.)
+#pragma once
+#include <cstdint>
+
+namespace mcdc {
+
+// Surface classes recognised at mcdc_problem_create ("implementations may classify
+// into typed surfaces; results must equal the general formula up to rounding").
+enum SurfType : int {
+  ST_PLANE_X = 0,  // q.x = position, q.y = sign of the linear coefficient
+  ST_PLANE_Y = 1,
+  ST_PLANE_Z = 2,
+  ST_CYL_Z = 3,    // q.x = x0, q.y = y0, q.z = r^2, q.w = sign of A
+  ST_QUADRIC = 4   // general 10-coefficient form (planes with a general normal included)
+};
+
+enum Event : int { EV_CENSUS = 0, EV_SURFACE = 1, EV_COLLISION = 2 };
+
+// Particle bank in HBM, structure of arrays; index = slot * cap + i.
+// Full record 92 B: x y z ux uy uz t w (8 x f64), key (u64), meta {cell, last_surface, ctr, g} (4 x i32), hid (u32).
+// A fission birth record (A.6) uses x y z t w key meta.x(cell) hid = 56 B; ux/uy/uz are not allocated.
+struct Bank {
+  double *x, *y, *z, *ux, *uy, *uz, *t, *w;
+  unsigned long long *key;
+  int4 *meta;
+  uint32_t *hid;
+  uint32_t *count;   // [n_slots] particles stored per slot
+  uint32_t *cursor;  // [n_slots] consumption cursor (transport kernel refill)
+};
+
+// Device-resident problem tables (all pointers are device memory owned by the handle).
+struct Tables {
+  int G, M, S, C, K, Nt;
+  // cross sections, index mg = m * G + g
+  const double *sig_t, *inv_sig_t, *sig_s_tot, *sig_sc /* Sigma_s_tot + Sigma_c */, *sig_f, *nu;
+  const double *cdf_s;     // [M*G][G] running sums of Sigma_s[m][g][.] in increasing g'
+  const int *last_s;       // [M*G] last g' with a non-zero entry (fallback of the CDF scan)
+  const double *cdf_chi;   // [M][G] running sums of chi
+  const int *last_chi;     // [M]
+  const double *speed, *inv_speed;   // [G]
+  // geometry
+  const double *surf_coef; // [S][10] general form
+  const double4 *surf_q;   // [S] typed parameters
+  const int *surf_type;    // [S]
+  const int *surf_bc;      // [S]
+  const int *cell_off;     // [C+1]
+  const int *hs;           // packed half-space: surface << 1 | (sense > 0)
+  const int *cell_mat;     // [C]
+  const int *nb_off;       // [nhs+1] neighbour candidates of half-space slot i (cells across that surface)
+  const int *nb_cell;
+  // source
+  double src_lo[3], src_hi[3], src_t0, src_t1;
+  const double *src_cdf;   // [G]
+  int src_last;
+  int src_dir_mode;
+  double src_dir[3];
+  // source locator grid over the source box
+  int loc_n[3];
+  double loc_lo[3], loc_inv_d[3];
+  const int *loc_off;      // [nvox+1]
+  const int *loc_cell;
+  // tally mesh
+  double mesh_lo[3], mesh_hi[3], mesh_d[3], mesh_inv_d[3];
+  int mesh_n[3];
+  const double *T;         // [Nt+1]
+  const double *census;    // [K]
+  unsigned long long n_bins;
+};
+
+// Per-launch parameters of the transport kernel.
+struct StepParams {
+  int k;                    // census index of this step (0-based); C[k] is the step's end time
+  int is_last;              // k == K-1
+  double t_census;          // C[k]
+  int it_lo, it_n;          // time bins covered by the shared-memory tally slab
+  int slab_bins;            // it_n * G * nz*ny*nx, or 0 when tallies go straight to global memory
+  int n_slots;
+  uint32_t cap;             // bank capacity per slot
+  uint32_t hb;              // histories per slot (slot = hid / hb)
+  int in_is_birth;          // input bank holds fission birth records
+  int record_events;
+};
+
+// Device-side accumulators (one instance per handle).
+struct DevCounters {
+  double ledger[7];         // source production capture fission_abs leak census_final lost
+  unsigned long long n[7];  // histories segments collisions surf_hits census_events children lost_n
+  int overflow;             // a bank overflowed
+  int pad;
+};
+
+}  // namespace mcdc
