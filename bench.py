@@ -1,0 +1,296 @@
+#!/usr/bin/env python
+"""bench.py -- histories/s of the MC/DC hot path on B200 (contract: see the task statement / DESIGN.md).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload config3] [--histories H] [--sweep]
+  python bench.py --impl reference ...      # the oracle (CPU) arm on the same workload
+
+A "step" is one mcdc_run of the whole hot path (source generation, all census steps and fission
+generations, batch close-out) over one batch of synthetic histories of the named workload.
+N=1 workload: config 3 (7-group 17x17 pin lattice, 1e7 histories, 100 batches) -- the configuration
+BASELINE.json's north_star quotes the roofline target on (configs 3/4); it fits one GPU.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "histories/s"
+FP64_LANES_PER_SM = 64          # B200 (sm_100a): 64 fp64 FMA lanes per SM (nominal 37 TFLOP/s / (2*148*1.965 GHz))
+N_SM = 148
+
+
+def _peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return float(d["hbm_gbs"]), "measured", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.rows = []
+        self.proc = None
+        self.gpu_index = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                 "-i", str(self.gpu_index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _problem(args):
+    from workloads import configs as W
+
+    kw = {}
+    if args.histories:
+        kw["n_histories"] = int(args.histories)
+    if args.batches:
+        kw["n_batches"] = int(args.batches)
+    return W.get_config(args.workload, **kw)
+
+
+def _desc_bytes(p):
+    n = 0
+    for name in ("sigma_t", "sigma_c", "sigma_f", "nu", "chi", "sigma_s", "speed", "surf_coef", "surf_bc",
+                 "cell_offset", "hs_surface", "hs_sense", "cell_material", "src_group_pdf", "time_edges",
+                 "census_times"):
+        n += getattr(p, name).nbytes
+    return n + 31 * 8
+
+
+def algorithmic_bytes(p, c, n_hist, n_batches):
+    """176 B per segment + 112 B per fission child + 88 B per source history + close-out."""
+    closeout = 3 * 16 * p.n_bins * n_batches
+    return 176.0 * c["segments"] + 112.0 * c["children"] + 88.0 * n_hist + closeout
+
+
+# ------------------------------------------------------------------------------------------------
+def run_cpu_sample(p, seconds_target=15.0, first_history_id=0):
+    """Time the oracle as it stands on a bounded sample of the same workload (one host thread)."""
+    from oracle import Oracle
+
+    o = Oracle(p)
+    n = 2000
+    t0 = time.perf_counter(); o.run(n, p.seed, n_batches=1, first_history_id=first_history_id)
+    dt = time.perf_counter() - t0
+    rate = n / dt
+    n2 = int(max(2000, min(p.n_histories, rate * seconds_target)))
+    o.reset()
+    t0 = time.perf_counter(); o.run(n2, p.seed, n_batches=1, first_history_id=first_history_id)
+    dt = time.perf_counter() - t0
+    c = o.counters()
+    return {"value": n2 / dt, "unit": METRIC, "cores": 1, "kind": "oracle",
+            "sample": f"first {n2} histories of {p.name} (seed {p.seed}), single thread, {dt:.1f} s",
+            "segments_per_s": c["segments"] / dt}
+
+
+def bench_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    p = _problem(args)
+    vals = []
+    per_step = max(3.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        run_cpu_sample(p, seconds_target=min(2.0, per_step))
+    t0 = time.perf_counter()
+    for s in range(args.steps):
+        vals.append(run_cpu_sample(p, seconds_target=per_step, first_history_id=0))
+    dt = time.perf_counter() - t0
+    v = float(np.mean([x["value"] for x in vals]))
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": METRIC, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": p.name, "histories_per_step": p.n_histories, "n_batches": p.n_batches,
+                      "note": "oracle timed on a bounded sample of the workload per step"},
+           "cpu_baseline": {"value": v, "unit": METRIC, "cores": 1, "kind": "oracle", "sample": vals[-1]["sample"]},
+           "e2e": {"value": v, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------
+def bench_gpu(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2409_04668_b200 as M
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    dev = f"cuda:{local}"
+    torch.cuda.set_device(dev)
+    p = _problem(args)
+    n_hist, n_b = p.n_histories, p.n_batches
+    from paper_2409_04668_b200.sharding import shard_range
+
+    # weak scaling: every rank runs n_hist histories of its own id range; no data-path collective
+    first_id = shard_range(n_hist * world, world, rank)[0]
+    g = M.Problem(p, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        g.reset(); g.run(n_hist, p.seed, n_b, first_history_id=first_id)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    g.reset()
+    launches0 = g.counters()["kernel_launches"]
+    ms_tr = 0.0
+    barrier()
+    t_wall0 = time.time()
+    ev0.record()
+    for _ in range(args.steps):
+        g.run(n_hist, p.seed, n_b, first_history_id=first_id)
+        ms_tr += g.counters()["ms_transport"]
+    ev1.record()
+    barrier()
+    t_wall1 = time.time()
+    ms = ev0.elapsed_time(ev1)
+    c = g.counters()
+    if world > 1:
+        t = torch.tensor([ms, ms_tr], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms, ms_tr = float(t[0]), float(t[1])
+    launches = c["kernel_launches"] - launches0
+    total_hist = n_hist * args.steps * world
+    value = total_hist / (ms * 1e-3)
+    seg_per_s = c["segments"] * world / (ms * 1e-3)
+
+    out = None
+    if rank == 0:
+        clocks = sampler.stop(t_wall0, t_wall1)
+        peak, peak_kind, sm_max = _peaks()
+        # dominant kernel: k_transport.  Algorithmic bytes of the steps it processed / its device time.
+        alg = algorithmic_bytes(p, {"segments": c["segments"], "children": c["children"]}, n_hist * args.steps,
+                                n_b * args.steps)
+        n_tr = max(1, (launches - args.steps * 2))
+        ach = alg / (ms_tr * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "kernel": "k_transport", "achieved": ach, "peak": peak, "unit": "GB/s",
+                    "frac": ach / peak, "traffic": None, "peak_kind": peak_kind,
+                    "note": "achieved = SURVEY 8(d) algorithmic bytes (176 B/segment + 112 B/child + 88 B/history + "
+                            "close-out) / summed k_transport device time; particle state is register-resident so "
+                            "DRAM traffic is far below this figure (see DESIGN.md, profiles/)",
+                    "launches": int(n_tr), "ms_kernel_total": ms_tr}
+        out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
+               "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+               "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+               "config": {"workload": p.name, "histories_per_step": n_hist, "n_batches": n_b, "seed": p.seed,
+                          "l2": "banks and tally accumulators exceed L2 (inputs larger than L2)" if n_hist >= 2_000_000
+                          else "small workload: L2-resident", "parallelism": f"history-range sharding x{world}"},
+               "segments_per_s": seg_per_s, "segments_per_history": c["segments"] / max(1, c["histories"]),
+               "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline}
+    # ---- e2e: host buffers in, host buffers out, through the C ABI (create + bind + run + get) ----
+    ws = g._ws
+    ptr = (ws.data_ptr() + 255) // 256 * 256
+    e2e_steps = max(1, min(args.steps, 3))
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        h = M.mcdc_problem_create(p)                      # H2D: the problem description
+        M.mcdc_workspace_bind(h, ptr, g.workspace_bytes, g.max_hist, g.max_slots, g._stream.cuda_stream)
+        M.mcdc_run_ex(h, n_hist, p.seed, n_b, first_id)
+        mean, sdev = M.mcdc_tallies_get(h, p.n_bins)      # D2H: sum and sumsq
+        M.mcdc_problem_destroy(h)
+    barrier()
+    dt = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([dt], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t[0])
+    if rank == 0:
+        out["e2e"] = {"value": n_hist * e2e_steps * world / dt, "unit": METRIC, "h2d_bytes_per_step": _desc_bytes(p),
+                      "d2h_bytes_per_step": 2 * 8 * p.n_bins, "steps": e2e_steps,
+                      "note": "mcdc_problem_create (host arrays) + workspace_bind + run_ex + tallies_get (host) per step"}
+        if world == 1 and not args.no_cpu:
+            out["cpu_baseline"] = run_cpu_sample(p, seconds_target=args.cpu_seconds)
+        print(json.dumps(out))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="config3")
+    ap.add_argument("--histories", type=float, default=0)
+    ap.add_argument("--batches", type=int, default=0)
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    args = ap.parse_args()
+    if args.impl == "reference":
+        bench_reference(args)
+    else:
+        bench_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

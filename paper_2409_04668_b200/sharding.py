@@ -1,0 +1,51 @@
+"""Host-side sharding of a run over ranks: histories are independent, so every rank takes a
+contiguous range of history ids (whole statistical batches) with the full problem and private tallies; the only
+exchange is one sum-reduction of the raw tally accumulators and ledgers at the end.  Pure bookkeeping -- no
+transport arithmetic here."""
+from __future__ import annotations
+
+import numpy as np
+
+
+def shard_range(n_total: int, world: int, rank: int, n_batches: int | None = None):
+    """(first_history_id, n_histories[, n_batches]) of `rank`.  With n_batches the split is by whole batches
+    (batch size n_total / n_batches), earlier ranks taking the remainder."""
+    if world < 1 or not (0 <= rank < world):
+        raise ValueError("bad world/rank")
+    if n_batches is None:
+        base, rem = divmod(n_total, world)
+        n = base + (1 if rank < rem else 0)
+        first = rank * base + min(rank, rem)
+        return first, n
+    if n_total % n_batches:
+        raise ValueError("n_batches must divide n_total")
+    hb = n_total // n_batches
+    base, rem = divmod(n_batches, world)
+    nb = base + (1 if rank < rem else 0)
+    first_b = rank * base + min(rank, rem)
+    return first_b * hb, nb * hb, nb
+
+
+def merge_statistics(sum_, sumsq, n_hist, n_batches):
+    """mean / sdev from reduced accumulators: sum over batches of S_b and S_b^2."""
+    hb = n_hist / n_batches
+    mean = sum_ / n_hist
+    if n_batches > 1:
+        var = (sumsq / (hb * hb) / n_batches - mean * mean) / (n_batches - 1)
+        sdev = np.sqrt(np.maximum(var, 0.0))
+    else:
+        sdev = np.zeros_like(mean)
+    return mean, sdev
+
+
+def all_reduce_tallies(sum_, sumsq, ledger, group=None):
+    """Sum-reduce raw accumulators over the process group (gloo on CPU tensors, nccl on CUDA tensors)."""
+    import torch
+    import torch.distributed as dist
+
+    out = []
+    for a in (sum_, sumsq, ledger):
+        t = a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a, dtype=np.float64))
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+        out.append(t if isinstance(a, torch.Tensor) else t.numpy())
+    return tuple(out)
