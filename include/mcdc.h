@@ -49,6 +49,11 @@ enum {
 
 enum { MCDC_BC_TRANSMISSION = 0, MCDC_BC_VACUUM = 1, MCDC_BC_REFLECTIVE = 2 };
 enum { MCDC_DIR_ISOTROPIC = 0, MCDC_DIR_FIXED = 1 };
+/* Schedulers: ASYNC = one persistent history kernel per sub-batch, census events do the
+ * population bookkeeping and the particle carries on; CENSUS_STEPPED = one kernel per census step,
+ * particles reaching the census time are parked in the census bank until every particle has arrived
+ * (the structure a population-control step needs).                                                 */
+enum { MCDC_SCHED_ASYNC = 0, MCDC_SCHED_CENSUS_STEPPED = 1 };
 
 /* Problem description.  Layouts are C row-major.
  *  sigma_s[m][g][g2] is the transfer cross section FROM group g TO group g2.
@@ -87,6 +92,7 @@ typedef struct {
   uint32_t n_batches;             /* >= 1                                                          */
   uint64_t first_history_id;      /* global id of the first history (resumable / shardable runs)   */
   int32_t record_history_events;  /* keep per-history event counts of this run (N x 4 uint32)      */
+  int32_t scheduler;              /* MCDC_SCHED_*; both give the same trajectories and tallies      */
 } mcdc_run_opts;
 
 typedef struct {

@@ -12,7 +12,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libmcdc.so")
+_LIB_PATH = os.environ.get("MCDC_LIB_PATH") or os.path.join(_HERE, "libmcdc.so")
 
 EXPORTED_SYMBOLS = [
     "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size",
@@ -49,7 +49,8 @@ class ProblemDesc(C.Structure):
 
 
 class RunOpts(C.Structure):
-    _fields_ = [("n_batches", C.c_uint32), ("first_history_id", C.c_uint64), ("record_history_events", C.c_int32)]
+    _fields_ = [("n_batches", C.c_uint32), ("first_history_id", C.c_uint64), ("record_history_events", C.c_int32),
+                ("scheduler", C.c_int32)]
 
 
 class Counters(C.Structure):
@@ -189,8 +190,11 @@ def mcdc_run(h, n_histories, seed):
     _check(lib().mcdc_run(h, int(n_histories), int(seed)), "mcdc_run", h)
 
 
-def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False):
-    o = RunOpts(int(n_batches), int(first_history_id), int(bool(record_history_events)))
+SCHED_ASYNC, SCHED_CENSUS_STEPPED = 0, 1
+
+
+def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False, scheduler=0):
+    o = RunOpts(int(n_batches), int(first_history_id), int(bool(record_history_events)), int(scheduler))
     _check(lib().mcdc_run_ex(h, int(n_histories), int(seed), C.byref(o)), "mcdc_run_ex", h)
 
 
@@ -271,11 +275,12 @@ class Problem:
     def reset(self):
         mcdc_problem_reset(self._h)
 
-    def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False):
+    def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False,
+            scheduler=0):
         n = int(n_histories if n_histories is not None else self.prob.n_histories)
         s = int(seed if seed is not None else self.prob.seed)
         b = int(n_batches if n_batches is not None else self.prob.n_batches)
-        mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events)
+        mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events, scheduler)
         self._last_n = n
 
     def tallies(self):

@@ -107,7 +107,7 @@ __device__ __forceinline__ Vec3 quad_grad(const double *__restrict__ c, double x
   return g;
 }
 
-// smallest positive root of a u^2 + 2 k u + c (half-b form), per A.4; INF when none
+// smallest positive root of a u^2 + 2 k u + c (half-b form) per A.4: q = -(k + sign(k) sqrt(k^2 - a c)), roots q/a and c/q
 __device__ __forceinline__ double quad_root(double a, double k, double c) {
   const double INF = CUDART_INF;
   if (a == 0.0) {
@@ -117,7 +117,8 @@ __device__ __forceinline__ double quad_root(double a, double k, double c) {
   }
   double disc = k * k - a * c;
   if (disc < 0.0) return INF;
-  double q = -(k + copysign(sqrt(disc), k));
+  const double sq = sqrt(disc);
+  const double q = (k < 0.0) ? (sq - k) : -(k + sq);      // sign(+-0) = +1 as in A.4
   double best = INF;
   double u1 = q / a;
   if (u1 > 0.0) best = u1;
@@ -128,25 +129,49 @@ __device__ __forceinline__ double quad_root(double a, double k, double c) {
   return best;
 }
 
-// distance to surface s along (ux,uy,uz) from (x,y,z); on => the particle sits on s (c := 0)
-__device__ __forceinline__ double surf_distance(const Tables &T, int s, bool on, double x, double y, double z,
-                                                double ux, double uy, double uz) {
+// same roots for a > 0 (cylinders): only the root that is the smallest positive one is divided out.
+//   c > 0: both roots share the sign of -k; the smaller is c/q.   c < 0: one positive root, q/a if k < 0 else c/q.
+//   c == 0 (on the surface): roots 0 and -2k/a.
+__device__ __forceinline__ double quad_root_pos_a(double a, double k, double c) {
   const double INF = CUDART_INF;
-  const int type = __ldg(T.surf_type + s);
-  const double4 q = ldg_d4(T.surf_q + s);
+  if (!(a > 0.0)) return INF;                              // parallel to the axis (A.4 plane branch with b = 0)
+  const double disc = k * k - a * c;
+  if (disc < 0.0) return INF;
+  const double sq = sqrt(disc);
+  const double q = (k < 0.0) ? (sq - k) : -(k + sq);      // -(k + sign(k) sqrt(disc)), sign(+-0) = +1 as in A.4
+  double u;
+  if (c > 0.0) {
+    if (k >= 0.0) return INF;
+    u = c / q;
+  } else if (c < 0.0) {
+    u = (k < 0.0) ? q / a : c / q;
+  } else {
+    if (k >= 0.0) return INF;
+    u = q / a;
+  }
+  return (u > 0.0) ? u : INF;
+}
+
+// distance to surface s along (ux,uy,uz) from (x,y,z); on => the particle sits on s (c := 0)
+__device__ __forceinline__ double surf_distance(const Tables &T, int s, int type, bool on, double x, double y, double z,
+                                                double ux, double uy, double uz, double ix, double iy, double iz) {
+  // (ix, iy, iz) = 1 / (ux, uy, uz), computed once per segment
+  const double INF = CUDART_INF;
   if (type <= ST_PLANE_Z) {
     if (on) return INF;
+    const double pos = __ldg((const double *)(T.surf_q + s));
     double r = (type == ST_PLANE_X) ? x : ((type == ST_PLANE_Y) ? y : z);
-    double u = (type == ST_PLANE_X) ? ux : ((type == ST_PLANE_Y) ? uy : uz);
-    double d = (q.x - r) / u;                      // u == 0: +-inf or NaN, both rejected below
+    double iu = (type == ST_PLANE_X) ? ix : ((type == ST_PLANE_Y) ? iy : iz);
+    double d = (pos - r) * iu;                     // u == 0: iu = inf -> +-inf or NaN, both rejected below
     return (d > 0.0 && d < INF) ? d : INF;
   }
+  const double4 q = ldg_d4(T.surf_q + s);
   if (type == ST_CYL_Z) {
     double dx = x - q.x, dy = y - q.y;
     double a = ux * ux + uy * uy;
     double k = dx * ux + dy * uy;
     double c = on ? 0.0 : (dx * dx + dy * dy - q.z);
-    return quad_root(a, k, c);
+    return quad_root_pos_a(a, k, c);
   }
   const double *c = T.surf_coef + 10 * s;
   double a = __ldg(c + 0) * ux * ux + __ldg(c + 1) * uy * uy + __ldg(c + 2) * uz * uz + __ldg(c + 3) * ux * uy +
@@ -159,9 +184,8 @@ __device__ __forceinline__ double surf_distance(const Tables &T, int s, bool on,
 
 // sense (+1 / -1) of surface s at r for a particle travelling along u (A.3 tie rule); from_dir forces
 // the direction rule (the surface just crossed, A.5)
-__device__ __forceinline__ int surf_sense(const Tables &T, int s, bool from_dir, double x, double y, double z,
+__device__ __forceinline__ int surf_sense(const Tables &T, int s, int type, bool from_dir, double x, double y, double z,
                                           double ux, double uy, double uz) {
-  const int type = __ldg(T.surf_type + s);
   const double4 q = ldg_d4(T.surf_q + s);
   double f, b;
   if (type <= ST_PLANE_Z) {
@@ -188,9 +212,9 @@ __device__ __forceinline__ bool cell_contains(const Tables &T, int c, int crosse
                                               double ux, double uy, double uz) {
   const int e = __ldg(T.cell_off + c + 1);
   for (int i = __ldg(T.cell_off + c); i < e; ++i) {
-    int h = __ldg(T.hs + i);
-    int s = h >> 1, want = (h & 1) ? 1 : -1;
-    if (surf_sense(T, s, s == crossed, x, y, z, ux, uy, uz) != want) return false;
+    int h = __ldg(T.hs + i);                            // packed: surface << 4 | type << 1 | (sense > 0)
+    int s = h >> 4, want = (h & 1) ? 1 : -1;
+    if (surf_sense(T, s, (h >> 1) & 7, s == crossed, x, y, z, ux, uy, uz) != want) return false;
   }
   return true;
 }
@@ -234,9 +258,8 @@ __device__ __forceinline__ int locate_source(const Tables &T, double x, double y
 }
 
 // specular reflection about grad f at the hit point (A.5)
-__device__ __forceinline__ void reflect(const Tables &T, int s, double x, double y, double z, double &ux, double &uy,
-                                        double &uz) {
-  const int type = __ldg(T.surf_type + s);
+__device__ __forceinline__ void reflect(const Tables &T, int s, int type, double x, double y, double z, double &ux,
+                                        double &uy, double &uz) {
   if (type == ST_PLANE_X) { ux = -ux; return; }
   if (type == ST_PLANE_Y) { uy = -uy; return; }
   if (type == ST_PLANE_Z) { uz = -uz; return; }

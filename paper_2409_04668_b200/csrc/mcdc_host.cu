@@ -85,10 +85,15 @@ struct mcdc_problem {
   cudaStream_t stream = nullptr;
   Bank bankA, bankB, bankS1, bankS2;
   double *x_acc = nullptr;
+  uint32_t *counts_dev = nullptr;
+  FissionQueue queue;
+  uint32_t *d_hist_cursor = nullptr;   // handle-owned
+  unsigned long long *d_head_tail = nullptr;
   // bookkeeping
   uint64_t histories = 0, batches = 0, batch_size = 0, launches = 0;
   double ms_run = 0.0, ms_transport = 0.0;
-  int n_sm = 148, blocks_per_sm = 1;
+  int n_sm = 148, blocks_per_sm = 1, blocks_per_sm_hist = 1;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
   std::string cuda_err;
 };
 
@@ -319,17 +324,18 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   std::vector<double4> q(S);
   for (int s = 0; s < S; ++s) classify_surface(&p->surf_coef[(size_t)10 * s], type[s], q[s]);
   std::vector<int> hs(nhs);
-  for (int i = 0; i < nhs; ++i) hs[i] = (p->hs_surface[i] << 1) | (p->hs_sense[i] > 0 ? 1 : 0);
+  for (int i = 0; i < nhs; ++i) hs[i] = (p->hs_surface[i] << 4) | (type[p->hs_surface[i]] << 1) | (p->hs_sense[i] > 0 ? 1 : 0);
   std::vector<Box> box(C);
   for (int c = 0; c < C; ++c) box[c] = cell_box(*p, type, q, c);
   // cells listing half-space (s, sense): index 2*s + (sense>0)
   std::vector<std::vector<int>> users((size_t)2 * S);
+  auto user_key = [&](int i) { return (size_t)2 * p->hs_surface[i] + (p->hs_sense[i] > 0 ? 1 : 0); };
   for (int c = 0; c < C; ++c)
-    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) users[(size_t)hs[i]].push_back(c);
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) users[user_key(i)].push_back(c);
   std::vector<int> nb_off(nhs + 1, 0), nb_cell;
   for (int c = 0; c < C; ++c)
     for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
-      const std::vector<int> &cand = users[(size_t)(hs[i] ^ 1)];          // same surface, opposite sense
+      const std::vector<int> &cand = users[user_key(i) ^ 1];          // same surface, opposite sense
       for (int c2 : cand)
         if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);  // increasing id by construction
       nb_off[i + 1] = (int)nb_cell.size();
@@ -393,6 +399,8 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   p->d_sum = ar.zeros<double>(p->n_bins); p->d_sumsq = ar.zeros<double>(p->n_bins);
   p->d_pop_w = ar.zeros<double>(p->K); p->d_pop_n = ar.zeros<unsigned long long>(p->K);
   p->d_cnt = ar.zeros<DevCounters>(1);
+  p->d_hist_cursor = ar.zeros<uint32_t>(1);
+  p->d_head_tail = ar.zeros<unsigned long long>(2);
   if (ar.err != cudaSuccess) {
     ar.release();
     delete p;
@@ -438,16 +446,27 @@ constexpr size_t BIRTH_BYTES = 5 * 8 + 8 + 16 + 4;   // x y z t w, key, meta, hi
 struct WsLayout {
   size_t total = 0;
   size_t x_acc = 0, counts = 0, bank[4] = {0, 0, 0, 0};
-  size_t fixed = 0;          // bytes that do not scale with the bank capacity
+  size_t q_flag = 0, q_data = 0;
+  uint64_t q_cap = 0;
+  size_t fixed = 0;          // bytes zeroed at bind (accumulators, counts, queue flags)
 };
 
 // slots * cap particles per bank; two full banks (live, census) and two birth banks (fission ping-pong)
-WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap) {
+uint64_t queue_capacity(uint64_t hist) {               // power of two, 2^20 .. 2^25 entries
+  uint64_t c = 1ull << 20;
+  while (c < hist && c < (1ull << 25)) c <<= 1;
+  return c;
+}
+
+WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap, uint64_t hist) {
   WsLayout L;
   size_t off = 0;
   L.x_acc = off; off += align_up((size_t)slots * p->n_bins * sizeof(double), 256);
   L.counts = off; off += align_up((size_t)8 * slots * sizeof(uint32_t), 256);
+  L.q_cap = queue_capacity(hist);
+  L.q_flag = off; off += align_up((size_t)L.q_cap * sizeof(uint32_t), 256);
   L.fixed = off;
+  L.q_data = off; off += (size_t)6 * align_up((size_t)L.q_cap * 8, 256) + align_up((size_t)L.q_cap * 16, 256);
   const size_t n = (size_t)slots * cap;
   for (int b = 0; b < 4; ++b) {
     L.bank[b] = off;
@@ -480,7 +499,7 @@ uint64_t default_cap(uint64_t hist, uint32_t slots) {
 
 extern "C" int mcdc_workspace_size(const mcdc_problem *p, uint64_t max_hist, uint32_t max_slots, size_t *bytes) {
   if (!p || !bytes || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
-  *bytes = layout(p, max_slots, default_cap(max_hist, max_slots)).total;
+  *bytes = layout(p, max_slots, default_cap(max_hist, max_slots), max_hist).total;
   return MCDC_OK;
 }
 
@@ -489,23 +508,37 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
   if (!p || !dev_ptr || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
   if (((uintptr_t)dev_ptr & 255u) != 0) return MCDC_ERR_ARG;
   uint64_t cap = default_cap(max_hist, max_slots);
-  WsLayout L = layout(p, max_slots, cap);
+  WsLayout L = layout(p, max_slots, cap, max_hist);
   if (bytes < L.total) return MCDC_ERR_NO_WORKSPACE;
   // a larger workspace buys larger banks: grow cap while it fits
   {
     uint64_t lo = cap, hi = cap * 64;
     while (lo + 32 <= hi) {
       uint64_t mid = align_up((size_t)((lo + hi) / 2), 32);
-      if (mid * max_slots <= 0xFFFFFFF0ull && layout(p, max_slots, mid).total <= bytes) lo = mid; else hi = mid - 32;
+      if (mid * max_slots <= 0xFFFFFFF0ull && layout(p, max_slots, mid, max_hist).total <= bytes) lo = mid; else hi = mid - 32;
     }
     cap = lo;
-    L = layout(p, max_slots, cap);
+    L = layout(p, max_slots, cap, max_hist);
   }
   p->ws = (char *)dev_ptr; p->ws_bytes = bytes; p->ws_hist = max_hist; p->ws_slots = max_slots;
   p->cap = (uint32_t)cap;
   p->stream = (cudaStream_t)cuda_stream;
   p->x_acc = (double *)(p->ws + L.x_acc);
   uint32_t *cnt = (uint32_t *)(p->ws + L.counts);
+  p->counts_dev = cnt;
+  {
+    char *qd = p->ws + L.q_data;
+    auto take = [&](size_t bytes) { char *r = qd; qd += align_up(bytes, 256); return r; };
+    FissionQueue &Q = p->queue;
+    Q.x = (double *)take(L.q_cap * 8); Q.y = (double *)take(L.q_cap * 8); Q.z = (double *)take(L.q_cap * 8);
+    Q.t = (double *)take(L.q_cap * 8); Q.w = (double *)take(L.q_cap * 8);
+    Q.key = (unsigned long long *)take(L.q_cap * 8);
+    Q.meta = (int4 *)take(L.q_cap * 16);
+    Q.flag = (uint32_t *)(p->ws + L.q_flag);
+    Q.mask = (uint32_t)(L.q_cap - 1);
+    Q.head_tail = p->d_head_tail;
+  }
+  CK(cudaMemsetAsync(p->d_head_tail, 0, 2 * sizeof(unsigned long long), (cudaStream_t)cuda_stream));
   const size_t n = (size_t)max_slots * cap;
   carve_bank(p->bankA, p->ws, L.bank[0], n, true, cnt + 0 * max_slots, cnt + 1 * max_slots);
   carve_bank(p->bankB, p->ws, L.bank[1], n, true, cnt + 2 * max_slots, cnt + 3 * max_slots);
@@ -541,7 +574,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
                  cudaEvent_t ev0, cudaEvent_t ev1) {
   const uint32_t ns = sb.n_slots;
   const uint32_t ws_ns = p->ws_slots;
-  uint32_t *counts_dev = (uint32_t *)((char *)p->x_acc + align_up((size_t)ws_ns * p->n_bins * sizeof(double), 256));
+  uint32_t *counts_dev = p->counts_dev;
   std::vector<uint32_t> h_counts((size_t)8 * ws_ns);
   CK(cudaMemsetAsync(counts_dev, 0, (size_t)8 * ws_ns * sizeof(uint32_t), p->stream));
   Bank A = p->bankA, Bk = p->bankB, S1 = p->bankS1, S2 = p->bankS2;
@@ -633,11 +666,46 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   return MCDC_OK;
 }
 
+// ---- asynchronous scheduler: one k_history launch per sub-batch, no host synchronisation ----
+int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
+                       cudaEvent_t ev0, cudaEvent_t ev1) {
+  HistoryArgs ha;
+  ha.q = p->queue;
+  ha.hist_cursor = p->d_hist_cursor;
+  ha.seed_mixed = mix64(seed + MCDC_GAMMA);
+  ha.first_history = first_history_id + sb.first_local;
+  ha.n_hist = sb.n_hist; ha.hb = sb.hs;
+  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
+  ha.aggregate = ((size_t)p->G * p->n_spatial <= 4096) ? 1 : 0;
+  CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
+  // consumers' cursor := producers' cursor (drops whatever an aborted launch may have left behind)
+  CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
+  const size_t smem = (size_t)p->K * (sizeof(double) + sizeof(uint32_t)) + 8;
+  const int max_grid = p->n_sm * p->blocks_per_sm_hist;
+  int grid = (int)std::min<uint64_t>((uint64_t)max_grid, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + TRANSPORT_THREADS - 1) / TRANSPORT_THREADS));
+  (void)ev0; (void)ev1;
+  cudaEvent_t a, b;
+  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  CK(cudaEventRecord(a, p->stream));
+  k_history<<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
+  CK(cudaEventRecord(b, p->stream));
+  p->ev_pairs.emplace_back(a, b);
+  p->launches++;
+  if (sb.closeout) {
+    int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
+    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)sb.n_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    p->launches++;
+  }
+  CK(cudaGetLastError());
+  return MCDC_OK;
+}
+
 }  // namespace
 
 extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts) {
   if (!p || n_histories == 0) return MCDC_ERR_ARG;
-  mcdc_run_opts def = {1u, 0ull, 0};
+  mcdc_run_opts def = {1u, 0ull, 0, 0};
   if (!opts) opts = &def;
   const uint32_t B = opts->n_batches ? opts->n_batches : 1u;
   if (n_histories % B != 0) return MCDC_ERR_ARG;
@@ -645,6 +713,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   if (p->batch_size != 0 && p->batch_size != hb) return MCDC_ERR_ARG;
   if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
   const bool record = opts->record_history_events != 0;
+  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED;
+  if (opts->scheduler != MCDC_SCHED_ASYNC && !stepped) return MCDC_ERR_ARG;
   if (record) {
     if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
     CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
@@ -663,6 +733,9 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
     size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
       p->blocks_per_sm = occ;
+    occ = 1;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_history, TRANSPORT_THREADS, (size_t)p->K * 12 + 8) == cudaSuccess && occ > 0)
+      p->blocks_per_sm_hist = occ;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
   CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1)); CK(cudaEventCreate(&ev0)); CK(cudaEventCreate(&ev1));
@@ -678,7 +751,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       SubBatch sb;
       sb.n_slots = std::min<uint32_t>(per_sub, B - b);
       sb.first_local = (uint64_t)b * hb; sb.n_hist = (uint32_t)(sb.n_slots * hb); sb.hs = (uint32_t)hb; sb.closeout = 1;
-      rc = run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+      rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
+                   : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
     }
   } else {                                               // one batch = several pieces spread over the slots
     const uint64_t per_sub = std::min<uint64_t>(p->ws_hist, slot_max * p->ws_slots);
@@ -690,7 +764,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
         sb.n_slots = (uint32_t)((n + sb.hs - 1) / sb.hs);
         sb.first_local = (uint64_t)b * hb + off; sb.n_hist = (uint32_t)n;
         sb.closeout = (off + n >= hb) ? 2 : 0;
-        rc = run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+        rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
+                   : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
       }
     }
   }
@@ -699,6 +774,12 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   float ms = 0.f;
   cudaEventElapsedTime(&ms, e_run0, e_run1);
   p->ms_run = ms;
+  for (auto &pr : p->ev_pairs) {
+    float m2 = 0.f;
+    if (se == cudaSuccess && cudaEventElapsedTime(&m2, pr.first, pr.second) == cudaSuccess) p->ms_transport += m2;
+    cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+  }
+  p->ev_pairs.clear();
   cudaEventDestroy(e_run0); cudaEventDestroy(e_run1); cudaEventDestroy(ev0); cudaEventDestroy(ev1);
   if (rc != MCDC_OK) return rc;
   if (se != cudaSuccess) return cuda_fail(p, se, "cudaStreamSynchronize");

@@ -7,7 +7,7 @@
 // ballot-aggregated appends.  Track-length scores go to a shared-memory copy of the step's tally slab
 // (match_any-aggregated when few bins are hit) and are flushed with fp64 RED to the slot's accumulator.
 #pragma once
-#include "mcdc_device.cuh"
+#include "mcdc_step.cuh"
 
 namespace mcdc {
 
@@ -41,10 +41,31 @@ __device__ __forceinline__ uint32_t warp_append(uint32_t *counter, bool want) {
 // ------------------------------------------------------------------------------------------------
 struct TallySink {
   double *slab;      // shared memory, or nullptr
-  double *global_x;  // slot accumulator x[slot][n_bins]
+  double *global_x;  // this lane's slot accumulator x[slot][n_bins]
   long long slab_lo; // first global bin held by the slab
   int slab_bins;
+  int aggregate;     // global mode: merge equal addresses inside the warp before the RED
 };
+
+// warp-converged sum of `val` over the lanes whose key equals the leader's, for up to `max_leaders` distinct keys;
+// returns true when the caller's contribution was absorbed by a leader (leader lanes get the total in val).
+template <class K>
+__device__ __forceinline__ bool warp_merge_equal(K key, bool valid, double &val, int max_leaders) {
+  unsigned peers = __match_any_sync(MCDC_FULL, key);
+  const int my_leader = __ffs(peers) - 1;
+  unsigned leaders = __ballot_sync(MCDC_FULL, valid && lane_id() == my_leader);
+  if (__popc(leaders) > max_leaders) return false;          // many distinct keys: little to gain
+  double mine = val;
+  bool absorbed = valid && lane_id() != my_leader;
+  while (leaders) {
+    const int l = __ffs(leaders) - 1;
+    leaders &= leaders - 1u;
+    const K lk = __shfl_sync(MCDC_FULL, key, l);
+    const double v = warp_sum((valid && key == lk) ? mine : 0.0);
+    if (lane_id() == l) val = v;
+  }
+  return absorbed;
+}
 
 __device__ __forceinline__ void tally_add_converged(const TallySink &S, long long bin, double val) {
   unsigned valid = __ballot_sync(MCDC_FULL, bin >= 0);
@@ -55,20 +76,13 @@ __device__ __forceinline__ void tally_add_converged(const TallySink &S, long lon
       atomicAdd(S.global_x + bin, val);
       bin = -1;
     }
-    int b = (bin >= 0) ? (int)rel : -1;
-    unsigned peers = __match_any_sync(MCDC_FULL, b);
-    unsigned leaders = __ballot_sync(MCDC_FULL, b >= 0 && lane_id() == __ffs(peers) - 1);
-    if (__popc(leaders) <= 3) {
-      while (leaders) {
-        int l = __ffs(leaders) - 1;
-        leaders &= leaders - 1u;
-        int lb = __shfl_sync(MCDC_FULL, b, l);
-        double v = warp_sum((b == lb) ? val : 0.0);
-        if (lane_id() == l) atomicAdd(S.slab + lb, v);
-      }
-    } else if (b >= 0) {
-      atomicAdd(S.slab + b, val);
-    }
+    const int b = (bin >= 0) ? (int)rel : -1;
+    const bool absorbed = warp_merge_equal<int>(b, b >= 0, val, 3);
+    if (b >= 0 && !absorbed) atomicAdd(S.slab + b, val);
+  } else if (S.aggregate) {
+    double *addr = (bin >= 0) ? S.global_x + bin : nullptr;
+    const bool absorbed = warp_merge_equal<unsigned long long>((unsigned long long)addr, bin >= 0, val, 3);
+    if (bin >= 0 && !absorbed) atomicAdd(addr, val);
   } else if (bin >= 0) {
     atomicAdd(S.global_x + bin, val);
   }
@@ -273,11 +287,55 @@ __global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank o
 }
 
 // ------------------------------------------------------------------------------------------------
-// Transport kernel: one census step (or one fission generation inside it) for every slot.
+// per-thread accumulators in shared memory (no atomics: one column per thread), flushed once per block
 // ------------------------------------------------------------------------------------------------
-enum { LED_PRODUCTION = 0, LED_CAPTURE, LED_FISSION_ABS, LED_LEAK, LED_CENSUS_FINAL, LED_LOST, LED_N };
-enum { CNT_COLL = 0, CNT_SURF, CNT_CENSUS, CNT_CHILDREN, CNT_LOST, CNT_N };
+struct BlockAccum {
+  double led[LED_N][TRANSPORT_THREADS];
+  uint32_t cnt[CNT_N][TRANSPORT_THREADS];
+  double scratch[32];
+};
 
+__device__ __forceinline__ void accum_zero(BlockAccum &B) {
+#pragma unroll
+  for (int e = 0; e < LED_N; ++e) B.led[e][threadIdx.x] = 0.0;
+#pragma unroll
+  for (int e = 0; e < CNT_N; ++e) B.cnt[e][threadIdx.x] = 0u;
+}
+
+__device__ __forceinline__ void accum_flush(BlockAccum &B, DevCounters *cnt) {
+  const int tid = threadIdx.x;
+  for (int e = 0; e < LED_N; ++e) block_atomic_add(&cnt->ledger[1 + e], B.led[e][tid], B.scratch);
+  unsigned long long *us = (unsigned long long *)B.scratch;
+  const unsigned long long nseg = (unsigned long long)B.cnt[CNT_COLL][tid] + B.cnt[CNT_SURF][tid] + B.cnt[CNT_CENSUS][tid];
+  block_atomic_add_u64(&cnt->n[1], nseg, us);
+  block_atomic_add_u64(&cnt->n[2], B.cnt[CNT_COLL][tid], us);
+  block_atomic_add_u64(&cnt->n[3], B.cnt[CNT_SURF][tid], us);
+  block_atomic_add_u64(&cnt->n[4], B.cnt[CNT_CENSUS][tid], us);
+  block_atomic_add_u64(&cnt->n[5], B.cnt[CNT_CHILDREN][tid], us);
+  block_atomic_add_u64(&cnt->n[6], B.cnt[CNT_LOST][tid], us);
+}
+
+// per-history event counts of a particle whose stay in this thread ends
+__device__ __forceinline__ void record_particle(BlockAccum &B, uint32_t *ev, uint32_t hid, uint32_t &pc_coll,
+                                                uint32_t &pc_surf, uint32_t &pc_child, uint32_t pc_census) {
+  const int tid = threadIdx.x;
+  B.cnt[CNT_COLL][tid] += pc_coll; B.cnt[CNT_SURF][tid] += pc_surf; B.cnt[CNT_CHILDREN][tid] += pc_child;
+  B.cnt[CNT_CENSUS][tid] += pc_census;
+  if (ev != nullptr) {
+    uint32_t *e4 = ev + (size_t)hid * 4;
+    if (pc_coll) atomicAdd(e4 + 0, pc_coll);
+    if (pc_surf) atomicAdd(e4 + 1, pc_surf);
+    if (pc_child) atomicAdd(e4 + 2, pc_child);
+    if (pc_census) atomicAdd(e4 + 3, pc_census);
+  }
+  pc_coll = pc_surf = pc_child = 0u;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Census-stepped transport kernel: one census step (or one fission generation inside it) for every slot.
+// Particles that reach the census time are parked in the census bank (A.8); fission children go to the
+// fission bank and are transported by the next launch of the same step.
+// ------------------------------------------------------------------------------------------------
 struct TransportArgs {
   Bank in, census_out, sec_out;
   double *x_acc;                 // [n_slots][n_bins] batch accumulators
@@ -289,18 +347,13 @@ struct TransportArgs {
 
 __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepParams P, TransportArgs A) {
   extern __shared__ double slab[];                       // [P.slab_bins]
-  __shared__ double s_led[LED_N][TRANSPORT_THREADS];
-  __shared__ uint32_t s_cnt[CNT_N][TRANSPORT_THREADS];
-  __shared__ double s_scratch[32];
+  __shared__ BlockAccum acc;
   __shared__ int s_flag;
-  const double INF = CUDART_INF;
   const int tid = threadIdx.x, lane = tid & 31;
-#pragma unroll
-  for (int e = 0; e < LED_N; ++e) s_led[e][tid] = 0.0;
-#pragma unroll
-  for (int e = 0; e < CNT_N; ++e) s_cnt[e][tid] = 0u;
+  accum_zero(acc);
   double popw = 0.0;
   uint32_t popn = 0u;
+  uint32_t *ev_out = P.record_events ? A.ev : nullptr;
 
   for (int probe = 0; probe < P.n_slots; ++probe) {
     const int slot = (int)((blockIdx.x + (unsigned)probe) % (unsigned)P.n_slots);
@@ -317,14 +370,13 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
     S.global_x = A.x_acc + (size_t)slot * T.n_bins;
     S.slab_lo = (long long)P.it_lo * T.G * T.mesh_n[2] * T.mesh_n[1] * T.mesh_n[0];
     S.slab_bins = P.slab_bins;
+    S.aggregate = 0;
     const size_t base_in = (size_t)slot * P.cap;
 
-    // ---- per-lane particle state (registers) ----
     bool have = false, exhausted = false;
-    double x = 0, y = 0, z = 0, ux = 0, uy = 0, uz = 1, t = 0, w = 0;
-    unsigned long long key = 0;
-    uint32_t ctr = 0, hid = 0;
-    int g = 0, cell = 0, last_surf = -1;
+    PState p;
+    p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
+    p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
     uint32_t pc_coll = 0, pc_surf = 0, pc_child = 0;
 
     for (;;) {
@@ -340,22 +392,14 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
           uint32_t i = base + (uint32_t)__popc(need & ((1u << lane) - 1u));
           if (i < n_in) {
             size_t j = base_in + i;
-            x = A.in.x[j]; y = A.in.y[j]; z = A.in.z[j]; t = A.in.t[j]; w = A.in.w[j];
-            key = A.in.key[j]; hid = A.in.hid[j];
+            p.x = A.in.x[j]; p.y = A.in.y[j]; p.z = A.in.z[j]; p.t = A.in.t[j]; p.w = A.in.w[j];
+            p.key = A.in.key[j]; p.hid = A.in.hid[j];
             int4 m = A.in.meta[j];
-            cell = m.x;
-            if (P.in_is_birth) {                         // A.6 init_child
-              ctr = 0u;
-              double xi_g = draw(key, ctr);
-              int mat = __ldg(T.cell_mat + cell);
-              g = sample_cdf(T.cdf_chi + (size_t)mat * T.G, T.G, __ldg(T.last_chi + mat), xi_g);
-              double xi_mu, xi_phi;
-              draw2(key, ctr, xi_mu, xi_phi);
-              isotropic(xi_mu, xi_phi, ux, uy, uz);
-              last_surf = -1;
-            } else {
-              ux = A.in.ux[j]; uy = A.in.uy[j]; uz = A.in.uz[j];
-              last_surf = m.y; ctr = (uint32_t)m.z; g = m.w;
+            p.cell = m.x;
+            if (P.in_is_birth) init_child(T, p);
+            else {
+              p.ux = A.in.ux[j]; p.uy = A.in.uy[j]; p.uz = A.in.uz[j];
+              p.last_surf = m.y; p.ctr = (uint32_t)m.z; p.g = m.w;
             }
             pc_coll = pc_surf = pc_child = 0u;
             have = true;
@@ -364,81 +408,33 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
       }
       if (__ballot_sync(MCDC_FULL, have) == 0u) break;
 
-      // ---------------- distances (A.2, A.4) ----------------
       double d = 0.0;
       int ev = -1, i_star = -1;
-      if (have) {
-        const int mat = __ldg(T.cell_mat + cell);
-        const int mg = mat * T.G + g;
-        const double xi = draw(key, ctr);
-        const double sig_t = __ldg(T.sig_t + mg);
-        const double d_coll = (sig_t > 0.0) ? -log(xi) * __ldg(T.inv_sig_t + mg) : INF;
-        double d_surf = INF;
-        const int e = __ldg(T.cell_off + cell + 1);
-        for (int i = __ldg(T.cell_off + cell); i < e; ++i) {
-          int s = __ldg(T.hs + i) >> 1;
-          double u = surf_distance(T, s, s == last_surf, x, y, z, ux, uy, uz);
-          if (u < d_surf) { d_surf = u; i_star = i; }
-        }
-        const double d_time = __ldg(T.speed + g) * (P.t_census - t);
-        if (d_time <= d_surf && d_time <= d_coll) { ev = EV_CENSUS; d = d_time; }
-        else if (d_surf <= d_coll)               { ev = EV_SURFACE; d = d_surf; }
-        else                                     { ev = EV_COLLISION; d = d_coll; }
-      }
-
-      // ---------------- score (A.7, pre-move state), then move (A.2) ----------------
-      score_track(T, S, have, x, y, z, ux, uy, uz, t, w, g, d);
+      if (have) ev = find_event(T, p, P.t_census, d, i_star);
+      score_track(T, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
       bool to_census = false;
       int n_children = 0;
-      uint32_t c0 = 0u;
+      uint32_t c0 = 0u, pc_census = 0u;
       if (have) {
-        x += d * ux; y += d * uy; z += d * uz;
-        t = (ev == EV_CENSUS) ? P.t_census : t + d * __ldg(T.inv_speed + g);
+        p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
+        p.t = (ev == EV_CENSUS) ? P.t_census : p.t + d * __ldg(T.inv_speed + p.g);
         if (ev == EV_CENSUS) {                           // A.8
-          s_cnt[CNT_CENSUS][tid] += 1u;
-          popw += w; popn += 1u;
-          if (d > 0.0) last_surf = -1;
-          if (P.is_last) s_led[LED_CENSUS_FINAL][tid] += w; else to_census = true;
+          pc_census = 1u;
+          popw += p.w; popn += 1u;
+          if (d > 0.0) p.last_surf = -1;
+          if (P.is_last) acc.led[LED_CENSUS_FINAL][tid] += p.w; else to_census = true;
           have = false;
-        } else if (ev == EV_SURFACE) {                   // A.5
+        } else if (ev == EV_SURFACE) {
           pc_surf += 1u;
-          const int s_star = __ldg(T.hs + i_star) >> 1;
-          last_surf = s_star;
-          const int bc = __ldg(T.surf_bc + s_star);
-          if (bc == 1) { s_led[LED_LEAK][tid] += w; have = false; }
-          else if (bc == 2) reflect(T, s_star, x, y, z, ux, uy, uz);
-          else {
-            int c = locate_neighbour(T, i_star, s_star, x, y, z, ux, uy, uz);
-            if (c < 0) { s_led[LED_LOST][tid] += w; s_cnt[CNT_LOST][tid] += 1u; have = false; }
-            else cell = c;
-          }
-        } else {                                         // A.6
+          have = surface_event(T, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
+        } else {
           pc_coll += 1u;
-          last_surf = -1;
-          const int mat = __ldg(T.cell_mat + cell);
-          const int mg = mat * T.G + g;
-          const double yv = draw(key, ctr) * __ldg(T.sig_t + mg);
-          const double s_tot = __ldg(T.sig_s_tot + mg);
-          if (yv < s_tot) {
-            double xi_g = draw(key, ctr);
-            g = sample_cdf(T.cdf_s + (size_t)mg * T.G, T.G, __ldg(T.last_s + mg), xi_g * s_tot);
-            double xi_mu, xi_phi;
-            draw2(key, ctr, xi_mu, xi_phi);
-            isotropic(xi_mu, xi_phi, ux, uy, uz);
-          } else if (yv < __ldg(T.sig_sc + mg) || __ldg(T.sig_f + mg) == 0.0) {
-            s_led[LED_CAPTURE][tid] += w; have = false;
-          } else {
-            double xi_nu = draw(key, ctr);
-            n_children = (int)floor(__ldg(T.nu + mg) + xi_nu);
-            c0 = ctr;
-            s_led[LED_FISSION_ABS][tid] += w;
-            s_led[LED_PRODUCTION][tid] += (double)n_children * w;
-            pc_child += (uint32_t)n_children;
-            have = false;
-          }
+          int r = collision_event(T, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
+                                  &acc.led[LED_PRODUCTION][tid]);
+          if (r != -1) have = false;
+          if (r > 0) { n_children = r; pc_child += (uint32_t)r; }
         }
       }
-
       // ---------------- hand-off: census bank (A.8) ----------------
       {
         uint32_t i = warp_append(A.census_out.count + slot, to_census);
@@ -447,9 +443,9 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
           else {
             size_t j = (size_t)slot * P.cap + i;
             Bank &O = A.census_out;
-            O.x[j] = x; O.y[j] = y; O.z[j] = z; O.ux[j] = ux; O.uy[j] = uy; O.uz[j] = uz;
-            O.t[j] = t; O.w[j] = w; O.key[j] = key; O.hid[j] = hid;
-            O.meta[j] = make_int4(cell, last_surf, (int)ctr, g);
+            O.x[j] = p.x; O.y[j] = p.y; O.z[j] = p.z; O.ux[j] = p.ux; O.uy[j] = p.uy; O.uz[j] = p.uz;
+            O.t[j] = p.t; O.w[j] = p.w; O.key[j] = p.key; O.hid[j] = p.hid;
+            O.meta[j] = make_int4(p.cell, p.last_surf, (int)p.ctr, p.g);
           }
         }
       }
@@ -472,24 +468,13 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
             if (i >= P.cap) { atomicExch(&A.cnt->overflow, 1); break; }
             size_t j = (size_t)slot * P.cap + i;
             Bank &O = A.sec_out;
-            O.x[j] = x; O.y[j] = y; O.z[j] = z; O.t[j] = t; O.w[j] = w; O.hid[j] = hid;
-            O.key[j] = child_key(key, c0, (uint32_t)c);
-            O.meta[j] = make_int4(cell, -1, 0, 0);
+            O.x[j] = p.x; O.y[j] = p.y; O.z[j] = p.z; O.t[j] = p.t; O.w[j] = p.w; O.hid[j] = p.hid;
+            O.key[j] = child_key(p.key, c0, (uint32_t)c);
+            O.meta[j] = make_int4(p.cell, -1, 0, 0);
           }
         }
       }
-      // ---------------- per-particle counters at the end of a particle's stay ----------------
-      if (!have && (pc_coll | pc_surf | pc_child | (uint32_t)(ev == EV_CENSUS))) {
-        s_cnt[CNT_COLL][tid] += pc_coll; s_cnt[CNT_SURF][tid] += pc_surf; s_cnt[CNT_CHILDREN][tid] += pc_child;
-        if (P.record_events && A.ev != nullptr) {
-          uint32_t *e4 = A.ev + (size_t)hid * 4;
-          if (pc_coll) atomicAdd(e4 + 0, pc_coll);
-          if (pc_surf) atomicAdd(e4 + 1, pc_surf);
-          if (pc_child) atomicAdd(e4 + 2, pc_child);
-          if (ev == EV_CENSUS) atomicAdd(e4 + 3, 1u);
-        }
-        pc_coll = pc_surf = pc_child = 0u;
-      }
+      if (!have && ev >= 0) record_particle(acc, ev_out, p.hid, pc_coll, pc_surf, pc_child, pc_census);
     }
 
     // ---- flush the slab into the slot's accumulator ----
@@ -500,19 +485,249 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
     }
     __syncthreads();
   }
+  accum_flush(acc, A.cnt);
+  block_atomic_add(A.pop_w + P.k, popw, acc.scratch);
+  block_atomic_add_u64(A.pop_n + P.k, (unsigned long long)popn, (unsigned long long *)acc.scratch);
+}
 
-  // ---- block totals -> global counters ----
-  for (int e = 0; e < LED_N; ++e) block_atomic_add(&A.cnt->ledger[1 + e], s_led[e][tid], s_scratch);
-  unsigned long long *us = (unsigned long long *)s_scratch;
-  const unsigned long long nseg = (unsigned long long)s_cnt[CNT_COLL][tid] + s_cnt[CNT_SURF][tid] + s_cnt[CNT_CENSUS][tid];
-  block_atomic_add_u64(&A.cnt->n[1], nseg, us);
-  block_atomic_add_u64(&A.cnt->n[2], s_cnt[CNT_COLL][tid], us);
-  block_atomic_add_u64(&A.cnt->n[3], s_cnt[CNT_SURF][tid], us);
-  block_atomic_add_u64(&A.cnt->n[4], s_cnt[CNT_CENSUS][tid], us);
-  block_atomic_add_u64(&A.cnt->n[5], s_cnt[CNT_CHILDREN][tid], us);
-  block_atomic_add_u64(&A.cnt->n[6], s_cnt[CNT_LOST][tid], us);
-  block_atomic_add(A.pop_w + P.k, popw, s_scratch);
-  block_atomic_add_u64(A.pop_n + P.k, (unsigned long long)popn, us);
+// ------------------------------------------------------------------------------------------------
+// Asynchronous history kernel: ONE launch per sub-batch.  Idle lanes take work from (1) the in-kernel
+// fission queue (children first, so lineages finish promptly) and (2) the source-history cursor, building the
+// source particle directly in registers.  A particle keeps its registers across census boundaries: the
+// census event only does the population bookkeeping (A.8) and moves on to the next census interval -- in
+// analog transport nothing has to wait there, so no census barrier is needed.
+// A fission parent turns into its first child in place; the other children are pushed to the queue.
+// ------------------------------------------------------------------------------------------------
+struct FissionQueue {             // ring buffer in HBM, structure of arrays, capacity mask+1 (power of two)
+  double *x, *y, *z, *t, *w;
+  unsigned long long *key;
+  int4 *meta;                     // {cell, census index k, hid, unused}
+  uint32_t *flag;                 // entry i is readable when flag[i & mask] == (uint32)(i + 1)
+  uint32_t mask;
+  unsigned long long *head_tail;  // [0] consumers' cursor, [1] producers' cursor (monotonic over launches)
+};
+
+struct HistoryArgs {
+  FissionQueue q;
+  uint32_t *hist_cursor;          // next source history of this sub-batch
+  unsigned long long seed_mixed, first_history;
+  uint32_t n_hist, hb;            // histories in the sub-batch, histories per slot
+  double *x_acc;
+  DevCounters *cnt;
+  double *pop_w;
+  unsigned long long *pop_n;
+  uint32_t *ev;
+  int aggregate;
+};
+
+__device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
+  uint32_t v;
+  asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_u32(uint32_t *p, uint32_t v) {
+  asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned long long *p) {
+  unsigned long long v;
+  asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+
+__global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, HistoryArgs A) {
+  extern __shared__ double s_dyn[];                      // pop_w[K] then pop_n[K] (u32)
+  __shared__ BlockAccum acc;
+  const int tid = threadIdx.x, lane = tid & 31;
+  const unsigned lt_mask = (1u << lane) - 1u;
+  double *s_popw = s_dyn;
+  uint32_t *s_popn = (uint32_t *)(s_dyn + T.K);
+  for (int k = tid; k < T.K; k += TRANSPORT_THREADS) { s_popw[k] = 0.0; s_popn[k] = 0u; }
+  accum_zero(acc);
+  __syncthreads();
+  unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
+  const unsigned long long q_cap = (unsigned long long)A.q.mask + 1ull;
+
+  bool have = false, src_done = false;
+  PState p;
+  p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
+  p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
+  int pk = 0;                                            // index of the particle's next census time
+  uint32_t slot = 0u;
+  uint32_t pc_coll = 0, pc_surf = 0, pc_child = 0, pc_census = 0, n_src = 0, n_src_lost = 0;
+
+  for (;;) {
+    // ---------------- acquire work for idle lanes ----------------
+    unsigned need = __ballot_sync(MCDC_FULL, !have);
+    if (need != 0u) {
+      // (1) fission queue
+      uint32_t got = 0u;
+      unsigned long long qbase = 0ull;
+      int abort_run = 0;
+      if (lane == 0) {
+        abort_run = *(volatile int *)&A.cnt->overflow;
+        unsigned long long h = ld_volatile_u64(q_head), t = ld_volatile_u64(q_tail);
+        if (t > h) {
+          unsigned long long want = min((unsigned long long)__popc(need), t - h);
+          if (atomicCAS(q_head, h, h + want) == h) { got = (uint32_t)want; qbase = h; }
+        }
+      }
+      if (__shfl_sync(MCDC_FULL, abort_run, 0)) break;   // a queue overflow was flagged: the run is void, leave
+      got = __shfl_sync(MCDC_FULL, got, 0);
+      qbase = __shfl_sync(MCDC_FULL, qbase, 0);
+      if (!have && (uint32_t)__popc(need & lt_mask) < got) {
+        const unsigned long long i = qbase + (unsigned long long)__popc(need & lt_mask);
+        const uint32_t j = (uint32_t)i & A.q.mask;
+        const uint32_t expect = (uint32_t)(i + 1ull);
+        bool ready = true;
+        for (uint32_t spin = 0; ld_acquire_u32(A.q.flag + j) != expect; ++spin) {
+          if ((spin & 255u) == 255u && (*(volatile int *)&A.cnt->overflow || spin > (1u << 26))) {
+            atomicExch(&A.cnt->overflow, 1);             // producer gave up (overflow) or never published
+            ready = false;
+            break;
+          }
+        }
+        if (ready) {
+        p.x = A.q.x[j]; p.y = A.q.y[j]; p.z = A.q.z[j]; p.t = A.q.t[j]; p.w = A.q.w[j];
+        p.key = A.q.key[j];
+        const int4 m = A.q.meta[j];
+        p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z;
+        slot = p.hid / A.hb;
+        init_child(T, p);
+        have = true;
+        }
+      }
+      // (2) source histories
+      unsigned need2 = __ballot_sync(MCDC_FULL, !have);
+      if (need2 != 0u && !src_done) {
+        const int leader = __ffs(need2) - 1;
+        uint32_t base = 0u;
+        if (lane == leader) base = atomicAdd(A.hist_cursor, (uint32_t)__popc(need2));
+        base = __shfl_sync(MCDC_FULL, base, leader);
+        if (base >= A.n_hist || base + (uint32_t)__popc(need2) >= A.n_hist) src_done = true;
+        if (!have) {
+          const uint32_t i = base + (uint32_t)__popc(need2 & lt_mask);
+          if (i < A.n_hist && base < A.n_hist) {
+            n_src += 1u;
+            p.hid = i;
+            slot = i / A.hb;
+            const bool ok = source_particle(T, A.seed_mixed, A.first_history + i, p);
+            pk = T.K - 1;
+            for (int k = 0; k < T.K; ++k)
+              if (__ldg(T.census + k) > p.t) { pk = k; break; }
+            if (ok) have = true; else n_src_lost += 1u;
+          }
+        }
+      }
+    }
+    if (__ballot_sync(MCDC_FULL, have) == 0u) {
+      if (!src_done) continue;
+      unsigned long long h = 0, t = 0;
+      if (lane == 0) { h = ld_volatile_u64(q_head); t = ld_volatile_u64(q_tail); }
+      h = __shfl_sync(MCDC_FULL, h, 0); t = __shfl_sync(MCDC_FULL, t, 0);
+      if (t <= h) break;
+      continue;
+    }
+
+    // ---------------- one segment ----------------
+    double d = 0.0;
+    int ev = -1, i_star = -1;
+    const double t_census = have ? __ldg(T.census + pk) : 0.0;
+    if (have) ev = find_event(T, p, t_census, d, i_star);
+    {
+      TallySink S;
+      S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
+      S.aggregate = A.aggregate;
+      score_track(T, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
+    }
+    int n_push = 0, census_k = -1;
+    uint32_t c0 = 0u;
+    bool ended = false;                                  // the particle (as an identity) ended in this iteration
+    if (have) {
+      p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
+      p.t = (ev == EV_CENSUS) ? t_census : p.t + d * __ldg(T.inv_speed + p.g);
+      if (ev == EV_CENSUS) {                             // A.8: bookkeeping only, then the next interval
+        pc_census += 1u;
+        census_k = pk;
+        if (d > 0.0) p.last_surf = -1;
+        if (pk == T.K - 1) { acc.led[LED_CENSUS_FINAL][tid] += p.w; have = false; ended = true; }
+        else pk += 1;
+      } else if (ev == EV_SURFACE) {
+        pc_surf += 1u;
+        have = surface_event(T, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
+        ended = !have;
+      } else {
+        pc_coll += 1u;
+        const int r = collision_event(T, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
+                                      &acc.led[LED_PRODUCTION][tid]);
+        if (r != -1) { ended = true; have = false; }
+        if (r > 0) { pc_child += (uint32_t)r; n_push = r - 1; }
+        if (r > 0) have = true;                          // continues below as child 0
+      }
+    }
+    // ---------------- census population (A.8), merged inside the warp ----------------
+    if (__ballot_sync(MCDC_FULL, census_k >= 0) != 0u) {
+      double v = p.w;
+      const bool absorbed = warp_merge_equal<int>(census_k, census_k >= 0, v, 4);
+      if (census_k >= 0) {
+        if (!absorbed) atomicAdd(s_popw + census_k, v);
+        atomicAdd(s_popn + census_k, 1u);
+      }
+    }
+    // ---------------- fission: push children 1..n-1, become child 0 (A.6) ----------------
+    {
+      unsigned fis = __ballot_sync(MCDC_FULL, n_push > 0);
+      if (fis != 0u) {
+        int pre = n_push;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          int v = __shfl_up_sync(MCDC_FULL, pre, o);
+          if (lane >= o) pre += v;
+        }
+        const int total = __shfl_sync(MCDC_FULL, pre, 31);
+        unsigned long long base = 0ull;
+        int ok = 1;
+        if (lane == 0) {
+          base = atomicAdd(q_tail, (unsigned long long)total);
+          if (base + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) ok = 0;
+        }
+        base = __shfl_sync(MCDC_FULL, base, 0) + (unsigned long long)(pre - n_push);
+        ok = __shfl_sync(MCDC_FULL, ok, 0);
+        if (!ok) { if (lane == 0) atomicExch(&A.cnt->overflow, 1); }
+        if (n_push > 0 && ok) {
+          for (int c = 0; c < n_push; ++c) {
+            const uint32_t j = (uint32_t)(base + (unsigned long long)c) & A.q.mask;
+            A.q.x[j] = p.x; A.q.y[j] = p.y; A.q.z[j] = p.z; A.q.t[j] = p.t; A.q.w[j] = p.w;
+            A.q.key[j] = child_key(p.key, c0, (uint32_t)(c + 1));
+            A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, 0);
+          }
+          __threadfence();
+          for (int c = 0; c < n_push; ++c) {
+            const unsigned long long i = base + (unsigned long long)c;
+            st_release_u32(A.q.flag + ((uint32_t)i & A.q.mask), (uint32_t)(i + 1ull));
+          }
+        }
+      }
+    }
+    if (ended) {
+      record_particle(acc, A.ev, p.hid, pc_coll, pc_surf, pc_child, pc_census);
+      pc_census = 0u;
+      if (have) {                                        // fission parent -> its first child, in place
+        p.key = child_key(p.key, c0, 0u);
+        init_child(T, p);
+      }
+    }
+  }
+
+  // ---- block totals ----
+  __syncthreads();
+  for (int k = tid; k < T.K; k += TRANSPORT_THREADS) {
+    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, s_popw[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
+  }
+  accum_flush(acc, A.cnt);
+  block_atomic_add(&A.cnt->ledger[0], (double)n_src, acc.scratch);
+  block_atomic_add(&A.cnt->ledger[6], (double)n_src_lost, acc.scratch);
+  block_atomic_add_u64(&A.cnt->n[0], (unsigned long long)n_src, (unsigned long long *)acc.scratch);
+  block_atomic_add_u64(&A.cnt->n[6], (unsigned long long)n_src_lost, (unsigned long long *)acc.scratch);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -45,7 +45,7 @@ struct Tables {
   const int *surf_type;    // [S]
   const int *surf_bc;      // [S]
   const int *cell_off;     // [C+1]
-  const int *hs;           // packed half-space: surface << 1 | (sense > 0)
+  const int *hs;           // packed half-space: surface << 4 | type << 1 | (sense > 0)
   const int *cell_mat;     // [C]
   const int *nb_off;       // [nhs+1] neighbour candidates of half-space slot i (cells across that surface)
   const int *nb_cell;

@@ -6,7 +6,7 @@ much tighter bound the shared trajectories allow)."""
 import numpy as np
 import pytest
 
-pytestmark = pytest.mark.gpu
+pytestmark = [pytest.mark.gpu, pytest.mark.timeout(300)]
 
 LEDGER = ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost")
 COUNTS = ("histories", "segments", "collisions", "surf_hits", "census_events", "children", "lost_n", "batches")
@@ -21,12 +21,12 @@ def M():
     return M
 
 
-def _pair(M, p, record=True, **gkw):
+def _pair(M, p, record=True, scheduler=0, **gkw):
     from oracle import Oracle
     o = Oracle(p)
     o.run(p.n_histories, p.seed, n_batches=p.n_batches, record_history_events=record)
     g = M.Problem(p, **gkw)
-    g.run(record_history_events=record)
+    g.run(record_history_events=record, scheduler=scheduler)
     return o, g
 
 
@@ -51,10 +51,11 @@ def _check_tallies(o, g, rtol, official=True):
         assert mg.sum() == pytest.approx(mo.sum(), rel=1e-3)
 
 
-def test_config0_bit_exact_event_counts_and_1e9_tallies(M):
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_config0_bit_exact_event_counts_and_1e9_tallies(M, scheduler):
     from workloads import configs as W
     p = W.config0_infinite_medium()                     # 1e5 histories, 20 batches: BASELINE config 0 as stated
-    o, g = _pair(M, p)
+    o, g = _pair(M, p, scheduler=scheduler)
     _check_counters(o, g)
     eo, eg = o.history_events(), g.history_events()
     same = np.all(eo == eg, axis=1).mean()
@@ -70,12 +71,13 @@ def test_config0_bit_exact_event_counts_and_1e9_tallies(M):
     g.close()
 
 
+@pytest.mark.parametrize("scheduler", [0, 1])
 @pytest.mark.parametrize("name,N,B", [("config1", 200_000, 20), ("config1a", 200_000, 20),
                                       ("config2", 300_000, 20), ("config3", 100_000, 20)])
-def test_larger_configs_match_the_oracle(M, name, N, B):
+def test_larger_configs_match_the_oracle(M, name, N, B, scheduler):
     from workloads import configs as W
     p = W.get_config(name, n_histories=N, n_batches=B)
-    o, g = _pair(M, p)
+    o, g = _pair(M, p, scheduler=scheduler)
     _check_counters(o, g)
     eo, eg = o.history_events(), g.history_events()
     assert np.all(eo == eg, axis=1).mean() >= 0.99999
@@ -85,11 +87,12 @@ def test_larger_configs_match_the_oracle(M, name, N, B):
     g.close()
 
 
+@pytest.mark.parametrize("scheduler", [0, 1])
 @pytest.mark.parametrize("N,B", [(1, 1), (31, 1), (33, 3), (257, 1), (1000, 8)])
-def test_ragged_and_tiny_runs(M, N, B):
+def test_ragged_and_tiny_runs(M, N, B, scheduler):
     from workloads import configs as W
     p = W.config3_pin_lattice(n_histories=N, n_batches=B)
-    o, g = _pair(M, p)
+    o, g = _pair(M, p, scheduler=scheduler)
     _check_counters(o, g)
     assert np.array_equal(o.history_events(), g.history_events())
     _check_tallies(o, g, rtol=1e-9, official=False)
@@ -105,16 +108,17 @@ def test_sub_batching_and_split_batches_do_not_change_results(M):
     ref_ev = g.history_events(); ref_s, ref_q = g.tally_sums(); ref_c = g.counters()
     g.close()
     for nh, nb in ((16_000, 4), (8_000, 16), (4_000, 1), (1_000, 4)):
-        h = M.Problem(p, max_histories_per_subbatch=nh, max_batches_in_flight=nb)
-        h.run(record_history_events=True)
-        assert np.array_equal(h.history_events(), ref_ev)
-        s, q = h.tally_sums()
-        assert np.allclose(s, ref_s, rtol=1e-12, atol=1e-14 * np.abs(ref_s).max())
-        assert np.allclose(q, ref_q, rtol=1e-11, atol=1e-14 * np.abs(ref_q).max())
-        c = h.counters()
-        for k in LEDGER + COUNTS:
-            assert c[k] == ref_c[k], (nh, nb, k)
-        h.close()
+        for scheduler in (0, 1):
+            h = M.Problem(p, max_histories_per_subbatch=nh, max_batches_in_flight=nb)
+            h.run(record_history_events=True, scheduler=scheduler)
+            assert np.array_equal(h.history_events(), ref_ev)
+            s, q = h.tally_sums()
+            assert np.allclose(s, ref_s, rtol=1e-12, atol=1e-14 * np.abs(ref_s).max())
+            assert np.allclose(q, ref_q, rtol=1e-11, atol=1e-14 * np.abs(ref_q).max())
+            c = h.counters()
+            for k in LEDGER + COUNTS:
+                assert c[k] == ref_c[k], (nh, nb, scheduler, k)
+            h.close()
     co = o.counters()
     for k in LEDGER + COUNTS:
         assert co[k] == ref_c[k]
@@ -163,11 +167,12 @@ def test_bank_overflow_is_detected(M):
     p = W.config0_infinite_medium(n_histories=2000, n_batches=1)
     p.sigma_f = p.sigma_f.copy(); p.sigma_c = p.sigma_c.copy(); p.nu = p.nu.copy()
     p.sigma_f[0, 0] = 0.45; p.sigma_c[0, 0] = 0.05; p.nu[0, 0] = 3.0       # c = 1.85: grows ~ e^{0.85 t}
-    g = M.Problem(p)
-    with pytest.raises(M.McdcError) as e:
-        g.run()
-    assert e.value.code == -6
-    g.close()
+    for scheduler in (0, 1):
+        g = M.Problem(p)
+        with pytest.raises(M.McdcError) as e:
+            g.run(scheduler=scheduler)
+        assert e.value.code == -6
+        g.close()
 
 
 def test_full_size_config3_sampled_against_the_oracle(M):
