@@ -1,5 +1,5 @@
 // mcdc_device.cuh -- device functions of the transport engine (sm_100a).
-// RNG, geometry (A.3-A.5), collision physics (A.6).
+// RNG, table access, geometry (A.3-A.5).
 #pragma once
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -8,6 +8,62 @@
 namespace mcdc {
 
 #define MCDC_FULL 0xFFFFFFFFu
+
+// dynamic shared memory of the transport kernels (staged tables first, kernel-specific data after)
+extern __shared__ __align__(16) unsigned char g_smem[];
+
+// ------------------------------------------------------------------------------------------------
+// Table accessor.  STAGED = true: the blob's hot prefix was copied to the start of dynamic shared memory
+// and every table read is an LDS; false: reads go to the global blob (L1/L2 cached).
+// ------------------------------------------------------------------------------------------------
+template <bool STAGED>
+struct TB {
+  const Tables &T;
+  __device__ __forceinline__ explicit TB(const Tables &t) : T(t) {}
+  template <class V>
+  __device__ __forceinline__ V ld(uint32_t off, int i) const {
+    if (STAGED) return reinterpret_cast<const V *>(g_smem + off)[i];
+    return reinterpret_cast<const V *>(T.blob + off)[i];
+  }
+  __device__ __forceinline__ double sig_t(int mg) const { return ld<double>(T.o_sig_t, mg); }
+  __device__ __forceinline__ double inv_sig_t(int mg) const { return ld<double>(T.o_inv_sig_t, mg); }
+  __device__ __forceinline__ double sig_s_tot(int mg) const { return ld<double>(T.o_sig_s_tot, mg); }
+  __device__ __forceinline__ double sig_sc(int mg) const { return ld<double>(T.o_sig_sc, mg); }
+  __device__ __forceinline__ double sig_f(int mg) const { return ld<double>(T.o_sig_f, mg); }
+  __device__ __forceinline__ double nu(int mg) const { return ld<double>(T.o_nu, mg); }
+  __device__ __forceinline__ double cdf_s(int i) const { return ld<double>(T.o_cdf_s, i); }
+  __device__ __forceinline__ int last_s(int mg) const { return ld<int>(T.o_last_s, mg); }
+  __device__ __forceinline__ double cdf_chi(int i) const { return ld<double>(T.o_cdf_chi, i); }
+  __device__ __forceinline__ int last_chi(int m) const { return ld<int>(T.o_last_chi, m); }
+  __device__ __forceinline__ double speed(int g) const { return ld<double>(T.o_speed, g); }
+  __device__ __forceinline__ double inv_speed(int g) const { return ld<double>(T.o_inv_speed, g); }
+  __device__ __forceinline__ double time_edge(int i) const { return ld<double>(T.o_T, i); }
+  __device__ __forceinline__ double census(int k) const { return ld<double>(T.o_census, k); }
+  __device__ __forceinline__ double src_cdf(int g) const { return ld<double>(T.o_src_cdf, g); }
+  __device__ __forceinline__ double2 surf_q01(int s) const { return ld<double2>(T.o_surf_q, 2 * s); }
+  __device__ __forceinline__ double2 surf_q23(int s) const { return ld<double2>(T.o_surf_q, 2 * s + 1); }
+  __device__ __forceinline__ double surf_q0(int s) const { return ld<double>(T.o_surf_q, 4 * s); }
+  __device__ __forceinline__ int surf_bc(int s) const { return ld<int>(T.o_surf_bc, s); }
+  __device__ __forceinline__ int cell_off(int c) const { return ld<int>(T.o_cell_off, c); }
+  __device__ __forceinline__ int hs(int i) const { return ld<int>(T.o_hs, i); }
+  __device__ __forceinline__ int cell_mat(int c) const { return ld<int>(T.o_cell_mat, c); }
+  __device__ __forceinline__ int nb_off(int i) const { return ld<int>(T.o_nb_off, i); }
+  __device__ __forceinline__ int nb_cell(int i) const { return ld<int>(T.o_nb_cell, i); }
+  __device__ __forceinline__ int loc_off(int i) const { return ld<int>(T.o_loc_off, i); }
+  __device__ __forceinline__ int loc_cell(int i) const { return ld<int>(T.o_loc_cell, i); }
+  // general quadric coefficients: from shared memory only when they are part of the staged prefix
+  __device__ __forceinline__ double coef(int s, int j) const {
+    if (STAGED && T.o_surf_coef < T.hot_bytes) return reinterpret_cast<const double *>(g_smem + T.o_surf_coef)[10 * s + j];
+    return reinterpret_cast<const double *>(T.blob + T.o_surf_coef)[10 * s + j];
+  }
+};
+
+// cooperative copy of the hot prefix into shared memory (call from all threads, then __syncthreads)
+__device__ __forceinline__ void stage_tables(const Tables &T) {
+  const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
+  uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
+  for (uint32_t i = threadIdx.x; i < T.hot_bytes / 16u; i += blockDim.x) dst[i] = src[i];
+}
 
 // ------------------------------------------------------------------------------------------------
 // RNG: counter-based, keyed by a 64-bit particle key; draw index = particle counter (Appendix B).
@@ -25,8 +81,8 @@ __device__ __forceinline__ unsigned long long child_key(unsigned long long kp, u
 }
 
 // Philox4x32-10 on counter (block, 0, 0, 0); returns the two 64-bit halves (o1:o0) and (o3:o2).
-__device__ __forceinline__ void philox_block(unsigned long long key, uint32_t block,
-                                             unsigned long long &lo64, unsigned long long &hi64) {
+// Not inlined: ~80 instructions called from a handful of sites keeps the kernels inside the i-cache.
+__device__ __noinline__ ulonglong2 philox_block(unsigned long long key, uint32_t block) {
   uint32_t c0 = block, c1 = 0u, c2 = 0u, c3 = 0u;
   uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
 #pragma unroll
@@ -37,8 +93,10 @@ __device__ __forceinline__ void philox_block(unsigned long long key, uint32_t bl
     c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
     k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
   }
-  lo64 = ((unsigned long long)c1 << 32) | c0;
-  hi64 = ((unsigned long long)c3 << 32) | c2;
+  ulonglong2 r;
+  r.x = ((unsigned long long)c1 << 32) | c0;
+  r.y = ((unsigned long long)c3 << 32) | c2;
+  return r;
 }
 
 // u = ((x >> 12) + 0.5) * 2^-52, built exactly: [1,2) mantissa trick then one exact subtraction.
@@ -48,22 +106,20 @@ __device__ __forceinline__ double u64_to_unit(unsigned long long x) {
 }
 
 __device__ __forceinline__ double draw(unsigned long long key, uint32_t &ctr) {
-  unsigned long long lo, hi;
-  philox_block(key, ctr >> 1, lo, hi);
-  unsigned long long x = (ctr & 1u) ? hi : lo;
+  const ulonglong2 b = philox_block(key, ctr >> 1);
+  const unsigned long long x = (ctr & 1u) ? b.y : b.x;
   ctr += 1u;
   return u64_to_unit(x);
 }
 // two consecutive draws; when ctr is even they come from one Philox block
 __device__ __forceinline__ void draw2(unsigned long long key, uint32_t &ctr, double &a, double &b) {
-  unsigned long long lo, hi;
-  philox_block(key, ctr >> 1, lo, hi);
+  ulonglong2 blk = philox_block(key, ctr >> 1);
   if (ctr & 1u) {
-    a = u64_to_unit(hi);
-    philox_block(key, (ctr + 1u) >> 1, lo, hi);
-    b = u64_to_unit(lo);
+    a = u64_to_unit(blk.y);
+    blk = philox_block(key, (ctr + 1u) >> 1);
+    b = u64_to_unit(blk.x);
   } else {
-    a = u64_to_unit(lo); b = u64_to_unit(hi);
+    a = u64_to_unit(blk.x); b = u64_to_unit(blk.y);
   }
   ctr += 2u;
 }
@@ -77,33 +133,23 @@ __device__ __forceinline__ void isotropic(double xi_mu, double xi_phi, double &u
   ux = st * c; uy = st * s; uz = mu;
 }
 
-// first index with xi < cdf[i]; fallback `last`
-__device__ __forceinline__ int sample_cdf(const double *__restrict__ cdf, int n, int last, double xi) {
-  for (int i = 0; i < n; ++i)
-    if (xi < __ldg(cdf + i)) return i;
-  return last;
-}
-
 // ------------------------------------------------------------------------------------------------
 // Geometry
 // ------------------------------------------------------------------------------------------------
 struct Vec3 { double x, y, z; };
 
-__device__ __forceinline__ double4 ldg_d4(const double4 *p) {
-  const double2 a = __ldg((const double2 *)p), b = __ldg((const double2 *)p + 1);
-  return make_double4(a.x, a.y, b.x, b.y);
+template <class TBT>
+__device__ __forceinline__ double quad_f(const TBT &tb, int s, double x, double y, double z) {
+  return tb.coef(s, 0) * x * x + tb.coef(s, 1) * y * y + tb.coef(s, 2) * z * z + tb.coef(s, 3) * x * y +
+         tb.coef(s, 4) * x * z + tb.coef(s, 5) * y * z + tb.coef(s, 6) * x + tb.coef(s, 7) * y + tb.coef(s, 8) * z +
+         tb.coef(s, 9);
 }
-
-__device__ __forceinline__ double quad_f(const double *__restrict__ c, double x, double y, double z) {
-  return __ldg(c + 0) * x * x + __ldg(c + 1) * y * y + __ldg(c + 2) * z * z + __ldg(c + 3) * x * y +
-         __ldg(c + 4) * x * z + __ldg(c + 5) * y * z + __ldg(c + 6) * x + __ldg(c + 7) * y + __ldg(c + 8) * z +
-         __ldg(c + 9);
-}
-__device__ __forceinline__ Vec3 quad_grad(const double *__restrict__ c, double x, double y, double z) {
+template <class TBT>
+__device__ __forceinline__ Vec3 quad_grad(const TBT &tb, int s, double x, double y, double z) {
   Vec3 g;
-  g.x = 2.0 * __ldg(c + 0) * x + __ldg(c + 3) * y + __ldg(c + 4) * z + __ldg(c + 6);
-  g.y = 2.0 * __ldg(c + 1) * y + __ldg(c + 3) * x + __ldg(c + 5) * z + __ldg(c + 7);
-  g.z = 2.0 * __ldg(c + 2) * z + __ldg(c + 4) * x + __ldg(c + 5) * y + __ldg(c + 8);
+  g.x = 2.0 * tb.coef(s, 0) * x + tb.coef(s, 3) * y + tb.coef(s, 4) * z + tb.coef(s, 6);
+  g.y = 2.0 * tb.coef(s, 1) * y + tb.coef(s, 3) * x + tb.coef(s, 5) * z + tb.coef(s, 7);
+  g.z = 2.0 * tb.coef(s, 2) * z + tb.coef(s, 4) * x + tb.coef(s, 5) * y + tb.coef(s, 8);
   return g;
 }
 
@@ -152,53 +198,55 @@ __device__ __forceinline__ double quad_root_pos_a(double a, double k, double c) 
   return (u > 0.0) ? u : INF;
 }
 
-// distance to surface s along (ux,uy,uz) from (x,y,z); on => the particle sits on s (c := 0)
-__device__ __forceinline__ double surf_distance(const Tables &T, int s, int type, bool on, double x, double y, double z,
+// distance to surface s along (ux,uy,uz) from (x,y,z); on => the particle sits on s (c := 0);
+// (ix, iy, iz) = 1 / (ux, uy, uz), computed once per segment
+template <class TBT>
+__device__ __forceinline__ double surf_distance(const TBT &tb, int s, int type, bool on, double x, double y, double z,
                                                 double ux, double uy, double uz, double ix, double iy, double iz) {
-  // (ix, iy, iz) = 1 / (ux, uy, uz), computed once per segment
   const double INF = CUDART_INF;
   if (type <= ST_PLANE_Z) {
     if (on) return INF;
-    const double pos = __ldg((const double *)(T.surf_q + s));
+    const double pos = tb.surf_q0(s);
     double r = (type == ST_PLANE_X) ? x : ((type == ST_PLANE_Y) ? y : z);
     double iu = (type == ST_PLANE_X) ? ix : ((type == ST_PLANE_Y) ? iy : iz);
     double d = (pos - r) * iu;                     // u == 0: iu = inf -> +-inf or NaN, both rejected below
     return (d > 0.0 && d < INF) ? d : INF;
   }
-  const double4 q = ldg_d4(T.surf_q + s);
   if (type == ST_CYL_Z) {
-    double dx = x - q.x, dy = y - q.y;
+    const double2 q01 = tb.surf_q01(s);
+    const double r2 = tb.surf_q23(s).x;
+    double dx = x - q01.x, dy = y - q01.y;
     double a = ux * ux + uy * uy;
     double k = dx * ux + dy * uy;
-    double c = on ? 0.0 : (dx * dx + dy * dy - q.z);
+    double c = on ? 0.0 : (dx * dx + dy * dy - r2);
     return quad_root_pos_a(a, k, c);
   }
-  const double *c = T.surf_coef + 10 * s;
-  double a = __ldg(c + 0) * ux * ux + __ldg(c + 1) * uy * uy + __ldg(c + 2) * uz * uz + __ldg(c + 3) * ux * uy +
-             __ldg(c + 4) * ux * uz + __ldg(c + 5) * uy * uz;
-  Vec3 g = quad_grad(c, x, y, z);
+  double a = tb.coef(s, 0) * ux * ux + tb.coef(s, 1) * uy * uy + tb.coef(s, 2) * uz * uz + tb.coef(s, 3) * ux * uy +
+             tb.coef(s, 4) * ux * uz + tb.coef(s, 5) * uy * uz;
+  Vec3 g = quad_grad(tb, s, x, y, z);
   double b = g.x * ux + g.y * uy + g.z * uz;
-  double cc = on ? 0.0 : quad_f(c, x, y, z);
+  double cc = on ? 0.0 : quad_f(tb, s, x, y, z);
   return quad_root(a, 0.5 * b, cc);
 }
 
 // sense (+1 / -1) of surface s at r for a particle travelling along u (A.3 tie rule); from_dir forces
 // the direction rule (the surface just crossed, A.5)
-__device__ __forceinline__ int surf_sense(const Tables &T, int s, int type, bool from_dir, double x, double y, double z,
+template <class TBT>
+__device__ __forceinline__ int surf_sense(const TBT &tb, int s, int type, bool from_dir, double x, double y, double z,
                                           double ux, double uy, double uz) {
-  const double4 q = ldg_d4(T.surf_q + s);
   double f, b;
   if (type <= ST_PLANE_Z) {
+    const double2 q = tb.surf_q01(s);
     double r = (type == ST_PLANE_X) ? x : ((type == ST_PLANE_Y) ? y : z);
     double u = (type == ST_PLANE_X) ? ux : ((type == ST_PLANE_Y) ? uy : uz);
     f = q.y * (r - q.x); b = q.y * u;
   } else if (type == ST_CYL_Z) {
-    double dx = x - q.x, dy = y - q.y;
-    f = q.w * (dx * dx + dy * dy - q.z); b = q.w * (dx * ux + dy * uy);
+    const double2 q01 = tb.surf_q01(s), q23 = tb.surf_q23(s);
+    double dx = x - q01.x, dy = y - q01.y;
+    f = q23.y * (dx * dx + dy * dy - q23.x); b = q23.y * (dx * ux + dy * uy);
   } else {
-    const double *c = T.surf_coef + 10 * s;
-    f = quad_f(c, x, y, z);
-    Vec3 g = quad_grad(c, x, y, z);
+    f = quad_f(tb, s, x, y, z);
+    Vec3 g = quad_grad(tb, s, x, y, z);
     b = g.x * ux + g.y * uy + g.z * uz;
   }
   if (!from_dir) {
@@ -208,39 +256,44 @@ __device__ __forceinline__ int surf_sense(const Tables &T, int s, int type, bool
   return (b < 0.0) ? -1 : 1;
 }
 
-__device__ __forceinline__ bool cell_contains(const Tables &T, int c, int crossed, double x, double y, double z,
+template <class TBT>
+__device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed, double x, double y, double z,
                                               double ux, double uy, double uz) {
-  const int e = __ldg(T.cell_off + c + 1);
-  for (int i = __ldg(T.cell_off + c); i < e; ++i) {
-    int h = __ldg(T.hs + i);                            // packed: surface << 4 | type << 1 | (sense > 0)
-    int s = h >> 4, want = (h & 1) ? 1 : -1;
-    if (surf_sense(T, s, (h >> 1) & 7, s == crossed, x, y, z, ux, uy, uz) != want) return false;
+  const int e = tb.cell_off(c + 1);
+  for (int i = tb.cell_off(c); i < e; ++i) {
+    const int h = tb.hs(i);                             // packed: surface << 4 | type << 1 | (sense > 0)
+    const int s = h >> 4, want = (h & 1) ? 1 : -1;
+    if (surf_sense(tb, s, (h >> 1) & 7, s == crossed, x, y, z, ux, uy, uz) != want) return false;
   }
   return true;
 }
 
 // full search in increasing cell id (A.3); slow path
-__device__ __noinline__ int locate_all(const Tables &T, int crossed, double x, double y, double z, double ux,
-                                       double uy, double uz) {
-  for (int c = 0; c < T.C; ++c)
-    if (cell_contains(T, c, crossed, x, y, z, ux, uy, uz)) return c;
+template <class TBT>
+__device__ __noinline__ int locate_all(const TBT &tb, int crossed, double x, double y, double z, double ux, double uy,
+                                       double uz) {
+  for (int c = 0; c < tb.T.C; ++c)
+    if (cell_contains(tb, c, crossed, x, y, z, ux, uy, uz)) return c;
   return -1;
 }
 
 // cell after crossing the surface of half-space slot `slot` of the current cell (A.5, transmission)
-__device__ __forceinline__ int locate_neighbour(const Tables &T, int slot, int s_star, double x, double y, double z,
+template <class TBT>
+__device__ __forceinline__ int locate_neighbour(const TBT &tb, int slot, int s_star, double x, double y, double z,
                                                 double ux, double uy, double uz) {
-  const int e = __ldg(T.nb_off + slot + 1);
-  for (int i = __ldg(T.nb_off + slot); i < e; ++i) {
-    int c = __ldg(T.nb_cell + i);
-    if (cell_contains(T, c, s_star, x, y, z, ux, uy, uz)) return c;
+  const int e = tb.nb_off(slot + 1);
+  for (int i = tb.nb_off(slot); i < e; ++i) {
+    const int c = tb.nb_cell(i);
+    if (cell_contains(tb, c, s_star, x, y, z, ux, uy, uz)) return c;
   }
-  return locate_all(T, s_star, x, y, z, ux, uy, uz);
+  return locate_all(tb, s_star, x, y, z, ux, uy, uz);
 }
 
 // source-particle location through the locator grid over the source box
-__device__ __forceinline__ int locate_source(const Tables &T, double x, double y, double z, double ux, double uy,
+template <class TBT>
+__device__ __forceinline__ int locate_source(const TBT &tb, double x, double y, double z, double ux, double uy,
                                              double uz) {
+  const Tables &T = tb.T;
   int v[3];
   const double r[3] = {x, y, z};
 #pragma unroll
@@ -248,22 +301,23 @@ __device__ __forceinline__ int locate_source(const Tables &T, double x, double y
     int i = (int)floor((r[a] - T.loc_lo[a]) * T.loc_inv_d[a]);
     v[a] = min(max(i, 0), T.loc_n[a] - 1);
   }
-  int vox = (v[2] * T.loc_n[1] + v[1]) * T.loc_n[0] + v[0];
-  const int e = __ldg(T.loc_off + vox + 1);
-  for (int i = __ldg(T.loc_off + vox); i < e; ++i) {
-    int c = __ldg(T.loc_cell + i);
-    if (cell_contains(T, c, -1, x, y, z, ux, uy, uz)) return c;
+  const int vox = (v[2] * T.loc_n[1] + v[1]) * T.loc_n[0] + v[0];
+  const int e = tb.loc_off(vox + 1);
+  for (int i = tb.loc_off(vox); i < e; ++i) {
+    const int c = tb.loc_cell(i);
+    if (cell_contains(tb, c, -1, x, y, z, ux, uy, uz)) return c;
   }
-  return locate_all(T, -1, x, y, z, ux, uy, uz);
+  return locate_all(tb, -1, x, y, z, ux, uy, uz);
 }
 
 // specular reflection about grad f at the hit point (A.5)
-__device__ __forceinline__ void reflect(const Tables &T, int s, int type, double x, double y, double z, double &ux,
+template <class TBT>
+__device__ __forceinline__ void reflect(const TBT &tb, int s, int type, double x, double y, double z, double &ux,
                                         double &uy, double &uz) {
   if (type == ST_PLANE_X) { ux = -ux; return; }
   if (type == ST_PLANE_Y) { uy = -uy; return; }
   if (type == ST_PLANE_Z) { uz = -uz; return; }
-  Vec3 g = quad_grad(T.surf_coef + 10 * s, x, y, z);
+  Vec3 g = quad_grad(tb, s, x, y, z);
   double inv = 1.0 / sqrt(g.x * g.x + g.y * g.y + g.z * g.z);
   double nx = g.x * inv, ny = g.y * inv, nz = g.z * inv;
   double dot = ux * nx + uy * ny + uz * nz;

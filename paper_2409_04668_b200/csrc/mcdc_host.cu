@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <limits>
 #include <string>
@@ -93,6 +94,8 @@ struct mcdc_problem {
   uint64_t histories = 0, batches = 0, batch_size = 0, launches = 0;
   double ms_run = 0.0, ms_transport = 0.0;
   int n_sm = 148, blocks_per_sm = 1, blocks_per_sm_hist = 1;
+  bool stage_tables = false;
+  int refill_min = 8;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
   std::string cuda_err;
 };
@@ -377,17 +380,33 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   Tables &t = p->tab;
   DeviceArena &ar = p->arena;
   t.G = G; t.M = M; t.S = S; t.C = C; t.K = p->K; t.Nt = p->Nt;
-  t.sig_t = ar.upload(p->sigma_t); t.inv_sig_t = ar.upload(inv_sig_t); t.sig_s_tot = ar.upload(s_tot);
-  t.sig_sc = ar.upload(s_sc); t.sig_f = ar.upload(p->sigma_f); t.nu = ar.upload(p->nu);
-  t.cdf_s = ar.upload(cdf_s); t.last_s = ar.upload(last_s); t.cdf_chi = ar.upload(cdf_chi);
-  t.last_chi = ar.upload(last_chi); t.speed = ar.upload(p->speed); t.inv_speed = ar.upload(inv_speed);
-  t.surf_coef = ar.upload(p->surf_coef); t.surf_q = ar.upload(q); t.surf_type = ar.upload(type);
-  t.surf_bc = ar.upload(p->surf_bc); t.cell_off = ar.upload(p->cell_off); t.hs = ar.upload(hs);
-  t.cell_mat = ar.upload(p->cell_mat); t.nb_off = ar.upload(nb_off); t.nb_cell = ar.upload(nb_cell);
-  t.src_cdf = ar.upload(src_cdf); t.src_last = src_last; t.src_dir_mode = p->src_dir_mode;
+  // one blob, 16-byte aligned pieces, hot tables first
+  std::vector<unsigned char> blob;
+  auto put = [&](const void *src, size_t bytes) -> uint32_t {
+    size_t off = (blob.size() + 15) / 16 * 16;
+    blob.resize(off + std::max<size_t>(bytes, 16), 0);
+    if (bytes) std::memcpy(blob.data() + off, src, bytes);
+    return (uint32_t)off;
+  };
+  auto putd = [&](const std::vector<double> &v) { return put(v.data(), v.size() * sizeof(double)); };
+  auto puti = [&](const std::vector<int> &v) { return put(v.data(), v.size() * sizeof(int)); };
+  t.o_sig_t = putd(p->sigma_t); t.o_inv_sig_t = putd(inv_sig_t); t.o_sig_s_tot = putd(s_tot); t.o_sig_sc = putd(s_sc);
+  t.o_sig_f = putd(p->sigma_f); t.o_nu = putd(p->nu); t.o_cdf_s = putd(cdf_s); t.o_last_s = puti(last_s);
+  t.o_cdf_chi = putd(cdf_chi); t.o_last_chi = puti(last_chi); t.o_speed = putd(p->speed); t.o_inv_speed = putd(inv_speed);
+  t.o_T = putd(p->T); t.o_census = putd(p->census); t.o_src_cdf = putd(src_cdf);
+  t.o_surf_q = put(q.data(), q.size() * sizeof(double4));
+  t.o_surf_bc = puti(p->surf_bc); t.o_cell_off = puti(p->cell_off); t.o_hs = puti(hs); t.o_cell_mat = puti(p->cell_mat);
+  t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell); t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
+  bool any_quadric = false;
+  for (int s = 0; s < S; ++s) any_quadric = any_quadric || type[s] == ST_QUADRIC;
+  size_t hot = (blob.size() + 15) / 16 * 16;
+  t.o_surf_coef = putd(p->surf_coef);
+  if (any_quadric) hot = (blob.size() + 15) / 16 * 16;
+  blob.resize((blob.size() + 15) / 16 * 16, 0);
+  t.hot_bytes = (uint32_t)hot;
+  t.blob = ar.upload(blob);
+  t.src_last = src_last; t.src_dir_mode = p->src_dir_mode;
   t.src_t0 = p->src_t0; t.src_t1 = p->src_t1;
-  t.loc_off = ar.upload(loc_off); t.loc_cell = ar.upload(loc_cell);
-  t.T = ar.upload(p->T); t.census = ar.upload(p->census);
   for (int a = 0; a < 3; ++a) {
     t.src_lo[a] = p->src_lo[a]; t.src_hi[a] = p->src_hi[a]; t.src_dir[a] = p->src_dir[a];
     t.loc_n[a] = loc_n[a]; t.loc_lo[a] = loc_lo[a]; t.loc_inv_d[a] = loc_inv_d[a];
@@ -555,6 +574,7 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
 namespace {
 
 constexpr int SLAB_MAX_BINS = 8192;   // 64 KB of shared memory for the privatised tally slab
+constexpr int MAX_STAGE_BYTES = 96 * 1024;   // largest hot-table prefix staged in shared memory
 
 int step_of(const mcdc_problem *p, double t) {          // smallest k with C[k] > t, else K-1
   for (int k = 0; k < p->K; ++k)
@@ -681,14 +701,18 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
   // consumers' cursor := producers' cursor (drops whatever an aborted launch may have left behind)
   CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
-  const size_t smem = (size_t)p->K * (sizeof(double) + sizeof(uint32_t)) + 8;
+  const bool staged = p->stage_tables;
+  ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
+  ha.refill_min = p->refill_min;
+  const size_t smem = ha.smem_tables + (size_t)p->K * (sizeof(double) + sizeof(uint32_t)) + 8;
   const int max_grid = p->n_sm * p->blocks_per_sm_hist;
   int grid = (int)std::min<uint64_t>((uint64_t)max_grid, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + TRANSPORT_THREADS - 1) / TRANSPORT_THREADS));
   (void)ev0; (void)ev1;
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
-  k_history<<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
+  if (staged) k_history<true><<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
+  else k_history<false><<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
   p->launches++;
@@ -733,9 +757,20 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
     size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
       p->blocks_per_sm = occ;
-    occ = 1;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_history, TRANSPORT_THREADS, (size_t)p->K * 12 + 8) == cudaSuccess && occ > 0)
-      p->blocks_per_sm_hist = occ;
+    // stage the hot tables in shared memory when that does not cost occupancy beyond the register limit
+    const size_t pop_bytes = (size_t)p->K * 12 + 8;
+    int occ_plain = 1, occ_staged = 0;
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_plain, k_history<false>, TRANSPORT_THREADS, pop_bytes);
+    const size_t staged_bytes = align_up(p->tab.hot_bytes, 16) + pop_bytes;
+    if (staged_bytes <= (size_t)MAX_STAGE_BYTES) {
+      cudaFuncSetAttribute(k_history<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)staged_bytes);
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_staged, k_history<true>, TRANSPORT_THREADS, staged_bytes);
+    }
+    const char *env = getenv("MCDC_STAGE_TABLES");
+    p->stage_tables = occ_staged >= std::max(1, occ_plain) || (occ_staged >= 1 && occ_plain <= 2 && occ_staged * 2 >= occ_plain * 2 - 1);
+    if (env) p->stage_tables = (atoi(env) != 0) && occ_staged >= 1;
+    p->blocks_per_sm_hist = std::max(1, p->stage_tables ? occ_staged : occ_plain);
+    if (const char *e2 = getenv("MCDC_REFILL_MIN")) p->refill_min = std::max(1, std::min(32, atoi(e2)));
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
   CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1)); CK(cudaEventCreate(&ev0)); CK(cudaEventCreate(&ev1));

@@ -92,10 +92,12 @@ __device__ __forceinline__ void tally_add_converged(const TallySink &S, long lon
 // A.7 track-length scoring: 4-D DDA from the pre-move state.  Warp-converged: every lane calls it,
 // lanes without a segment pass active = false.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void score_track(const Tables &T, const TallySink &S, bool active, double x, double y,
+template <class TBT>
+__device__ __forceinline__ void score_track(const TBT &tb, const TallySink &S, bool active, double x, double y,
                                             double z, double ux, double uy, double uz, double t, double w, int g,
                                             double d) {
   const double INF = CUDART_INF;
+  const Tables &T = tb.T;
   const double r[3] = {x, y, z}, o[3] = {ux, uy, uz};
   double inv_o[3];
   double u_in = 0.0, u_out = d, u_cur = 0.0;
@@ -104,7 +106,7 @@ __device__ __forceinline__ void score_track(const Tables &T, const TallySink &S,
   double v = 0.0;
   bool more = active;
   if (more) {
-    v = __ldg(T.speed + g);
+    v = tb.speed(g);
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       const double lo = T.mesh_lo[a], hi = T.mesh_hi[a];
@@ -118,8 +120,8 @@ __device__ __forceinline__ void score_track(const Tables &T, const TallySink &S,
         u_in = fmax(u_in, u0); u_out = fmin(u_out, u1);
       }
     }
-    u_in = fmax(u_in, (__ldg(T.T) - t) * v);
-    u_out = fmin(u_out, (__ldg(T.T + T.Nt) - t) * v);
+    u_in = fmax(u_in, (tb.time_edge(0) - t) * v);
+    u_out = fmin(u_out, (tb.time_edge(T.Nt) - t) * v);
     if (!(u_in < u_out)) more = false;
   }
   if (more) {
@@ -131,12 +133,12 @@ __device__ __forceinline__ void score_track(const Tables &T, const TallySink &S,
         idx[a] = (q < 0.0) ? 0 : ((q > (double)(n - 1)) ? n - 1 : (int)q);
       }
     }
-    const double t_in = t + u_in * __ldg(T.inv_speed + g);
+    const double t_in = t + u_in * tb.inv_speed(g);
     // largest it with T[it] <= t_in (binary search over the edge array)
     int lo = 0, hi = T.Nt - 1;
     while (lo < hi) {
       int mid = (lo + hi + 1) >> 1;
-      if (__ldg(T.T + mid) <= t_in) lo = mid; else hi = mid - 1;
+      if (tb.time_edge(mid) <= t_in) lo = mid; else hi = mid - 1;
     }
     it = lo;
     u_cur = u_in;
@@ -154,7 +156,7 @@ __device__ __forceinline__ void score_track(const Tables &T, const TallySink &S,
         else edge = T.mesh_lo[a] + (double)(idx[a] + (o[a] > 0.0 ? 1 : 0)) * T.mesh_d[a];
         cross[a] = (edge - r[a]) * inv_o[a];
       }
-      const double cross_t = (__ldg(T.T + it + 1) - t) * v;
+      const double cross_t = (tb.time_edge(it + 1) - t) * v;
       double u_next = fmin(fmin(u_out, cross_t), fmin(cross[0], fmin(cross[1], cross[2])));
       bin = ((((long long)it * T.G + g) * T.mesh_n[2] + idx[2]) * T.mesh_n[1] + idx[1]) * T.mesh_n[0] + idx[0];
       val = w * fmax(u_next - u_cur, 0.0);
@@ -214,79 +216,6 @@ __device__ __forceinline__ void block_atomic_add_u64(unsigned long long *dst, un
 }
 
 // ------------------------------------------------------------------------------------------------
-// Source kernel (A.3): one thread per history of the sub-batch; histories whose birth time falls
-// in census step k are appended to the live bank of their batch slot.
-// ------------------------------------------------------------------------------------------------
-struct SourceParams {
-  unsigned long long seed_mixed;       // M(seed + gamma)
-  unsigned long long first_history;    // global id of local history 0 of this sub-batch
-  uint32_t n_hist;                     // histories in this sub-batch
-  uint32_t hb;                         // histories per slot
-  uint32_t cap;
-  int k;                               // census step being fed
-  int single_step;                     // all sources are born in step k (skip the time filter)
-};
-
-__global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank out, DevCounters *cnt) {
-  __shared__ double scratch[32];
-  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-  bool live = i < P.n_hist;
-  double x = 0, y = 0, z = 0, ux = 0, uy = 0, uz = 1, t = 0;
-  double xi_x = 0, xi_y = 0, xi_z = 0, xi_t = 0;
-  int g = 0, cell = -1;
-  uint32_t ctr = 0;
-  unsigned long long key = 0;
-  if (live) {
-    key = mix64(P.seed_mixed ^ (P.first_history + i));
-    draw2(key, ctr, xi_x, xi_y);
-    draw2(key, ctr, xi_z, xi_t);
-    t = T.src_t0 + xi_t * (T.src_t1 - T.src_t0);
-    if (!P.single_step) {
-      int k0 = T.K - 1;                  // smallest k with C[k] > t (last step when none, D15)
-      for (int k = 0; k < T.K; ++k)
-        if (__ldg(T.census + k) > t) { k0 = k; break; }
-      if (k0 != P.k) live = false;
-    }
-  }
-  if (live) {
-    double xi_g = draw(key, ctr);
-    x = T.src_lo[0] + xi_x * (T.src_hi[0] - T.src_lo[0]);
-    y = T.src_lo[1] + xi_y * (T.src_hi[1] - T.src_lo[1]);
-    z = T.src_lo[2] + xi_z * (T.src_hi[2] - T.src_lo[2]);
-    g = sample_cdf(T.src_cdf, T.G, T.src_last, xi_g);
-    if (T.src_dir_mode == 0) {
-      double xi_mu, xi_phi;
-      draw2(key, ctr, xi_mu, xi_phi);
-      isotropic(xi_mu, xi_phi, ux, uy, uz);
-    } else {
-      ux = T.src_dir[0]; uy = T.src_dir[1]; uz = T.src_dir[2];
-    }
-    cell = locate_source(T, x, y, z, ux, uy, uz);
-  }
-  const bool lost = live && cell < 0;
-  const bool keep = live && cell >= 0;
-  const int slot = keep ? (int)(i / P.hb) : -1;
-  uint32_t idx = warp_append_by_slot(out.count, slot);
-  if (keep) {
-    if (idx >= P.cap) {
-      atomicExch(&cnt->overflow, 1);
-    } else {
-      size_t j = (size_t)slot * P.cap + idx;
-      out.x[j] = x; out.y[j] = y; out.z[j] = z;
-      out.ux[j] = ux; out.uy[j] = uy; out.uz[j] = uz;
-      out.t[j] = t; out.w[j] = 1.0;
-      out.key[j] = key;
-      out.meta[j] = make_int4(cell, -1, (int)ctr, g);
-      out.hid[j] = i;
-    }
-  }
-  block_atomic_add(&cnt->ledger[0], live ? 1.0 : 0.0, scratch);
-  block_atomic_add(&cnt->ledger[6], lost ? 1.0 : 0.0, scratch);
-  block_atomic_add_u64(&cnt->n[0], live ? 1ull : 0ull, (unsigned long long *)scratch);
-  block_atomic_add_u64(&cnt->n[6], lost ? 1ull : 0ull, (unsigned long long *)scratch);
-}
-
-// ------------------------------------------------------------------------------------------------
 // per-thread accumulators in shared memory (no atomics: one column per thread), flushed once per block
 // ------------------------------------------------------------------------------------------------
 struct BlockAccum {
@@ -332,9 +261,61 @@ __device__ __forceinline__ void record_particle(BlockAccum &B, uint32_t *ev, uin
 }
 
 // ------------------------------------------------------------------------------------------------
+// Source kernel of the census-stepped scheduler (A.3): one thread per history of the sub-batch; histories
+// whose birth time falls in census step k are appended to the live bank of their batch slot.
+// ------------------------------------------------------------------------------------------------
+struct SourceParams {
+  unsigned long long seed_mixed;       // M(seed + gamma)
+  unsigned long long first_history;    // global id of local history 0 of this sub-batch
+  uint32_t n_hist;                     // histories in this sub-batch
+  uint32_t hb;                         // histories per slot
+  uint32_t cap;
+  int k;                               // census step being fed
+  int single_step;                     // all sources are born in step k (skip the time filter)
+};
+
+__global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank out, DevCounters *cnt) {
+  __shared__ double scratch[32];
+  const TB<false> tb(T);
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  bool live = i < P.n_hist;
+  PState p;
+  p.x = p.y = p.z = p.ux = p.uy = p.t = 0.0; p.uz = 1.0; p.w = 1.0;
+  p.key = 0; p.ctr = 0; p.hid = i; p.g = 0; p.cell = -1; p.last_surf = -1;
+  if (live) {
+    source_position(T, P.seed_mixed, P.first_history + i, p);
+    if (!P.single_step && census_index(tb, p.t) != P.k) live = false;
+  }
+  bool ok = false;
+  if (live) ok = flight_init(tb, p, FI_SOURCE);
+  const bool lost = live && !ok;
+  const bool keep = live && ok;
+  const int slot = keep ? (int)(i / P.hb) : -1;
+  uint32_t idx = warp_append_by_slot(out.count, slot);
+  if (keep) {
+    if (idx >= P.cap) {
+      atomicExch(&cnt->overflow, 1);
+    } else {
+      size_t j = (size_t)slot * P.cap + idx;
+      out.x[j] = p.x; out.y[j] = p.y; out.z[j] = p.z;
+      out.ux[j] = p.ux; out.uy[j] = p.uy; out.uz[j] = p.uz;
+      out.t[j] = p.t; out.w[j] = p.w;
+      out.key[j] = p.key;
+      out.meta[j] = make_int4(p.cell, -1, (int)p.ctr, p.g);
+      out.hid[j] = i;
+    }
+  }
+  block_atomic_add(&cnt->ledger[0], live ? 1.0 : 0.0, scratch);
+  block_atomic_add(&cnt->ledger[6], lost ? 1.0 : 0.0, scratch);
+  block_atomic_add_u64(&cnt->n[0], live ? 1ull : 0ull, (unsigned long long *)scratch);
+  block_atomic_add_u64(&cnt->n[6], lost ? 1ull : 0ull, (unsigned long long *)scratch);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Census-stepped transport kernel: one census step (or one fission generation inside it) for every slot.
 // Particles that reach the census time are parked in the census bank (A.8); fission children go to the
-// fission bank and are transported by the next launch of the same step.
+// fission bank and are transported by the next launch of the same step.  Dynamic shared memory = the
+// step's tally slab (tables are read from the global blob here).
 // ------------------------------------------------------------------------------------------------
 struct TransportArgs {
   Bank in, census_out, sec_out;
@@ -346,9 +327,10 @@ struct TransportArgs {
 };
 
 __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepParams P, TransportArgs A) {
-  extern __shared__ double slab[];                       // [P.slab_bins]
+  double *slab = reinterpret_cast<double *>(g_smem);     // [P.slab_bins]
   __shared__ BlockAccum acc;
   __shared__ int s_flag;
+  const TB<false> tb(T);
   const int tid = threadIdx.x, lane = tid & 31;
   accum_zero(acc);
   double popw = 0.0;
@@ -374,6 +356,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
     const size_t base_in = (size_t)slot * P.cap;
 
     bool have = false, exhausted = false;
+    int fi = FI_NONE;
     PState p;
     p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
     p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
@@ -396,10 +379,11 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
             p.key = A.in.key[j]; p.hid = A.in.hid[j];
             int4 m = A.in.meta[j];
             p.cell = m.x;
-            if (P.in_is_birth) init_child(T, p);
+            if (P.in_is_birth) { p.ctr = 0u; fi = FI_CHILD; }
             else {
               p.ux = A.in.ux[j]; p.uy = A.in.uy[j]; p.uz = A.in.uz[j];
               p.last_surf = m.y; p.ctr = (uint32_t)m.z; p.g = m.w;
+              fi = FI_NONE;
             }
             pc_coll = pc_surf = pc_child = 0u;
             have = true;
@@ -407,17 +391,18 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
         }
       }
       if (__ballot_sync(MCDC_FULL, have) == 0u) break;
+      if (have && fi != FI_NONE) { flight_init(tb, p, fi); fi = FI_NONE; }
 
       double d = 0.0;
       int ev = -1, i_star = -1;
-      if (have) ev = find_event(T, p, P.t_census, d, i_star);
-      score_track(T, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
+      if (have) ev = find_event(tb, p, P.t_census, d, i_star);
+      score_track(tb, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
       bool to_census = false;
       int n_children = 0;
       uint32_t c0 = 0u, pc_census = 0u;
       if (have) {
         p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
-        p.t = (ev == EV_CENSUS) ? P.t_census : p.t + d * __ldg(T.inv_speed + p.g);
+        p.t = (ev == EV_CENSUS) ? P.t_census : p.t + d * tb.inv_speed(p.g);
         if (ev == EV_CENSUS) {                           // A.8
           pc_census = 1u;
           popw += p.w; popn += 1u;
@@ -426,12 +411,12 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
           have = false;
         } else if (ev == EV_SURFACE) {
           pc_surf += 1u;
-          have = surface_event(T, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
+          have = surface_event(tb, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
         } else {
           pc_coll += 1u;
-          int r = collision_event(T, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
+          int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
                                   &acc.led[LED_PRODUCTION][tid]);
-          if (r != -1) have = false;
+          if (r == -1) fi = FI_SCATTER; else have = false;
           if (r > 0) { n_children = r; pc_child += (uint32_t)r; }
         }
       }
@@ -491,12 +476,17 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
 }
 
 // ------------------------------------------------------------------------------------------------
-// Asynchronous history kernel: ONE launch per sub-batch.  Idle lanes take work from (1) the in-kernel
-// fission queue (children first, so lineages finish promptly) and (2) the source-history cursor, building the
-// source particle directly in registers.  A particle keeps its registers across census boundaries: the
-// census event only does the population bookkeeping (A.8) and moves on to the next census interval -- in
-// analog transport nothing has to wait there, so no census barrier is needed.
-// A fission parent turns into its first child in place; the other children are pushed to the queue.
+// Asynchronous history kernel: ONE launch per sub-batch.
+//  * Idle lanes take work from (1) the in-kernel fission queue (children first, so lineages finish promptly)
+//    and (2) the source-history cursor, building the source particle directly in registers.  Refills are
+//    batched: the acquire phase runs only when REFILL_MIN lanes of the warp are idle (or none is busy).
+//  * Every lane that starts a flight -- new source, new child, or a particle that just scattered -- samples
+//    its group and direction in one shared phase (flight_init) instead of three divergent code paths.
+//  * A particle keeps its registers across census boundaries: the census event only does the population
+//    bookkeeping (A.8) and moves on to the next census interval; in analog transport nothing has to wait
+//    there, so there is no census barrier.
+//  * A fission parent turns into its first child in place; the other children are published to the queue.
+//  * Tables are read from their shared-memory copy when STAGED.
 // ------------------------------------------------------------------------------------------------
 struct FissionQueue {             // ring buffer in HBM, structure of arrays, capacity mask+1 (power of two)
   double *x, *y, *z, *t, *w;
@@ -518,6 +508,8 @@ struct HistoryArgs {
   unsigned long long *pop_n;
   uint32_t *ev;
   int aggregate;
+  int refill_min;                 // idle lanes per warp that trigger a refill
+  uint32_t smem_tables;           // bytes of dynamic shared memory in front of the census arrays
 };
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
@@ -534,13 +526,15 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
   return v;
 }
 
+template <bool STAGED>
 __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, HistoryArgs A) {
-  extern __shared__ double s_dyn[];                      // pop_w[K] then pop_n[K] (u32)
   __shared__ BlockAccum acc;
+  const TB<STAGED> tb(T);
   const int tid = threadIdx.x, lane = tid & 31;
   const unsigned lt_mask = (1u << lane) - 1u;
-  double *s_popw = s_dyn;
-  uint32_t *s_popn = (uint32_t *)(s_dyn + T.K);
+  double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables);
+  uint32_t *s_popn = reinterpret_cast<uint32_t *>(s_popw + T.K);
+  if (STAGED) stage_tables(T);
   for (int k = tid; k < T.K; k += TRANSPORT_THREADS) { s_popw[k] = 0.0; s_popn[k] = 0u; }
   accum_zero(acc);
   __syncthreads();
@@ -548,6 +542,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
   const unsigned long long q_cap = (unsigned long long)A.q.mask + 1ull;
 
   bool have = false, src_done = false;
+  int fi = FI_NONE;
   PState p;
   p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
   p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
@@ -556,9 +551,9 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
   uint32_t pc_coll = 0, pc_surf = 0, pc_child = 0, pc_census = 0, n_src = 0, n_src_lost = 0;
 
   for (;;) {
-    // ---------------- acquire work for idle lanes ----------------
-    unsigned need = __ballot_sync(MCDC_FULL, !have);
-    if (need != 0u) {
+    // ---------------- phase A: acquire work for idle lanes (batched) ----------------
+    const unsigned need = __ballot_sync(MCDC_FULL, !have);
+    if (__popc(need) >= A.refill_min || need == MCDC_FULL) {
       // (1) fission queue
       uint32_t got = 0u;
       unsigned long long qbase = 0ull;
@@ -587,17 +582,18 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
           }
         }
         if (ready) {
-        p.x = A.q.x[j]; p.y = A.q.y[j]; p.z = A.q.z[j]; p.t = A.q.t[j]; p.w = A.q.w[j];
-        p.key = A.q.key[j];
-        const int4 m = A.q.meta[j];
-        p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z;
-        slot = p.hid / A.hb;
-        init_child(T, p);
-        have = true;
+          p.x = A.q.x[j]; p.y = A.q.y[j]; p.z = A.q.z[j]; p.t = A.q.t[j]; p.w = A.q.w[j];
+          p.key = A.q.key[j];
+          const int4 m = A.q.meta[j];
+          p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z;
+          p.ctr = 0u;
+          slot = p.hid / A.hb;
+          fi = FI_CHILD;
+          have = true;
         }
       }
       // (2) source histories
-      unsigned need2 = __ballot_sync(MCDC_FULL, !have);
+      const unsigned need2 = __ballot_sync(MCDC_FULL, !have);
       if (need2 != 0u && !src_done) {
         const int leader = __ffs(need2) - 1;
         uint32_t base = 0u;
@@ -610,11 +606,10 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
             n_src += 1u;
             p.hid = i;
             slot = i / A.hb;
-            const bool ok = source_particle(T, A.seed_mixed, A.first_history + i, p);
-            pk = T.K - 1;
-            for (int k = 0; k < T.K; ++k)
-              if (__ldg(T.census + k) > p.t) { pk = k; break; }
-            if (ok) have = true; else n_src_lost += 1u;
+            source_position(T, A.seed_mixed, A.first_history + i, p);
+            pk = census_index(tb, p.t);
+            fi = FI_SOURCE;
+            have = true;
           }
         }
       }
@@ -628,23 +623,31 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
       continue;
     }
 
-    // ---------------- one segment ----------------
+    // ---------------- phase B: group / direction / cell of every flight that starts now ----------------
+    if (have && fi != FI_NONE) {
+      const bool ok = flight_init(tb, p, fi);
+      fi = FI_NONE;
+      if (!ok) { n_src_lost += 1u; have = false; }       // a source particle outside every cell (A.3)
+    }
+
+    // ---------------- phase C/D: one segment: distances, score, move ----------------
     double d = 0.0;
     int ev = -1, i_star = -1;
-    const double t_census = have ? __ldg(T.census + pk) : 0.0;
-    if (have) ev = find_event(T, p, t_census, d, i_star);
+    const double t_census = have ? tb.census(pk) : 0.0;
+    if (have) ev = find_event(tb, p, t_census, d, i_star);
     {
       TallySink S;
       S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
       S.aggregate = A.aggregate;
-      score_track(T, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
+      score_track(tb, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
     }
+    // ---------------- phase E: the event ----------------
     int n_push = 0, census_k = -1;
     uint32_t c0 = 0u;
     bool ended = false;                                  // the particle (as an identity) ended in this iteration
     if (have) {
       p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
-      p.t = (ev == EV_CENSUS) ? t_census : p.t + d * __ldg(T.inv_speed + p.g);
+      p.t = (ev == EV_CENSUS) ? t_census : p.t + d * tb.inv_speed(p.g);
       if (ev == EV_CENSUS) {                             // A.8: bookkeeping only, then the next interval
         pc_census += 1u;
         census_k = pk;
@@ -653,15 +656,18 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
         else pk += 1;
       } else if (ev == EV_SURFACE) {
         pc_surf += 1u;
-        have = surface_event(T, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
+        have = surface_event(tb, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
         ended = !have;
       } else {
         pc_coll += 1u;
-        const int r = collision_event(T, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
+        const int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
                                       &acc.led[LED_PRODUCTION][tid]);
-        if (r != -1) { ended = true; have = false; }
-        if (r > 0) { pc_child += (uint32_t)r; n_push = r - 1; }
-        if (r > 0) have = true;                          // continues below as child 0
+        if (r == -1) fi = FI_SCATTER;
+        else {
+          ended = true;
+          have = r > 0;                                  // continues below as its first child
+          if (r > 0) { pc_child += (uint32_t)r; n_push = r - 1; }
+        }
       }
     }
     // ---------------- census population (A.8), merged inside the warp ----------------
@@ -673,38 +679,35 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
         atomicAdd(s_popn + census_k, 1u);
       }
     }
-    // ---------------- fission: push children 1..n-1, become child 0 (A.6) ----------------
-    {
-      unsigned fis = __ballot_sync(MCDC_FULL, n_push > 0);
-      if (fis != 0u) {
-        int pre = n_push;
+    // ---------------- fission: publish children 1..n-1, become child 0 (A.6) ----------------
+    if (__ballot_sync(MCDC_FULL, n_push > 0) != 0u) {
+      int pre = n_push;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-          int v = __shfl_up_sync(MCDC_FULL, pre, o);
-          if (lane >= o) pre += v;
+      for (int o = 1; o < 32; o <<= 1) {
+        int v = __shfl_up_sync(MCDC_FULL, pre, o);
+        if (lane >= o) pre += v;
+      }
+      const int total = __shfl_sync(MCDC_FULL, pre, 31);
+      unsigned long long base = 0ull;
+      int ok = 1;
+      if (lane == 0) {
+        base = atomicAdd(q_tail, (unsigned long long)total);
+        if (base + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) ok = 0;
+      }
+      base = __shfl_sync(MCDC_FULL, base, 0) + (unsigned long long)(pre - n_push);
+      ok = __shfl_sync(MCDC_FULL, ok, 0);
+      if (!ok && lane == 0) atomicExch(&A.cnt->overflow, 1);
+      if (n_push > 0 && ok) {
+        for (int c = 0; c < n_push; ++c) {
+          const uint32_t j = (uint32_t)(base + (unsigned long long)c) & A.q.mask;
+          A.q.x[j] = p.x; A.q.y[j] = p.y; A.q.z[j] = p.z; A.q.t[j] = p.t; A.q.w[j] = p.w;
+          A.q.key[j] = child_key(p.key, c0, (uint32_t)(c + 1));
+          A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, 0);
         }
-        const int total = __shfl_sync(MCDC_FULL, pre, 31);
-        unsigned long long base = 0ull;
-        int ok = 1;
-        if (lane == 0) {
-          base = atomicAdd(q_tail, (unsigned long long)total);
-          if (base + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) ok = 0;
-        }
-        base = __shfl_sync(MCDC_FULL, base, 0) + (unsigned long long)(pre - n_push);
-        ok = __shfl_sync(MCDC_FULL, ok, 0);
-        if (!ok) { if (lane == 0) atomicExch(&A.cnt->overflow, 1); }
-        if (n_push > 0 && ok) {
-          for (int c = 0; c < n_push; ++c) {
-            const uint32_t j = (uint32_t)(base + (unsigned long long)c) & A.q.mask;
-            A.q.x[j] = p.x; A.q.y[j] = p.y; A.q.z[j] = p.z; A.q.t[j] = p.t; A.q.w[j] = p.w;
-            A.q.key[j] = child_key(p.key, c0, (uint32_t)(c + 1));
-            A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, 0);
-          }
-          __threadfence();
-          for (int c = 0; c < n_push; ++c) {
-            const unsigned long long i = base + (unsigned long long)c;
-            st_release_u32(A.q.flag + ((uint32_t)i & A.q.mask), (uint32_t)(i + 1ull));
-          }
+        __threadfence();
+        for (int c = 0; c < n_push; ++c) {
+          const unsigned long long i = base + (unsigned long long)c;
+          st_release_u32(A.q.flag + ((uint32_t)i & A.q.mask), (uint32_t)(i + 1ull));
         }
       }
     }
@@ -713,7 +716,8 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
       pc_census = 0u;
       if (have) {                                        // fission parent -> its first child, in place
         p.key = child_key(p.key, c0, 0u);
-        init_child(T, p);
+        p.ctr = 0u;
+        fi = FI_CHILD;
       }
     }
   }

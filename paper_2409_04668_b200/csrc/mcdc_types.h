@@ -29,42 +29,44 @@ struct Bank {
   uint32_t *cursor;  // [n_slots] consumption cursor (transport kernel refill)
 };
 
-// Device-resident problem tables (all pointers are device memory owned by the handle).
+// Device-resident problem tables.  Every array lives in ONE contiguous blob (16-byte aligned pieces); the
+// struct holds byte offsets into it, so that a kernel can address the same tables either in global memory
+// (blob) or in its shared-memory copy of the blob's hot prefix (first hot_bytes bytes).
 struct Tables {
   int G, M, S, C, K, Nt;
+  const unsigned char *blob;   // global copy of the blob
+  uint32_t hot_bytes;          // prefix a kernel may stage in shared memory (everything the hot loop reads)
   // cross sections, index mg = m * G + g
-  const double *sig_t, *inv_sig_t, *sig_s_tot, *sig_sc /* Sigma_s_tot + Sigma_c */, *sig_f, *nu;
-  const double *cdf_s;     // [M*G][G] running sums of Sigma_s[m][g][.] in increasing g'
-  const int *last_s;       // [M*G] last g' with a non-zero entry (fallback of the CDF scan)
-  const double *cdf_chi;   // [M][G] running sums of chi
-  const int *last_chi;     // [M]
-  const double *speed, *inv_speed;   // [G]
+  uint32_t o_sig_t, o_inv_sig_t, o_sig_s_tot, o_sig_sc /* Sigma_s_tot + Sigma_c */, o_sig_f, o_nu;
+  uint32_t o_cdf_s;     // [M*G][G] running sums of Sigma_s[m][g][.] in increasing g'
+  uint32_t o_last_s;    // [M*G] last g' with a non-zero entry (fallback of the CDF scan)
+  uint32_t o_cdf_chi;   // [M][G] running sums of chi
+  uint32_t o_last_chi;  // [M]
+  uint32_t o_speed, o_inv_speed;   // [G]
+  uint32_t o_T;         // [Nt+1]
+  uint32_t o_census;    // [K]
+  uint32_t o_src_cdf;   // [G]
   // geometry
-  const double *surf_coef; // [S][10] general form
-  const double4 *surf_q;   // [S] typed parameters
-  const int *surf_type;    // [S]
-  const int *surf_bc;      // [S]
-  const int *cell_off;     // [C+1]
-  const int *hs;           // packed half-space: surface << 4 | type << 1 | (sense > 0)
-  const int *cell_mat;     // [C]
-  const int *nb_off;       // [nhs+1] neighbour candidates of half-space slot i (cells across that surface)
-  const int *nb_cell;
+  uint32_t o_surf_q;    // [S] double4 typed parameters
+  uint32_t o_surf_bc;   // [S]
+  uint32_t o_cell_off;  // [C+1]
+  uint32_t o_hs;        // packed half-space: surface << 4 | type << 1 | (sense > 0)
+  uint32_t o_cell_mat;  // [C]
+  uint32_t o_nb_off;    // [nhs+1] neighbour candidates of half-space slot i (cells across that surface)
+  uint32_t o_nb_cell;
+  uint32_t o_loc_off;   // [nvox+1] source locator grid
+  uint32_t o_loc_cell;
+  uint32_t o_surf_coef; // [S][10] general form (inside the hot prefix only when a general quadric exists)
   // source
   double src_lo[3], src_hi[3], src_t0, src_t1;
-  const double *src_cdf;   // [G]
   int src_last;
   int src_dir_mode;
   double src_dir[3];
-  // source locator grid over the source box
   int loc_n[3];
   double loc_lo[3], loc_inv_d[3];
-  const int *loc_off;      // [nvox+1]
-  const int *loc_cell;
   // tally mesh
   double mesh_lo[3], mesh_hi[3], mesh_d[3], mesh_inv_d[3];
   int mesh_n[3];
-  const double *T;         // [Nt+1]
-  const double *census;    // [K]
   unsigned long long n_bins;
 };
 
