@@ -25,6 +25,12 @@ struct TB {
     if (STAGED) return reinterpret_cast<const V *>(g_smem + off)[i];
     return reinterpret_cast<const V *>(T.blob + off)[i];
   }
+  // load at an absolute byte offset of the blob
+  template <class V>
+  __device__ __forceinline__ V ldb(uint32_t byte_off) const {
+    if (STAGED) return *reinterpret_cast<const V *>(g_smem + byte_off);
+    return *reinterpret_cast<const V *>(T.blob + byte_off);
+  }
   __device__ __forceinline__ double sig_t(int mg) const { return ld<double>(T.o_sig_t, mg); }
   __device__ __forceinline__ double inv_sig_t(int mg) const { return ld<double>(T.o_inv_sig_t, mg); }
   __device__ __forceinline__ double sig_s_tot(int mg) const { return ld<double>(T.o_sig_s_tot, mg); }
@@ -87,8 +93,9 @@ __device__ __noinline__ ulonglong2 philox_block(unsigned long long key, uint32_t
   uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
 #pragma unroll
   for (int r = 0; r < 10; ++r) {
-    uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-    uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE.U32 each
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
     uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
     c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
     k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
@@ -261,20 +268,26 @@ __device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed,
                                               double ux, double uy, double uz) {
   const int e = tb.cell_off(c + 1);
   for (int i = tb.cell_off(c); i < e; ++i) {
-    const int h = tb.hs(i);                             // packed: surface << 4 | type << 1 | (sense > 0)
-    const int s = h >> 4, want = (h & 1) ? 1 : -1;
+    const int h = tb.hs(i);                             // packed: surface << 6 | bc << 4 | type << 1 | (sense > 0)
+    const int s = h >> 6, want = (h & 1) ? 1 : -1;
     if (surf_sense(tb, s, (h >> 1) & 7, s == crossed, x, y, z, ux, uy, uz) != want) return false;
   }
   return true;
 }
 
-// full search in increasing cell id (A.3); slow path
-template <class TBT>
-__device__ __noinline__ int locate_all(const TBT &tb, int crossed, double x, double y, double z, double ux, double uy,
-                                       double uz) {
-  for (int c = 0; c < tb.T.C; ++c)
+// full search in increasing cell id (A.3); slow path.  Not inlined, and it works on the device-memory copy of
+// the tables so that no caller has to take the address of its kernel parameter block.
+__device__ __noinline__ int locate_all_dev(const Tables *gT, int crossed, double x, double y, double z, double ux,
+                                           double uy, double uz) {
+  const TB<false> tb(*gT);
+  for (int c = 0; c < gT->C; ++c)
     if (cell_contains(tb, c, crossed, x, y, z, ux, uy, uz)) return c;
   return -1;
+}
+template <class TBT>
+__device__ __forceinline__ int locate_all(const TBT &tb, int crossed, double x, double y, double z, double ux, double uy,
+                                          double uz) {
+  return locate_all_dev(tb.T.self_dev, crossed, x, y, z, ux, uy, uz);
 }
 
 // cell after crossing the surface of half-space slot `slot` of the current cell (A.5, transmission)

@@ -12,7 +12,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/mcdc.h"
-#include "mcdc_kernels.cuh"
+#include "mcdc_pool.cuh"
 
 using namespace mcdc;
 
@@ -95,6 +95,9 @@ struct mcdc_problem {
   double ms_run = 0.0, ms_transport = 0.0;
   int n_sm = 148, blocks_per_sm = 1, blocks_per_sm_hist = 1;
   bool stage_tables = false;
+  int hist_threads = 512;
+  uint32_t pool_slots = 0;
+  size_t pool_smem = 0;
   int refill_min = 8;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
   std::string cuda_err;
@@ -224,7 +227,7 @@ void classify_surface(const double *c, int &type, double4 &q) {
   type = ST_QUADRIC;
 }
 
-Box cell_box(const mcdc_problem &P, const std::vector<int> &type, const std::vector<double4> &q, int c) {
+Box cell_box(const mcdc_problem &P, const std::vector<int> &type, const std::vector<double4> &q, int c, bool pad = true) {
   Box b;
   for (int a = 0; a < 3; ++a) { b.lo[a] = -HINF; b.hi[a] = HINF; }
   for (int i = P.cell_off[c]; i < P.cell_off[c + 1]; ++i) {
@@ -239,7 +242,7 @@ Box cell_box(const mcdc_problem &P, const std::vector<int> &type, const std::vec
       b.lo[1] = std::max(b.lo[1], q[s].y - r); b.hi[1] = std::min(b.hi[1], q[s].y + r);
     }
   }
-  for (int a = 0; a < 3; ++a) {                            // pad: a point within rounding of a face stays inside
+  for (int a = 0; a < 3 && pad; ++a) {                     // pad: a point within rounding of a face stays inside
     double ref = 1.0 + (std::isfinite(b.lo[a]) ? std::fabs(b.lo[a]) : 0.0) + (std::isfinite(b.hi[a]) ? std::fabs(b.hi[a]) : 0.0);
     b.lo[a] -= 1e-6 * ref; b.hi[a] += 1e-6 * ref;
   }
@@ -327,7 +330,8 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   std::vector<double4> q(S);
   for (int s = 0; s < S; ++s) classify_surface(&p->surf_coef[(size_t)10 * s], type[s], q[s]);
   std::vector<int> hs(nhs);
-  for (int i = 0; i < nhs; ++i) hs[i] = (p->hs_surface[i] << 4) | (type[p->hs_surface[i]] << 1) | (p->hs_sense[i] > 0 ? 1 : 0);
+  for (int i = 0; i < nhs; ++i)
+    hs[i] = (p->hs_surface[i] << 6) | (p->surf_bc[p->hs_surface[i]] << 4) | (type[p->hs_surface[i]] << 1) | (p->hs_sense[i] > 0 ? 1 : 0);
   std::vector<Box> box(C);
   for (int c = 0; c < C; ++c) box[c] = cell_box(*p, type, q, c);
   // cells listing half-space (s, sense): index 2*s + (sense>0)
@@ -343,6 +347,68 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
         if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);  // increasing id by construction
       nb_off[i + 1] = (int)nb_cell.size();
     }
+  // ---- typed cell records (mcdc_types.h): tightest axis-aligned plane per (axis, side) = face, the rest = other ----
+  std::vector<unsigned char> cell_rec((size_t)C * CELL_REC_BYTES, 0);
+  std::vector<int> other_list;
+  for (int c = 0; c < C; ++c) {
+    double bound[6];
+    int face[6];
+    for (int a = 0; a < 3; ++a) { bound[2 * a] = -HINF; bound[2 * a + 1] = HINF; face[2 * a] = face[2 * a + 1] = -1; }
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
+      const int s = p->hs_surface[i];
+      if (type[s] > ST_PLANE_Z) continue;
+      const int a = type[s] - ST_PLANE_X;
+      const bool below = (q[s].y > 0.0) == (p->hs_sense[i] < 0);          // coordinate < position
+      const int f = 2 * a + (below ? 1 : 0);
+      const bool tighter = below ? (q[s].x < bound[f]) : (q[s].x > bound[f]);
+      if (tighter) { bound[f] = q[s].x; face[f] = i; }                    // equal positions: the earlier slot stays
+    }
+    std::vector<int> others;
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
+      bool is_face = false;
+      for (int f = 0; f < 6; ++f) is_face = is_face || face[f] == i;
+      if (!is_face) others.push_back(i);
+    }
+    unsigned char *r = cell_rec.data() + (size_t)c * CELL_REC_BYTES;
+    std::memcpy(r + CR_BOUND, bound, sizeof(bound));
+    std::memcpy(r + CR_FACE, face, sizeof(face));
+    const int n_other = (int)others.size(), other_off = (int)other_list.size();
+    const int o01[2] = {n_other > 0 ? others[0] : -1, n_other > 1 ? others[1] : -1};
+    std::memcpy(r + CR_N_OTHER, &n_other, 4); std::memcpy(r + CR_OTHER_OFF, &other_off, 4);
+    std::memcpy(r + CR_OTHER0, o01, 8); std::memcpy(r + CR_MAT, &p->cell_mat[c], 4);
+    other_list.insert(other_list.end(), others.begin(), others.end());
+  }
+  // candidate neighbours: the one sharing the largest part of the face first (cells do not overlap, so the order
+  // of the tests cannot change which cell contains the point -- DESIGN.md section 2)
+  {
+    std::vector<Box> ubox(C);
+    for (int c = 0; c < C; ++c) ubox[c] = cell_box(*p, type, q, c, false);
+    auto overlap = [&](int c1, int c2) {
+      double m = 1.0;
+      int finite = 0;
+      for (int a = 0; a < 3; ++a) {
+        const double lo = std::max(ubox[c1].lo[a], ubox[c2].lo[a]), hi = std::min(ubox[c1].hi[a], ubox[c2].hi[a]);
+        if (!std::isfinite(lo) || !std::isfinite(hi)) continue;
+        const double w = hi - lo;
+        if (w > 1e-9 * (1.0 + std::fabs(lo) + std::fabs(hi))) { m *= w; finite++; }   // skip the shared (zero-width) axis
+        else if (w < -1e-9 * (1.0 + std::fabs(lo) + std::fabs(hi))) return -1.0;
+      }
+      return finite ? m : 0.0;
+    };
+    for (int c = 0; c < C; ++c)
+      for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i)
+        std::stable_sort(nb_cell.begin() + nb_off[i], nb_cell.begin() + nb_off[i + 1],
+                         [&](int x, int y) { return overlap(c, x) > overlap(c, y); });
+  }
+  // the tally mesh covers the geometry and the time grid covers the run: the score needs no clipping
+  int score_fast = 1;
+  for (int c = 0; c < C && score_fast; ++c) {
+    const Box b = cell_box(*p, type, q, c, false);
+    for (int a = 0; a < 3; ++a)
+      if (!(p->mesh_lo[a] <= b.lo[a]) || !(p->mesh_hi[a] >= b.hi[a])) score_fast = 0;
+  }
+  if (!(p->T[0] <= p->src_t0) || !(p->T[p->Nt] >= p->census[p->K - 1])) score_fast = 0;
+
   // ---- source locator grid ----
   int loc_n[3];
   double loc_lo[3], loc_inv_d[3];
@@ -396,7 +462,10 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   t.o_T = putd(p->T); t.o_census = putd(p->census); t.o_src_cdf = putd(src_cdf);
   t.o_surf_q = put(q.data(), q.size() * sizeof(double4));
   t.o_surf_bc = puti(p->surf_bc); t.o_cell_off = puti(p->cell_off); t.o_hs = puti(hs); t.o_cell_mat = puti(p->cell_mat);
-  t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell); t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
+  t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell);
+  t.o_cell_rec = put(cell_rec.data(), cell_rec.size()); t.o_other = puti(other_list);
+  t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
+  t.score_fast = score_fast;
   bool any_quadric = false;
   for (int s = 0; s < S; ++s) any_quadric = any_quadric || type[s] == ST_QUADRIC;
   size_t hot = (blob.size() + 15) / 16 * 16;
@@ -415,6 +484,11 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
     t.mesh_inv_d[a] = (p->mesh_n[a] > 1) ? 1.0 / t.mesh_d[a] : 0.0;
   }
   t.n_bins = p->n_bins;
+  {
+    Tables *dT = ar.zeros<Tables>(1);
+    t.self_dev = dT;
+    if (dT && cudaMemcpy(dT, &t, sizeof(Tables), cudaMemcpyHostToDevice) != cudaSuccess) ar.err = cudaErrorUnknown;
+  }
   p->d_sum = ar.zeros<double>(p->n_bins); p->d_sumsq = ar.zeros<double>(p->n_bins);
   p->d_pop_w = ar.zeros<double>(p->K); p->d_pop_n = ar.zeros<unsigned long long>(p->K);
   p->d_cnt = ar.zeros<DevCounters>(1);
@@ -459,8 +533,7 @@ extern "C" int mcdc_problem_reset(mcdc_problem *p) {
 // =============================================================================================
 namespace {
 
-constexpr size_t FULL_BYTES = 8 * 8 + 8 + 16 + 4;    // x y z ux uy uz t w, key, meta, hid = 92
-constexpr size_t BIRTH_BYTES = 5 * 8 + 8 + 16 + 4;   // x y z t w, key, meta, hid         = 68 (meta kept whole)
+// bank records: full = x y z ux uy uz t w, key, meta, hid = 92 B; birth = x y z t w, key, meta, hid = 68 B
 
 struct WsLayout {
   size_t total = 0;
@@ -574,7 +647,6 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
 namespace {
 
 constexpr int SLAB_MAX_BINS = 8192;   // 64 KB of shared memory for the privatised tally slab
-constexpr int MAX_STAGE_BYTES = 96 * 1024;   // largest hot-table prefix staged in shared memory
 
 int step_of(const mcdc_problem *p, double t) {          // smallest k with C[k] > t, else K-1
   for (int k = 0; k < p->K; ++k)
@@ -686,6 +758,34 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   return MCDC_OK;
 }
 
+// ---- k_pool instantiations: (tables staged, fast score, threads per block) ----
+#define MCDC_POOL_CASES(X) X(256) X(512) X(768) X(1024)
+template <bool STAGED, bool FAST>
+void pool_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  switch (nt) {
+#define X(N) case N: k_pool<STAGED, FAST, N><<<grid, N, smem, st>>>(T, A); break;
+    MCDC_POOL_CASES(X)
+#undef X
+  }
+}
+template <bool STAGED, bool FAST>
+cudaError_t pool_set_smem_nt(int nt, int bytes) {
+  switch (nt) {
+#define X(N) case N: return cudaFuncSetAttribute(k_pool<STAGED, FAST, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    MCDC_POOL_CASES(X)
+#undef X
+  }
+  return cudaErrorInvalidValue;
+}
+void pool_launch(bool staged, bool fast, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  if (staged) { if (fast) pool_launch_nt<true, true>(nt, grid, smem, st, T, A); else pool_launch_nt<true, false>(nt, grid, smem, st, T, A); }
+  else        { if (fast) pool_launch_nt<false, true>(nt, grid, smem, st, T, A); else pool_launch_nt<false, false>(nt, grid, smem, st, T, A); }
+}
+cudaError_t pool_set_smem(bool staged, bool fast, int nt, int bytes) {
+  if (staged) return fast ? pool_set_smem_nt<true, true>(nt, bytes) : pool_set_smem_nt<true, false>(nt, bytes);
+  return fast ? pool_set_smem_nt<false, true>(nt, bytes) : pool_set_smem_nt<false, false>(nt, bytes);
+}
+
 // ---- asynchronous scheduler: one k_history launch per sub-batch, no host synchronisation ----
 int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
                        cudaEvent_t ev0, cudaEvent_t ev1) {
@@ -704,15 +804,17 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
   ha.refill_min = p->refill_min;
-  const size_t smem = ha.smem_tables + (size_t)p->K * (sizeof(double) + sizeof(uint32_t)) + 8;
-  const int max_grid = p->n_sm * p->blocks_per_sm_hist;
-  int grid = (int)std::min<uint64_t>((uint64_t)max_grid, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + TRANSPORT_THREADS - 1) / TRANSPORT_THREADS));
+  ha.pool_slots = p->pool_slots;
+  if (const char *e3 = getenv("MCDC_AGGREGATE")) ha.aggregate = atoi(e3);
+  const size_t smem = p->pool_smem;
+  const int nt = p->hist_threads;
+  // one block per SM; fewer when the sub-batch is too small to fill the pools
+  int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + p->pool_slots - 1) / p->pool_slots));
   (void)ev0; (void)ev1;
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
-  if (staged) k_history<true><<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
-  else k_history<false><<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, ha);
+  pool_launch(staged, p->tab.score_fast != 0, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
   p->launches++;
@@ -757,19 +859,36 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
     size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
       p->blocks_per_sm = occ;
-    // stage the hot tables in shared memory when that does not cost occupancy beyond the register limit
-    const size_t pop_bytes = (size_t)p->K * 12 + 8;
-    int occ_plain = 1, occ_staged = 0;
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_plain, k_history<false>, TRANSPORT_THREADS, pop_bytes);
-    const size_t staged_bytes = align_up(p->tab.hot_bytes, 16) + pop_bytes;
-    if (staged_bytes <= (size_t)MAX_STAGE_BYTES) {
-      cudaFuncSetAttribute(k_history<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)staged_bytes);
-      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_staged, k_history<true>, TRANSPORT_THREADS, staged_bytes);
+    // pool kernel: one block per SM.  Stage the hot tables in shared memory when the rest still holds a pool of
+    // at least 2 particles per thread; otherwise the tables are read through L1/L2 and the pool takes the space.
+    {
+      int dev = 0, max_optin = 0;
+      cudaGetDevice(&dev);
+      cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+      const size_t pop_bytes = (size_t)p->K * 8 + align_up((size_t)p->K * 4, 16);
+      const size_t fixed = sizeof(PoolCtl) + 64 + pop_bytes;
+      const size_t hot = align_up(p->tab.hot_bytes, 16);
+      int nt = 512;
+      if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
+      if (nt != 256 && nt != 512 && nt != 768 && nt != 1024) nt = 512;
+      auto slots = [&](bool staged) -> long {
+        const long avail = (long)max_optin - (long)fixed - (long)(staged ? hot : 0);
+        if (avail <= 0) return 0;
+        long P = avail / (long)pool_bytes_per_slot();
+        P = std::min<long>(P, 8L * nt);
+        P = std::min<long>(P, 65528L);
+        return P / 8 * 8;
+      };
+      bool staged = slots(true) >= 2L * nt;
+      if (const char *e = getenv("MCDC_STAGE_TABLES")) staged = atoi(e) != 0 && slots(true) >= 64;
+      long P = slots(staged);
+      if (const char *e = getenv("MCDC_POOL")) P = std::min<long>(P, std::max<long>(64, atol(e) / 8 * 8));
+      if (P < 64) return MCDC_ERR_NOMEM;
+      p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)P;
+      p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)P * pool_bytes_per_slot();
+      cudaError_t e1 = pool_set_smem(staged, p->tab.score_fast != 0, nt, (int)p->pool_smem);
+      if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_pool)");
     }
-    const char *env = getenv("MCDC_STAGE_TABLES");
-    p->stage_tables = occ_staged >= std::max(1, occ_plain) || (occ_staged >= 1 && occ_plain <= 2 && occ_staged * 2 >= occ_plain * 2 - 1);
-    if (env) p->stage_tables = (atoi(env) != 0) && occ_staged >= 1;
-    p->blocks_per_sm_hist = std::max(1, p->stage_tables ? occ_staged : occ_plain);
     if (const char *e2 = getenv("MCDC_REFILL_MIN")) p->refill_min = std::max(1, std::min(32, atoi(e2)));
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;

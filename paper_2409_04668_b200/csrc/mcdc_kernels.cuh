@@ -7,7 +7,7 @@
 // ballot-aggregated appends.  Track-length scores go to a shared-memory copy of the step's tally slab
 // (match_any-aggregated when few bins are hit) and are flushed with fp64 RED to the slot's accumulator.
 #pragma once
-#include "mcdc_step.cuh"
+#include "mcdc_typed.cuh"
 
 namespace mcdc {
 
@@ -177,6 +177,68 @@ __device__ __forceinline__ void score_track(const TBT &tb, const TallySink &S, b
 }
 
 // ------------------------------------------------------------------------------------------------
+// A.7 when the mesh covers the whole geometry and the time grid covers [t0, C_K] (Tables::score_fast): the
+// segment needs no clipping (u_in = 0, u_out = d), axes with a single bin never produce a crossing, and the
+// time-bin index is carried by the particle (`it`, validated against the edge array, D16).  Same DDA otherwise.
+// Warp-converged: every lane calls it, lanes without a segment pass active = false.
+// ------------------------------------------------------------------------------------------------
+template <class TBT>
+__device__ __forceinline__ void score_track_fast(const TBT &tb, const TallySink &S, bool active, const PState &p, int &it_hint,
+                                                 double d) {
+  const double INF = CUDART_INF;
+  const Tables &T = tb.T;
+  const bool bx = T.mesh_n[0] > 1, by = T.mesh_n[1] > 1, bz = T.mesh_n[2] > 1;   // kernel-uniform
+  int ix = 0, iy = 0, iz = 0, it = 0;
+  double v = 0.0, u_cur = 0.0;
+  bool more = active && d > 0.0;
+  if (more) {
+    v = tb.speed(p.g);
+    if (bx) { const double q = floor((p.x - T.mesh_lo[0]) * T.mesh_inv_d[0]); ix = (q < 0.0) ? 0 : ((q > (double)(T.mesh_n[0] - 1)) ? T.mesh_n[0] - 1 : (int)q); }
+    if (by) { const double q = floor((p.y - T.mesh_lo[1]) * T.mesh_inv_d[1]); iy = (q < 0.0) ? 0 : ((q > (double)(T.mesh_n[1] - 1)) ? T.mesh_n[1] - 1 : (int)q); }
+    if (bz) { const double q = floor((p.z - T.mesh_lo[2]) * T.mesh_inv_d[2]); iz = (q < 0.0) ? 0 : ((q > (double)(T.mesh_n[2] - 1)) ? T.mesh_n[2] - 1 : (int)q); }
+    // largest it with T[it] <= t: try the carried index and its successor, else search
+    it = it_hint;
+    double t_lo = tb.time_edge(it), t_hi = tb.time_edge(it + 1);
+    if (p.t >= t_hi && it + 1 < T.Nt) { it += 1; t_lo = t_hi; t_hi = tb.time_edge(it + 1); }
+    if (!(t_lo <= p.t && (p.t < t_hi || it == T.Nt - 1))) {
+      int lo = 0, hi = T.Nt - 1;
+      while (lo < hi) {
+        const int mid = (lo + hi + 1) >> 1;
+        if (tb.time_edge(mid) <= p.t) lo = mid; else hi = mid - 1;
+      }
+      it = lo;
+    }
+  }
+  while (__any_sync(MCDC_FULL, more)) {
+    long long bin = -1;
+    double val = 0.0;
+    if (more) {
+      double cx = INF, cy = INF, cz = INF;
+      if (bx) cx = (T.mesh_lo[0] + (double)(ix + (p.ux > 0.0 ? 1 : 0)) * T.mesh_d[0] - p.x) * p.ix;
+      if (by) cy = (T.mesh_lo[1] + (double)(iy + (p.uy > 0.0 ? 1 : 0)) * T.mesh_d[1] - p.y) * p.iy;
+      if (bz) cz = (T.mesh_lo[2] + (double)(iz + (p.uz > 0.0 ? 1 : 0)) * T.mesh_d[2] - p.z) * p.iz;
+      if (p.ux == 0.0) cx = INF;                          // direction component 0: no crossing on that axis
+      if (p.uy == 0.0) cy = INF;
+      if (p.uz == 0.0) cz = INF;
+      const double ct = (tb.time_edge(it + 1) - p.t) * v;
+      const double u_next = fmin(fmin(d, ct), fmin(cx, fmin(cy, cz)));
+      bin = ((((long long)it * T.G + p.g) * T.mesh_n[2] + iz) * T.mesh_n[1] + iy) * T.mesh_n[0] + ix;
+      val = p.w * fmax(u_next - u_cur, 0.0);
+      u_cur = u_next;
+      if (u_next >= d) more = false;
+      else {
+        if (cx <= u_next) { ix += (p.ux > 0.0) ? 1 : -1; if (ix < 0 || ix >= T.mesh_n[0]) more = false; }
+        if (cy <= u_next) { iy += (p.uy > 0.0) ? 1 : -1; if (iy < 0 || iy >= T.mesh_n[1]) more = false; }
+        if (cz <= u_next) { iz += (p.uz > 0.0) ? 1 : -1; if (iz < 0 || iz >= T.mesh_n[2]) more = false; }
+        if (ct <= u_next) { it += 1; if (it >= T.Nt) { more = false; it = T.Nt - 1; } }
+      }
+    }
+    tally_add_converged(S, bin, val);
+  }
+  if (active) it_hint = it;
+}
+
+// ------------------------------------------------------------------------------------------------
 // match_any-aggregated append for lanes that may target different slots (source kernel)
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t warp_append_by_slot(uint32_t *counters, int slot) {
@@ -218,20 +280,24 @@ __device__ __forceinline__ void block_atomic_add_u64(unsigned long long *dst, un
 // ------------------------------------------------------------------------------------------------
 // per-thread accumulators in shared memory (no atomics: one column per thread), flushed once per block
 // ------------------------------------------------------------------------------------------------
-struct BlockAccum {
-  double led[LED_N][TRANSPORT_THREADS];
-  uint32_t cnt[CNT_N][TRANSPORT_THREADS];
+template <int NT>
+struct BlockAccumT {
+  double led[LED_N][NT];
+  uint32_t cnt[CNT_N][NT];
   double scratch[32];
 };
+typedef BlockAccumT<TRANSPORT_THREADS> BlockAccum;
 
-__device__ __forceinline__ void accum_zero(BlockAccum &B) {
+template <class BA>
+__device__ __forceinline__ void accum_zero(BA &B) {
 #pragma unroll
   for (int e = 0; e < LED_N; ++e) B.led[e][threadIdx.x] = 0.0;
 #pragma unroll
   for (int e = 0; e < CNT_N; ++e) B.cnt[e][threadIdx.x] = 0u;
 }
 
-__device__ __forceinline__ void accum_flush(BlockAccum &B, DevCounters *cnt) {
+template <class BA>
+__device__ __forceinline__ void accum_flush(BA &B, DevCounters *cnt) {
   const int tid = threadIdx.x;
   for (int e = 0; e < LED_N; ++e) block_atomic_add(&cnt->ledger[1 + e], B.led[e][tid], B.scratch);
   unsigned long long *us = (unsigned long long *)B.scratch;
@@ -245,7 +311,8 @@ __device__ __forceinline__ void accum_flush(BlockAccum &B, DevCounters *cnt) {
 }
 
 // per-history event counts of a particle whose stay in this thread ends
-__device__ __forceinline__ void record_particle(BlockAccum &B, uint32_t *ev, uint32_t hid, uint32_t &pc_coll,
+template <class BA>
+__device__ __forceinline__ void record_particle(BA &B, uint32_t *ev, uint32_t hid, uint32_t &pc_coll,
                                                 uint32_t &pc_surf, uint32_t &pc_child, uint32_t pc_census) {
   const int tid = threadIdx.x;
   B.cnt[CNT_COLL][tid] += pc_coll; B.cnt[CNT_SURF][tid] += pc_surf; B.cnt[CNT_CHILDREN][tid] += pc_child;
@@ -510,6 +577,7 @@ struct HistoryArgs {
   int aggregate;
   int refill_min;                 // idle lanes per warp that trigger a refill
   uint32_t smem_tables;           // bytes of dynamic shared memory in front of the census arrays
+  uint32_t pool_slots;            // k_pool: particles held in the block's shared-memory pool (multiple of 8)
 };
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
@@ -526,16 +594,20 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
   return v;
 }
 
-template <bool STAGED>
-__global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, HistoryArgs A) {
-  __shared__ BlockAccum acc;
+template <bool STAGED, int NT>
+__global__ void __launch_bounds__(NT, 1) k_history(Tables T, HistoryArgs A) {
+  __shared__ BlockAccumT<NT> acc;
   const TB<STAGED> tb(T);
   const int tid = threadIdx.x, lane = tid & 31;
   const unsigned lt_mask = (1u << lane) - 1u;
   double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables);
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(s_popw + T.K);
-  if (STAGED) stage_tables(T);
-  for (int k = tid; k < T.K; k += TRANSPORT_THREADS) { s_popw[k] = 0.0; s_popn[k] = 0u; }
+  if (STAGED) {
+    const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
+    uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
+    for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
+  }
+  for (int k = tid; k < T.K; k += NT) { s_popw[k] = 0.0; s_popn[k] = 0u; }
   accum_zero(acc);
   __syncthreads();
   unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
@@ -545,8 +617,10 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
   int fi = FI_NONE;
   PState p;
   p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
+  p.ix = p.iy = p.iz = 1.0;
   p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
   int pk = 0;                                            // index of the particle's next census time
+  int it = 0;                                            // carried time-bin index (validated in the score)
   uint32_t slot = 0u;
   uint32_t pc_coll = 0, pc_surf = 0, pc_child = 0, pc_census = 0, n_src = 0, n_src_lost = 0;
 
@@ -585,7 +659,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
           p.x = A.q.x[j]; p.y = A.q.y[j]; p.z = A.q.z[j]; p.t = A.q.t[j]; p.w = A.q.w[j];
           p.key = A.q.key[j];
           const int4 m = A.q.meta[j];
-          p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z;
+          p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z; it = m.w;
           p.ctr = 0u;
           slot = p.hid / A.hb;
           fi = FI_CHILD;
@@ -608,6 +682,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
             slot = i / A.hb;
             source_position(T, A.seed_mixed, A.first_history + i, p);
             pk = census_index(tb, p.t);
+            it = 0;
             fi = FI_SOURCE;
             have = true;
           }
@@ -631,15 +706,16 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
     }
 
     // ---------------- phase C/D: one segment: distances, score, move ----------------
-    double d = 0.0;
-    int ev = -1, i_star = -1;
+    double d = 0.0, pos_star = 0.0;
+    int ev = -1, slot_star = -1, which = -1;
     const double t_census = have ? tb.census(pk) : 0.0;
-    if (have) ev = find_event(tb, p, t_census, d, i_star);
+    if (have) ev = find_event_typed(tb, p, t_census, d, slot_star, which, pos_star);
     {
       TallySink S;
       S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
       S.aggregate = A.aggregate;
-      score_track(tb, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
+      if (T.score_fast) score_track_fast(tb, S, have, p, it, d);
+      else score_track(tb, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
     }
     // ---------------- phase E: the event ----------------
     int n_push = 0, census_k = -1;
@@ -648,16 +724,17 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
     if (have) {
       p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
       p.t = (ev == EV_CENSUS) ? t_census : p.t + d * tb.inv_speed(p.g);
-      if (ev == EV_CENSUS) {                             // A.8: bookkeeping only, then the next interval
+      if (ev == EV_SURFACE) {
+        pc_surf += 1u;
+        have = surface_event_typed(tb, p, slot_star, which, pos_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid],
+                                   &acc.cnt[CNT_LOST][tid]);
+        ended = !have;
+      } else if (ev == EV_CENSUS) {                      // A.8: bookkeeping only, then the next interval
         pc_census += 1u;
         census_k = pk;
         if (d > 0.0) p.last_surf = -1;
         if (pk == T.K - 1) { acc.led[LED_CENSUS_FINAL][tid] += p.w; have = false; ended = true; }
         else pk += 1;
-      } else if (ev == EV_SURFACE) {
-        pc_surf += 1u;
-        have = surface_event(tb, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
-        ended = !have;
       } else {
         pc_coll += 1u;
         const int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
@@ -702,7 +779,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
           const uint32_t j = (uint32_t)(base + (unsigned long long)c) & A.q.mask;
           A.q.x[j] = p.x; A.q.y[j] = p.y; A.q.z[j] = p.z; A.q.t[j] = p.t; A.q.w[j] = p.w;
           A.q.key[j] = child_key(p.key, c0, (uint32_t)(c + 1));
-          A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, 0);
+          A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, it);
         }
         __threadfence();
         for (int c = 0; c < n_push; ++c) {
@@ -724,7 +801,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_history(Tables T, History
 
   // ---- block totals ----
   __syncthreads();
-  for (int k = tid; k < T.K; k += TRANSPORT_THREADS) {
+  for (int k = tid; k < T.K; k += NT) {
     if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, s_popw[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
   }
   accum_flush(acc, A.cnt);

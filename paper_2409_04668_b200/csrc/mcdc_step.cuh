@@ -20,6 +20,7 @@ enum FlightInit : int {
 // particle state held in registers
 struct PState {
   double x, y, z, ux, uy, uz, t, w;
+  double ix, iy, iz;                // 1 / (ux, uy, uz), kept with the direction (history kernel only)
   unsigned long long key;
   uint32_t ctr, hid;
   int g, cell, last_surf;
@@ -58,6 +59,7 @@ __device__ __forceinline__ bool flight_init(const TBT &tb, PState &p, int kind) 
     draw2(p.key, p.ctr, xi_mu, xi_phi);
     isotropic(xi_mu, xi_phi, p.ux, p.uy, p.uz);
   }
+  p.ix = 1.0 / p.ux; p.iy = 1.0 / p.uy; p.iz = 1.0 / p.uz;
   p.last_surf = -1;
   if (kind == FI_SOURCE) {
     p.cell = locate_source(tb, p.x, p.y, p.z, p.ux, p.uy, p.uz);
@@ -107,7 +109,7 @@ __device__ __forceinline__ int find_event(const TBT &tb, PState &p, double t_cen
   const int e = tb.cell_off(p.cell + 1);
   for (int i = tb.cell_off(p.cell); i < e; ++i) {
     const int h = tb.hs(i);
-    const int s = h >> 4;
+    const int s = h >> 6;
     const double u = surf_distance(tb, s, (h >> 1) & 7, s == p.last_surf, p.x, p.y, p.z, p.ux, p.uy, p.uz, ix, iy, iz);
     if (u < d_surf) { d_surf = u; i_star = i; }
   }
@@ -123,7 +125,7 @@ template <class TBT>
 __device__ __forceinline__ bool surface_event(const TBT &tb, PState &p, int i_star, double *led_leak, double *led_lost,
                                               uint32_t *cnt_lost) {
   const int h = tb.hs(i_star);
-  const int s_star = h >> 4;
+  const int s_star = h >> 6;
   p.last_surf = s_star;
   const int bc = tb.surf_bc(s_star);
   if (bc == 1) { *led_leak += p.w; return false; }

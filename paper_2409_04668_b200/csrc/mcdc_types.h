@@ -50,13 +50,17 @@ struct Tables {
   uint32_t o_surf_q;    // [S] double4 typed parameters
   uint32_t o_surf_bc;   // [S]
   uint32_t o_cell_off;  // [C+1]
-  uint32_t o_hs;        // packed half-space: surface << 4 | type << 1 | (sense > 0)
+  uint32_t o_hs;        // packed half-space: surface << 6 | bc << 4 | type << 1 | (sense > 0)
   uint32_t o_cell_mat;  // [C]
   uint32_t o_nb_off;    // [nhs+1] neighbour candidates of half-space slot i (cells across that surface)
   uint32_t o_nb_cell;
   uint32_t o_loc_off;   // [nvox+1] source locator grid
   uint32_t o_loc_cell;
+  uint32_t o_cell_rec;  // [C] typed cell records, CELL_REC_BYTES each (layout below)
+  uint32_t o_other;     // overflow list of "other" half-space slots (cells with more than two)
   uint32_t o_surf_coef; // [S][10] general form (inside the hot prefix only when a general quadric exists)
+  const Tables *self_dev;  // device-memory copy of this struct (slow paths that must not take the parameter's address)
+  int score_fast;       // the tally mesh covers the geometry and the time grid covers [t0, C_K]: no clipping needed
   // source
   double src_lo[3], src_hi[3], src_t0, src_t1;
   int src_last;
@@ -69,6 +73,18 @@ struct Tables {
   int mesh_n[3];
   unsigned long long n_bins;
 };
+
+// Typed cell record (built at mcdc_problem_create): the tightest axis-aligned plane of each (axis, side) is a
+// "face"; every other half-space of the cell (cylinders, general quadrics, redundant planes) is an "other".
+//   +0  double bound[6]   [2a] = lower plane position on axis a (-inf if none), [2a+1] = upper (+inf)
+//   +48 int    face[6]    half-space slot (index into o_hs) of that face, -1 if none
+//   +72 int    n_other
+//   +76 int    other_off  index into o_other of the cell's full "other" slot list
+//   +80 int    other0, other1   the first two "other" slots (copies)
+//   +88 int    material
+//   +92 int    pad[3]
+constexpr uint32_t CELL_REC_BYTES = 104;   // 26 words: odd multiple of 8 bytes, spreads cells over the banks
+constexpr uint32_t CR_BOUND = 0, CR_FACE = 48, CR_N_OTHER = 72, CR_OTHER_OFF = 76, CR_OTHER0 = 80, CR_MAT = 88;
 
 // Per-launch parameters of the transport kernel.
 struct StepParams {
