@@ -225,15 +225,15 @@ def bench_gpu(args):
     if rank == 0:
         clocks = sampler.stop(t_wall0, t_wall1)
         peak, peak_kind, sm_max = _peaks()
-        # dominant kernel: k_transport.  Algorithmic bytes of the steps it processed / its device time.
+        # dominant kernel: k_warp.  Algorithmic bytes of the steps it processed / its device time.
         alg = algorithmic_bytes(p, {"segments": c["segments"], "children": c["children"]}, n_hist * args.steps,
                                 n_b * args.steps)
         n_tr = max(1, (launches - args.steps * 2))
         ach = alg / (ms_tr * 1e-3) / 1e9
-        roofline = {"bound": "hbm", "kernel": "k_transport", "achieved": ach, "peak": peak, "unit": "GB/s",
+        roofline = {"bound": "hbm", "kernel": "k_warp", "achieved": ach, "peak": peak, "unit": "GB/s",
                     "frac": ach / peak, "traffic": None, "peak_kind": peak_kind,
                     "note": "achieved = SURVEY 8(d) algorithmic bytes (176 B/segment + 112 B/child + 88 B/history + "
-                            "close-out) / summed k_transport device time; particle state is register-resident so "
+                            "close-out) / summed k_warp device time; particle state is register-resident so "
                             "DRAM traffic is far below this figure (see DESIGN.md, profiles/)",
                     "launches": int(n_tr), "ms_kernel_total": ms_tr}
         out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libmcdc.so")
 SOURCES = ["mcdc_host.cu"]
-HEADERS = ["mcdc_types.h", "mcdc_device.cuh", "mcdc_step.cuh", "mcdc_typed.cuh", "mcdc_kernels.cuh", "mcdc_pool.cuh"]
+HEADERS = ["mcdc_types.h", "mcdc_device.cuh", "mcdc_step.cuh", "mcdc_kernels.cuh", "mcdc_warp.cuh"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

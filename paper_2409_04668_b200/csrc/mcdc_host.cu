@@ -1,6 +1,7 @@
 // mcdc_host.cu -- C ABI (include/mcdc.h) of libmcdc.so: validation, problem upload, the census-step
 // driver loop and result read-back.  All transport arithmetic runs in the kernels of mcdc_kernels.cuh.
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -12,7 +13,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/mcdc.h"
-#include "mcdc_pool.cuh"
+#include "mcdc_warp.cuh"
 
 using namespace mcdc;
 
@@ -98,7 +99,7 @@ struct mcdc_problem {
   int hist_threads = 512;
   uint32_t pool_slots = 0;
   size_t pool_smem = 0;
-  int refill_min = 8;
+  size_t n_cert = 0, n_transm = 0;   // transmission half-spaces with / without a certified neighbour
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
   std::string cuda_err;
 };
@@ -347,36 +348,26 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
         if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);  // increasing id by construction
       nb_off[i + 1] = (int)nb_cell.size();
     }
-  // ---- typed cell records (mcdc_types.h): tightest axis-aligned plane per (axis, side) = face, the rest = other ----
-  std::vector<unsigned char> cell_rec((size_t)C * CELL_REC_BYTES, 0);
-  std::vector<int> other_list;
+  // ---- typed cells (mcdc_types.h): tightest axis-aligned plane per (axis, side) = face, the rest = other ----
+  std::vector<std::array<double, 6>> bound(C);
+  std::vector<std::array<int, 6>> face(C);
+  std::vector<std::vector<int>> others(C);
   for (int c = 0; c < C; ++c) {
-    double bound[6];
-    int face[6];
-    for (int a = 0; a < 3; ++a) { bound[2 * a] = -HINF; bound[2 * a + 1] = HINF; face[2 * a] = face[2 * a + 1] = -1; }
+    for (int a = 0; a < 3; ++a) { bound[c][2 * a] = -HINF; bound[c][2 * a + 1] = HINF; face[c][2 * a] = face[c][2 * a + 1] = -1; }
     for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
       const int s = p->hs_surface[i];
       if (type[s] > ST_PLANE_Z) continue;
       const int a = type[s] - ST_PLANE_X;
       const bool below = (q[s].y > 0.0) == (p->hs_sense[i] < 0);          // coordinate < position
       const int f = 2 * a + (below ? 1 : 0);
-      const bool tighter = below ? (q[s].x < bound[f]) : (q[s].x > bound[f]);
-      if (tighter) { bound[f] = q[s].x; face[f] = i; }                    // equal positions: the earlier slot stays
+      const bool tighter = below ? (q[s].x < bound[c][f]) : (q[s].x > bound[c][f]);
+      if (tighter) { bound[c][f] = q[s].x; face[c][f] = i; }              // equal positions: the earlier slot stays
     }
-    std::vector<int> others;
     for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
       bool is_face = false;
-      for (int f = 0; f < 6; ++f) is_face = is_face || face[f] == i;
-      if (!is_face) others.push_back(i);
+      for (int f = 0; f < 6; ++f) is_face = is_face || face[c][f] == i;
+      if (!is_face) others[c].push_back(i);
     }
-    unsigned char *r = cell_rec.data() + (size_t)c * CELL_REC_BYTES;
-    std::memcpy(r + CR_BOUND, bound, sizeof(bound));
-    std::memcpy(r + CR_FACE, face, sizeof(face));
-    const int n_other = (int)others.size(), other_off = (int)other_list.size();
-    const int o01[2] = {n_other > 0 ? others[0] : -1, n_other > 1 ? others[1] : -1};
-    std::memcpy(r + CR_N_OTHER, &n_other, 4); std::memcpy(r + CR_OTHER_OFF, &other_off, 4);
-    std::memcpy(r + CR_OTHER0, o01, 8); std::memcpy(r + CR_MAT, &p->cell_mat[c], 4);
-    other_list.insert(other_list.end(), others.begin(), others.end());
   }
   // candidate neighbours: the one sharing the largest part of the face first (cells do not overlap, so the order
   // of the tests cannot change which cell contains the point -- DESIGN.md section 2)
@@ -408,6 +399,141 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
       if (!(p->mesh_lo[a] <= b.lo[a]) || !(p->mesh_hi[a] >= b.hi[a])) score_fast = 0;
   }
   if (!(p->T[0] <= p->src_t0) || !(p->T[p->Nt] >= p->census[p->K - 1])) score_fast = 0;
+
+  // ---- compact tables of k_warp (mcdc_types.h): certificates, one-bin cells, one-bin census intervals ----
+  // "Certificates": at a transmission the new cell is found by A.5's search over the cells on the other side.  Where
+  // geometry alone proves that ONE candidate n holds every point of the crossed surface patch, the kernel may take n
+  // without testing.  The patch of half-space (s, sense) of cell c lies inside R = c's bounding box (flattened onto the
+  // plane, or cut to the cylinder's bounding box).  n is certified when (1) it lists s with the opposite sense -- as its
+  // own face at the same position when s is a plane; (2) on every other axis n's plane bounds enclose R, where a bound
+  // that R takes from one of c's own planes may coincide (the kernel then requires the point to lie strictly inside c's
+  // forward faces) and any other bound must clear R by a margin; (3) each of n's remaining half-spaces holds on all of R
+  // by a margin (axis-aligned planes and z-cylinders only; a general quadric is never certified).  Cells do not overlap
+  // (header), so no other cell can hold such a point.  Points that fail the kernel's strict test take the full search.
+  std::vector<Box> ubox(C);
+  for (int c = 0; c < C; ++c) ubox[c] = cell_box(*p, type, q, c, false);
+  auto holds_on_box = [&](int t, int sense, const Box &R) -> bool {
+    if (type[t] <= ST_PLANE_Z) {
+      const int a = type[t] - ST_PLANE_X;
+      const double pos = q[t].x, m = 1e-9 * (1.0 + std::fabs(pos));
+      const bool below = (q[t].y > 0.0) == (sense < 0);                     // coordinate < position required
+      return below ? (R.hi[a] < pos - m) : (R.lo[a] > pos + m);
+    }
+    if (type[t] == ST_CYL_Z) {
+      const bool inside = (double)sense * q[t].w < 0.0;
+      const double x0 = q[t].x, y0 = q[t].y, r2 = q[t].z;
+      const double dxn = std::max(0.0, std::max(R.lo[0] - x0, x0 - R.hi[0])), dyn = std::max(0.0, std::max(R.lo[1] - y0, y0 - R.hi[1]));
+      const double dxx = std::max(std::fabs(R.lo[0] - x0), std::fabs(R.hi[0] - x0)), dyx = std::max(std::fabs(R.lo[1] - y0), std::fabs(R.hi[1] - y0));
+      return inside ? (dxx * dxx + dyx * dyx < r2 * (1.0 - 1e-9)) : (dxn * dxn + dyn * dyn > r2 * (1.0 + 1e-9));
+    }
+    return false;
+  };
+  auto encloses = [&](int n, int c, const Box &R, int skip_axis) -> bool {   // condition (2)
+    for (int b = 0; b < 3; ++b) {
+      if (b == skip_axis) continue;
+      const double m = 1e-9 * (1.0 + (std::isfinite(R.lo[b]) ? std::fabs(R.lo[b]) : 0.0) + (std::isfinite(R.hi[b]) ? std::fabs(R.hi[b]) : 0.0));
+      const bool lo_ok = bound[n][2 * b] <= bound[c][2 * b] || bound[n][2 * b] < R.lo[b] - m;
+      const bool hi_ok = bound[n][2 * b + 1] >= bound[c][2 * b + 1] || bound[n][2 * b + 1] > R.hi[b] + m;
+      if (!lo_ok || !hi_ok) return false;
+    }
+    return true;
+  };
+  auto certified = [&](int c, int i) -> int {                                // neighbour across half-space slot i of cell c
+    const int s = p->hs_surface[i];
+    if (p->surf_bc[s] != MCDC_BC_TRANSMISSION) return -1;
+    Box R = ubox[c];
+    int axis = -1, f = -1;
+    if (type[s] <= ST_PLANE_Z) {
+      axis = type[s] - ST_PLANE_X;
+      for (int k = 0; k < 2; ++k)
+        if (face[c][2 * axis + k] == i) f = 2 * axis + k;
+      if (f < 0) return -1;                                                   // a redundant plane: never the nearest one
+      R.lo[axis] = R.hi[axis] = bound[c][f];
+    } else if (type[s] == ST_CYL_Z) {
+      const double r = std::sqrt(q[s].z);
+      R.lo[0] = std::max(R.lo[0], q[s].x - r); R.hi[0] = std::min(R.hi[0], q[s].x + r);
+      R.lo[1] = std::max(R.lo[1], q[s].y - r); R.hi[1] = std::min(R.hi[1], q[s].y + r);
+    } else return -1;
+    for (int k = nb_off[i]; k < nb_off[i + 1]; ++k) {
+      const int n = nb_cell[k];
+      if (axis >= 0) {
+        const int fo = f ^ 1;
+        if (face[n][fo] < 0 || p->hs_surface[face[n][fo]] != s) continue;
+      }
+      if (!encloses(n, c, R, axis)) continue;
+      bool ok = true;
+      for (int o : others[n]) {
+        if (p->hs_surface[o] == s) continue;
+        ok = ok && holds_on_box(p->hs_surface[o], p->hs_sense[o], R);
+      }
+      if (ok) return n;
+    }
+    return -1;
+  };
+  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095;
+  std::vector<unsigned char> cell2((size_t)C * CELL2_BYTES, 0), other2;
+  size_t n_cert = 0, n_transm = 0;
+  for (int c = 0; c < C && warp_ok; ++c) {
+    unsigned char *r = cell2.data() + (size_t)c * CELL2_BYTES;
+    if (p->cell_off[c + 1] - p->cell_off[c] > 255 || others[c].size() > 255 || other2.size() / OTHER2_BYTES > 65000) { warp_ok = false; break; }
+    uint16_t fs[6], fn[6], fbc = 0;
+    uint8_t fi[6];
+    for (int f = 0; f < 6; ++f) {
+      fs[f] = fn[f] = (uint16_t)NONE16; fi[f] = 0;
+      const int i = face[c][f];
+      if (i < 0) continue;
+      const int s = p->hs_surface[i];
+      fs[f] = (uint16_t)s; fi[f] = (uint8_t)(i - p->cell_off[c]);
+      fbc |= (uint16_t)(p->surf_bc[s] << (2 * f));
+      const int n = certified(c, i);
+      if (p->surf_bc[s] == MCDC_BC_TRANSMISSION) { n_transm++; if (n >= 0) n_cert++; }
+      if (n >= 0) fn[f] = (uint16_t)n;
+    }
+    std::memcpy(r + C2_FACE_SURF, fs, 12); std::memcpy(r + C2_FACE_NB, fn, 12); std::memcpy(r + C2_FACE_IDX, fi, 6);
+    std::memcpy(r + C2_FACE_BC, &fbc, 2);
+    const uint32_t info = (uint32_t)others[c].size() | ((uint32_t)p->cell_mat[c] << 8) | ((uint32_t)(other2.size() / OTHER2_BYTES) << 16);
+    std::memcpy(r + C2_INFO, &info, 4);
+    for (int i : others[c]) {
+      const int s = p->hs_surface[i];
+      const int n = certified(c, i);
+      if (p->surf_bc[s] == MCDC_BC_TRANSMISSION) { n_transm++; if (n >= 0) n_cert++; }
+      const uint32_t w0 = (uint32_t)s | ((uint32_t)(n >= 0 ? n : (int)NONE16) << 16);
+      const uint32_t flags = (p->hs_sense[i] > 0 ? 1u : 0u) | ((uint32_t)type[s] << 1) | ((uint32_t)p->surf_bc[s] << 4);
+      const uint32_t w1 = (uint32_t)(i - p->cell_off[c]) | (flags << 8);
+      unsigned char e[8];
+      std::memcpy(e, &w0, 4); std::memcpy(e + 4, &w1, 4);
+      other2.insert(other2.end(), e, e + 8);
+    }
+    // the one spatial tally bin that holds the whole cell (the score is then a single addition)
+    uint32_t cbin = NONE32;
+    if (score_fast) {
+      int idx[3] = {0, 0, 0};
+      bool one = true;
+      for (int a = 0; a < 3 && one; ++a) {
+        if (p->mesh_n[a] == 1) continue;
+        const double d = (p->mesh_hi[a] - p->mesh_lo[a]) / p->mesh_n[a];
+        const double lo = ubox[c].lo[a], hi = ubox[c].hi[a];
+        if (!std::isfinite(lo) || !std::isfinite(hi)) { one = false; break; }
+        const double tol = 1e-12 * (1.0 + std::fabs(lo) + std::fabs(hi)) / d;
+        const double i_lo = std::floor((lo - p->mesh_lo[a]) / d + tol), i_hi = std::ceil((hi - p->mesh_lo[a]) / d - tol) - 1.0;
+        if (i_lo != i_hi || i_lo < 0.0 || i_lo > (double)(p->mesh_n[a] - 1)) one = false; else idx[a] = (int)i_lo;
+      }
+      if (one) cbin = (uint32_t)((idx[2] * p->mesh_n[1] + idx[1]) * p->mesh_n[0] + idx[0]);
+    }
+    std::memcpy(r + C2_BIN, &cbin, 4);
+  }
+  if (other2.empty()) other2.resize(OTHER2_BYTES, 0);
+  p->n_cert = n_cert; p->n_transm = n_transm;
+  // census interval k = (C[k-1] (or the source start), C[k]]: the time bin that holds all of it, if one does
+  std::vector<int> tbin_k(p->K, -1), it0_k(p->K, 0);
+  for (int k = 0; k < p->K; ++k) {
+    const double a_k = (k == 0) ? p->src_t0 : p->census[k - 1];
+    int j = 0;
+    for (int i = 0; i < p->Nt; ++i)
+      if (p->T[i] <= a_k) j = i;
+    it0_k[k] = j;
+    if (score_fast && p->T[j] <= a_k && p->census[k] <= p->T[j + 1]) tbin_k[k] = j;
+  }
 
   // ---- source locator grid ----
   int loc_n[3];
@@ -460,17 +586,20 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   t.o_sig_f = putd(p->sigma_f); t.o_nu = putd(p->nu); t.o_cdf_s = putd(cdf_s); t.o_last_s = puti(last_s);
   t.o_cdf_chi = putd(cdf_chi); t.o_last_chi = puti(last_chi); t.o_speed = putd(p->speed); t.o_inv_speed = putd(inv_speed);
   t.o_T = putd(p->T); t.o_census = putd(p->census); t.o_src_cdf = putd(src_cdf);
+  t.o_tbin_k = puti(tbin_k); t.o_it0_k = puti(it0_k);
   t.o_surf_q = put(q.data(), q.size() * sizeof(double4));
-  t.o_surf_bc = puti(p->surf_bc); t.o_cell_off = puti(p->cell_off); t.o_hs = puti(hs); t.o_cell_mat = puti(p->cell_mat);
-  t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell);
-  t.o_cell_rec = put(cell_rec.data(), cell_rec.size()); t.o_other = puti(other_list);
-  t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
-  t.score_fast = score_fast;
+  t.o_cell2 = put(cell2.data(), cell2.size()); t.o_other2 = put(other2.data(), other2.size());
   bool any_quadric = false;
   for (int s = 0; s < S; ++s) any_quadric = any_quadric || type[s] == ST_QUADRIC;
-  size_t hot = (blob.size() + 15) / 16 * 16;
+  // everything above is the hot prefix k_warp stages in shared memory; the generic tables below stay in L2
+  const size_t hot = (blob.size() + 15) / 16 * 16;
+  t.o_surf_bc = puti(p->surf_bc); t.o_cell_off = puti(p->cell_off); t.o_hs = puti(hs); t.o_cell_mat = puti(p->cell_mat);
+  t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell);
+  t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
   t.o_surf_coef = putd(p->surf_coef);
-  if (any_quadric) hot = (blob.size() + 15) / 16 * 16;
+  t.score_fast = score_fast;
+  t.warp_ok = warp_ok ? 1 : 0;
+  (void)any_quadric;
   blob.resize((blob.size() + 15) / 16 * 16, 0);
   t.hot_bytes = (uint32_t)hot;
   t.blob = ar.upload(blob);
@@ -558,7 +687,7 @@ WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap, uint64_t hi
   L.q_cap = queue_capacity(hist);
   L.q_flag = off; off += align_up((size_t)L.q_cap * sizeof(uint32_t), 256);
   L.fixed = off;
-  L.q_data = off; off += (size_t)6 * align_up((size_t)L.q_cap * 8, 256) + align_up((size_t)L.q_cap * 16, 256);
+  L.q_data = off; off += (size_t)5 * align_up((size_t)L.q_cap * 8, 256) + align_up((size_t)L.q_cap * 16, 256);
   const size_t n = (size_t)slots * cap;
   for (int b = 0; b < 4; ++b) {
     L.bank[b] = off;
@@ -623,7 +752,7 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
     auto take = [&](size_t bytes) { char *r = qd; qd += align_up(bytes, 256); return r; };
     FissionQueue &Q = p->queue;
     Q.x = (double *)take(L.q_cap * 8); Q.y = (double *)take(L.q_cap * 8); Q.z = (double *)take(L.q_cap * 8);
-    Q.t = (double *)take(L.q_cap * 8); Q.w = (double *)take(L.q_cap * 8);
+    Q.t = (double *)take(L.q_cap * 8);
     Q.key = (unsigned long long *)take(L.q_cap * 8);
     Q.meta = (int4 *)take(L.q_cap * 16);
     Q.flag = (uint32_t *)(p->ws + L.q_flag);
@@ -758,35 +887,67 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   return MCDC_OK;
 }
 
-// ---- k_pool instantiations: (tables staged, fast score, threads per block) ----
-#define MCDC_POOL_CASES(X) X(256) X(512) X(768) X(1024)
-template <bool STAGED, bool FAST>
-void pool_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+// ---- k_warp instantiations: (tables staged, per-history events recorded, threads per block) ----
+#define MCDC_WARP_CASES(X) X(256) X(384) X(512) X(640) X(768) X(1024)
+template <bool STAGED, bool RECORD>
+void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
-#define X(N) case N: k_pool<STAGED, FAST, N><<<grid, N, smem, st>>>(T, A); break;
-    MCDC_POOL_CASES(X)
+#define X(N) case N: k_warp<STAGED, RECORD, N><<<grid, N, smem, st>>>(T, A); break;
+    MCDC_WARP_CASES(X)
 #undef X
   }
 }
-template <bool STAGED, bool FAST>
-cudaError_t pool_set_smem_nt(int nt, int bytes) {
+template <bool STAGED, bool RECORD>
+cudaError_t warp_set_smem_nt(int nt, int bytes) {
   switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_pool<STAGED, FAST, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    MCDC_POOL_CASES(X)
+#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    MCDC_WARP_CASES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-void pool_launch(bool staged, bool fast, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (fast) pool_launch_nt<true, true>(nt, grid, smem, st, T, A); else pool_launch_nt<true, false>(nt, grid, smem, st, T, A); }
-  else        { if (fast) pool_launch_nt<false, true>(nt, grid, smem, st, T, A); else pool_launch_nt<false, false>(nt, grid, smem, st, T, A); }
+void warp_launch(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  if (staged) { if (record) warp_launch_nt<true, true>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false>(nt, grid, smem, st, T, A); }
+  else        { if (record) warp_launch_nt<false, true>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false>(nt, grid, smem, st, T, A); }
 }
-cudaError_t pool_set_smem(bool staged, bool fast, int nt, int bytes) {
-  if (staged) return fast ? pool_set_smem_nt<true, true>(nt, bytes) : pool_set_smem_nt<true, false>(nt, bytes);
-  return fast ? pool_set_smem_nt<false, true>(nt, bytes) : pool_set_smem_nt<false, false>(nt, bytes);
+cudaError_t warp_set_smem(bool staged, bool record, int nt, int bytes) {
+  if (staged) return record ? warp_set_smem_nt<true, true>(nt, bytes) : warp_set_smem_nt<true, false>(nt, bytes);
+  return record ? warp_set_smem_nt<false, true>(nt, bytes) : warp_set_smem_nt<false, false>(nt, bytes);
 }
 
-// ---- asynchronous scheduler: one k_history launch per sub-batch, no host synchronisation ----
+// shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
+int plan_warp_kernel(mcdc_problem *p, bool record) {
+  int dev = 0, max_optin = 0;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+  int nt = 512;
+  if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
+  if (nt != 256 && nt != 384 && nt != 512 && nt != 640 && nt != 768 && nt != 1024) nt = 512;
+  const int nw = nt / 32;
+  const size_t pop_bytes = align_up((size_t)p->K * 4, 16);
+  const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
+  const size_t hot = align_up(p->tab.hot_bytes, 16);
+  const size_t per_slot = warp_pool_bytes_per_slot(record);
+  auto slots = [&](bool staged) -> long {
+    const long avail = (long)max_optin - (long)fixed - (long)(staged ? hot : 0);
+    if (avail <= 0) return 0;
+    long W = avail / (long)(per_slot * nw);
+    W = std::min<long>(W, 248L);
+    return W / 8 * 8;                                  // keeps every array of the pool 8-byte aligned
+  };
+  bool staged = slots(true) >= 64;
+  if (const char *e = getenv("MCDC_STAGE_TABLES")) staged = atoi(e) != 0 && slots(true) >= 32;
+  long W = slots(staged);
+  if (const char *e = getenv("MCDC_POOL")) W = std::min<long>(W, std::max<long>(32, atol(e) / 8 * 8));
+  if (W < 32) return MCDC_ERR_NOMEM;
+  p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
+  p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
+  cudaError_t e1 = warp_set_smem(staged, record, nt, (int)p->pool_smem);
+  if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
+  return MCDC_OK;
+}
+
+// ---- asynchronous scheduler: one k_warp launch per sub-batch, no host synchronisation ----
 int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
                        cudaEvent_t ev0, cudaEvent_t ev1) {
   HistoryArgs ha;
@@ -803,18 +964,22 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
-  ha.refill_min = p->refill_min;
   ha.pool_slots = p->pool_slots;
   if (const char *e3 = getenv("MCDC_AGGREGATE")) ha.aggregate = atoi(e3);
   const size_t smem = p->pool_smem;
   const int nt = p->hist_threads;
   // one block per SM; fewer when the sub-batch is too small to fill the pools
-  int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + p->pool_slots - 1) / p->pool_slots));
+  const uint64_t per_block = (uint64_t)p->pool_slots * (nt / 32);
+  int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + per_block - 1) / per_block));
+  // chunk of source histories a warp reserves at a time: large enough to keep the cursor atomic cold, small enough
+  // that the last chunks still spread over all warps
+  ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)sb.n_hist / ((uint64_t)grid * (nt / 32) * 8)));
+  if (const char *e4 = getenv("MCDC_CHUNK")) ha.src_chunk = (uint32_t)std::max(1, atoi(e4));
   (void)ev0; (void)ev1;
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
-  pool_launch(staged, p->tab.score_fast != 0, nt, grid, smem, p->stream, p->tab, ha);
+  warp_launch(staged, record, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
   p->launches++;
@@ -839,8 +1004,9 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   if (p->batch_size != 0 && p->batch_size != hb) return MCDC_ERR_ARG;
   if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
   const bool record = opts->record_history_events != 0;
-  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED;
-  if (opts->scheduler != MCDC_SCHED_ASYNC && !stepped) return MCDC_ERR_ARG;
+  if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
+  // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
+  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u;
   if (record) {
     if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
     CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
@@ -859,37 +1025,10 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
     size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
       p->blocks_per_sm = occ;
-    // pool kernel: one block per SM.  Stage the hot tables in shared memory when the rest still holds a pool of
-    // at least 2 particles per thread; otherwise the tables are read through L1/L2 and the pool takes the space.
-    {
-      int dev = 0, max_optin = 0;
-      cudaGetDevice(&dev);
-      cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-      const size_t pop_bytes = (size_t)p->K * 8 + align_up((size_t)p->K * 4, 16);
-      const size_t fixed = sizeof(PoolCtl) + 64 + pop_bytes;
-      const size_t hot = align_up(p->tab.hot_bytes, 16);
-      int nt = 512;
-      if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
-      if (nt != 256 && nt != 512 && nt != 768 && nt != 1024) nt = 512;
-      auto slots = [&](bool staged) -> long {
-        const long avail = (long)max_optin - (long)fixed - (long)(staged ? hot : 0);
-        if (avail <= 0) return 0;
-        long P = avail / (long)pool_bytes_per_slot();
-        P = std::min<long>(P, 8L * nt);
-        P = std::min<long>(P, 65528L);
-        return P / 8 * 8;
-      };
-      bool staged = slots(true) >= 2L * nt;
-      if (const char *e = getenv("MCDC_STAGE_TABLES")) staged = atoi(e) != 0 && slots(true) >= 64;
-      long P = slots(staged);
-      if (const char *e = getenv("MCDC_POOL")) P = std::min<long>(P, std::max<long>(64, atol(e) / 8 * 8));
-      if (P < 64) return MCDC_ERR_NOMEM;
-      p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)P;
-      p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)P * pool_bytes_per_slot();
-      cudaError_t e1 = pool_set_smem(staged, p->tab.score_fast != 0, nt, (int)p->pool_smem);
-      if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_pool)");
-    }
-    if (const char *e2 = getenv("MCDC_REFILL_MIN")) p->refill_min = std::max(1, std::min(32, atoi(e2)));
+  }
+  if (!stepped) {
+    const int rcp = plan_warp_kernel(p, record);
+    if (rcp != MCDC_OK) return rcp;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
   CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1)); CK(cudaEventCreate(&ev0)); CK(cudaEventCreate(&ev1));

@@ -7,7 +7,7 @@
 // ballot-aggregated appends.  Track-length scores go to a shared-memory copy of the step's tally slab
 // (match_any-aggregated when few bins are hit) and are flushed with fp64 RED to the slot's accumulator.
 #pragma once
-#include "mcdc_typed.cuh"
+#include "mcdc_step.cuh"
 
 namespace mcdc {
 
@@ -543,22 +543,12 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
 }
 
 // ------------------------------------------------------------------------------------------------
-// Asynchronous history kernel: ONE launch per sub-batch.
-//  * Idle lanes take work from (1) the in-kernel fission queue (children first, so lineages finish promptly)
-//    and (2) the source-history cursor, building the source particle directly in registers.  Refills are
-//    batched: the acquire phase runs only when REFILL_MIN lanes of the warp are idle (or none is busy).
-//  * Every lane that starts a flight -- new source, new child, or a particle that just scattered -- samples
-//    its group and direction in one shared phase (flight_init) instead of three divergent code paths.
-//  * A particle keeps its registers across census boundaries: the census event only does the population
-//    bookkeeping (A.8) and moves on to the next census interval; in analog transport nothing has to wait
-//    there, so there is no census barrier.
-//  * A fission parent turns into its first child in place; the other children are published to the queue.
-//  * Tables are read from their shared-memory copy when STAGED.
+// Global fission queue and launch arguments of the asynchronous history kernel k_warp (mcdc_warp.cuh).
 // ------------------------------------------------------------------------------------------------
 struct FissionQueue {             // ring buffer in HBM, structure of arrays, capacity mask+1 (power of two)
-  double *x, *y, *z, *t, *w;
+  double *x, *y, *z, *t;
   unsigned long long *key;
-  int4 *meta;                     // {cell, census index k, hid, unused}
+  int4 *meta;                     // {cell, census index k, history id (when events are recorded), batch slot}
   uint32_t *flag;                 // entry i is readable when flag[i & mask] == (uint32)(i + 1)
   uint32_t mask;
   unsigned long long *head_tail;  // [0] consumers' cursor, [1] producers' cursor (monotonic over launches)
@@ -569,15 +559,15 @@ struct HistoryArgs {
   uint32_t *hist_cursor;          // next source history of this sub-batch
   unsigned long long seed_mixed, first_history;
   uint32_t n_hist, hb;            // histories in the sub-batch, histories per slot
+  uint32_t src_chunk;             // source histories a warp reserves per global atomic
   double *x_acc;
   DevCounters *cnt;
   double *pop_w;
   unsigned long long *pop_n;
   uint32_t *ev;
   int aggregate;
-  int refill_min;                 // idle lanes per warp that trigger a refill
   uint32_t smem_tables;           // bytes of dynamic shared memory in front of the census arrays
-  uint32_t pool_slots;            // k_pool: particles held in the block's shared-memory pool (multiple of 8)
+  uint32_t pool_slots;            // particles held in each warp's shared-memory pool
 };
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {
@@ -592,223 +582,6 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
   unsigned long long v;
   asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
   return v;
-}
-
-template <bool STAGED, int NT>
-__global__ void __launch_bounds__(NT, 1) k_history(Tables T, HistoryArgs A) {
-  __shared__ BlockAccumT<NT> acc;
-  const TB<STAGED> tb(T);
-  const int tid = threadIdx.x, lane = tid & 31;
-  const unsigned lt_mask = (1u << lane) - 1u;
-  double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables);
-  uint32_t *s_popn = reinterpret_cast<uint32_t *>(s_popw + T.K);
-  if (STAGED) {
-    const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
-    uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
-    for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
-  }
-  for (int k = tid; k < T.K; k += NT) { s_popw[k] = 0.0; s_popn[k] = 0u; }
-  accum_zero(acc);
-  __syncthreads();
-  unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
-  const unsigned long long q_cap = (unsigned long long)A.q.mask + 1ull;
-
-  bool have = false, src_done = false;
-  int fi = FI_NONE;
-  PState p;
-  p.x = p.y = p.z = p.ux = p.uy = p.t = p.w = 0.0; p.uz = 1.0;
-  p.ix = p.iy = p.iz = 1.0;
-  p.key = 0; p.ctr = 0; p.hid = 0; p.g = 0; p.cell = 0; p.last_surf = -1;
-  int pk = 0;                                            // index of the particle's next census time
-  int it = 0;                                            // carried time-bin index (validated in the score)
-  uint32_t slot = 0u;
-  uint32_t pc_coll = 0, pc_surf = 0, pc_child = 0, pc_census = 0, n_src = 0, n_src_lost = 0;
-
-  for (;;) {
-    // ---------------- phase A: acquire work for idle lanes (batched) ----------------
-    const unsigned need = __ballot_sync(MCDC_FULL, !have);
-    if (__popc(need) >= A.refill_min || need == MCDC_FULL) {
-      // (1) fission queue
-      uint32_t got = 0u;
-      unsigned long long qbase = 0ull;
-      int abort_run = 0;
-      if (lane == 0) {
-        abort_run = *(volatile int *)&A.cnt->overflow;
-        unsigned long long h = ld_volatile_u64(q_head), t = ld_volatile_u64(q_tail);
-        if (t > h) {
-          unsigned long long want = min((unsigned long long)__popc(need), t - h);
-          if (atomicCAS(q_head, h, h + want) == h) { got = (uint32_t)want; qbase = h; }
-        }
-      }
-      if (__shfl_sync(MCDC_FULL, abort_run, 0)) break;   // a queue overflow was flagged: the run is void, leave
-      got = __shfl_sync(MCDC_FULL, got, 0);
-      qbase = __shfl_sync(MCDC_FULL, qbase, 0);
-      if (!have && (uint32_t)__popc(need & lt_mask) < got) {
-        const unsigned long long i = qbase + (unsigned long long)__popc(need & lt_mask);
-        const uint32_t j = (uint32_t)i & A.q.mask;
-        const uint32_t expect = (uint32_t)(i + 1ull);
-        bool ready = true;
-        for (uint32_t spin = 0; ld_acquire_u32(A.q.flag + j) != expect; ++spin) {
-          if ((spin & 255u) == 255u && (*(volatile int *)&A.cnt->overflow || spin > (1u << 26))) {
-            atomicExch(&A.cnt->overflow, 1);             // producer gave up (overflow) or never published
-            ready = false;
-            break;
-          }
-        }
-        if (ready) {
-          p.x = A.q.x[j]; p.y = A.q.y[j]; p.z = A.q.z[j]; p.t = A.q.t[j]; p.w = A.q.w[j];
-          p.key = A.q.key[j];
-          const int4 m = A.q.meta[j];
-          p.cell = m.x; pk = m.y; p.hid = (uint32_t)m.z; it = m.w;
-          p.ctr = 0u;
-          slot = p.hid / A.hb;
-          fi = FI_CHILD;
-          have = true;
-        }
-      }
-      // (2) source histories
-      const unsigned need2 = __ballot_sync(MCDC_FULL, !have);
-      if (need2 != 0u && !src_done) {
-        const int leader = __ffs(need2) - 1;
-        uint32_t base = 0u;
-        if (lane == leader) base = atomicAdd(A.hist_cursor, (uint32_t)__popc(need2));
-        base = __shfl_sync(MCDC_FULL, base, leader);
-        if (base >= A.n_hist || base + (uint32_t)__popc(need2) >= A.n_hist) src_done = true;
-        if (!have) {
-          const uint32_t i = base + (uint32_t)__popc(need2 & lt_mask);
-          if (i < A.n_hist && base < A.n_hist) {
-            n_src += 1u;
-            p.hid = i;
-            slot = i / A.hb;
-            source_position(T, A.seed_mixed, A.first_history + i, p);
-            pk = census_index(tb, p.t);
-            it = 0;
-            fi = FI_SOURCE;
-            have = true;
-          }
-        }
-      }
-    }
-    if (__ballot_sync(MCDC_FULL, have) == 0u) {
-      if (!src_done) continue;
-      unsigned long long h = 0, t = 0;
-      if (lane == 0) { h = ld_volatile_u64(q_head); t = ld_volatile_u64(q_tail); }
-      h = __shfl_sync(MCDC_FULL, h, 0); t = __shfl_sync(MCDC_FULL, t, 0);
-      if (t <= h) break;
-      continue;
-    }
-
-    // ---------------- phase B: group / direction / cell of every flight that starts now ----------------
-    if (have && fi != FI_NONE) {
-      const bool ok = flight_init(tb, p, fi);
-      fi = FI_NONE;
-      if (!ok) { n_src_lost += 1u; have = false; }       // a source particle outside every cell (A.3)
-    }
-
-    // ---------------- phase C/D: one segment: distances, score, move ----------------
-    double d = 0.0, pos_star = 0.0;
-    int ev = -1, slot_star = -1, which = -1;
-    const double t_census = have ? tb.census(pk) : 0.0;
-    if (have) ev = find_event_typed(tb, p, t_census, d, slot_star, which, pos_star);
-    {
-      TallySink S;
-      S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
-      S.aggregate = A.aggregate;
-      if (T.score_fast) score_track_fast(tb, S, have, p, it, d);
-      else score_track(tb, S, have, p.x, p.y, p.z, p.ux, p.uy, p.uz, p.t, p.w, p.g, d);
-    }
-    // ---------------- phase E: the event ----------------
-    int n_push = 0, census_k = -1;
-    uint32_t c0 = 0u;
-    bool ended = false;                                  // the particle (as an identity) ended in this iteration
-    if (have) {
-      p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
-      p.t = (ev == EV_CENSUS) ? t_census : p.t + d * tb.inv_speed(p.g);
-      if (ev == EV_SURFACE) {
-        pc_surf += 1u;
-        have = surface_event_typed(tb, p, slot_star, which, pos_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid],
-                                   &acc.cnt[CNT_LOST][tid]);
-        ended = !have;
-      } else if (ev == EV_CENSUS) {                      // A.8: bookkeeping only, then the next interval
-        pc_census += 1u;
-        census_k = pk;
-        if (d > 0.0) p.last_surf = -1;
-        if (pk == T.K - 1) { acc.led[LED_CENSUS_FINAL][tid] += p.w; have = false; ended = true; }
-        else pk += 1;
-      } else {
-        pc_coll += 1u;
-        const int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
-                                      &acc.led[LED_PRODUCTION][tid]);
-        if (r == -1) fi = FI_SCATTER;
-        else {
-          ended = true;
-          have = r > 0;                                  // continues below as its first child
-          if (r > 0) { pc_child += (uint32_t)r; n_push = r - 1; }
-        }
-      }
-    }
-    // ---------------- census population (A.8), merged inside the warp ----------------
-    if (__ballot_sync(MCDC_FULL, census_k >= 0) != 0u) {
-      double v = p.w;
-      const bool absorbed = warp_merge_equal<int>(census_k, census_k >= 0, v, 4);
-      if (census_k >= 0) {
-        if (!absorbed) atomicAdd(s_popw + census_k, v);
-        atomicAdd(s_popn + census_k, 1u);
-      }
-    }
-    // ---------------- fission: publish children 1..n-1, become child 0 (A.6) ----------------
-    if (__ballot_sync(MCDC_FULL, n_push > 0) != 0u) {
-      int pre = n_push;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        int v = __shfl_up_sync(MCDC_FULL, pre, o);
-        if (lane >= o) pre += v;
-      }
-      const int total = __shfl_sync(MCDC_FULL, pre, 31);
-      unsigned long long base = 0ull;
-      int ok = 1;
-      if (lane == 0) {
-        base = atomicAdd(q_tail, (unsigned long long)total);
-        if (base + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) ok = 0;
-      }
-      base = __shfl_sync(MCDC_FULL, base, 0) + (unsigned long long)(pre - n_push);
-      ok = __shfl_sync(MCDC_FULL, ok, 0);
-      if (!ok && lane == 0) atomicExch(&A.cnt->overflow, 1);
-      if (n_push > 0 && ok) {
-        for (int c = 0; c < n_push; ++c) {
-          const uint32_t j = (uint32_t)(base + (unsigned long long)c) & A.q.mask;
-          A.q.x[j] = p.x; A.q.y[j] = p.y; A.q.z[j] = p.z; A.q.t[j] = p.t; A.q.w[j] = p.w;
-          A.q.key[j] = child_key(p.key, c0, (uint32_t)(c + 1));
-          A.q.meta[j] = make_int4(p.cell, pk, (int)p.hid, it);
-        }
-        __threadfence();
-        for (int c = 0; c < n_push; ++c) {
-          const unsigned long long i = base + (unsigned long long)c;
-          st_release_u32(A.q.flag + ((uint32_t)i & A.q.mask), (uint32_t)(i + 1ull));
-        }
-      }
-    }
-    if (ended) {
-      record_particle(acc, A.ev, p.hid, pc_coll, pc_surf, pc_child, pc_census);
-      pc_census = 0u;
-      if (have) {                                        // fission parent -> its first child, in place
-        p.key = child_key(p.key, c0, 0u);
-        p.ctr = 0u;
-        fi = FI_CHILD;
-      }
-    }
-  }
-
-  // ---- block totals ----
-  __syncthreads();
-  for (int k = tid; k < T.K; k += NT) {
-    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, s_popw[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
-  }
-  accum_flush(acc, A.cnt);
-  block_atomic_add(&A.cnt->ledger[0], (double)n_src, acc.scratch);
-  block_atomic_add(&A.cnt->ledger[6], (double)n_src_lost, acc.scratch);
-  block_atomic_add_u64(&A.cnt->n[0], (unsigned long long)n_src, (unsigned long long *)acc.scratch);
-  block_atomic_add_u64(&A.cnt->n[6], (unsigned long long)n_src_lost, (unsigned long long *)acc.scratch);
 }
 
 // ------------------------------------------------------------------------------------------------

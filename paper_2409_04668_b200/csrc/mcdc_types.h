@@ -56,11 +56,14 @@ struct Tables {
   uint32_t o_nb_cell;
   uint32_t o_loc_off;   // [nvox+1] source locator grid
   uint32_t o_loc_cell;
-  uint32_t o_cell_rec;  // [C] typed cell records, CELL_REC_BYTES each (layout below)
-  uint32_t o_other;     // overflow list of "other" half-space slots (cells with more than two)
+  uint32_t o_cell2;     // [C] compact cell records, CELL2_BYTES each (layout below)
+  uint32_t o_other2;    // "other" half-space entries, OTHER2_BYTES each
+  uint32_t o_tbin_k;    // [K] int: the one time bin that holds census interval k, -1 if it spans several
+  uint32_t o_it0_k;     // [K] int: time bin at the start of census interval k (hint of the general scorer)
   uint32_t o_surf_coef; // [S][10] general form (inside the hot prefix only when a general quadric exists)
   const Tables *self_dev;  // device-memory copy of this struct (slow paths that must not take the parameter's address)
   int score_fast;       // the tally mesh covers the geometry and the time grid covers [t0, C_K]: no clipping needed
+  int warp_ok;          // the problem fits the compact tables of k_warp (16-bit surface / cell ids, ...)
   // source
   double src_lo[3], src_hi[3], src_t0, src_t1;
   int src_last;
@@ -74,17 +77,23 @@ struct Tables {
   unsigned long long n_bins;
 };
 
-// Typed cell record (built at mcdc_problem_create): the tightest axis-aligned plane of each (axis, side) is a
-// "face"; every other half-space of the cell (cylinders, general quadrics, redundant planes) is an "other".
-//   +0  double bound[6]   [2a] = lower plane position on axis a (-inf if none), [2a+1] = upper (+inf)
-//   +48 int    face[6]    half-space slot (index into o_hs) of that face, -1 if none
-//   +72 int    n_other
-//   +76 int    other_off  index into o_other of the cell's full "other" slot list
-//   +80 int    other0, other1   the first two "other" slots (copies)
-//   +88 int    material
-//   +92 int    pad[3]
-constexpr uint32_t CELL_REC_BYTES = 104;   // 26 words: odd multiple of 8 bytes, spreads cells over the banks
-constexpr uint32_t CR_BOUND = 0, CR_FACE = 48, CR_N_OTHER = 72, CR_OTHER_OFF = 76, CR_OTHER0 = 80, CR_MAT = 88;
+// Compact hot tables of the warp-pool kernel k_warp (built at mcdc_problem_create, staged in shared memory).
+//
+// Cell record, CELL2_BYTES = 40, ten 32-bit words.  The tightest axis-aligned plane of each (axis, side) is a "face"
+// f = 2*axis + side (side 0 = lower bound); every other half-space of the cell (cylinders, general quadrics,
+// redundant planes) is an "other".
+//   +0  u16 face_surf[6]  surface id of the face (plane position = surf_q[s].x), NONE16 if the cell is unbounded there
+//   +12 u16 face_nb[6]    certified neighbour cell across the face (see mcdc_host.cu "certificates"), NONE16 = search
+//   +24 u8  face_idx[6]   position of the face's half-space in the cell's list (tie-break D5, generic look-ups)
+//   +30 u16 face_bc       2 bits per face: boundary condition of the face's surface
+//   +32 u8 n_other, u8 material, u16 other_off (first entry of the cell in the other table)
+//   +36 u32 cell_bin      spatial tally bin that contains the whole cell, NONE32 if it spans several bins
+// Other entry, OTHER2_BYTES = 8:
+//   +0  u16 surface, u16 nb (certified neighbour across it or NONE16)
+//   +4  u8 idx (position in the cell's half-space list), u8 flags = sense>0 | type<<1 | bc<<4, u16 pad
+constexpr uint32_t CELL2_BYTES = 40, OTHER2_BYTES = 8;
+constexpr uint32_t C2_FACE_SURF = 0, C2_FACE_NB = 12, C2_FACE_IDX = 24, C2_FACE_BC = 30, C2_INFO = 32, C2_BIN = 36;
+constexpr uint32_t NONE16 = 0xFFFFu, NONE32 = 0xFFFFFFFFu;
 
 // Per-launch parameters of the transport kernel.
 struct StepParams {

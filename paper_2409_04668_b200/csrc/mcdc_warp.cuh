@@ -1,0 +1,557 @@
+// mcdc_warp.cuh -- k_warp: the event-based history kernel (default scheduler, MCDC_SCHED_ASYNC).
+//
+// Replaces the paper's Harmonize runtime ("segregating them into like-operations ... executed
+// together in batches") with an ON-CHIP, PER-WARP event scheduler.  Every warp owns a pool of W particles in shared
+// memory (structure of arrays) and three index stacks -- F (needs a flight), C (collided), FREE -- that it edits
+// with ballots only: no atomics, no block barriers, warps never wait for one another.  Each round the warp picks
+// the stack that fills all 32 lanes and runs ONE kind of work on it:
+//   R  refill   free slots take fission children from the global ring queue, then new source histories (A.3, A.6)
+//   F  flight   distances, event choice, track-length score, move (A.2, A.4, A.7); census bookkeeping (A.8) and
+//               the surface event (A.5) are finished in the same round -- with a certified neighbour a crossing
+//               is a table look-up
+//   C  collide  reaction choice, scattering or fission (A.6); a fission parent continues as its first child,
+//               the other children go to the global queue
+// Particle records never travel through HBM; only the fission queue, the batch accumulators (fp64 RED) and the
+// counters do.  Trajectories depend on (seed, history id, lineage) alone, so the processing order is free
+// (DESIGN.md section 5).  Analog transport: every weight is 1 and is not stored.
+#pragma once
+#include "mcdc_kernels.cuh"
+
+namespace mcdc {
+
+// ---- slow paths: rare, not inlined, and they read the tables from global memory (device copy of Tables) ----
+
+// A.5 transmission without a certified neighbour: candidate cells of half-space `idx` of `cell`, then every cell
+__device__ __noinline__ int slow_cross(const Tables *gT, int cell, int idx, int s_star, double x, double y, double z,
+                                       double ux, double uy, double uz) {
+  const TB<false> tb(*gT);
+  const int slot = tb.cell_off(cell) + idx;
+  return locate_neighbour(tb, slot, s_star, x, y, z, ux, uy, uz);
+}
+// A.5 reflection off a surface that is not an axis-aligned plane
+__device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, double x, double y, double z, double *u) {
+  const TB<false> tb(*gT);
+  reflect(tb, s, type, x, y, z, u[0], u[1], u[2]);
+}
+// A.3 cell of a source particle
+__device__ __noinline__ int slow_locate_source(const Tables *gT, double x, double y, double z, double ux, double uy,
+                                               double uz) {
+  const TB<false> tb(*gT);
+  return locate_source(tb, x, y, z, ux, uy, uz);
+}
+// A.4 distance to a surface that is neither an axis-aligned plane face nor a z-cylinder
+__device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, bool on, double x, double y, double z,
+                                             double ux, double uy, double uz) {
+  const TB<false> tb(*gT);
+  return surf_distance(tb, s, type, on, x, y, z, ux, uy, uz, 1.0 / ux, 1.0 / uy, 1.0 / uz);
+}
+
+__device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
+
+// bytes of shared memory per pool slot: x y z ux uy uz t (7 x f64), key, ctr, cell|last, meta, 3 stack entries
+__host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record) { return 7 * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0); }
+
+struct WarpShared {                // block-wide totals (static shared memory)
+  double led[LED_N];
+  unsigned long long n_coll, n_surf, n_census, n_children, n_lost, n_src;
+};
+
+template <bool STAGED, bool RECORD, int NT>
+__global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
+  constexpr int NW = NT / 32;
+  const double INF = CUDART_INF;
+  __shared__ WarpShared sh;
+  const TB<STAGED> tb(T);
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const uint32_t W = A.pool_slots;                    // slots per warp
+  const uint32_t N = W * (uint32_t)NW;
+  // ---- carve the dynamic shared memory: [staged tables][census populations][pool arrays][stacks] ----
+  unsigned char *base = g_smem + A.smem_tables;
+  uint32_t *s_popn = reinterpret_cast<uint32_t *>(base); base += ((size_t)T.K * 4 + 15) / 16 * 16;
+  double *px = reinterpret_cast<double *>(base), *py = px + N, *pz = py + N, *pux = pz + N, *puy = pux + N, *puz = puy + N,
+         *pt = puz + N;
+  unsigned long long *pkey = reinterpret_cast<unsigned long long *>(pt + N);
+  uint32_t *pctr = reinterpret_cast<uint32_t *>(pkey + N), *pcl = pctr + N, *pmeta = pcl + N;
+  uint32_t *phid = pmeta + N;                          // only when RECORD
+  uint8_t *LF = reinterpret_cast<uint8_t *>(RECORD ? phid + N : phid), *LC = LF + N, *LFREE = LC + N;
+
+  if (STAGED) {
+    const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
+    uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
+    for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
+  }
+  for (int k = tid; k < T.K; k += NT) s_popn[k] = 0u;
+  if (tid == 0) {
+    for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
+    sh.n_coll = sh.n_surf = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
+  }
+  const uint32_t lb = (uint32_t)wid * W;               // first slot of this warp
+  for (uint32_t i = lane; i < W; i += 32) LFREE[lb + i] = (uint8_t)(W - 1u - i);
+  __syncthreads();
+
+  unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
+  const unsigned long long q_cap = (unsigned long long)A.q.mask + 1ull;
+  const Tables *gT = T.self_dev;
+  const int G = T.G;
+  const long long n_spatial = (long long)T.mesh_n[0] * T.mesh_n[1] * T.mesh_n[2];
+  // warp-uniform scheduler state
+  uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
+  uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
+  bool src_exhausted = false;
+  uint32_t c_coll = 0u, c_surf = 0u, c_census = 0u, c_children = 0u, c_lost = 0u, c_src = 0u;
+
+  for (;;) {
+    int phase;                                         // 0 = R, 1 = F, 2 = C
+    if (nF >= 32u) phase = 1;
+    else if (nC >= 32u) phase = 2;
+    else if (nFree > 0u && dry == 0u) phase = 0;
+    else if (nF > 0u && nF >= nC) phase = 1;
+    else if (nC > 0u) phase = 2;
+    else phase = 0;
+    if (dry) --dry;
+
+    if (phase == 0) {
+      // =============== R: acquire work for up to 32 free slots, initialise the new particles (A.3, A.6) ===============
+      const uint32_t want = min(32u, nFree);
+      // source histories come from the warp's own chunk of the sub-batch; one global atomic per chunk
+      if (src_next == src_end && !src_exhausted) {
+        uint32_t cb = 0u;
+        if (lane == 0) cb = atomicAdd(A.hist_cursor, A.src_chunk);
+        cb = __shfl_sync(MCDC_FULL, cb, 0);
+        if (cb >= A.n_hist) src_exhausted = true;
+        else { src_next = cb; src_end = min(cb + A.src_chunk, A.n_hist); }
+      }
+      const uint32_t n_src = min(want, src_end - src_next), src_base = src_next;
+      src_next += n_src;
+      const bool src_done = src_exhausted && src_next == src_end;
+      // the global queue only holds children that did not fit their parent's pool: look at it when this warp has
+      // no source left, and now and then otherwise
+      uint32_t got = 0u;
+      unsigned long long qbase = 0ull;
+      int flags = 0;                                   // 1 = abort (overflow flagged), 4 = queue empty
+      if (n_src < want && (src_done || (r_calls & 15u) == 0u)) {
+        if (lane == 0) {
+          if (*(volatile int *)&A.cnt->overflow) flags |= 1;
+          const unsigned long long h = ld_volatile_u64(q_head), t = ld_volatile_u64(q_tail);
+          if (t > h) {
+            const unsigned long long w = min((unsigned long long)(want - n_src), t - h);
+            if (atomicCAS(q_head, h, h + w) == h) { got = (uint32_t)w; qbase = h; }
+          } else flags |= 4;
+        }
+        flags = __shfl_sync(MCDC_FULL, flags, 0);
+        got = __shfl_sync(MCDC_FULL, got, 0);
+        qbase = __shfl_sync(MCDC_FULL, qbase, 0);
+      }
+      ++r_calls;
+      if (flags & 1) break;                            // a queue overflow was flagged somewhere: the run is void
+      const uint32_t total = got + n_src;
+      if (total == 0u) {
+        if (nF == 0u && nC == 0u) {
+          if (src_done && (flags & 4)) break;          // pool empty, no source left, queue empty
+          __nanosleep(256);
+        } else dry = 8u;                               // nothing to take right now: work on what the pool holds
+        continue;
+      }
+      const bool act = (uint32_t)lane < total;
+      const uint32_t i = act ? (uint32_t)LFREE[lb + nFree - 1u - (uint32_t)lane] : 0u;
+      nFree -= total;
+      double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
+      unsigned long long key = 0ull;
+      uint32_t ctr = 0u, hid = 0u, slot = 0u;
+      int cell = 0, pk = 0;
+      bool ok = act, is_src = false;
+      if (act && (uint32_t)lane >= n_src) {            // a fission child from the global queue (A.6)
+        const unsigned long long qi = qbase + (unsigned long long)((uint32_t)lane - n_src);
+        const uint32_t j = (uint32_t)qi & A.q.mask;
+        const uint32_t expect = (uint32_t)(qi + 1ull);
+        for (uint32_t spin = 0; ld_acquire_u32(A.q.flag + j) != expect; ++spin) {
+          if ((spin & 255u) == 255u && (*(volatile int *)&A.cnt->overflow || spin > (1u << 26))) {
+            atomicExch(&A.cnt->overflow, 1);           // producer gave up (overflow) or never published
+            ok = false;
+            break;
+          }
+        }
+        x = A.q.x[j]; y = A.q.y[j]; z = A.q.z[j]; t = A.q.t[j];
+        key = A.q.key[j];
+        const int4 m = A.q.meta[j];
+        cell = ok ? m.x : 0; pk = m.y; hid = (uint32_t)m.z; slot = (uint32_t)m.w;
+      } else if (act) {                                // a new source history (A.3): xi_x, xi_y, xi_z, xi_t
+        is_src = true;
+        hid = src_base + (uint32_t)lane;
+        slot = hid / A.hb;
+        key = mix64(A.seed_mixed ^ (A.first_history + (unsigned long long)hid));
+        double xi_x, xi_y, xi_z, xi_t;
+        draw2(key, ctr, xi_x, xi_y);
+        draw2(key, ctr, xi_z, xi_t);
+        x = T.src_lo[0] + xi_x * (T.src_hi[0] - T.src_lo[0]);
+        y = T.src_lo[1] + xi_y * (T.src_hi[1] - T.src_lo[1]);
+        z = T.src_lo[2] + xi_z * (T.src_hi[2] - T.src_lo[2]);
+        t = T.src_t0 + xi_t * (T.src_t1 - T.src_t0);
+        pk = census_index(tb, t);
+      }
+      // group: chi of the fission-site material (child) or the source pdf; then the direction
+      const double xi_g = draw(key, ctr);
+      int g;
+      if (is_src) g = sample_cdf([&](int q) { return tb.src_cdf(q); }, G, T.src_last, xi_g);
+      else {
+        const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
+        g = sample_cdf([&](int q) { return tb.cdf_chi(mat * G + q); }, G, tb.last_chi(mat), xi_g);
+      }
+      double ux, uy, uz;
+      if (is_src && T.src_dir_mode != 0) { ux = T.src_dir[0]; uy = T.src_dir[1]; uz = T.src_dir[2]; }
+      else {
+        double xi_mu, xi_phi;
+        draw2(key, ctr, xi_mu, xi_phi);
+        isotropic(xi_mu, xi_phi, ux, uy, uz);
+      }
+      if (is_src) {
+        cell = slow_locate_source(gT, x, y, z, ux, uy, uz);
+        if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
+      }
+      const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0);
+      if (m_lost) { c_lost += (uint32_t)__popc(m_lost); if (lane == 0) atomicAdd(&sh.led[LED_LOST], (double)__popc(m_lost)); }
+      c_src += n_src;
+      if (ok) {
+        const uint32_t gi = lb + i;
+        px[gi] = x; py[gi] = y; pz[gi] = z; pux[gi] = ux; puy[gi] = uy; puz[gi] = uz; pt[gi] = t;
+        pkey[gi] = key; pctr[gi] = ctr; pcl[gi] = (uint32_t)cell | (NONE16 << 16);
+        pmeta[gi] = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
+        if (RECORD) phid[gi] = hid;
+      }
+      const unsigned m_ok = __ballot_sync(MCDC_FULL, ok), m_bad = __ballot_sync(MCDC_FULL, act && !ok);
+      if (ok) LF[lb + nF + lanes_below(m_ok, lane)] = (uint8_t)i;
+      nF += (uint32_t)__popc(m_ok);
+      if (act && !ok) LFREE[lb + nFree + lanes_below(m_bad, lane)] = (uint8_t)i;
+      nFree += (uint32_t)__popc(m_bad);
+      __syncwarp();
+      continue;
+    }
+
+    if (phase == 1) {
+      // =============== F: one segment -- distances, event choice, score, move, census / surface event ===============
+      const uint32_t n = min(32u, nF);
+      nF -= n;
+      const bool act = (uint32_t)lane < n;
+      const uint32_t i = act ? (uint32_t)LF[lb + nF + (uint32_t)lane] : 0u;
+      const uint32_t gi = lb + i;
+      double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, t = 0.0;
+      unsigned long long key = 0ull;
+      uint32_t ctr = 0u, cl = NONE16 << 16, meta = 0u;
+      if (act) {
+        x = px[gi]; y = py[gi]; z = pz[gi]; ux = pux[gi]; uy = puy[gi]; uz = puz[gi]; t = pt[gi];
+        key = pkey[gi]; ctr = pctr[gi]; cl = pcl[gi]; meta = pmeta[gi];
+      }
+      const int cell = (int)(cl & 0xFFFFu), g = (int)(meta & 255u), pk = (int)((meta >> 8) & 4095u);
+      const uint32_t last = cl >> 16;                  // surface the particle sits on, NONE16 if none
+      const double ix = 1.0 / ux, iy = 1.0 / uy, iz = 1.0 / uz;
+      const uint32_t rec = T.o_cell2 + (uint32_t)cell * CELL2_BYTES;
+      const uint32_t info = tb.template ldb<uint32_t>(rec + C2_INFO);
+      const int n_other = (int)(info & 255u), mg = (int)((info >> 8) & 255u) * G + g;
+      const double xi = draw(key, ctr);                // always consumed (D3)
+      const double sig_t = tb.sig_t(mg);
+      const double d_coll = (sig_t > 0.0) ? -log(xi) * tb.inv_sig_t(mg) : INF;
+      // ---- faces: one candidate per axis, picked by the sign of the direction component ----
+      const int fx = (ux > 0.0) ? 1 : 0, fy = (uy > 0.0) ? 3 : 2, fz = (uz > 0.0) ? 5 : 4;
+      const uint32_t sfx = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fx);
+      const uint32_t sfy = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fy);
+      const uint32_t sfz = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fz);
+      const double bx = (sfx == NONE16) ? ((ux > 0.0) ? INF : -INF) : tb.surf_q0((int)sfx);
+      const double by = (sfy == NONE16) ? ((uy > 0.0) ? INF : -INF) : tb.surf_q0((int)sfy);
+      const double bz = (sfz == NONE16) ? ((uz > 0.0) ? INF : -INF) : tb.surf_q0((int)sfz);
+      const double dx = (bx - x) * ix, dy = (by - y) * iy, dz = (bz - z) * iz;   // 0 * inf = NaN: rejected below
+      double d_surf = INF;
+      int which = -1;                                  // 2*axis + side of the nearest face, 6 + j for other j
+      if (dx > 0.0 && dx < INF) { d_surf = dx; which = fx; }
+      if (dy > 0.0 && dy <= d_surf && dy < INF) {
+        // equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
+        if (dy < d_surf || tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fy) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which)) {
+          d_surf = dy; which = fy;
+        }
+      }
+      if (dz > 0.0 && dz <= d_surf && dz < INF) {
+        if (dz < d_surf || tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fz) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which)) {
+          d_surf = dz; which = fz;
+        }
+      }
+      // ---- other half-spaces (cylinders, general quadrics, redundant planes), list order, strict < ----
+      const uint32_t orec = T.o_other2 + (info >> 16) * OTHER2_BYTES;
+      for (int j = 0; j < n_other; ++j) {
+        const uint2 e = tb.template ldb<uint2>(orec + (uint32_t)j * OTHER2_BYTES);
+        const uint32_t s = e.x & 0xFFFFu;
+        const int type = (int)((e.y >> 9) & 7u);
+        double u;
+        if (type == ST_CYL_Z) {
+          const double2 q01 = tb.surf_q01((int)s);
+          const double r2 = tb.surf_q23((int)s).x;
+          const double ex = x - q01.x, ey = y - q01.y;
+          u = quad_root_pos_a(ux * ux + uy * uy, ex * ux + ey * uy, (s == last) ? 0.0 : (ex * ex + ey * ey - r2));
+        } else {
+          u = slow_distance(gT, (int)s, type, s == last, x, y, z, ux, uy, uz);
+        }
+        if (u < d_surf) { d_surf = u; which = 6 + j; }
+      }
+      const double t_census = tb.census(pk);
+      const double d_time = tb.speed(g) * (t_census - t);
+      int ev;
+      double d;
+      if (d_time <= d_surf && d_time <= d_coll) { d = d_time; ev = EV_CENSUS; }
+      else if (d_surf <= d_coll) { d = d_surf; ev = EV_SURFACE; }
+      else { d = d_coll; ev = EV_COLLISION; }
+      if (!act) { ev = -1; d = 0.0; }
+
+      // ---- track-length score (A.7) from the pre-move state ----
+      {
+        const uint32_t slot = meta >> 20;
+        TallySink S;
+        S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
+        S.aggregate = A.aggregate;
+        const uint32_t cbin = tb.template ldb<uint32_t>(rec + C2_BIN);
+        const int tbin = tb.template ld<int>(T.o_tbin_k, pk);
+        const bool one_bin = cbin != NONE32 && tbin >= 0;      // the whole segment lies in one tally bin
+        if (__any_sync(MCDC_FULL, act && !one_bin)) {
+          PState p;
+          p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = 1.0;
+          p.key = 0ull; p.ctr = 0u; p.hid = 0u; p.g = g; p.cell = cell; p.last_surf = -1;
+          int it = tb.template ld<int>(T.o_it0_k, pk);
+          if (T.score_fast) score_track_fast(tb, S, act && !one_bin, p, it, d);
+          else score_track(tb, S, act && !one_bin, x, y, z, ux, uy, uz, t, 1.0, g, d);
+        }
+        if (__any_sync(MCDC_FULL, act && one_bin)) {
+          const bool sc = act && one_bin && d > 0.0;
+          const long long bin = sc ? (long long)(tbin * G + g) * n_spatial + (long long)cbin : -1;
+          tally_add_converged(S, bin, d);
+        }
+      }
+      // ---- move (A.3) ----
+      x += d * ux; y += d * uy; z += d * uz;
+      t = (ev == EV_CENSUS) ? t_census : t + d * tb.inv_speed(g);
+      bool alive = act, lost = false;
+      uint32_t new_cl = cl;
+      int census_k = -1;
+      if (ev == EV_CENSUS) {                           // A.8: bookkeeping only, then the next interval
+        census_k = pk;
+        if (d > 0.0) new_cl = (cl & 0xFFFFu) | (NONE16 << 16);
+        if (pk == T.K - 1) alive = false;
+        else meta += 1u << 8;
+      } else if (ev == EV_SURFACE) {                   // A.5
+        uint32_t s_star, nb;
+        int bc, type, idx;
+        if (which < 6) {
+          s_star = (which == fx) ? sfx : ((which == fy) ? sfy : sfz);
+          nb = tb.template ldb<uint16_t>(rec + C2_FACE_NB + 2u * which);
+          bc = (int)((tb.template ldb<uint16_t>(rec + C2_FACE_BC) >> (2 * which)) & 3u);
+          type = which >> 1;                           // ST_PLANE_X/Y/Z
+          idx = -1;
+        } else {
+          const uint2 e = tb.template ldb<uint2>(orec + (uint32_t)(which - 6) * OTHER2_BYTES);
+          s_star = e.x & 0xFFFFu; nb = e.x >> 16;
+          idx = (int)(e.y & 255u); type = (int)((e.y >> 9) & 7u); bc = (int)((e.y >> 12) & 3u);
+        }
+        new_cl = (cl & 0xFFFFu) | (s_star << 16);
+        if (bc == 1) {                                 // vacuum: leaks
+          alive = false;
+          atomicAdd(&sh.led[LED_LEAK], 1.0);
+        } else if (bc == 2) {                          // reflective: specular, stays in the cell
+          if (type == ST_PLANE_X) ux = -ux;
+          else if (type == ST_PLANE_Y) uy = -uy;
+          else if (type == ST_PLANE_Z) uz = -uz;
+          else { double u3[3] = {ux, uy, uz}; slow_reflect(gT, (int)s_star, type, x, y, z, u3); ux = u3[0]; uy = u3[1]; uz = u3[2]; }
+          pux[gi] = ux; puy[gi] = uy; puz[gi] = uz;
+        } else {                                       // transmission: the cell on the other side
+          // a certified neighbour holds every point of this surface patch that lies strictly inside the cell's
+          // forward faces (mcdc_host.cu); anything else takes the full search of A.5
+          const int ax = (which < 6) ? (which >> 1) : -1;
+          const bool in_x = ax == 0 || ((ux > 0.0) ? (x < bx) : ((ux < 0.0) ? (x > bx) : true));
+          const bool in_y = ax == 1 || ((uy > 0.0) ? (y < by) : ((uy < 0.0) ? (y > by) : true));
+          const bool in_z = ax == 2 || ((uz > 0.0) ? (z < bz) : ((uz < 0.0) ? (z > bz) : true));
+          int c2;
+          if (nb != NONE16 && in_x && in_y && in_z) c2 = (int)nb;
+          else {
+            if (idx < 0) idx = (int)tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
+            c2 = slow_cross(gT, cell, idx, (int)s_star, x, y, z, ux, uy, uz);
+          }
+          if (c2 < 0) { alive = false; lost = true; atomicAdd(&sh.led[LED_LOST], 1.0); }
+          else new_cl = (uint32_t)c2 | (s_star << 16);
+        }
+      }
+      if (act) {
+        px[gi] = x; py[gi] = y; pz[gi] = z; pt[gi] = t; pctr[gi] = ctr;
+        if (new_cl != cl) pcl[gi] = new_cl;
+        if (ev == EV_CENSUS) pmeta[gi] = meta;
+        if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)phid[gi] * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
+      }
+      // ---- census population (A.8): one shared-memory add per distinct census index in the warp ----
+      const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
+      if (m_cen) {
+        const unsigned peers = __match_any_sync(MCDC_FULL, census_k);
+        if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
+        c_census += (uint32_t)__popc(m_cen);
+        const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
+        if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
+      }
+      {
+        const unsigned m_s = __ballot_sync(MCDC_FULL, ev == EV_SURFACE), m_lost = __ballot_sync(MCDC_FULL, lost);
+        c_surf += (uint32_t)__popc(m_s);
+        c_lost += (uint32_t)__popc(m_lost);
+      }
+      // ---- hand the slots on: F again, C, or FREE ----
+      const bool toF = alive && ev != EV_COLLISION, toC = alive && ev == EV_COLLISION, dead = act && !alive;
+      const unsigned mF = __ballot_sync(MCDC_FULL, toF), mC = __ballot_sync(MCDC_FULL, toC), mD = __ballot_sync(MCDC_FULL, dead);
+      if (toF) LF[lb + nF + lanes_below(mF, lane)] = (uint8_t)i;
+      if (toC) LC[lb + nC + lanes_below(mC, lane)] = (uint8_t)i;
+      if (dead) LFREE[lb + nFree + lanes_below(mD, lane)] = (uint8_t)i;
+      nF += (uint32_t)__popc(mF); nC += (uint32_t)__popc(mC); nFree += (uint32_t)__popc(mD);
+      __syncwarp();
+      continue;
+    }
+
+    // =============== C: collisions (A.6) ===============
+    {
+      const uint32_t n = min(32u, nC);
+      nC -= n;
+      const bool act = (uint32_t)lane < n;
+      const uint32_t i = act ? (uint32_t)LC[lb + nC + (uint32_t)lane] : 0u;
+      const uint32_t gi = lb + i;
+      unsigned long long key = 0ull;
+      uint32_t ctr = 0u, cl = 0u, meta = 0u;
+      if (act) { key = pkey[gi]; ctr = pctr[gi]; cl = pcl[gi]; meta = pmeta[gi]; }
+      const int cell = (int)(cl & 0xFFFFu);
+      int g = (int)(meta & 255u);
+      const bool born = g == 255;                      // a fission child placed in this pool: only its flight is sampled
+      if (born) g = 0;
+      const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
+      const int mg = mat * G + g;
+      // reaction: scatter, capture, fission in this order (D6)
+      const double yv = draw(key, ctr) * tb.sig_t(mg);
+      if (born) ctr = 0u;                              // nothing drawn yet from a new child's stream
+      int kind = FI_NONE, n_child = 0;                 // kind of the outgoing flight; children of a fission
+      bool alive = false, captured = false, fissioned = false;
+      uint32_t c0 = 0u;
+      if (born) { kind = FI_CHILD; alive = true; }
+      else if (act) {
+        if (yv < tb.sig_s_tot(mg)) { kind = FI_SCATTER; alive = true; }
+        else if (yv < tb.sig_sc(mg) || tb.sig_f(mg) == 0.0) captured = true;
+        else {
+          const double xi_nu = draw(key, ctr);
+          n_child = (int)floor(tb.nu(mg) + xi_nu);
+          c0 = ctr;
+          fissioned = true;
+          if (n_child > 0) { kind = FI_CHILD; alive = true; }
+        }
+      }
+      {
+        const unsigned m_cap = __ballot_sync(MCDC_FULL, captured), m_fis = __ballot_sync(MCDC_FULL, fissioned);
+        if (lane == 0 && m_cap) atomicAdd(&sh.led[LED_CAPTURE], (double)__popc(m_cap));
+        if (m_fis) {
+          const uint32_t kids = __reduce_add_sync(MCDC_FULL, (uint32_t)n_child);
+          if (lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], (double)__popc(m_fis)); atomicAdd(&sh.led[LED_PRODUCTION], (double)kids); }
+          c_children += kids;
+        }
+        c_coll += (uint32_t)__popc(__ballot_sync(MCDC_FULL, act && !born));
+      }
+      if (RECORD && act && !born) {
+        atomicAdd(A.ev + (size_t)phid[gi] * 4 + 0, 1u);
+        if (n_child > 0) atomicAdd(A.ev + (size_t)phid[gi] * 4 + 2, (uint32_t)n_child);
+      }
+      // fission: publish children 1..n-1 to the global queue, continue as child 0
+      const int n_push = (n_child > 1) ? n_child - 1 : 0;
+      if (__ballot_sync(MCDC_FULL, n_push > 0) != 0u) {
+        int pre = n_push;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+          const int v = __shfl_up_sync(MCDC_FULL, pre, o);
+          if (lane >= o) pre += v;
+        }
+        const int total = __shfl_sync(MCDC_FULL, pre, 31);
+        if ((uint32_t)total <= nFree) {                // the children fit this warp's pool: they join its C stack
+          if (n_push > 0) {
+            const double x = px[gi], y = py[gi], z = pz[gi], t = pt[gi];
+            for (int c = 0; c < n_push; ++c) {
+              const uint32_t r = (uint32_t)(pre - n_push + c);
+              const uint32_t i2 = (uint32_t)LFREE[lb + nFree - 1u - r], g2 = lb + i2;
+              px[g2] = x; py[g2] = y; pz[g2] = z; pt[g2] = t;
+              pkey[g2] = child_key(key, c0, (uint32_t)(c + 1)); pctr[g2] = 0u;
+              pcl[g2] = (cl & 0xFFFFu) | (NONE16 << 16);
+              pmeta[g2] = (meta & ~255u) | 255u;
+              if (RECORD) phid[g2] = phid[gi];
+              LC[lb + nC + r] = (uint8_t)i2;
+            }
+          }
+          nFree -= (uint32_t)total; nC += (uint32_t)total;
+        } else {                                       // pool full: publish them to the global queue
+          unsigned long long qb = 0ull;
+          int okq = 1;
+          if (lane == 0) {
+            qb = atomicAdd(q_tail, (unsigned long long)total);
+            if (qb + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) okq = 0;
+          }
+          qb = __shfl_sync(MCDC_FULL, qb, 0) + (unsigned long long)(pre - n_push);
+          okq = __shfl_sync(MCDC_FULL, okq, 0);
+          if (!okq && lane == 0) atomicExch(&A.cnt->overflow, 1);
+          if (n_push > 0 && okq) {
+            const double x = px[gi], y = py[gi], z = pz[gi], t = pt[gi];
+            const int4 qm = make_int4(cell, (int)((meta >> 8) & 4095u), RECORD ? (int)phid[gi] : 0, (int)(meta >> 20));
+            for (int c = 0; c < n_push; ++c) {
+              const uint32_t j = (uint32_t)(qb + (unsigned long long)c) & A.q.mask;
+              A.q.x[j] = x; A.q.y[j] = y; A.q.z[j] = z; A.q.t[j] = t;
+              A.q.key[j] = child_key(key, c0, (uint32_t)(c + 1));
+              A.q.meta[j] = qm;
+            }
+            __threadfence();
+            for (int c = 0; c < n_push; ++c) {
+              const unsigned long long qi = qb + (unsigned long long)c;
+              st_release_u32(A.q.flag + ((uint32_t)qi & A.q.mask), (uint32_t)(qi + 1ull));
+            }
+          }
+        }
+      }
+      if (fissioned && n_child > 0) { key = child_key(key, c0, 0u); ctr = 0u; }   // fission parent -> its first child, in place
+      // group and direction of the outgoing flight (A.6): one draw for the group, two for the direction
+      if (__any_sync(MCDC_FULL, alive)) {
+        const double xi_g = draw(key, ctr);
+        if (kind == FI_SCATTER) g = sample_cdf([&](int q) { return tb.cdf_s(mg * G + q); }, G, tb.last_s(mg), xi_g * tb.sig_s_tot(mg));
+        else g = sample_cdf([&](int q) { return tb.cdf_chi(mat * G + q); }, G, tb.last_chi(mat), xi_g);
+        double xi_mu, xi_phi, ux, uy, uz;
+        draw2(key, ctr, xi_mu, xi_phi);
+        isotropic(xi_mu, xi_phi, ux, uy, uz);
+        if (alive) {
+          pux[gi] = ux; puy[gi] = uy; puz[gi] = uz;
+          pkey[gi] = key; pctr[gi] = ctr;
+          pmeta[gi] = (meta & ~255u) | (uint32_t)g;
+          pcl[gi] = (cl & 0xFFFFu) | (NONE16 << 16);
+        }
+      }
+      const unsigned mF = __ballot_sync(MCDC_FULL, alive), mD = __ballot_sync(MCDC_FULL, act && !alive);
+      if (alive) LF[lb + nF + lanes_below(mF, lane)] = (uint8_t)i;
+      if (act && !alive) LFREE[lb + nFree + lanes_below(mD, lane)] = (uint8_t)i;
+      nF += (uint32_t)__popc(mF); nFree += (uint32_t)__popc(mD);
+      __syncwarp();
+    }
+  }
+
+  // ---- warp totals -> block totals -> global ----
+  if (lane == 0) {
+    atomicAdd(&sh.n_coll, (unsigned long long)c_coll); atomicAdd(&sh.n_surf, (unsigned long long)c_surf);
+    atomicAdd(&sh.n_census, (unsigned long long)c_census); atomicAdd(&sh.n_children, (unsigned long long)c_children);
+    atomicAdd(&sh.n_lost, (unsigned long long)c_lost); atomicAdd(&sh.n_src, (unsigned long long)c_src);
+  }
+  __syncthreads();
+  for (int k = tid; k < T.K; k += NT) {
+    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
+  }
+  if (tid == 0) {
+    DevCounters *cnt = A.cnt;
+    for (int e = 0; e < LED_N; ++e)
+      if (sh.led[e] != 0.0) atomicAdd(&cnt->ledger[1 + e], sh.led[e]);
+    atomicAdd(&cnt->ledger[0], (double)sh.n_src);
+    atomicAdd(&cnt->n[0], sh.n_src);
+    atomicAdd(&cnt->n[1], sh.n_coll + sh.n_surf + sh.n_census);
+    atomicAdd(&cnt->n[2], sh.n_coll);
+    atomicAdd(&cnt->n[3], sh.n_surf);
+    atomicAdd(&cnt->n[4], sh.n_census);
+    atomicAdd(&cnt->n[5], sh.n_children);
+    atomicAdd(&cnt->n[6], sh.n_lost);
+  }
+}
+
+}  // namespace mcdc
