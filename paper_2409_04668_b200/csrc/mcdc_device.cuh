@@ -187,21 +187,13 @@ __device__ __forceinline__ double quad_root(double a, double k, double c) {
 //   c == 0 (on the surface): roots 0 and -2k/a.
 __device__ __forceinline__ double quad_root_pos_a(double a, double k, double c) {
   const double INF = CUDART_INF;
-  if (!(a > 0.0)) return INF;                              // parallel to the axis (A.4 plane branch with b = 0)
   const double disc = k * k - a * c;
-  if (disc < 0.0) return INF;
+  // no root ahead: parallel to the axis (A.4 plane branch with b = 0), no real root, or both roots behind (c >= 0, k >= 0)
+  if (!(a > 0.0) || disc < 0.0 || (c >= 0.0 && k >= 0.0)) return INF;
   const double sq = sqrt(disc);
   const double q = (k < 0.0) ? (sq - k) : -(k + sq);      // -(k + sign(k) sqrt(disc)), sign(+-0) = +1 as in A.4
-  double u;
-  if (c > 0.0) {
-    if (k >= 0.0) return INF;
-    u = c / q;
-  } else if (c < 0.0) {
-    u = (k < 0.0) ? q / a : c / q;
-  } else {
-    if (k >= 0.0) return INF;
-    u = q / a;
-  }
+  const bool c_over_q = (c > 0.0) || (c < 0.0 && !(k < 0.0));
+  const double u = (c_over_q ? c : q) / (c_over_q ? q : a);   // one division for whichever root is the one ahead
   return (u > 0.0) ? u : INF;
 }
 

@@ -888,7 +888,9 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 }
 
 // ---- k_warp instantiations: (tables staged, per-history events recorded, threads per block) ----
+#ifndef MCDC_WARP_CASES
 #define MCDC_WARP_CASES(X) X(256) X(384) X(512) X(640) X(768) X(1024)
+#endif
 template <bool STAGED, bool RECORD>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
@@ -958,7 +960,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   ha.n_hist = sb.n_hist; ha.hb = sb.hs;
   ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
-  ha.aggregate = ((size_t)p->G * p->n_spatial <= 4096) ? 1 : 0;
+  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;   // in-warp merge of equal bins pays only on tiny meshes
   CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
   // consumers' cursor := producers' cursor (drops whatever an aborted launch may have left behind)
   CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));

@@ -17,6 +17,13 @@
 #pragma once
 #include "mcdc_kernels.cuh"
 
+#ifndef MCDC_STORE_INV
+#define MCDC_STORE_INV 1        // keep 1/direction in the pool (else recomputed every flight)
+#endif
+#ifndef MCDC_SCORE_NOINLINE
+#define MCDC_SCORE_NOINLINE 0   // general (multi-bin) scorer out of line
+#endif
+
 namespace mcdc {
 
 // ---- slow paths: rare, not inlined, and they read the tables from global memory (device copy of Tables) ----
@@ -46,14 +53,41 @@ __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, 
   return surf_distance(tb, s, type, on, x, y, z, ux, uy, uz, 1.0 / ux, 1.0 / uy, 1.0 / uz);
 }
 
+// A.7 for segments that may touch several tally bins (4-D DDA).  Warp-converged: every lane calls it.
+template <bool STAGED>
+#if MCDC_SCORE_NOINLINE
+__device__ __noinline__
+#else
+__device__ __forceinline__
+#endif
+void general_score(const Tables *gT, double *x_acc_slot, int aggregate, bool active,
+                                           const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d) {
+  // the pre-move state is still in the pool: x y z ux uy uz 1/ux 1/uy 1/uz t, N slots apart
+  const double x = pool[gi], y = pool[N + gi], z = pool[2 * N + gi], ux = pool[3 * N + gi], uy = pool[4 * N + gi],
+               uz = pool[5 * N + gi], ix = pool[6 * N + gi], iy = pool[7 * N + gi], iz = pool[8 * N + gi], t = pool[9 * N + gi];
+  const TB<STAGED> tb(*gT);
+  TallySink S;
+  S.slab = nullptr; S.global_x = x_acc_slot; S.slab_lo = 0; S.slab_bins = 0; S.aggregate = aggregate;
+  if (gT->score_fast) {
+    PState p;
+    p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = 1.0;
+    p.key = 0ull; p.ctr = 0u; p.hid = 0u; p.g = g; p.cell = 0; p.last_surf = -1;
+    int it = tb.template ld<int>(gT->o_it0_k, pk);
+    score_track_fast(tb, S, active, p, it, d);
+  } else {
+    score_track(tb, S, active, x, y, z, ux, uy, uz, t, 1.0, g, d);
+  }
+}
+
 __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
 
-// bytes of shared memory per pool slot: x y z ux uy uz t (7 x f64), key, ctr, cell|last, meta, 3 stack entries
-__host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record) { return 7 * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0); }
+// bytes of shared memory per pool slot: x y z ux uy uz 1/ux 1/uy 1/uz t (10 x f64), key, ctr, cell|last, meta, 3 stack entries
+__host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record) { return 10 * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0); }
 
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
   unsigned long long n_coll, n_surf, n_census, n_children, n_lost, n_src;
+  uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
 
 template <bool STAGED, bool RECORD, int NT>
@@ -66,14 +100,17 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   const uint32_t W = A.pool_slots;                    // slots per warp
   const uint32_t N = W * (uint32_t)NW;
   // ---- carve the dynamic shared memory: [staged tables][census populations][pool arrays][stacks] ----
-  unsigned char *base = g_smem + A.smem_tables;
-  uint32_t *s_popn = reinterpret_cast<uint32_t *>(base); base += ((size_t)T.K * 4 + 15) / 16 * 16;
-  double *px = reinterpret_cast<double *>(base), *py = px + N, *pz = py + N, *pux = pz + N, *puy = pux + N, *puz = puy + N,
-         *pt = puz + N;
-  unsigned long long *pkey = reinterpret_cast<unsigned long long *>(pt + N);
-  uint32_t *pctr = reinterpret_cast<uint32_t *>(pkey + N), *pcl = pctr + N, *pmeta = pcl + N;
-  uint32_t *phid = pmeta + N;                          // only when RECORD
-  uint8_t *LF = reinterpret_cast<uint8_t *>(RECORD ? phid + N : phid), *LC = LF + N, *LFREE = LC + N;
+  // One offset and the stride N address every array (pointers would cost two registers each):
+  //   f64  x y z ux uy uz 1/ux 1/uy 1/uz t  -> PD(k, slot), k = 0..9        u64  key       -> PK(slot)
+  //   u32  ctr, cell|last<<16, meta = g | census index<<8 | batch slot<<20, [history id]  -> PU(k, slot)
+  //   u8   stacks F, C, FREE -> PL(k, position)
+  uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
+  const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16);
+#define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + ((uint32_t)(k) * N + (slot)) * 8u))
+#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (10u * N + (slot)) * 8u))
+#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + 88u * N + ((uint32_t)(k) * N + (slot)) * 4u))
+#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + (RECORD ? 104u : 100u) * N + (uint32_t)(k) * N + (pos)))
+  enum { D_X = 0, D_Y, D_Z, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_T, U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
 
   if (STAGED) {
     const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
@@ -85,8 +122,9 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
     sh.n_coll = sh.n_surf = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
   }
+  if (lane < 8) sh.wcnt[wid][lane] = 0u;
   const uint32_t lb = (uint32_t)wid * W;               // first slot of this warp
-  for (uint32_t i = lane; i < W; i += 32) LFREE[lb + i] = (uint8_t)(W - 1u - i);
+  for (uint32_t i = lane; i < W; i += 32) PL(L_FREE, lb + i) = (uint8_t)(W - 1u - i);
   __syncthreads();
 
   unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
@@ -98,7 +136,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
   bool src_exhausted = false;
-  uint32_t c_coll = 0u, c_surf = 0u, c_census = 0u, c_children = 0u, c_lost = 0u, c_src = 0u;
+  enum { W_COLL = 0, W_SURF, W_CENSUS, W_CHILDREN, W_LOST, W_SRC };
+#define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
   for (;;) {
     int phase;                                         // 0 = R, 1 = F, 2 = C
@@ -153,7 +192,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         continue;
       }
       const bool act = (uint32_t)lane < total;
-      const uint32_t i = act ? (uint32_t)LFREE[lb + nFree - 1u - (uint32_t)lane] : 0u;
+      const uint32_t i = act ? (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane) : 0u;
       nFree -= total;
       double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
       unsigned long long key = 0ull;
@@ -209,19 +248,20 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
       }
       const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0);
-      if (m_lost) { c_lost += (uint32_t)__popc(m_lost); if (lane == 0) atomicAdd(&sh.led[LED_LOST], (double)__popc(m_lost)); }
-      c_src += n_src;
+      if (m_lost) { WCNT(W_LOST, (uint32_t)__popc(m_lost)); if (lane == 0) atomicAdd(&sh.led[LED_LOST], (double)__popc(m_lost)); }
+      WCNT(W_SRC, n_src);
       if (ok) {
         const uint32_t gi = lb + i;
-        px[gi] = x; py[gi] = y; pz[gi] = z; pux[gi] = ux; puy[gi] = uy; puz[gi] = uz; pt[gi] = t;
-        pkey[gi] = key; pctr[gi] = ctr; pcl[gi] = (uint32_t)cell | (NONE16 << 16);
-        pmeta[gi] = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
-        if (RECORD) phid[gi] = hid;
+        PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz; PD(D_T, gi) = t;
+        PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+        PK(gi) = key; PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
+        PU(U_META, gi) = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
+        if (RECORD) PU(U_HID, gi) = hid;
       }
       const unsigned m_ok = __ballot_sync(MCDC_FULL, ok), m_bad = __ballot_sync(MCDC_FULL, act && !ok);
-      if (ok) LF[lb + nF + lanes_below(m_ok, lane)] = (uint8_t)i;
+      if (ok) PL(L_F, lb + nF + lanes_below(m_ok, lane)) = (uint8_t)i;
       nF += (uint32_t)__popc(m_ok);
-      if (act && !ok) LFREE[lb + nFree + lanes_below(m_bad, lane)] = (uint8_t)i;
+      if (act && !ok) PL(L_FREE, lb + nFree + lanes_below(m_bad, lane)) = (uint8_t)i;
       nFree += (uint32_t)__popc(m_bad);
       __syncwarp();
       continue;
@@ -232,24 +272,35 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       const uint32_t n = min(32u, nF);
       nF -= n;
       const bool act = (uint32_t)lane < n;
-      const uint32_t i = act ? (uint32_t)LF[lb + nF + (uint32_t)lane] : 0u;
+      const uint32_t i = act ? (uint32_t)PL(L_F, lb + nF + (uint32_t)lane) : 0u;
       const uint32_t gi = lb + i;
-      double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, t = 0.0;
-      unsigned long long key = 0ull;
-      uint32_t ctr = 0u, cl = NONE16 << 16, meta = 0u;
-      if (act) {
-        x = px[gi]; y = py[gi]; z = pz[gi]; ux = pux[gi]; uy = puy[gi]; uz = puz[gi]; t = pt[gi];
-        key = pkey[gi]; ctr = pctr[gi]; cl = pcl[gi]; meta = pmeta[gi];
+      // distance to collision first: the random-number state is dead before the geometry needs its registers
+      uint32_t cl = NONE16 << 16, meta = 0u;
+      double d_coll;
+      {
+        unsigned long long key = 0ull;
+        uint32_t ctr = 0u;
+        if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
+        const double xi = draw(key, ctr);              // always consumed (D3)
+        if (act) PU(U_CTR, gi) = ctr;
+        d_coll = -log(xi);
       }
       const int cell = (int)(cl & 0xFFFFu), g = (int)(meta & 255u), pk = (int)((meta >> 8) & 4095u);
       const uint32_t last = cl >> 16;                  // surface the particle sits on, NONE16 if none
-      const double ix = 1.0 / ux, iy = 1.0 / uy, iz = 1.0 / uz;
       const uint32_t rec = T.o_cell2 + (uint32_t)cell * CELL2_BYTES;
       const uint32_t info = tb.template ldb<uint32_t>(rec + C2_INFO);
       const int n_other = (int)(info & 255u), mg = (int)((info >> 8) & 255u) * G + g;
-      const double xi = draw(key, ctr);                // always consumed (D3)
-      const double sig_t = tb.sig_t(mg);
-      const double d_coll = (sig_t > 0.0) ? -log(xi) * tb.inv_sig_t(mg) : INF;
+      d_coll = (tb.sig_t(mg) > 0.0) ? d_coll * tb.inv_sig_t(mg) : INF;
+      double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, ix = INF, iy = INF, iz = 1.0;
+      if (act) {
+        x = PD(D_X, gi); y = PD(D_Y, gi); z = PD(D_Z, gi); ux = PD(D_UX, gi); uy = PD(D_UY, gi); uz = PD(D_UZ, gi);
+#if MCDC_STORE_INV
+        ix = PD(D_IX, gi); iy = PD(D_IY, gi); iz = PD(D_IZ, gi);
+#endif
+      }
+#if !MCDC_STORE_INV
+      ix = 1.0 / ux; iy = 1.0 / uy; iz = 1.0 / uz;
+#endif
       // ---- faces: one candidate per axis, picked by the sign of the direction component ----
       const int fx = (ux > 0.0) ? 1 : 0, fy = (uy > 0.0) ? 3 : 2, fz = (uz > 0.0) ? 5 : 4;
       const uint32_t sfx = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fx);
@@ -259,20 +310,16 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       const double by = (sfy == NONE16) ? ((uy > 0.0) ? INF : -INF) : tb.surf_q0((int)sfy);
       const double bz = (sfz == NONE16) ? ((uz > 0.0) ? INF : -INF) : tb.surf_q0((int)sfz);
       const double dx = (bx - x) * ix, dy = (by - y) * iy, dz = (bz - z) * iz;   // 0 * inf = NaN: rejected below
-      double d_surf = INF;
-      int which = -1;                                  // 2*axis + side of the nearest face, 6 + j for other j
-      if (dx > 0.0 && dx < INF) { d_surf = dx; which = fx; }
-      if (dy > 0.0 && dy <= d_surf && dy < INF) {
-        // equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
-        if (dy < d_surf || tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fy) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which)) {
-          d_surf = dy; which = fy;
-        }
-      }
-      if (dz > 0.0 && dz <= d_surf && dz < INF) {
-        if (dz < d_surf || tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fz) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which)) {
-          d_surf = dz; which = fz;
-        }
-      }
+      // nearest face; equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
+      const bool vx = dx > 0.0 && dx < INF, vy = dy > 0.0 && dy < INF, vz = dz > 0.0 && dz < INF;
+      double d_surf = vx ? dx : INF;
+      int which = vx ? fx : -1;                        // 2*axis + side of the nearest face, 6 + j for other j
+      bool ty = vy && dy < d_surf;
+      if (vy && dy == d_surf) ty = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fy) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
+      if (ty) { d_surf = dy; which = fy; }
+      bool tz = vz && dz < d_surf;
+      if (vz && dz == d_surf) tz = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fz) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
+      if (tz) { d_surf = dz; which = fz; }
       // ---- other half-spaces (cylinders, general quadrics, redundant planes), list order, strict < ----
       const uint32_t orec = T.o_other2 + (info >> 16) * OTHER2_BYTES;
       for (int j = 0; j < n_other; ++j) {
@@ -290,6 +337,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         }
         if (u < d_surf) { d_surf = u; which = 6 + j; }
       }
+      double t = act ? PD(D_T, gi) : 0.0;
       const double t_census = tb.census(pk);
       const double d_time = tb.speed(g) * (t_census - t);
       int ev;
@@ -308,14 +356,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const uint32_t cbin = tb.template ldb<uint32_t>(rec + C2_BIN);
         const int tbin = tb.template ld<int>(T.o_tbin_k, pk);
         const bool one_bin = cbin != NONE32 && tbin >= 0;      // the whole segment lies in one tally bin
-        if (__any_sync(MCDC_FULL, act && !one_bin)) {
-          PState p;
-          p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = 1.0;
-          p.key = 0ull; p.ctr = 0u; p.hid = 0u; p.g = g; p.cell = cell; p.last_surf = -1;
-          int it = tb.template ld<int>(T.o_it0_k, pk);
-          if (T.score_fast) score_track_fast(tb, S, act && !one_bin, p, it, d);
-          else score_track(tb, S, act && !one_bin, x, y, z, ux, uy, uz, t, 1.0, g, d);
-        }
+        if (__any_sync(MCDC_FULL, act && !one_bin))
+          general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d);
         if (__any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
           const long long bin = sc ? (long long)(tbin * G + g) * n_spatial + (long long)cbin : -1;
@@ -334,29 +376,30 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (pk == T.K - 1) alive = false;
         else meta += 1u << 8;
       } else if (ev == EV_SURFACE) {                   // A.5
-        uint32_t s_star, nb;
-        int bc, type, idx;
-        if (which < 6) {
-          s_star = (which == fx) ? sfx : ((which == fy) ? sfy : sfz);
-          nb = tb.template ldb<uint16_t>(rec + C2_FACE_NB + 2u * which);
-          bc = (int)((tb.template ldb<uint16_t>(rec + C2_FACE_BC) >> (2 * which)) & 3u);
-          type = which >> 1;                           // ST_PLANE_X/Y/Z
-          idx = -1;
-        } else {
-          const uint2 e = tb.template ldb<uint2>(orec + (uint32_t)(which - 6) * OTHER2_BYTES);
-          s_star = e.x & 0xFFFFu; nb = e.x >> 16;
-          idx = (int)(e.y & 255u); type = (int)((e.y >> 9) & 7u); bc = (int)((e.y >> 12) & 3u);
-        }
+        const bool is_face = which < 6;
+        const int wf = is_face ? which : 0, jo = is_face ? 0 : which - 6;
+        const uint2 e = tb.template ldb<uint2>(orec + (uint32_t)jo * OTHER2_BYTES);
+        const uint32_t nb_f = tb.template ldb<uint16_t>(rec + C2_FACE_NB + 2u * wf);
+        const uint32_t bc_f = (tb.template ldb<uint16_t>(rec + C2_FACE_BC) >> (2 * wf)) & 3u;
+        const uint32_t s_f = (which == fx) ? sfx : ((which == fy) ? sfy : sfz);
+        const uint32_t s_star = is_face ? s_f : (e.x & 0xFFFFu), nb = is_face ? nb_f : (e.x >> 16);
+        const int bc = (int)(is_face ? bc_f : ((e.y >> 12) & 3u));
+        const int type = is_face ? (which >> 1) : (int)((e.y >> 9) & 7u);   // faces: ST_PLANE_X/Y/Z = axis
+        int idx = is_face ? -1 : (int)(e.y & 255u);
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
         if (bc == 1) {                                 // vacuum: leaks
           alive = false;
           atomicAdd(&sh.led[LED_LEAK], 1.0);
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
-          if (type == ST_PLANE_X) ux = -ux;
-          else if (type == ST_PLANE_Y) uy = -uy;
-          else if (type == ST_PLANE_Z) uz = -uz;
-          else { double u3[3] = {ux, uy, uz}; slow_reflect(gT, (int)s_star, type, x, y, z, u3); ux = u3[0]; uy = u3[1]; uz = u3[2]; }
-          pux[gi] = ux; puy[gi] = uy; puz[gi] = uz;
+          if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
+          else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
+          else if (type == ST_PLANE_Z) { PD(D_UZ, gi) = -uz; PD(D_IZ, gi) = -iz; }
+          else {
+            double u3[3] = {ux, uy, uz};
+            slow_reflect(gT, (int)s_star, type, x, y, z, u3);
+            PD(D_UX, gi) = u3[0]; PD(D_UY, gi) = u3[1]; PD(D_UZ, gi) = u3[2];
+            PD(D_IX, gi) = 1.0 / u3[0]; PD(D_IY, gi) = 1.0 / u3[1]; PD(D_IZ, gi) = 1.0 / u3[2];
+          }
         } else {                                       // transmission: the cell on the other side
           // a certified neighbour holds every point of this surface patch that lies strictly inside the cell's
           // forward faces (mcdc_host.cu); anything else takes the full search of A.5
@@ -375,31 +418,31 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         }
       }
       if (act) {
-        px[gi] = x; py[gi] = y; pz[gi] = z; pt[gi] = t; pctr[gi] = ctr;
-        if (new_cl != cl) pcl[gi] = new_cl;
-        if (ev == EV_CENSUS) pmeta[gi] = meta;
-        if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)phid[gi] * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
+        PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_T, gi) = t;
+        if (new_cl != cl) PU(U_CL, gi) = new_cl;
+        if (ev == EV_CENSUS) PU(U_META, gi) = meta;
+        if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
       }
       // ---- census population (A.8): one shared-memory add per distinct census index in the warp ----
       const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
       if (m_cen) {
         const unsigned peers = __match_any_sync(MCDC_FULL, census_k);
         if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
-        c_census += (uint32_t)__popc(m_cen);
+        WCNT(W_CENSUS, (uint32_t)__popc(m_cen));
         const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
         if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
       }
       {
         const unsigned m_s = __ballot_sync(MCDC_FULL, ev == EV_SURFACE), m_lost = __ballot_sync(MCDC_FULL, lost);
-        c_surf += (uint32_t)__popc(m_s);
-        c_lost += (uint32_t)__popc(m_lost);
+        WCNT(W_SURF, (uint32_t)__popc(m_s));
+        WCNT(W_LOST, (uint32_t)__popc(m_lost));
       }
       // ---- hand the slots on: F again, C, or FREE ----
       const bool toF = alive && ev != EV_COLLISION, toC = alive && ev == EV_COLLISION, dead = act && !alive;
       const unsigned mF = __ballot_sync(MCDC_FULL, toF), mC = __ballot_sync(MCDC_FULL, toC), mD = __ballot_sync(MCDC_FULL, dead);
-      if (toF) LF[lb + nF + lanes_below(mF, lane)] = (uint8_t)i;
-      if (toC) LC[lb + nC + lanes_below(mC, lane)] = (uint8_t)i;
-      if (dead) LFREE[lb + nFree + lanes_below(mD, lane)] = (uint8_t)i;
+      if (toF) PL(L_F, lb + nF + lanes_below(mF, lane)) = (uint8_t)i;
+      if (toC) PL(L_C, lb + nC + lanes_below(mC, lane)) = (uint8_t)i;
+      if (dead) PL(L_FREE, lb + nFree + lanes_below(mD, lane)) = (uint8_t)i;
       nF += (uint32_t)__popc(mF); nC += (uint32_t)__popc(mC); nFree += (uint32_t)__popc(mD);
       __syncwarp();
       continue;
@@ -410,11 +453,11 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       const uint32_t n = min(32u, nC);
       nC -= n;
       const bool act = (uint32_t)lane < n;
-      const uint32_t i = act ? (uint32_t)LC[lb + nC + (uint32_t)lane] : 0u;
+      const uint32_t i = act ? (uint32_t)PL(L_C, lb + nC + (uint32_t)lane) : 0u;
       const uint32_t gi = lb + i;
       unsigned long long key = 0ull;
       uint32_t ctr = 0u, cl = 0u, meta = 0u;
-      if (act) { key = pkey[gi]; ctr = pctr[gi]; cl = pcl[gi]; meta = pmeta[gi]; }
+      if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
       const int cell = (int)(cl & 0xFFFFu);
       int g = (int)(meta & 255u);
       const bool born = g == 255;                      // a fission child placed in this pool: only its flight is sampled
@@ -445,13 +488,13 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (m_fis) {
           const uint32_t kids = __reduce_add_sync(MCDC_FULL, (uint32_t)n_child);
           if (lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], (double)__popc(m_fis)); atomicAdd(&sh.led[LED_PRODUCTION], (double)kids); }
-          c_children += kids;
+          WCNT(W_CHILDREN, kids);
         }
-        c_coll += (uint32_t)__popc(__ballot_sync(MCDC_FULL, act && !born));
+        WCNT(W_COLL, (uint32_t)__popc(__ballot_sync(MCDC_FULL, act && !born)));
       }
       if (RECORD && act && !born) {
-        atomicAdd(A.ev + (size_t)phid[gi] * 4 + 0, 1u);
-        if (n_child > 0) atomicAdd(A.ev + (size_t)phid[gi] * 4 + 2, (uint32_t)n_child);
+        atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + 0, 1u);
+        if (n_child > 0) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + 2, (uint32_t)n_child);
       }
       // fission: publish children 1..n-1 to the global queue, continue as child 0
       const int n_push = (n_child > 1) ? n_child - 1 : 0;
@@ -465,16 +508,16 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const int total = __shfl_sync(MCDC_FULL, pre, 31);
         if ((uint32_t)total <= nFree) {                // the children fit this warp's pool: they join its C stack
           if (n_push > 0) {
-            const double x = px[gi], y = py[gi], z = pz[gi], t = pt[gi];
+            const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
             for (int c = 0; c < n_push; ++c) {
               const uint32_t r = (uint32_t)(pre - n_push + c);
-              const uint32_t i2 = (uint32_t)LFREE[lb + nFree - 1u - r], g2 = lb + i2;
-              px[g2] = x; py[g2] = y; pz[g2] = z; pt[g2] = t;
-              pkey[g2] = child_key(key, c0, (uint32_t)(c + 1)); pctr[g2] = 0u;
-              pcl[g2] = (cl & 0xFFFFu) | (NONE16 << 16);
-              pmeta[g2] = (meta & ~255u) | 255u;
-              if (RECORD) phid[g2] = phid[gi];
-              LC[lb + nC + r] = (uint8_t)i2;
+              const uint32_t i2 = (uint32_t)PL(L_FREE, lb + nFree - 1u - r), g2 = lb + i2;
+              PD(D_X, g2) = x; PD(D_Y, g2) = y; PD(D_Z, g2) = z; PD(D_T, g2) = t;
+              PK(g2) = child_key(key, c0, (uint32_t)(c + 1)); PU(U_CTR, g2) = 0u;
+              PU(U_CL, g2) = (cl & 0xFFFFu) | (NONE16 << 16);
+              PU(U_META, g2) = (meta & ~255u) | 255u;
+              if (RECORD) PU(U_HID, g2) = PU(U_HID, gi);
+              PL(L_C, lb + nC + r) = (uint8_t)i2;
             }
           }
           nFree -= (uint32_t)total; nC += (uint32_t)total;
@@ -489,8 +532,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           okq = __shfl_sync(MCDC_FULL, okq, 0);
           if (!okq && lane == 0) atomicExch(&A.cnt->overflow, 1);
           if (n_push > 0 && okq) {
-            const double x = px[gi], y = py[gi], z = pz[gi], t = pt[gi];
-            const int4 qm = make_int4(cell, (int)((meta >> 8) & 4095u), RECORD ? (int)phid[gi] : 0, (int)(meta >> 20));
+            const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
+            const int4 qm = make_int4(cell, (int)((meta >> 8) & 4095u), RECORD ? (int)PU(U_HID, gi) : 0, (int)(meta >> 20));
             for (int c = 0; c < n_push; ++c) {
               const uint32_t j = (uint32_t)(qb + (unsigned long long)c) & A.q.mask;
               A.q.x[j] = x; A.q.y[j] = y; A.q.z[j] = z; A.q.t[j] = t;
@@ -515,25 +558,28 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         draw2(key, ctr, xi_mu, xi_phi);
         isotropic(xi_mu, xi_phi, ux, uy, uz);
         if (alive) {
-          pux[gi] = ux; puy[gi] = uy; puz[gi] = uz;
-          pkey[gi] = key; pctr[gi] = ctr;
-          pmeta[gi] = (meta & ~255u) | (uint32_t)g;
-          pcl[gi] = (cl & 0xFFFFu) | (NONE16 << 16);
+          PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
+          PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+          PK(gi) = key; PU(U_CTR, gi) = ctr;
+          PU(U_META, gi) = (meta & ~255u) | (uint32_t)g;
+          PU(U_CL, gi) = (cl & 0xFFFFu) | (NONE16 << 16);
         }
       }
       const unsigned mF = __ballot_sync(MCDC_FULL, alive), mD = __ballot_sync(MCDC_FULL, act && !alive);
-      if (alive) LF[lb + nF + lanes_below(mF, lane)] = (uint8_t)i;
-      if (act && !alive) LFREE[lb + nFree + lanes_below(mD, lane)] = (uint8_t)i;
+      if (alive) PL(L_F, lb + nF + lanes_below(mF, lane)) = (uint8_t)i;
+      if (act && !alive) PL(L_FREE, lb + nFree + lanes_below(mD, lane)) = (uint8_t)i;
       nF += (uint32_t)__popc(mF); nFree += (uint32_t)__popc(mD);
       __syncwarp();
     }
   }
 
   // ---- warp totals -> block totals -> global ----
+  __syncwarp();
   if (lane == 0) {
-    atomicAdd(&sh.n_coll, (unsigned long long)c_coll); atomicAdd(&sh.n_surf, (unsigned long long)c_surf);
-    atomicAdd(&sh.n_census, (unsigned long long)c_census); atomicAdd(&sh.n_children, (unsigned long long)c_children);
-    atomicAdd(&sh.n_lost, (unsigned long long)c_lost); atomicAdd(&sh.n_src, (unsigned long long)c_src);
+    const uint32_t *wc = sh.wcnt[wid];
+    atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_surf, (unsigned long long)wc[W_SURF]);
+    atomicAdd(&sh.n_census, (unsigned long long)wc[W_CENSUS]); atomicAdd(&sh.n_children, (unsigned long long)wc[W_CHILDREN]);
+    atomicAdd(&sh.n_lost, (unsigned long long)wc[W_LOST]); atomicAdd(&sh.n_src, (unsigned long long)wc[W_SRC]);
   }
   __syncthreads();
   for (int k = tid; k < T.K; k += NT) {
@@ -553,5 +599,11 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
     atomicAdd(&cnt->n[6], sh.n_lost);
   }
 }
+
+#undef PD
+#undef PK
+#undef PU
+#undef PL
+#undef WCNT
 
 }  // namespace mcdc
