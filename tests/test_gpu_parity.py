@@ -99,6 +99,23 @@ def test_ragged_and_tiny_runs(M, N, B, scheduler):
     g.close()
 
 
+@pytest.mark.parametrize("scheduler", [0, 1])
+@pytest.mark.parametrize("covering", [False, True])
+def test_stress_geometry_takes_the_slow_paths_and_still_matches(M, covering, scheduler):
+    """General quadric cells, a reflective sphere, a face with two neighbours (no certified neighbour), lost source
+    particles, a tally mesh that clips / is unaligned with the cells, census times off the tally time edges."""
+    from workloads import configs as W
+    p = W.stress_geometry(n_histories=240_000, n_batches=12, covering_mesh=covering)
+    o, g = _pair(M, p, scheduler=scheduler)
+    co, cg = _check_counters(o, g)
+    assert cg["lost_n"] > 0 and cg["leak"] > 0 and cg["children"] > 0
+    assert np.all(o.history_events() == g.history_events(), axis=1).mean() >= 0.99999
+    _check_tallies(o, g, rtol=1e-9)
+    wo, no = o.census(); wg, ng = g.census()
+    assert np.array_equal(no, ng) and np.array_equal(wo, wg)
+    g.close()
+
+
 def test_sub_batching_and_split_batches_do_not_change_results(M):
     """A workspace too small for the whole run forces several sub-batches; a batch larger than a slot is split
     into pieces spread over the slots."""

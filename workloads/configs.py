@@ -429,5 +429,45 @@ CONFIGS = {
 }
 
 
+# ----------------------------------------------------------------------------------------
+# Stress geometry (parity tests only): what the five configs do not reach -- a general quadric (sphere) cell,
+# a reflective sphere with nothing inside (sources drawn there are lost), a face shared with two neighbours
+# (no certified neighbour), a z-cylinder inside one of them, a tally mesh smaller than the geometry or
+# unaligned with the cells, census times that do not coincide with the tally time edges, two groups.
+# ----------------------------------------------------------------------------------------
+def stress_geometry(n_histories=60_000, n_batches=12, covering_mesh=False):
+    G = 2
+    mats, ss = _materials([
+        dict(sigma_t=[0.6, 0.9], sigma_c=[0.1, 0.2], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+             sigma_s=[[0.3, 0.2], [0.1, 0.6]]),
+        dict(sigma_t=[0.8, 1.2], sigma_c=[0.15, 0.4], sigma_f=[0.05, 0.1], nu=[2.2, 2.5], chi=[0.7, 0.3],
+             sigma_s=[[0.4, 0.2], [0.0, 0.7]]),
+    ], G)
+    surfs = [plane_x(0.0), plane_x(2.0), plane_x(6.0), plane_y(0.0), plane_y(2.0), plane_y(4.0), plane_z(0.0),
+             plane_z(4.0), sphere(1.0, 2.0, 2.0, 0.7), sphere(5.0, 1.0, 2.0, 0.4), cylinder_z(4.0, 3.0, 0.5)]
+    bcs = [BC_REFLECTIVE, BC_TRANSMISSION, BC_VACUUM, BC_VACUUM, BC_TRANSMISSION, BC_VACUUM, BC_VACUUM,
+           BC_REFLECTIVE, BC_TRANSMISSION, BC_REFLECTIVE, BC_TRANSMISSION]
+    cells = [
+        ([(8, -1)], 1),                                                              # fuel sphere
+        ([(0, +1), (1, -1), (3, +1), (5, -1), (6, +1), (7, -1), (8, +1)], 0),        # x in [0,2], outside it
+        ([(1, +1), (2, -1), (3, +1), (4, -1), (6, +1), (7, -1), (9, +1)], 1),        # y in [0,2], outside the mirror ball
+        ([(1, +1), (2, -1), (4, +1), (5, -1), (6, +1), (7, -1), (10, +1)], 0),       # y in [2,4], outside the pin
+        ([(10, -1), (6, +1), (7, -1)], 1),                                           # the pin
+    ]
+    src = dict(lo=[0.2, 0.2, 0.2], hi=[5.8, 3.8, 3.8], t0=0.0, t1=1.5, pdf=[0.6, 0.4])
+    if covering_mesh:
+        mesh = dict(lo=[0.0, 0.0, 0.0], hi=[6.0, 4.0, 4.0], n=[7, 5, 3])
+        T = np.array([0.0, 0.5, 2.0, 3.5, 6.0])
+    else:
+        mesh = dict(lo=[0.5, 0.5, 0.0], hi=[5.5, 3.5, 4.0], n=[5, 3, 2])
+        T = np.array([0.25, 0.5, 2.0, 3.5, 5.0])
+    census = np.array([1.3, 2.9, 6.0])
+    return _assemble("stress_geometry" + ("_covering" if covering_mesh else ""), mats, ss, [1.0, 0.4], surfs, bcs,
+                     cells, src, mesh, T, census, n_histories, n_batches, run_seed(9))
+
+
+CONFIGS["stress"] = stress_geometry
+
+
 def get_config(name: str, **kw) -> Problem:
     return CONFIGS[name](**kw)
