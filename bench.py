@@ -26,8 +26,12 @@ if ROOT not in sys.path:
 import numpy as np  # noqa: E402
 
 METRIC = "histories/s"
-FP64_LANES_PER_SM = 64          # B200 (sm_100a): 64 fp64 FMA lanes per SM (nominal 37 TFLOP/s / (2*148*1.965 GHz))
 N_SM = 148
+ISSUE_LANES_PER_SM = 128        # 4 warp schedulers x 32 lanes: one warp instruction per scheduler per cycle
+# From the committed ncu capture of k_warp on this workload (profiles/r01d_k_warp.md): per launch of 1e7 config-3
+# histories, dram__bytes_read.sum + dram__bytes_write.sum, and thread instructions per track segment.
+NCU = {"config3_pin_lattice": {"dram_bytes_per_history": 3.23, "thread_inst_per_segment": 1003.0,
+                               "source": "profiles/r01d_k_warp.md"}}
 
 
 def _peaks():
@@ -228,22 +232,35 @@ def bench_gpu(args):
         # dominant kernel: k_warp.  Algorithmic bytes of the steps it processed / its device time.
         alg = algorithmic_bytes(p, {"segments": c["segments"], "children": c["children"]}, n_hist * args.steps,
                                 n_b * args.steps)
-        n_tr = max(1, (launches - args.steps * 2))
+        n_tr = max(1, launches // 2)                       # one k_warp + one k_closeout launch per sub-batch
         ach = alg / (ms_tr * 1e-3) / 1e9
+        ncu = NCU.get(p.name)
+        traffic = ncu["dram_bytes_per_history"] * n_hist * args.steps / n_tr if ncu else None
         roofline = {"bound": "hbm", "kernel": "k_warp", "achieved": ach, "peak": peak, "unit": "GB/s",
-                    "frac": ach / peak, "traffic": None, "peak_kind": peak_kind,
+                    "frac": ach / peak, "traffic": traffic, "peak_kind": peak_kind,
                     "note": "achieved = SURVEY 8(d) algorithmic bytes (176 B/segment + 112 B/child + 88 B/history + "
-                            "close-out) / summed k_warp device time; particle state is register-resident so "
-                            "DRAM traffic is far below this figure (see DESIGN.md, profiles/)",
+                            "close-out) / summed k_warp device time (CUDA events on the library's stream); particle "
+                            "state lives in shared memory, so the DRAM traffic (bytes per launch, from the ncu capture "
+                            "in profiles/) is far below this figure and the kernel is issue-bound: see roofline_alu",
                     "launches": int(n_tr), "ms_kernel_total": ms_tr}
+        roofline_alu = None
+        if ncu:
+            ti = ncu["thread_inst_per_segment"] * c["segments"] / (ms_tr * 1e-3)
+            pk = N_SM * ISSUE_LANES_PER_SM * sm_max * 1e6
+            roofline_alu = {"bound": "alu", "kernel": "k_warp", "achieved": ti / 1e12, "peak": pk / 1e12,
+                            "unit": "T thread-inst/s", "frac": ti / pk,
+                            "note": "instruction issue: thread instructions per segment from the ncu capture x segments/s, "
+                                    "against 148 SMs x 4 schedulers x 32 lanes x max SM clock (DESIGN.md section 6)"}
         out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                "config": {"workload": p.name, "histories_per_step": n_hist, "n_batches": n_b, "seed": p.seed,
-                          "l2": "banks and tally accumulators exceed L2 (inputs larger than L2)" if n_hist >= 2_000_000
-                          else "small workload: L2-resident", "parallelism": f"history-range sharding x{world}"},
+                          "l2": "the path has no input buffers (histories are generated on chip from seed and id); its "
+                                "only global data, the per-batch tally accumulators, are rewritten by the close-out of "
+                                "every step, so no step can reuse a previous step's cache contents",
+                          "parallelism": f"history-range sharding x{world}"},
                "segments_per_s": seg_per_s, "segments_per_history": c["segments"] / max(1, c["histories"]),
-               "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline}
+               "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu}
     # ---- e2e: host buffers in, host buffers out, through the C ABI (create + bind + run + get) ----
     ws = g._ws
     ptr = (ws.data_ptr() + 255) // 256 * 256
@@ -268,10 +285,50 @@ def bench_gpu(args):
                       "note": "mcdc_problem_create (host arrays) + workspace_bind + run_ex + tallies_get (host) per step"}
         if world == 1 and not args.no_cpu:
             out["cpu_baseline"] = run_cpu_sample(p, seconds_target=args.cpu_seconds)
-        print(json.dumps(out))
     g.close()
+    if args.sweep and world == 1:
+        out["sweep"] = run_sweep(M, args, dev, peak)
+    if rank == 0:
+        print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_sweep(M, args, dev, peak):
+    """BASELINE config 4: the config-3 problem at 1e5 .. 1e9 histories (1e9 as device-sized sub-batches)."""
+    import torch
+    from workloads import configs as W
+
+    rows = []
+    for n in (10 ** 5, 10 ** 6, 10 ** 7, 10 ** 8, 10 ** 9):
+        if n > args.sweep_max:
+            break
+        nb = 20 if n == 10 ** 5 else 100
+        p = W.config3_pin_lattice(n_histories=n, n_batches=nb)
+        sub = min(n, 250_000_000)                         # histories per sub-batch (one k_warp launch)
+        g = M.Problem(p, max_histories_per_subbatch=sub, max_batches_in_flight=min(nb, max(1, sub // (n // nb))),
+                      device=dev, async_only=True)
+        reps = 3 if n <= 10 ** 7 else 1
+        g.run(min(n, 10 ** 7) // nb * nb, p.seed, nb)   # warm-up
+        g.reset()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        ms_k = 0.0
+        for _ in range(reps):
+            g.run(n, p.seed, nb)
+            ms_k += g.counters()["ms_transport"]
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        c = g.counters()
+        alg = algorithmic_bytes(p, c, n * reps, nb * reps)
+        rows.append({"histories": n, "n_batches": nb, "histories_per_s": n * reps / (ms * 1e-3),
+                     "segments_per_s": c["segments"] / (ms * 1e-3), "ms_per_run": ms / reps,
+                     "alg_GBps": alg / (ms_k * 1e-3) / 1e9, "frac_of_hbm_peak": alg / (ms_k * 1e-3) / 1e9 / peak,
+                     "launches_per_run": (c["kernel_launches"]) // reps, "workspace_bytes": g.workspace_bytes})
+        g.close()
+    return rows
 
 
 def main():
@@ -285,6 +342,8 @@ def main():
     ap.add_argument("--batches", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--sweep", action="store_true", help="also run the config-4 batch-size sweep (adds a 'sweep' key)")
+    ap.add_argument("--sweep-max", type=float, default=1e9)
     args = ap.parse_args()
     if args.impl == "reference":
         bench_reference(args)

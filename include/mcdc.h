@@ -116,6 +116,11 @@ int mcdc_problem_reset(mcdc_problem *p);
  * census and fission banks, per-batch tally accumulators).                                        */
 int mcdc_workspace_size(const mcdc_problem *p, uint64_t max_histories_per_subbatch,
                         uint32_t max_batches_in_flight, size_t *bytes);
+/* The smaller workspace that is enough for MCDC_SCHED_ASYNC alone (no particle banks: per-batch
+ * tally accumulators and the fission queue).  A handle bound with it refuses
+ * MCDC_SCHED_CENSUS_STEPPED with MCDC_ERR_NO_WORKSPACE.                                           */
+int mcdc_workspace_size_async(const mcdc_problem *p, uint64_t max_histories_per_subbatch,
+                              uint32_t max_batches_in_flight, size_t *bytes);
 /* dev_ptr: device memory of at least `bytes` (256-byte aligned); cuda_stream: cudaStream_t.       */
 int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes, uint64_t max_histories_per_subbatch,
                         uint32_t max_batches_in_flight, void *cuda_stream);

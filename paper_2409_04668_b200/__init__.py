@@ -12,6 +12,7 @@ from .api import (  # noqa: F401
     mcdc_problem_destroy,
     mcdc_problem_reset,
     mcdc_workspace_size,
+    mcdc_workspace_size_async,
     mcdc_workspace_bind,
     mcdc_run,
     mcdc_run_ex,

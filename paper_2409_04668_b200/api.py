@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("MCDC_LIB_PATH") or os.path.join(_HERE, "libmcdc.so")
 
 EXPORTED_SYMBOLS = [
-    "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size",
+    "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size", "mcdc_workspace_size_async",
     "mcdc_workspace_bind", "mcdc_run", "mcdc_run_ex", "mcdc_tallies_get", "mcdc_tally_sums_get",
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version",
@@ -86,6 +86,8 @@ def lib():
     L.mcdc_problem_reset.argtypes = [vp]; L.mcdc_problem_reset.restype = C.c_int
     L.mcdc_workspace_size.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
     L.mcdc_workspace_size.restype = C.c_int
+    L.mcdc_workspace_size_async.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
+    L.mcdc_workspace_size_async.restype = C.c_int
     L.mcdc_workspace_bind.argtypes = [vp, vp, C.c_size_t, C.c_uint64, C.c_uint32, vp]
     L.mcdc_workspace_bind.restype = C.c_int
     L.mcdc_run.argtypes = [vp, C.c_uint64, C.c_uint64]; L.mcdc_run.restype = C.c_int
@@ -180,6 +182,13 @@ def mcdc_workspace_size(h, max_histories_per_subbatch, max_batches_in_flight) ->
     return int(n.value)
 
 
+def mcdc_workspace_size_async(h, max_histories_per_subbatch, max_batches_in_flight) -> int:
+    n = C.c_size_t(0)
+    _check(lib().mcdc_workspace_size_async(h, int(max_histories_per_subbatch), int(max_batches_in_flight), C.byref(n)),
+           "mcdc_workspace_size_async", h)
+    return int(n.value)
+
+
 def mcdc_workspace_bind(h, dev_ptr, nbytes, max_histories_per_subbatch, max_batches_in_flight, cuda_stream=0):
     _check(lib().mcdc_workspace_bind(h, C.c_void_p(int(dev_ptr)), int(nbytes), int(max_histories_per_subbatch),
                                      int(max_batches_in_flight), C.c_void_p(int(cuda_stream))),
@@ -234,7 +243,7 @@ class Problem:
     """Handle + PyTorch-owned workspace.  Marshalling only; all work happens in libmcdc.so."""
 
     def __init__(self, prob, max_histories_per_subbatch=None, max_batches_in_flight=None, device="cuda:0",
-                 workspace_scale=1.0):
+                 workspace_scale=1.0, async_only=False):
         import torch  # device memory and stream only
 
         if not torch.cuda.is_available():
@@ -247,12 +256,14 @@ class Problem:
         self._h = mcdc_problem_create(prob)
         nb = int(max_batches_in_flight or max(1, getattr(prob, "n_batches", 1)))
         nh = int(max_histories_per_subbatch or max(1, getattr(prob, "n_histories", 1)))
+        self._async_only = bool(async_only)
         self._bind(nh, nb, workspace_scale)
 
     def _bind(self, nh, nb, scale=1.0):
         import torch
 
-        nbytes = int(mcdc_workspace_size(self._h, nh, nb) * scale)
+        size = mcdc_workspace_size_async if self._async_only else mcdc_workspace_size
+        nbytes = int(size(self._h, nh, nb) * scale)
         self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
         ptr = (self._ws.data_ptr() + 255) // 256 * 256
         self._stream = torch.cuda.current_stream(self.device)

@@ -724,15 +724,24 @@ extern "C" int mcdc_workspace_size(const mcdc_problem *p, uint64_t max_hist, uin
   return MCDC_OK;
 }
 
+extern "C" int mcdc_workspace_size_async(const mcdc_problem *p, uint64_t max_hist, uint32_t max_slots, size_t *bytes) {
+  if (!p || !bytes || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
+  *bytes = layout(p, max_slots, 0, max_hist).total;      // no particle banks: accumulators and the fission queue only
+  return MCDC_OK;
+}
+
 extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes, uint64_t max_hist, uint32_t max_slots,
                                    void *cuda_stream) {
   if (!p || !dev_ptr || max_hist == 0 || max_slots == 0 || max_hist > 0xFFFFFFF0ull) return MCDC_ERR_ARG;
   if (((uintptr_t)dev_ptr & 255u) != 0) return MCDC_ERR_ARG;
   uint64_t cap = default_cap(max_hist, max_slots);
   WsLayout L = layout(p, max_slots, cap, max_hist);
-  if (bytes < L.total) return MCDC_ERR_NO_WORKSPACE;
-  // a larger workspace buys larger banks: grow cap while it fits
-  {
+  if (bytes < L.total) {                                  // enough for the asynchronous scheduler alone?
+    cap = 0;
+    L = layout(p, max_slots, 0, max_hist);
+    if (bytes < L.total) return MCDC_ERR_NO_WORKSPACE;
+  } else {
+    // a larger workspace buys larger banks: grow cap while it fits
     uint64_t lo = cap, hi = cap * 64;
     while (lo + 32 <= hi) {
       uint64_t mid = align_up((size_t)((lo + hi) / 2), 32);
@@ -977,6 +986,8 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   // that the last chunks still spread over all warps
   ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)sb.n_hist / ((uint64_t)grid * (nt / 32) * 8)));
   if (const char *e4 = getenv("MCDC_CHUNK")) ha.src_chunk = (uint32_t)std::max(1, atoi(e4));
+  ha.n_slots = sb.n_slots;
+  ha.n_chunks = sb.n_slots * ((sb.hs + ha.src_chunk - 1) / ha.src_chunk);
   (void)ev0; (void)ev1;
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
@@ -1038,7 +1049,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   CK(cudaEventRecord(e_run0, p->stream));
 
   // ---- plan sub-batches ----
-  const uint64_t slot_max = std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist));
+  if (stepped && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
+  const uint64_t slot_max = stepped ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
   int rc = MCDC_OK;
   if (hb <= slot_max) {                                  // whole batches, one per slot
     const uint32_t per_sub = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(p->ws_slots, p->ws_hist / hb));

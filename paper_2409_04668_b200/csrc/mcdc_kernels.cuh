@@ -560,6 +560,7 @@ struct HistoryArgs {
   unsigned long long seed_mixed, first_history;
   uint32_t n_hist, hb;            // histories in the sub-batch, histories per slot
   uint32_t src_chunk;             // source histories a warp reserves per global atomic
+  uint32_t n_slots, n_chunks;     // batch slots of the sub-batch; chunks in all = n_slots * ceil(hb / src_chunk)
   double *x_acc;
   DevCounters *cnt;
   double *pop_w;

@@ -153,12 +153,19 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       // =============== R: acquire work for up to 32 free slots, initialise the new particles (A.3, A.6) ===============
       const uint32_t want = min(32u, nFree);
       // source histories come from the warp's own chunk of the sub-batch; one global atomic per chunk
-      if (src_next == src_end && !src_exhausted) {
-        uint32_t cb = 0u;
-        if (lane == 0) cb = atomicAdd(A.hist_cursor, A.src_chunk);
-        cb = __shfl_sync(MCDC_FULL, cb, 0);
-        if (cb >= A.n_hist) src_exhausted = true;
-        else { src_next = cb; src_end = min(cb + A.src_chunk, A.n_hist); }
+      // Chunks are dealt round-robin over the batch slots, so the warps in flight spread their scores over all the
+      // slot accumulators instead of contending for the hot bins of one.
+      while (src_next == src_end && !src_exhausted) {   // (a ragged last slot can yield an empty chunk)
+        uint32_t ci = 0u;
+        if (lane == 0) ci = atomicAdd(A.hist_cursor, 1u);
+        ci = __shfl_sync(MCDC_FULL, ci, 0);
+        if (ci >= A.n_chunks) src_exhausted = true;
+        else {
+          const uint32_t slot = ci % A.n_slots, j = ci / A.n_slots;
+          const unsigned long long lo = (unsigned long long)slot * A.hb + (unsigned long long)j * A.src_chunk;
+          const unsigned long long hi = min(min(lo + A.src_chunk, (unsigned long long)(slot + 1u) * A.hb), (unsigned long long)A.n_hist);
+          src_next = (uint32_t)min(lo, hi); src_end = (uint32_t)hi;
+        }
       }
       const uint32_t n_src = min(want, src_end - src_next), src_base = src_next;
       src_next += n_src;
