@@ -143,6 +143,16 @@ int mcdc_census_get(const mcdc_problem *p, double *pop_w, uint64_t *pop_n, size_
  * first_history_id+h of the LAST run (needs record_history_events).                               */
 int mcdc_history_events_get(const mcdc_problem *p, uint32_t *ev, size_t n_histories);
 
+/* What mcdc_problem_create derived from the geometry: how many transmission
+ * half-spaces have a certified neighbour, how many cells lie in one spatial tally bin, the bytes of
+ * tables the history kernel stages in shared memory, and whether the problem fits that kernel's
+ * compact tables at all (else MCDC_SCHED_CENSUS_STEPPED is used).                                 */
+typedef struct {
+  uint64_t transmission_halfspaces, certified_halfspaces, cells, one_bin_cells, hot_table_bytes;
+  int32_t warp_kernel_ok, score_fast;
+} mcdc_problem_info;
+int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
+
 const char *mcdc_strerror(int code);
 const char *mcdc_last_cuda_error(const mcdc_problem *p);
 /* "major.minor sm_XX" of the build; never fails.                                                  */

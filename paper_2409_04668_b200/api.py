@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.environ.get("MCDC_LIB_PATH") or os.path.join(_HERE, "libmcdc.so")
 
 EXPORTED_SYMBOLS = [
-    "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size", "mcdc_workspace_size_async",
+    "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size", "mcdc_workspace_size_async", "mcdc_problem_info_get",
     "mcdc_workspace_bind", "mcdc_run", "mcdc_run_ex", "mcdc_tallies_get", "mcdc_tally_sums_get",
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version",
@@ -67,6 +67,11 @@ class Counters(C.Structure):
 _lib = None
 
 
+class ProblemInfo(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("transmission_halfspaces", "certified_halfspaces", "cells", "one_bin_cells",
+                                          "hot_table_bytes")] + [("warp_kernel_ok", C.c_int32), ("score_fast", C.c_int32)]
+
+
 def lib_path() -> str:
     return _LIB_PATH
 
@@ -88,6 +93,7 @@ def lib():
     L.mcdc_workspace_size.restype = C.c_int
     L.mcdc_workspace_size_async.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
     L.mcdc_workspace_size_async.restype = C.c_int
+    L.mcdc_problem_info_get.argtypes = [vp, C.POINTER(ProblemInfo)]; L.mcdc_problem_info_get.restype = C.c_int
     L.mcdc_workspace_bind.argtypes = [vp, vp, C.c_size_t, C.c_uint64, C.c_uint32, vp]
     L.mcdc_workspace_bind.restype = C.c_int
     L.mcdc_run.argtypes = [vp, C.c_uint64, C.c_uint64]; L.mcdc_run.restype = C.c_int
@@ -180,6 +186,12 @@ def mcdc_workspace_size(h, max_histories_per_subbatch, max_batches_in_flight) ->
     _check(lib().mcdc_workspace_size(h, int(max_histories_per_subbatch), int(max_batches_in_flight), C.byref(n)),
            "mcdc_workspace_size", h)
     return int(n.value)
+
+
+def mcdc_problem_info_get(h) -> dict:
+    info = ProblemInfo()
+    _check(lib().mcdc_problem_info_get(h, C.byref(info)), "mcdc_problem_info_get", h)
+    return {n: int(getattr(info, n)) for n, _ in ProblemInfo._fields_}
 
 
 def mcdc_workspace_size_async(h, max_histories_per_subbatch, max_batches_in_flight) -> int:
@@ -285,6 +297,9 @@ class Problem:
 
     def reset(self):
         mcdc_problem_reset(self._h)
+
+    def info(self):
+        return mcdc_problem_info_get(self._h)
 
     def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False,
             scheduler=0):

@@ -99,7 +99,7 @@ struct mcdc_problem {
   int hist_threads = 512;
   uint32_t pool_slots = 0;
   size_t pool_smem = 0;
-  size_t n_cert = 0, n_transm = 0;   // transmission half-spaces with / without a certified neighbour
+  size_t n_cert = 0, n_transm = 0, n_one_bin = 0;   // certified / all transmission half-spaces; cells in one tally bin
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
   std::string cuda_err;
 };
@@ -521,6 +521,7 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
       if (one) cbin = (uint32_t)((idx[2] * p->mesh_n[1] + idx[1]) * p->mesh_n[0] + idx[0]);
     }
     std::memcpy(r + C2_BIN, &cbin, 4);
+    if (cbin != NONE32) p->n_one_bin++;
   }
   if (other2.empty()) other2.resize(OTHER2_BYTES, 0);
   p->n_cert = n_cert; p->n_transm = n_transm;
@@ -1163,6 +1164,14 @@ extern "C" int mcdc_history_events_get(const mcdc_problem *cp, uint32_t *ev, siz
   if (!p || !ev) return MCDC_ERR_ARG;
   if (n != p->ev_n || !p->d_ev) return MCDC_ERR_SIZE;
   CK(cudaMemcpy(ev, p->d_ev, n * 4 * sizeof(uint32_t), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info) {
+  if (!p || !info) return MCDC_ERR_ARG;
+  info->transmission_halfspaces = p->n_transm; info->certified_halfspaces = p->n_cert;
+  info->cells = (uint64_t)p->C; info->one_bin_cells = p->n_one_bin; info->hot_table_bytes = p->tab.hot_bytes;
+  info->warp_kernel_ok = p->tab.warp_ok; info->score_fast = p->tab.score_fast;
   return MCDC_OK;
 }
 

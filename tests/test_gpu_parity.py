@@ -222,3 +222,40 @@ def test_full_size_config3_sampled_against_the_oracle(M):
     tot_o, tot_g = mo.sum(), mean.sum()
     assert tot_g == pytest.approx(tot_o, rel=0.03)
     g.close()
+
+
+def test_certificates_one_bin_cells_and_async_only_workspace(M):
+    """What problem creation derives from the geometry, and the small workspace that serves
+    the asynchronous scheduler alone."""
+    from workloads import configs as W
+    p3 = W.config3_pin_lattice(n_histories=4000, n_batches=4)
+    g = M.Problem(p3, async_only=True)
+    i3 = g.info()
+    # 289 moderator cells x (4 pitch planes + cylinder) + 289 fuel cylinders, minus the 68 reflective outer planes
+    assert i3["transmission_halfspaces"] == 289 * 6 - 68 and i3["certified_halfspaces"] == i3["transmission_halfspaces"]
+    assert i3["cells"] == 578 and i3["one_bin_cells"] == 578 and i3["warp_kernel_ok"] == 1 and i3["score_fast"] == 1
+    assert i3["hot_table_bytes"] < 64 * 1024
+    full = M.mcdc_workspace_size(g._h, 4000, 4)
+    assert g.workspace_bytes < full
+    g.run(record_history_events=True)
+    ev = g.history_events()
+    with pytest.raises(M.McdcError) as e:
+        g.run(scheduler=1)                               # no particle banks in this workspace
+    assert e.value.code == -5
+    g.close()
+    h = M.Problem(p3)
+    h.run(record_history_events=True)
+    assert np.array_equal(h.history_events(), ev)
+    h.close()
+    ps = W.stress_geometry(n_histories=1200, n_batches=12)
+    g = M.Problem(ps)
+    i_s = g.info()
+    # certified: only the pin <-> its box (z-cylinder); nothing next to a sphere, nothing on the two-neighbour face
+    assert 0 < i_s["certified_halfspaces"] < i_s["transmission_halfspaces"]
+    assert i_s["one_bin_cells"] == 0 and i_s["score_fast"] == 0
+    g.close()
+    p2 = W.config2_lduct(n_histories=1000, n_batches=1)
+    g = M.Problem(p2)
+    i2 = g.info()
+    assert i2["certified_halfspaces"] == i2["transmission_halfspaces"] > 0 and i2["one_bin_cells"] == 0
+    g.close()
