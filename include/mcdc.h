@@ -153,6 +153,21 @@ typedef struct {
 } mcdc_problem_info;
 int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
 
+/* Multi-GPU domain replication (PAPER.md:59 "domain-replicated MPI", :173-177):
+ * every rank runs its own history-id range on a full copy of the problem, and the raw accumulators are
+ * summed over ranks once at the end.  These calls expose the handle's accumulators as ONE fp64 vector
+ * so that the caller can reduce it with any collective (ncclAllReduce on a device buffer, gloo/MPI on
+ * a host buffer) and put the sum back:
+ *   [0, n_bins) sum   [n_bins, 2 n_bins) sumsq   then pop_w[K], pop_n[K], ledger[7] (source production
+ *   capture fission_abs leak census_final lost), counts[7] (histories segments collisions surf_hits
+ *   census_events children lost_n), roulette[2] (gain, loss), histories, batches.
+ * Integer entries are stored as doubles (exact below 2^53).  on_device != 0: buf is DEVICE memory
+ * (copies run on the bound stream, synchronous on return); else HOST memory.  n must equal
+ * mcdc_state_size.  Import REPLACES the handle's accumulators; ranks must use the same batch size. */
+int mcdc_state_size(const mcdc_problem *p, size_t *n_doubles);
+int mcdc_state_export(const mcdc_problem *p, double *buf, size_t n_doubles, int on_device);
+int mcdc_state_import(mcdc_problem *p, const double *buf, size_t n_doubles, int on_device);
+
 const char *mcdc_strerror(int code);
 const char *mcdc_last_cuda_error(const mcdc_problem *p);
 /* "major.minor sm_XX" of the build; never fails.                                                  */

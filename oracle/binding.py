@@ -32,10 +32,16 @@ class Counters(C.Structure):
     _fields_ = [(n, C.c_double) for n in
                 ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost")] + \
                [(n, C.c_uint64) for n in
-                ("histories", "segments", "collisions", "surf_hits", "census_events", "children", "lost_n", "batches")]
+                ("histories", "segments", "collisions", "surf_hits", "census_events", "children", "lost_n", "batches")] + \
+               [("vr_gain", C.c_double), ("vr_loss", C.c_double), ("pc_removed", C.c_uint64), ("pc_added", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class _Technique(C.Structure):
+    _fields_ = [("implicit_capture", C.c_int32), ("wr_threshold", C.c_double), ("wr_survive", C.c_double),
+                ("population_control", C.c_int32), ("pc_target", C.c_uint64)]
 
 
 class _RunOpts(C.Structure):
@@ -89,6 +95,11 @@ def _load():
     L.orc_score_segment.argtypes = [vp, _dp, _dp, C.c_double, C.c_int, C.c_double, C.c_double]
     L.orc_score_segment.restype = C.c_int
     L.orc_close_batch.argtypes = [vp, C.c_uint64]; L.orc_close_batch.restype = C.c_int
+    L.orc_technique_set.argtypes = [vp, C.POINTER(_Technique)]; L.orc_technique_set.restype = C.c_int
+    L.orc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.orc_census_after_get.restype = C.c_int
+    L.orc_population_control.argtypes = [vp, C.c_size_t, _dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.c_uint64,
+                                         _ip, _dp]
+    L.orc_population_control.restype = C.c_int
     _lib = L
     return L
 
@@ -184,6 +195,27 @@ class Oracle:
 
     def reset(self):
         self._L.orc_reset(self._h)
+
+    def set_technique(self, implicit_capture=False, wr_threshold=0.0, wr_survive=0.0, population_control=False,
+                      pc_target=0):
+        t = _Technique(int(implicit_capture), float(wr_threshold), float(wr_survive), int(population_control),
+                       int(pc_target))
+        if self._L.orc_technique_set(self._h, C.byref(t)) != 0:
+            raise RuntimeError("orc_technique_set failed")
+
+    def census_after(self):
+        K = self.prob.n_census
+        w = np.empty(K); n = np.empty(K, dtype=np.uint64)
+        self._L.orc_census_after_get(self._h, _d(w), n.ctypes.data_as(C.POINTER(C.c_uint64)), K)
+        return w, n
+
+    def population_control(self, w, key, ctr, target):
+        w = np.ascontiguousarray(w, dtype=np.float64); key = np.ascontiguousarray(key, dtype=np.uint64)
+        ctr = np.ascontiguousarray(ctr, dtype=np.uint32)
+        n_out = np.zeros(len(w), dtype=np.int32); w_t = C.c_double(0.0)
+        self._L.orc_population_control(self._h, len(w), _d(w), key.ctypes.data_as(C.POINTER(C.c_uint64)),
+                                       ctr.ctypes.data_as(C.POINTER(C.c_uint32)), int(target), _i(n_out), C.byref(w_t))
+        return n_out, w_t.value
 
     def run(self, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False,
             bank_fifo=False, reverse_histories=False):

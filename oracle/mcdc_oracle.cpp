@@ -101,6 +101,8 @@ struct orc_problem {
   // results
   std::vector<double> x, sum, sumsq;         // batch accumulator, sum of S_b, sum of S_b^2
   std::vector<double> pop_w; std::vector<uint64_t> pop_n;
+  std::vector<double> pop_w_after; std::vector<uint64_t> pop_n_after;   // after the population control (G.3)
+  orc_technique tech;                        // Appendix G of DESIGN.md; all zero = analog
   orc_counters cnt;
   uint64_t batch_size;                       // histories per batch (must agree over runs)
   std::vector<uint32_t> hist_ev;             // [n][4] of the last run
@@ -351,18 +353,39 @@ void collision_event(orc_problem &P, Particle &p, std::deque<BankItem> &bank) {
   const int m = P.cell_material[p.cell], G = P.G;
   const size_t mg = (size_t)m * G + p.g;
   double xi = draw(p.key, p.ctr);
-  double y = xi * P.sigma_t[mg];
   double s_tot = P.sigma_s_tot[mg];
-  if (y < s_tot) {                                    // scatter
+  bool scatter;
+  if (P.tech.implicit_capture) {
+    // G.1 implicit capture: the captured fraction leaves the weight, the reaction is scatter | fission
+    double w_c = p.w * (P.sigma_c[mg] / P.sigma_t[mg]);
+    P.cnt.capture += w_c;
+    p.w -= w_c;
+    double s_r = s_tot + P.sigma_f[mg];
+    if (!(s_r > 0.0)) {                               // nothing but capture can happen here
+      P.cnt.capture += p.w; p.w = 0.0; p.alive = false; return;
+    }
+    double y = xi * s_r;
+    scatter = (y < s_tot) || P.sigma_f[mg] == 0.0;
+  } else {
+    double y = xi * P.sigma_t[mg];
+    scatter = y < s_tot;
+    if (!scatter && (y < s_tot + P.sigma_c[mg] || P.sigma_f[mg] == 0.0)) {   // capture (Sigma_f == 0 falls through to capture)
+      P.cnt.capture += p.w; p.alive = false; return;
+    }
+  }
+  if (scatter) {
+    // G.2 weight roulette of the surviving particle, before its outgoing flight is sampled
+    if (P.tech.wr_threshold > 0.0 && p.w < P.tech.wr_threshold) {
+      double xi_r = draw(p.key, p.ctr);
+      if (xi_r * P.tech.wr_survive < p.w) { P.cnt.vr_gain += P.tech.wr_survive - p.w; p.w = P.tech.wr_survive; }
+      else { P.cnt.vr_loss += p.w; p.alive = false; return; }
+    }
     double xi_g = draw(p.key, p.ctr);
     int gp = sample_cdf(&P.sigma_s[mg * G], G, xi_g * s_tot);
     double xi_mu = draw(p.key, p.ctr), xi_phi = draw(p.key, p.ctr);
     isotropic(xi_mu, xi_phi, p.ux, p.uy, p.uz);
     p.g = gp;
     return;
-  }
-  if (y < s_tot + P.sigma_c[mg] || P.sigma_f[mg] == 0.0) {   // capture (Sigma_f == 0 falls through to capture)
-    P.cnt.capture += p.w; p.alive = false; return;
   }
   double xi_nu = draw(p.key, p.ctr);                  // fission
   int n = (int)std::floor(P.nu[mg] + xi_nu);
@@ -390,8 +413,9 @@ void census_event(orc_problem &P, Particle &p, double d) {
   p.k += 1;
 }
 
-// A.2 transport one particle until it dies
-void transport(orc_problem &P, Particle &p, std::deque<BankItem> &bank) {
+// A.2 transport one particle until it dies -- or, with stop_at_census (G.3), until it has had a census event
+// that left it alive (the particle then waits in the census bank of its batch)
+bool transport(orc_problem &P, Particle &p, std::deque<BankItem> &bank, bool stop_at_census = false) {
   while (p.alive) {
     const int m = P.cell_material[p.cell];
     const double sig_t = P.sigma_t[(size_t)m * P.G + p.g];
@@ -416,9 +440,40 @@ void transport(orc_problem &P, Particle &p, std::deque<BankItem> &bank) {
     p.x += d * p.ux; p.y += d * p.uy; p.z += d * p.uz;
     p.t = (ev == 0) ? P.census[p.k] : p.t + d / v;
     P.cnt.segments += 1;
-    if (ev == 0) census_event(P, p, d);
+    if (ev == 0) { census_event(P, p, d); if (stop_at_census && p.alive) return true; }
     else if (ev == 1) surface_event(P, p, s_star);
     else collision_event(P, p, bank);
+  }
+  return false;
+}
+
+// G.3 population control of one batch's census bank at census k: splitting-roulette to the weight
+// w_t = W / target.  W is summed in 2^-40 fixed point so that it does not depend on the order of the bank.
+// `owner` (the local history index a particle descends from) rides along for the per-history event counts.
+const double FIX40 = 1099511627776.0;   // 2^40
+typedef std::pair<uint64_t, Particle> Owned;
+void population_control(orc_problem &P, const std::vector<Owned> &arrived, uint64_t target, int k,
+                        std::vector<Owned> &out) {
+  uint64_t w_fix = 0;
+  for (const Owned &a : arrived) w_fix += (uint64_t)(a.second.w * FIX40);
+  if (w_fix == 0 || target == 0) return;
+  const double w_t = ((double)w_fix / FIX40) / (double)target;
+  for (const Owned &a : arrived) {
+    Particle q = a.second;
+    double xi = draw(q.key, q.ctr);                   // the particle's own stream
+    int n = (int)std::floor(q.w / w_t + xi);
+    double dw = (double)n * w_t - q.w;
+    if (dw > 0.0) P.cnt.vr_gain += dw; else P.cnt.vr_loss += -dw;
+    if (n == 0) { P.cnt.pc_removed += 1; continue; }
+    P.cnt.pc_added += (uint64_t)(n - 1);
+    uint32_t c0 = q.ctr;
+    for (int j = 0; j < n; ++j) {
+      Particle c = q;                                 // same r, Omega, t, g, cell, last_surface, k
+      c.w = w_t;
+      if (j > 0) { c.key = child_key(q.key, c0, (uint32_t)j); c.ctr = 0; }
+      out.emplace_back(a.first, c);
+      P.pop_w_after[k] += w_t; P.pop_n_after[k] += 1;
+    }
   }
 }
 
@@ -521,8 +576,42 @@ int orc_create(const orc_desc *d, orc_problem **out) {
   P->n_bins = (size_t)d->Nt * d->G * d->mesh_n[2] * d->mesh_n[1] * d->mesh_n[0];
   build_boxes(*P);
   P->cur_ev = nullptr;
+  std::memset(&P->tech, 0, sizeof(P->tech));
   orc_reset(P);
   *out = P;
+  return 0;
+}
+
+int orc_technique_set(orc_problem *P, const orc_technique *t) {
+  if (!P) return -1;
+  if (!t) { std::memset(&P->tech, 0, sizeof(P->tech)); return 0; }
+  if (t->wr_threshold > 0.0 && !(t->wr_survive >= t->wr_threshold)) return -1;
+  P->tech = *t;
+  return 0;
+}
+
+int orc_census_after_get(const orc_problem *P, double *w, uint64_t *n, size_t K) {
+  if (K != (size_t)P->K) return -4;
+  for (size_t k = 0; k < K; ++k) { w[k] = P->pop_w_after[k]; n[k] = P->pop_n_after[k]; }
+  return 0;
+}
+
+// unit-level: the control applied to a bank given as arrays (pins of G.3); n_out[i] = copies of particle i
+int orc_population_control(orc_problem *P, size_t n, const double *w, const uint64_t *key, const uint32_t *ctr,
+                           uint64_t target, int32_t *n_out, double *w_t_out) {
+  std::vector<Owned> in, out;
+  for (size_t i = 0; i < n; ++i) {
+    Particle q; std::memset(&q, 0, sizeof(q));
+    q.w = w[i]; q.key = key[i]; q.ctr = ctr[i]; q.alive = true;
+    in.emplace_back((uint64_t)i, q);
+  }
+  orc_counters save = P->cnt;
+  std::vector<double> sw = P->pop_w_after; std::vector<uint64_t> sn = P->pop_n_after;
+  population_control(*P, in, target, 0, out);
+  P->cnt = save; P->pop_w_after = sw; P->pop_n_after = sn;
+  for (size_t i = 0; i < n; ++i) n_out[i] = 0;
+  for (const Owned &o : out) n_out[o.first] += 1;
+  *w_t_out = out.empty() ? 0.0 : out[0].second.w;
   return 0;
 }
 
@@ -531,6 +620,7 @@ void orc_destroy(orc_problem *p) { delete p; }
 void orc_reset(orc_problem *P) {
   P->x.assign(P->n_bins, 0.0); P->sum.assign(P->n_bins, 0.0); P->sumsq.assign(P->n_bins, 0.0);
   P->pop_w.assign(P->K, 0.0); P->pop_n.assign(P->K, 0);
+  P->pop_w_after.assign(P->K, 0.0); P->pop_n_after.assign(P->K, 0);
   std::memset(&P->cnt, 0, sizeof(P->cnt));
   P->batch_size = 0; P->hist_ev.clear(); P->cur_ev = nullptr;
 }
@@ -546,6 +636,44 @@ int orc_run(orc_problem *P, uint64_t n_histories, uint64_t seed, const orc_run_o
   P->batch_size = hb;
   if (o->record_history_events) P->hist_ev.assign((size_t)n_histories * 4, 0u); else P->hist_ev.clear();
   std::deque<BankItem> bank;
+  if (P->tech.population_control) {
+    // G.3: batch-synchronous census steps.  Step k transports every particle whose next census is C[k]
+    // (sources born in the step, survivors of the control at C[k-1], and all their fission progeny) up to
+    // C[k]; the arrivals are controlled and become the live bank of step k+1.
+    const uint64_t target = P->tech.pc_target ? P->tech.pc_target : hb;
+    for (uint32_t b = 0; b < B; ++b) {
+      std::vector<Owned> src;                              // (local history index, particle) of the batch
+      for (uint64_t i = 0; i < hb; ++i) {
+        uint64_t local = (uint64_t)b * hb + (o->reverse_histories ? (hb - 1 - i) : i);
+        P->cnt.histories += 1;
+        Particle p = source_particle(*P, seed, o->first_history_id + local);
+        if (p.alive) src.emplace_back(local, p);
+      }
+      std::vector<Owned> live, arrived;
+      for (int k = 0; k < P->K; ++k) {
+        for (auto &sp : src) if (sp.second.k == k) live.push_back(sp);
+        arrived.clear();
+        for (auto &lp : live) {
+          P->cur_ev = o->record_history_events ? &P->hist_ev[(size_t)lp.first * 4] : nullptr;
+          BankItem first; first.is_birth = false; first.p = lp.second;
+          bank.push_back(first);
+          while (!bank.empty()) {
+            BankItem it;
+            if (o->bank_fifo) { it = bank.front(); bank.pop_front(); }
+            else              { it = bank.back();  bank.pop_back(); }
+            if (it.is_birth) init_child(*P, it.p);
+            if (transport(*P, it.p, bank, true)) arrived.emplace_back(lp.first, it.p);
+          }
+        }
+        live.clear();
+        if (k == P->K - 1) break;
+        population_control(*P, arrived, target, k, live);
+      }
+      close_batch(*P);
+    }
+    P->cur_ev = nullptr;
+    return 0;
+  }
   for (uint32_t b = 0; b < B; ++b) {
     for (uint64_t i = 0; i < hb; ++i) {
       uint64_t local = (uint64_t)b * hb + (o->reverse_histories ? (hb - 1 - i) : i);

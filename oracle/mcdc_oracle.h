@@ -42,7 +42,28 @@ typedef struct {
 typedef struct {
   double source, production, capture, fission_abs, leak, census_final, lost;
   uint64_t histories, segments, collisions, surf_hits, census_events, children, lost_n, batches;
+  /* variance reduction (Appendix G of DESIGN.md): weight created / removed by weight roulette and by the
+   * population control at census, and the particles the control removed / added                         */
+  double vr_gain, vr_loss;
+  uint64_t pc_removed, pc_added;
 } orc_counters;
+
+/* Techniques named by the paper ("a variance reduction event"; "time-dependent
+ * population control"), in the reading of DESIGN.md Appendix G:
+ *  implicit_capture: at a collision capture += w Sigma_c/Sigma_t, w -= that, and the reaction is sampled
+ *    from scatter | fission alone (y = xi (Sigma_s_tot + Sigma_f));
+ *  weight roulette: a particle that scattered with w < wr_threshold draws xi; xi wr_survive < w keeps it
+ *    with w = wr_survive, else it dies;
+ *  population_control (splitting-roulette) at every census but the last, per statistical batch: with
+ *    W = sum over the batch's arrivals of trunc(w 2^40) 2^-40 and w_t = W / pc_target, a particle becomes
+ *    n = floor(w / w_t + xi) particles of weight w_t (copy 0 keeps its stream, copy j >= 1 takes the
+ *    stream child_key(key, ctr after xi, j)).                                                          */
+typedef struct {
+  int32_t implicit_capture;
+  double wr_threshold, wr_survive;       /* wr_threshold <= 0: no roulette                       */
+  int32_t population_control;
+  uint64_t pc_target;                    /* 0: the number of source histories of the batch        */
+} orc_technique;
 
 typedef struct {
   uint32_t n_batches;         /* B, must divide n_histories                                  */
@@ -53,6 +74,7 @@ typedef struct {
 } orc_run_opts;
 
 int  orc_create(const orc_desc *d, orc_problem **out);   /* deep copy; 0 or negative error   */
+int  orc_technique_set(orc_problem *p, const orc_technique *t);   /* NULL: analog (the default)        */
 void orc_destroy(orc_problem *p);
 void orc_reset(orc_problem *p);
 int  orc_run(orc_problem *p, uint64_t n_histories, uint64_t seed, const orc_run_opts *o);
@@ -61,6 +83,8 @@ int  orc_tally_sums_get(const orc_problem *p, double *sum, double *sumsq, size_t
 int  orc_counters_get(const orc_problem *p, orc_counters *c);
 int  orc_census_get(const orc_problem *p, double *pop_w, uint64_t *pop_n, size_t K);
 int  orc_history_events_get(const orc_problem *p, uint32_t *ev /* [n][4] */, size_t n);
+/* weight and number of particles that left the population control at census k (zero where no control ran) */
+int  orc_census_after_get(const orc_problem *p, double *pop_w, uint64_t *pop_n, size_t K);
 
 /* unit-level entry points used by the pins (tests/test_oracle_*.py) */
 uint64_t orc_mix64(uint64_t z);
@@ -77,6 +101,9 @@ int      orc_stream(const orc_problem *p, double r[3], double omega[3], int32_t 
 int      orc_score_segment(orc_problem *p, const double r[3], const double omega[3], double t, int g,
                            double w, double d);
 int      orc_close_batch(orc_problem *p, uint64_t histories_in_batch);
+/* the population control of G.3 applied to a bank given as arrays: n_out[i] = copies made of particle i */
+int      orc_population_control(orc_problem *p, size_t n, const double *w, const uint64_t *key, const uint32_t *ctr,
+                                uint64_t target, int32_t *n_out, double *w_t_out);
 
 #ifdef __cplusplus
 }
