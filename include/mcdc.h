@@ -102,7 +102,34 @@ typedef struct {
   uint64_t kernel_launches;       /* launches of this library's kernels since create/reset          */
   double ms_run;                  /* device time of the last mcdc_run (CUDA events on its stream)   */
   double ms_transport;            /* of which: transport kernels of the last run                    */
+  /* variance reduction (mcdc_technique): weight created / removed by the weight roulette and by the
+   * population control, particles the control removed / added.  The ledger then reads
+   * source + production + vr_gain == capture + fission_abs + leak + census_final + lost + vr_loss
+   * (to rounding: weights are no longer integers).                                                 */
+  double vr_gain, vr_loss;
+  uint64_t pc_removed, pc_added;
 } mcdc_counters;
+
+/* Techniques the paper names without defining them: "a variance reduction event" among the events
+ * that end a flight and "time-dependent population control"; SURVEY.md
+ * 8(f) NEXT-1; definition in DESIGN.md Appendix G.
+ *  implicit_capture: at a collision capture += w Sigma_c/Sigma_t, w -= that, and the reaction is
+ *    sampled from scatter | fission alone (y = xi (Sigma_s_tot + Sigma_f)).
+ *  wr_threshold > 0: a particle that scattered with w < wr_threshold draws xi; if xi wr_survive < w it
+ *    continues with w = wr_survive (wr_survive >= wr_threshold), else it dies.
+ *  population_control: at every census but the last, per statistical batch, splitting-roulette to the
+ *    weight w_t = W / pc_target (W = the batch's arriving weight summed in 2^-40 fixed point;
+ *    pc_target = 0 means the batch's number of source histories): a particle becomes
+ *    floor(w / w_t + xi) particles of weight w_t.  Needs the census-stepped scheduler (chosen
+ *    automatically) and batches that fit one slot of the workspace, else MCDC_ERR_ARG.             */
+typedef struct {
+  int32_t implicit_capture;
+  double wr_threshold, wr_survive;
+  int32_t population_control;
+  uint64_t pc_target;
+} mcdc_technique;
+/* t == NULL restores analog transport (the default).  Takes effect from the next run.              */
+int mcdc_technique_set(mcdc_problem *p, const mcdc_technique *t);
 
 /* Validates and deep-copies *d, classifies surfaces, builds cell-neighbour tables and uploads the
  * problem to the current CUDA device.  *out is untouched on error.                                */
@@ -139,6 +166,8 @@ int mcdc_tally_sums_get(const mcdc_problem *p, double *sum, double *sumsq, size_
 int mcdc_counters_get(const mcdc_problem *p, mcdc_counters *c);
 /* Population bookkeeping at census: summed weight and number of particles that reached census k.  */
 int mcdc_census_get(const mcdc_problem *p, double *pop_w, uint64_t *pop_n, size_t n_census);
+/* Weight and number of particles that LEFT the population control at census k (zero where none ran). */
+int mcdc_census_after_get(const mcdc_problem *p, double *pop_w, uint64_t *pop_n, size_t n_census);
 /* ev[h][0..3] = collisions, surface events, fission children, census events of history
  * first_history_id+h of the LAST run (needs record_history_events).                               */
 int mcdc_history_events_get(const mcdc_problem *p, uint32_t *ev, size_t n_histories);
@@ -160,7 +189,7 @@ int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
  * a host buffer) and put the sum back:
  *   [0, n_bins) sum   [n_bins, 2 n_bins) sumsq   then pop_w[K], pop_n[K], ledger[7] (source production
  *   capture fission_abs leak census_final lost), counts[7] (histories segments collisions surf_hits
- *   census_events children lost_n), roulette[2] (gain, loss), histories, batches.
+ *   census_events children lost_n), vr[2] (gain, loss), pc[2] (removed, added), histories, batches.
  * Integer entries are stored as doubles (exact below 2^53).  on_device != 0: buf is DEVICE memory
  * (copies run on the bound stream, synchronous on return); else HOST memory.  n must equal
  * mcdc_state_size.  Import REPLACES the handle's accumulators; ranks must use the same batch size. */

@@ -22,6 +22,11 @@ from .api import (  # noqa: F401
     mcdc_counters_get,
     mcdc_census_get,
     mcdc_history_events_get,
+    mcdc_technique_set,
+    mcdc_census_after_get,
+    mcdc_state_size,
+    mcdc_state_export,
+    mcdc_state_import,
     mcdc_strerror,
     mcdc_version,
     EXPORTED_SYMBOLS,

@@ -18,7 +18,8 @@ EXPORTED_SYMBOLS = [
     "mcdc_problem_create", "mcdc_problem_destroy", "mcdc_problem_reset", "mcdc_workspace_size", "mcdc_workspace_size_async", "mcdc_problem_info_get",
     "mcdc_workspace_bind", "mcdc_run", "mcdc_run_ex", "mcdc_tallies_get", "mcdc_tally_sums_get",
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
-    "mcdc_last_cuda_error", "mcdc_version",
+    "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
+    "mcdc_state_size", "mcdc_state_export", "mcdc_state_import",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -58,10 +59,16 @@ class Counters(C.Structure):
                 ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost")] + \
                [(n, C.c_uint64) for n in ("histories", "segments", "collisions", "surf_hits", "census_events",
                                           "children", "lost_n", "batches", "kernel_launches")] + \
-               [("ms_run", C.c_double), ("ms_transport", C.c_double)]
+               [("ms_run", C.c_double), ("ms_transport", C.c_double), ("vr_gain", C.c_double), ("vr_loss", C.c_double),
+                ("pc_removed", C.c_uint64), ("pc_added", C.c_uint64)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class Technique(C.Structure):
+    _fields_ = [("implicit_capture", C.c_int32), ("wr_threshold", C.c_double), ("wr_survive", C.c_double),
+                ("population_control", C.c_int32), ("pc_target", C.c_uint64)]
 
 
 _lib = None
@@ -104,6 +111,12 @@ def lib():
     L.mcdc_census_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.mcdc_census_get.restype = C.c_int
     L.mcdc_history_events_get.argtypes = [vp, C.POINTER(C.c_uint32), C.c_size_t]
     L.mcdc_history_events_get.restype = C.c_int
+    L.mcdc_technique_set.argtypes = [vp, C.POINTER(Technique)]; L.mcdc_technique_set.restype = C.c_int
+    L.mcdc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]
+    L.mcdc_census_after_get.restype = C.c_int
+    L.mcdc_state_size.argtypes = [vp, C.POINTER(C.c_size_t)]; L.mcdc_state_size.restype = C.c_int
+    L.mcdc_state_export.argtypes = [vp, vp, C.c_size_t, C.c_int]; L.mcdc_state_export.restype = C.c_int
+    L.mcdc_state_import.argtypes = [vp, vp, C.c_size_t, C.c_int]; L.mcdc_state_import.restype = C.c_int
     L.mcdc_strerror.argtypes = [C.c_int]; L.mcdc_strerror.restype = C.c_char_p
     L.mcdc_last_cuda_error.argtypes = [vp]; L.mcdc_last_cuda_error.restype = C.c_char_p
     L.mcdc_version.argtypes = []; L.mcdc_version.restype = C.c_char_p
@@ -250,6 +263,34 @@ def mcdc_history_events_get(h, n_histories):
     return ev
 
 
+def mcdc_technique_set(h, implicit_capture=False, wr_threshold=0.0, wr_survive=0.0, population_control=False,
+                       pc_target=0):
+    t = Technique(int(bool(implicit_capture)), float(wr_threshold), float(wr_survive), int(bool(population_control)),
+                  int(pc_target))
+    _check(lib().mcdc_technique_set(h, C.byref(t)), "mcdc_technique_set", h)
+
+
+def mcdc_census_after_get(h, n_census):
+    w = np.empty(n_census); n = np.empty(n_census, dtype=np.uint64)
+    _check(lib().mcdc_census_after_get(h, _d(w), n.ctypes.data_as(C.POINTER(C.c_uint64)), n_census),
+           "mcdc_census_after_get", h)
+    return w, n
+
+
+def mcdc_state_size(h) -> int:
+    n = C.c_size_t(0)
+    _check(lib().mcdc_state_size(h, C.byref(n)), "mcdc_state_size", h)
+    return int(n.value)
+
+
+def mcdc_state_export(h, ptr, n_doubles, on_device):
+    _check(lib().mcdc_state_export(h, C.c_void_p(int(ptr)), int(n_doubles), int(bool(on_device))), "mcdc_state_export", h)
+
+
+def mcdc_state_import(h, ptr, n_doubles, on_device):
+    _check(lib().mcdc_state_import(h, C.c_void_p(int(ptr)), int(n_doubles), int(bool(on_device))), "mcdc_state_import", h)
+
+
 # ---- convenience wrapper: owns the handle and the torch workspace ------------------------------
 class Problem:
     """Handle + PyTorch-owned workspace.  Marshalling only; all work happens in libmcdc.so."""
@@ -325,3 +366,25 @@ class Problem:
 
     def history_events(self):
         return mcdc_history_events_get(self._h, self._last_n)
+
+    def set_technique(self, **kw):
+        mcdc_technique_set(self._h, **kw)
+
+    def census_after(self):
+        return mcdc_census_after_get(self._h, int(self.prob.n_census))
+
+    # ---- multi-rank: the accumulators as one fp64 vector (include/mcdc.h) ----
+    def state_size(self):
+        return mcdc_state_size(self._h)
+
+    def state_export(self, tensor):
+        """tensor: contiguous float64 torch tensor of state_size() elements, on this device or on the host."""
+        mcdc_state_export(self._h, tensor.data_ptr(), tensor.numel(), tensor.is_cuda)
+
+    def state_import(self, tensor):
+        mcdc_state_import(self._h, tensor.data_ptr(), tensor.numel(), tensor.is_cuda)
+
+    def all_reduce(self, group=None):
+        """Sum the accumulators of all ranks into every rank's handle (NCCL on the device buffer)."""
+        from .sharding import all_reduce_state
+        all_reduce_state(self, group=group, device=self.device)

@@ -37,6 +37,7 @@ struct TB {
   __device__ __forceinline__ double sig_sc(int mg) const { return ld<double>(T.o_sig_sc, mg); }
   __device__ __forceinline__ double sig_f(int mg) const { return ld<double>(T.o_sig_f, mg); }
   __device__ __forceinline__ double nu(int mg) const { return ld<double>(T.o_nu, mg); }
+  __device__ __forceinline__ double cap_frac(int mg) const { return ld<double>(T.o_cap_frac, mg); }
   __device__ __forceinline__ double cdf_s(int i) const { return ld<double>(T.o_cdf_s, i); }
   __device__ __forceinline__ int last_s(int mg) const { return ld<int>(T.o_last_s, mg); }
   __device__ __forceinline__ double cdf_chi(int i) const { return ld<double>(T.o_cdf_chi, i); }

@@ -73,8 +73,10 @@ struct mcdc_problem {
   // device
   DeviceArena arena;
   Tables tab;
-  double *d_sum = nullptr, *d_sumsq = nullptr, *d_pop_w = nullptr;
-  unsigned long long *d_pop_n = nullptr;
+  double *d_sum = nullptr, *d_sumsq = nullptr, *d_pop_w = nullptr, *d_pop_w_after = nullptr;
+  unsigned long long *d_pop_n = nullptr, *d_pop_n_after = nullptr;
+  unsigned long long *d_wfix = nullptr;   // [ws_slots] arriving weight of a batch in 2^-40 fixed point (workspace)
+  mcdc_technique tech = {0, 0.0, 0.0, 0, 0ull};
   DevCounters *d_cnt = nullptr;
   uint32_t *d_ev = nullptr;      // [n][4] of the last run (cudaMalloc'ed on demand)
   size_t ev_n = 0;
@@ -587,6 +589,12 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   t.o_sig_f = putd(p->sigma_f); t.o_nu = putd(p->nu); t.o_cdf_s = putd(cdf_s); t.o_last_s = puti(last_s);
   t.o_cdf_chi = putd(cdf_chi); t.o_last_chi = puti(last_chi); t.o_speed = putd(p->speed); t.o_inv_speed = putd(inv_speed);
   t.o_T = putd(p->T); t.o_census = putd(p->census); t.o_src_cdf = putd(src_cdf);
+  {
+    std::vector<double> cap_frac((size_t)M * G);          // Sigma_c / Sigma_t (implicit capture, Appendix G.1)
+    for (size_t i = 0; i < cap_frac.size(); ++i) cap_frac[i] = p->sigma_t[i] > 0.0 ? p->sigma_c[i] / p->sigma_t[i] : 0.0;
+    t.o_cap_frac = putd(cap_frac);
+  }
+  t.implicit_capture = 0; t.wr_threshold = 0.0; t.wr_survive = 0.0;
   t.o_tbin_k = puti(tbin_k); t.o_it0_k = puti(it0_k);
   t.o_surf_q = put(q.data(), q.size() * sizeof(double4));
   t.o_cell2 = put(cell2.data(), cell2.size()); t.o_other2 = put(other2.data(), other2.size());
@@ -621,6 +629,7 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   }
   p->d_sum = ar.zeros<double>(p->n_bins); p->d_sumsq = ar.zeros<double>(p->n_bins);
   p->d_pop_w = ar.zeros<double>(p->K); p->d_pop_n = ar.zeros<unsigned long long>(p->K);
+  p->d_pop_w_after = ar.zeros<double>(p->K); p->d_pop_n_after = ar.zeros<unsigned long long>(p->K);
   p->d_cnt = ar.zeros<DevCounters>(1);
   p->d_hist_cursor = ar.zeros<uint32_t>(1);
   p->d_head_tail = ar.zeros<unsigned long long>(2);
@@ -649,6 +658,8 @@ extern "C" int mcdc_problem_reset(mcdc_problem *p) {
   CK(cudaMemsetAsync(p->d_sumsq, 0, p->n_bins * sizeof(double), p->stream));
   CK(cudaMemsetAsync(p->d_pop_w, 0, p->K * sizeof(double), p->stream));
   CK(cudaMemsetAsync(p->d_pop_n, 0, p->K * sizeof(unsigned long long), p->stream));
+  CK(cudaMemsetAsync(p->d_pop_w_after, 0, p->K * sizeof(double), p->stream));
+  CK(cudaMemsetAsync(p->d_pop_n_after, 0, p->K * sizeof(unsigned long long), p->stream));
   CK(cudaMemsetAsync(p->d_cnt, 0, sizeof(DevCounters), p->stream));
   if (p->x_acc) CK(cudaMemsetAsync(p->x_acc, 0, (size_t)p->ws_slots * p->n_bins * sizeof(double), p->stream));
   CK(cudaStreamSynchronize(p->stream));
@@ -684,7 +695,7 @@ WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap, uint64_t hi
   WsLayout L;
   size_t off = 0;
   L.x_acc = off; off += align_up((size_t)slots * p->n_bins * sizeof(double), 256);
-  L.counts = off; off += align_up((size_t)8 * slots * sizeof(uint32_t), 256);
+  L.counts = off; off += align_up((size_t)10 * slots * sizeof(uint32_t), 256);   // 8 bank counters + one u64 (wfix) per slot
   L.q_cap = queue_capacity(hist);
   L.q_flag = off; off += align_up((size_t)L.q_cap * sizeof(uint32_t), 256);
   L.fixed = off;
@@ -775,6 +786,7 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
   carve_bank(p->bankB, p->ws, L.bank[1], n, true, cnt + 2 * max_slots, cnt + 3 * max_slots);
   carve_bank(p->bankS1, p->ws, L.bank[2], n, false, cnt + 4 * max_slots, cnt + 5 * max_slots);
   carve_bank(p->bankS2, p->ws, L.bank[3], n, false, cnt + 6 * max_slots, cnt + 7 * max_slots);
+  p->d_wfix = reinterpret_cast<unsigned long long *>(cnt + 8 * max_slots);
   CK(cudaMemsetAsync(p->ws, 0, L.fixed, p->stream));
   CK(cudaStreamSynchronize(p->stream));
   return MCDC_OK;
@@ -886,7 +898,33 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
         live_total += hc[s];
       }
     }
-    std::swap(A, Bk);
+    if (p->tech.population_control && k < p->K - 1 && live_total > 0) {
+      // Appendix G.3: the census bank Bk is controlled into the (consumed) live bank A, batch by batch
+      uint32_t n_max = 0;
+      {
+        const uint32_t *hc = h_counts.data() + (Bk.count - counts_dev);
+        for (uint32_t s = 0; s < ns; ++s) n_max = std::max(n_max, hc[s]);
+      }
+      PcParams pc;
+      pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs;
+      const dim3 grid((n_max + 255) / 256, ns);
+      CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
+      CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
+      k_pc_weight<<<grid, 256, 0, p->stream>>>(Bk, p->cap, p->d_wfix);
+      k_pc_apply<<<grid, 256, 0, p->stream>>>(Bk, A, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
+      p->launches += 2;
+      CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+      CK(cudaStreamSynchronize(p->stream));
+      CK(cudaGetLastError());
+      const uint32_t *hc = h_counts.data() + (A.count - counts_dev);
+      live_total = 0;
+      for (uint32_t s = 0; s < ns; ++s) {
+        if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
+        live_total += hc[s];
+      }
+    } else {
+      std::swap(A, Bk);
+    }
     CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));
   }
   if (sb.closeout) {
@@ -899,7 +937,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 
 // ---- k_warp instantiations: (tables staged, per-history events recorded, threads per block) ----
 #ifndef MCDC_WARP_CASES
-#define MCDC_WARP_CASES(X) X(256) X(384) X(512) X(640) X(768) X(1024)
+#define MCDC_WARP_CASES(X) X(256) X(512) X(1024)
 #endif
 template <bool STAGED, bool RECORD>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
@@ -934,7 +972,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record) {
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   int nt = 512;
   if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
-  if (nt != 256 && nt != 384 && nt != 512 && nt != 640 && nt != 768 && nt != 1024) nt = 512;
+  if (nt != 256 && nt != 512 && nt != 1024) nt = 512;
   const int nw = nt / 32;
   const size_t pop_bytes = align_up((size_t)p->K * 4, 16);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
@@ -1020,7 +1058,9 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   const bool record = opts->record_history_events != 0;
   if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
   // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
-  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u;
+  // ... and so do the techniques the history kernel does not implement
+  const bool vr = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->tech.population_control;
+  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u || vr;
   if (record) {
     if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
     CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
@@ -1053,6 +1093,7 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   if (stepped && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
   const uint64_t slot_max = stepped ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
   int rc = MCDC_OK;
+  if (p->tech.population_control && hb > slot_max) return MCDC_ERR_ARG;   // the control acts on whole batches
   if (hb <= slot_max) {                                  // whole batches, one per slot
     const uint32_t per_sub = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(p->ws_slots, p->ws_hist / hb));
     for (uint32_t b = 0; b < B && rc == MCDC_OK; b += per_sub) {
@@ -1145,6 +1186,7 @@ extern "C" int mcdc_counters_get(const mcdc_problem *cp, mcdc_counters *c) {
   c->leak = h.ledger[4]; c->census_final = h.ledger[5]; c->lost = h.ledger[6];
   c->histories = h.n[0]; c->segments = h.n[1]; c->collisions = h.n[2]; c->surf_hits = h.n[3];
   c->census_events = h.n[4]; c->children = h.n[5]; c->lost_n = h.n[6];
+  c->vr_gain = h.ledger[7]; c->vr_loss = h.ledger[8]; c->pc_removed = h.n[7]; c->pc_added = h.n[8];
   c->batches = p->batches; c->kernel_launches = p->launches;
   c->ms_run = p->ms_run; c->ms_transport = p->ms_transport;
   return MCDC_OK;
@@ -1156,6 +1198,91 @@ extern "C" int mcdc_census_get(const mcdc_problem *cp, double *pop_w, uint64_t *
   if (K != (size_t)p->K) return MCDC_ERR_SIZE;
   CK(cudaMemcpy(pop_w, p->d_pop_w, K * sizeof(double), cudaMemcpyDeviceToHost));
   CK(cudaMemcpy(pop_n, p->d_pop_n, K * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_census_after_get(const mcdc_problem *cp, double *pop_w, uint64_t *pop_n, size_t K) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !pop_w || !pop_n) return MCDC_ERR_ARG;
+  if (K != (size_t)p->K) return MCDC_ERR_SIZE;
+  CK(cudaMemcpy(pop_w, p->d_pop_w_after, K * sizeof(double), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(pop_n, p->d_pop_n_after, K * sizeof(uint64_t), cudaMemcpyDeviceToHost));
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_technique_set(mcdc_problem *p, const mcdc_technique *t) {
+  if (!p) return MCDC_ERR_ARG;
+  mcdc_technique z = {0, 0.0, 0.0, 0, 0ull};
+  if (!t) t = &z;
+  if (t->wr_threshold > 0.0 && !(t->wr_survive >= t->wr_threshold)) return MCDC_ERR_ARG;
+  if (t->wr_threshold < 0.0 || t->wr_threshold != t->wr_threshold) return MCDC_ERR_ARG;
+  p->tech = *t;
+  p->tab.implicit_capture = t->implicit_capture ? 1 : 0;   // Tables travel by value with every launch
+  p->tab.wr_threshold = t->wr_threshold > 0.0 ? t->wr_threshold : 0.0;
+  p->tab.wr_survive = t->wr_survive;
+  return MCDC_OK;
+}
+
+// ---- multi-rank reduction support (include/mcdc.h "Multi-GPU domain replication") ----
+namespace {
+size_t state_doubles(const mcdc_problem *p) { return 2 * p->n_bins + 2 * (size_t)p->K + 9 + 9 + 2; }
+}
+extern "C" int mcdc_state_size(const mcdc_problem *p, size_t *n) {
+  if (!p || !n) return MCDC_ERR_ARG;
+  *n = state_doubles(p);
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_state_export(const mcdc_problem *cp, double *buf, size_t n, int on_device) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !buf) return MCDC_ERR_ARG;
+  if (n != state_doubles(p)) return MCDC_ERR_SIZE;
+  const size_t nb = p->n_bins, K = (size_t)p->K;
+  const cudaMemcpyKind big = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+  CK(cudaMemcpyAsync(buf, p->d_sum, nb * sizeof(double), big, p->stream));
+  CK(cudaMemcpyAsync(buf + nb, p->d_sumsq, nb * sizeof(double), big, p->stream));
+  CK(cudaMemcpyAsync(buf + 2 * nb, p->d_pop_w, K * sizeof(double), big, p->stream));
+  // the integer tail goes through the host (a few hundred bytes)
+  std::vector<unsigned long long> pn(K);
+  DevCounters h;
+  CK(cudaMemcpyAsync(pn.data(), p->d_pop_n, K * sizeof(unsigned long long), cudaMemcpyDeviceToHost, p->stream));
+  CK(cudaMemcpyAsync(&h, p->d_cnt, sizeof(h), cudaMemcpyDeviceToHost, p->stream));
+  CK(cudaStreamSynchronize(p->stream));
+  std::vector<double> tail(K + 20);
+  for (size_t k = 0; k < K; ++k) tail[k] = (double)pn[k];
+  for (int e = 0; e < 9; ++e) { tail[K + e] = h.ledger[e]; tail[K + 9 + e] = (double)h.n[e]; }
+  tail[K + 18] = (double)p->histories; tail[K + 19] = (double)p->batches;
+  double *dst = buf + 2 * nb + K;
+  if (on_device) {
+    CK(cudaMemcpyAsync(dst, tail.data(), tail.size() * sizeof(double), cudaMemcpyHostToDevice, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+  } else std::memcpy(dst, tail.data(), tail.size() * sizeof(double));
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_state_import(mcdc_problem *p, const double *buf, size_t n, int on_device) {
+  if (!p || !buf) return MCDC_ERR_ARG;
+  if (n != state_doubles(p)) return MCDC_ERR_SIZE;
+  const size_t nb = p->n_bins, K = (size_t)p->K;
+  const cudaMemcpyKind big = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  CK(cudaMemcpyAsync(p->d_sum, buf, nb * sizeof(double), big, p->stream));
+  CK(cudaMemcpyAsync(p->d_sumsq, buf + nb, nb * sizeof(double), big, p->stream));
+  CK(cudaMemcpyAsync(p->d_pop_w, buf + 2 * nb, K * sizeof(double), big, p->stream));
+  std::vector<double> tail(K + 20);
+  const double *src = buf + 2 * nb + K;
+  if (on_device) {
+    CK(cudaMemcpyAsync(tail.data(), src, tail.size() * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+  } else std::memcpy(tail.data(), src, tail.size() * sizeof(double));
+  std::vector<unsigned long long> pn(K);
+  for (size_t k = 0; k < K; ++k) pn[k] = (unsigned long long)llround(tail[k]);
+  DevCounters h;
+  std::memset(&h, 0, sizeof(h));
+  for (int e = 0; e < 9; ++e) { h.ledger[e] = tail[K + e]; h.n[e] = (unsigned long long)llround(tail[K + 9 + e]); }
+  CK(cudaMemcpyAsync(p->d_pop_n, pn.data(), K * sizeof(unsigned long long), cudaMemcpyHostToDevice, p->stream));
+  CK(cudaMemcpyAsync(p->d_cnt, &h, sizeof(h), cudaMemcpyHostToDevice, p->stream));
+  CK(cudaStreamSynchronize(p->stream));
+  p->histories = (uint64_t)llround(tail[K + 18]); p->batches = (uint64_t)llround(tail[K + 19]);
   return MCDC_OK;
 }
 

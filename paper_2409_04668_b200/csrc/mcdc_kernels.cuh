@@ -482,7 +482,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
         } else {
           pc_coll += 1u;
           int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
-                                  &acc.led[LED_PRODUCTION][tid]);
+                                  &acc.led[LED_PRODUCTION][tid], &acc.led[LED_VR_GAIN][tid], &acc.led[LED_VR_LOSS][tid]);
           if (r == -1) fi = FI_SCATTER; else have = false;
           if (r > 0) { n_children = r; pc_child += (uint32_t)r; }
         }
@@ -540,6 +540,86 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
   accum_flush(acc, A.cnt);
   block_atomic_add(A.pop_w + P.k, popw, acc.scratch);
   block_atomic_add_u64(A.pop_n + P.k, (unsigned long long)popn, (unsigned long long *)acc.scratch);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Population control at census (Appendix G.3; "time-dependent population control"), census-stepped
+// scheduler.  Per batch slot: k_pc_weight sums the arriving weight in 2^-40 fixed point (an integer sum: the
+// result does not depend on the order of the bank), k_pc_apply turns every particle of the census bank into
+// floor(w / w_t + xi) particles of weight w_t = W / target in the next live bank.  Grid: (chunks of 256, slots).
+// ------------------------------------------------------------------------------------------------
+#define MCDC_FIX40 1099511627776.0   // 2^40
+
+__global__ void __launch_bounds__(256) k_pc_weight(Bank in, uint32_t cap, unsigned long long *wfix) {
+  __shared__ unsigned long long scratch[32];
+  const int slot = blockIdx.y;
+  const uint32_t n = min(in.count[slot], cap);
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  unsigned long long v = 0ull;
+  if (i < n) v = (unsigned long long)(in.w[(size_t)slot * cap + i] * MCDC_FIX40);   // truncation, as the oracle's cast
+  block_atomic_add_u64(wfix + slot, v, scratch);
+}
+
+struct PcParams {
+  uint32_t cap;
+  int k;                              // census index
+  unsigned long long target;          // particles per batch after the control
+};
+
+__global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P, const unsigned long long *wfix,
+                                                  DevCounters *cnt, double *pop_w_after, unsigned long long *pop_n_after) {
+  __shared__ double scratch[32];
+  const int slot = blockIdx.y, lane = lane_id();
+  const uint32_t n_in = min(in.count[slot], P.cap);
+  const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+  const unsigned long long W = wfix[slot];
+  const bool have = i < n_in && W != 0ull;
+  const size_t j = (size_t)slot * P.cap + (have ? i : 0u);
+  const double w_t = ((double)W / MCDC_FIX40) / (double)P.target;
+  double w = 0.0, gain = 0.0, loss = 0.0;
+  unsigned long long key = 0ull;
+  uint32_t ctr = 0u;
+  int4 m = make_int4(0, -1, 0, 0);
+  int n = 0;
+  if (have) {
+    w = in.w[j]; key = in.key[j]; m = in.meta[j]; ctr = (uint32_t)m.z;
+  }
+  const double xi = draw(key, ctr);                      // the particle's own stream
+  if (have) {
+    n = (int)floor(w / w_t + xi);
+    const double dw = (double)n * w_t - w;
+    if (dw > 0.0) gain = dw; else loss = -dw;
+  }
+  // ballot-free inclusive scan of the copies over the warp, one atomic per warp on the slot's counter
+  int pre = n;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int v = __shfl_up_sync(MCDC_FULL, pre, o);
+    if (lane >= o) pre += v;
+  }
+  const int total = __shfl_sync(MCDC_FULL, pre, 31);
+  uint32_t base = 0u;
+  if (lane == 0 && total > 0) base = atomicAdd(out.count + slot, (uint32_t)total);
+  base = __shfl_sync(MCDC_FULL, base, 0) + (uint32_t)(pre - n);
+  if (n > 0) {
+    const double x = in.x[j], y = in.y[j], z = in.z[j], ux = in.ux[j], uy = in.uy[j], uz = in.uz[j], t = in.t[j];
+    const uint32_t hid = in.hid[j];
+    for (int c = 0; c < n; ++c) {
+      const uint32_t o = base + (uint32_t)c;
+      if (o >= P.cap) { atomicExch(&cnt->overflow, 1); break; }
+      const size_t q = (size_t)slot * P.cap + o;
+      out.x[q] = x; out.y[q] = y; out.z[q] = z; out.ux[q] = ux; out.uy[q] = uy; out.uz[q] = uz; out.t[q] = t;
+      out.w[q] = w_t; out.hid[q] = hid;
+      out.key[q] = (c == 0) ? key : child_key(key, ctr, (uint32_t)c);   // copy 0 keeps its stream
+      out.meta[q] = make_int4(m.x, m.y, (c == 0) ? (int)ctr : 0, m.w);
+    }
+  }
+  block_atomic_add(&cnt->ledger[1 + LED_VR_GAIN], gain, scratch);
+  block_atomic_add(&cnt->ledger[1 + LED_VR_LOSS], loss, scratch);
+  block_atomic_add_u64(&cnt->n[7], (have && n == 0) ? 1ull : 0ull, (unsigned long long *)scratch);
+  block_atomic_add_u64(&cnt->n[8], (n > 1) ? (unsigned long long)(n - 1) : 0ull, (unsigned long long *)scratch);
+  block_atomic_add(pop_w_after + P.k, (double)n * w_t, scratch);
+  block_atomic_add_u64(pop_n_after + P.k, (unsigned long long)n, (unsigned long long *)scratch);
 }
 
 // ------------------------------------------------------------------------------------------------

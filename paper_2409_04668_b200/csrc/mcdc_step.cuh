@@ -6,7 +6,7 @@
 
 namespace mcdc {
 
-enum { LED_PRODUCTION = 0, LED_CAPTURE, LED_FISSION_ABS, LED_LEAK, LED_CENSUS_FINAL, LED_LOST, LED_N };
+enum { LED_PRODUCTION = 0, LED_CAPTURE, LED_FISSION_ABS, LED_LEAK, LED_CENSUS_FINAL, LED_LOST, LED_VR_GAIN, LED_VR_LOSS, LED_N };
 enum { CNT_COLL = 0, CNT_SURF, CNT_CENSUS, CNT_CHILDREN, CNT_LOST, CNT_N };
 
 // what a lane still has to sample before its particle can fly (draw order of A.3 / A.6 is kept per particle)
@@ -136,16 +136,38 @@ __device__ __forceinline__ bool surface_event(const TBT &tb, PState &p, int i_st
   return true;
 }
 
-// A.6 reaction choice.  Returns -1: scattered (the caller must run flight_init(FI_SCATTER) before the next
-// segment); -2: captured; n >= 0: absorbed by fission with n children, c0 = parent's counter after the nu draw.
+// A.6 reaction choice, with the techniques of Appendix G when the problem asks for them.  Returns -1: scattered
+// (the caller must run flight_init(FI_SCATTER) before the next segment); -2: dead (captured, or killed by the
+// weight roulette); n >= 0: absorbed by fission with n children, c0 = parent's counter after the nu draw.
 template <class TBT>
 __device__ __forceinline__ int collision_event(const TBT &tb, PState &p, uint32_t &c0, double *led_capture,
-                                               double *led_fis, double *led_prod) {
+                                               double *led_fis, double *led_prod, double *led_gain, double *led_loss) {
+  const Tables &T = tb.T;
   p.last_surf = -1;
-  const int mg = tb.cell_mat(p.cell) * tb.T.G + p.g;
-  const double yv = draw(p.key, p.ctr) * tb.sig_t(mg);
-  if (yv < tb.sig_s_tot(mg)) return -1;
-  if (yv < tb.sig_sc(mg) || tb.sig_f(mg) == 0.0) { *led_capture += p.w; return -2; }
+  const int mg = tb.cell_mat(p.cell) * T.G + p.g;
+  const double xi = draw(p.key, p.ctr);
+  const double s_tot = tb.sig_s_tot(mg), sig_f = tb.sig_f(mg);
+  bool scatter;
+  if (T.implicit_capture) {                                // G.1
+    const double w_c = p.w * tb.cap_frac(mg);
+    *led_capture += w_c;
+    p.w -= w_c;
+    const double s_r = s_tot + sig_f;
+    if (!(s_r > 0.0)) { *led_capture += p.w; p.w = 0.0; return -2; }
+    scatter = (xi * s_r < s_tot) || sig_f == 0.0;
+  } else {
+    const double yv = xi * tb.sig_t(mg);
+    scatter = yv < s_tot;
+    if (!scatter && (yv < tb.sig_sc(mg) || sig_f == 0.0)) { *led_capture += p.w; return -2; }
+  }
+  if (scatter) {
+    if (T.wr_threshold > 0.0 && p.w < T.wr_threshold) {    // G.2
+      const double xi_r = draw(p.key, p.ctr);
+      if (xi_r * T.wr_survive < p.w) { *led_gain += T.wr_survive - p.w; p.w = T.wr_survive; }
+      else { *led_loss += p.w; return -2; }
+    }
+    return -1;
+  }
   const double xi_nu = draw(p.key, p.ctr);
   const int n = (int)floor(tb.nu(mg) + xi_nu);
   c0 = p.ctr;

@@ -46,6 +46,7 @@ struct Tables {
   uint32_t o_T;         // [Nt+1]
   uint32_t o_census;    // [K]
   uint32_t o_src_cdf;   // [G]
+  uint32_t o_cap_frac;  // [M*G] Sigma_c / Sigma_t
   // geometry
   uint32_t o_surf_q;    // [S] double4 typed parameters
   uint32_t o_surf_bc;   // [S]
@@ -64,6 +65,9 @@ struct Tables {
   const Tables *self_dev;  // device-memory copy of this struct (slow paths that must not take the parameter's address)
   int score_fast;       // the tally mesh covers the geometry and the time grid covers [t0, C_K]: no clipping needed
   int warp_ok;          // the problem fits the compact tables of k_warp (16-bit surface / cell ids, ...)
+  // techniques (include/mcdc.h mcdc_technique, DESIGN.md Appendix G); all zero = analog
+  int implicit_capture;
+  double wr_threshold, wr_survive;
   // source
   double src_lo[3], src_hi[3], src_t0, src_t1;
   int src_last;
@@ -111,8 +115,8 @@ struct StepParams {
 
 // Device-side accumulators (one instance per handle).
 struct DevCounters {
-  double ledger[7];         // source production capture fission_abs leak census_final lost
-  unsigned long long n[7];  // histories segments collisions surf_hits census_events children lost_n
+  double ledger[9];         // source production capture fission_abs leak census_final lost vr_gain vr_loss
+  unsigned long long n[9];  // histories segments collisions surf_hits census_events children lost_n pc_removed pc_added
   int overflow;             // a bank overflowed
   int pad;
 };

@@ -49,3 +49,20 @@ def all_reduce_tallies(sum_, sumsq, ledger, group=None):
         dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
         out.append(t if isinstance(a, torch.Tensor) else t.numpy())
     return tuple(out)
+
+
+def all_reduce_state(problem, group=None, device=None):
+    """The one exchange of a domain-replicated run: export the handle's accumulators as one
+    fp64 vector, sum it over the ranks (NCCL when `device` is a CUDA device, gloo on the host otherwise) and import
+    the sum back, so that every rank's tallies_get / counters_get answer for the whole job.  `problem` is anything with
+    state_size / state_export / state_import (paper_2409_04668_b200.Problem)."""
+    import torch
+    import torch.distributed as dist
+
+    n = problem.state_size()
+    buf = torch.empty(n, dtype=torch.float64, device=device if device is not None else "cpu")
+    problem.state_export(buf)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+    problem.state_import(buf)
+    return buf
