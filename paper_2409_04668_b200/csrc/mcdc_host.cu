@@ -699,7 +699,7 @@ WsLayout layout(const mcdc_problem *p, uint32_t slots, uint64_t cap, uint64_t hi
   L.q_cap = queue_capacity(hist);
   L.q_flag = off; off += align_up((size_t)L.q_cap * sizeof(uint32_t), 256);
   L.fixed = off;
-  L.q_data = off; off += (size_t)5 * align_up((size_t)L.q_cap * 8, 256) + align_up((size_t)L.q_cap * 16, 256);
+  L.q_data = off; off += (size_t)6 * align_up((size_t)L.q_cap * 8, 256) + align_up((size_t)L.q_cap * 16, 256);
   const size_t n = (size_t)slots * cap;
   for (int b = 0; b < 4; ++b) {
     L.bank[b] = off;
@@ -773,7 +773,7 @@ extern "C" int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes,
     auto take = [&](size_t bytes) { char *r = qd; qd += align_up(bytes, 256); return r; };
     FissionQueue &Q = p->queue;
     Q.x = (double *)take(L.q_cap * 8); Q.y = (double *)take(L.q_cap * 8); Q.z = (double *)take(L.q_cap * 8);
-    Q.t = (double *)take(L.q_cap * 8);
+    Q.t = (double *)take(L.q_cap * 8); Q.w = (double *)take(L.q_cap * 8);
     Q.key = (unsigned long long *)take(L.q_cap * 8);
     Q.meta = (int4 *)take(L.q_cap * 16);
     Q.flag = (uint32_t *)(p->ws + L.q_flag);
@@ -939,34 +939,43 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 #ifndef MCDC_WARP_CASES
 #define MCDC_WARP_CASES(X) X(256) X(512) X(1024)
 #endif
-template <bool STAGED, bool RECORD>
+template <bool STAGED, bool RECORD, bool WEIGHTED>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
-#define X(N) case N: k_warp<STAGED, RECORD, N><<<grid, N, smem, st>>>(T, A); break;
+#define X(N) case N: k_warp<STAGED, RECORD, WEIGHTED, N><<<grid, N, smem, st>>>(T, A); break;
     MCDC_WARP_CASES(X)
 #undef X
   }
 }
-template <bool STAGED, bool RECORD>
+template <bool STAGED, bool RECORD, bool WEIGHTED>
 cudaError_t warp_set_smem_nt(int nt, int bytes) {
   switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, WEIGHTED, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     MCDC_WARP_CASES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-void warp_launch(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (record) warp_launch_nt<true, true>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false>(nt, grid, smem, st, T, A); }
-  else        { if (record) warp_launch_nt<false, true>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false>(nt, grid, smem, st, T, A); }
+template <bool WEIGHTED>
+void warp_launch_w(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  if (staged) { if (record) warp_launch_nt<true, true, WEIGHTED>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, WEIGHTED>(nt, grid, smem, st, T, A); }
+  else        { if (record) warp_launch_nt<false, true, WEIGHTED>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, WEIGHTED>(nt, grid, smem, st, T, A); }
 }
-cudaError_t warp_set_smem(bool staged, bool record, int nt, int bytes) {
-  if (staged) return record ? warp_set_smem_nt<true, true>(nt, bytes) : warp_set_smem_nt<true, false>(nt, bytes);
-  return record ? warp_set_smem_nt<false, true>(nt, bytes) : warp_set_smem_nt<false, false>(nt, bytes);
+void warp_launch(bool staged, bool record, bool weighted, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  if (weighted) warp_launch_w<true>(staged, record, nt, grid, smem, st, T, A);
+  else warp_launch_w<false>(staged, record, nt, grid, smem, st, T, A);
+}
+template <bool WEIGHTED>
+cudaError_t warp_set_smem_w(bool staged, bool record, int nt, int bytes) {
+  if (staged) return record ? warp_set_smem_nt<true, true, WEIGHTED>(nt, bytes) : warp_set_smem_nt<true, false, WEIGHTED>(nt, bytes);
+  return record ? warp_set_smem_nt<false, true, WEIGHTED>(nt, bytes) : warp_set_smem_nt<false, false, WEIGHTED>(nt, bytes);
+}
+cudaError_t warp_set_smem(bool staged, bool record, bool weighted, int nt, int bytes) {
+  return weighted ? warp_set_smem_w<true>(staged, record, nt, bytes) : warp_set_smem_w<false>(staged, record, nt, bytes);
 }
 
 // shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
-int plan_warp_kernel(mcdc_problem *p, bool record) {
+int plan_warp_kernel(mcdc_problem *p, bool record, bool weighted) {
   int dev = 0, max_optin = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
@@ -974,10 +983,10 @@ int plan_warp_kernel(mcdc_problem *p, bool record) {
   if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
   if (nt != 256 && nt != 512 && nt != 1024) nt = 512;
   const int nw = nt / 32;
-  const size_t pop_bytes = align_up((size_t)p->K * 4, 16);
+  const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8, 16) : 0);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
   const size_t hot = align_up(p->tab.hot_bytes, 16);
-  const size_t per_slot = warp_pool_bytes_per_slot(record);
+  const size_t per_slot = warp_pool_bytes_per_slot(record, weighted);
   auto slots = [&](bool staged) -> long {
     const long avail = (long)max_optin - (long)fixed - (long)(staged ? hot : 0);
     if (avail <= 0) return 0;
@@ -992,7 +1001,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record) {
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
-  cudaError_t e1 = warp_set_smem(staged, record, nt, (int)p->pool_smem);
+  cudaError_t e1 = warp_set_smem(staged, record, weighted, nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
   return MCDC_OK;
 }
@@ -1031,7 +1040,8 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
-  warp_launch(staged, record, nt, grid, smem, p->stream, p->tab, ha);
+  const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0;
+  warp_launch(staged, record, weighted, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
   p->launches++;
@@ -1058,9 +1068,9 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   const bool record = opts->record_history_events != 0;
   if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
   // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
-  // ... and so do the techniques the history kernel does not implement
-  const bool vr = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->tech.population_control;
-  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u || vr;
+  // ... and so does the population control, which needs every particle of a batch parked at the census
+  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u ||
+                       p->tech.population_control;
   if (record) {
     if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
     CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
@@ -1081,7 +1091,7 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       p->blocks_per_sm = occ;
   }
   if (!stepped) {
-    const int rcp = plan_warp_kernel(p, record);
+    const int rcp = plan_warp_kernel(p, record, p->tech.implicit_capture || p->tech.wr_threshold > 0.0);
     if (rcp != MCDC_OK) return rcp;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;

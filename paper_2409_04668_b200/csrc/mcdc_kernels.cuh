@@ -626,7 +626,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
 // Global fission queue and launch arguments of the asynchronous history kernel k_warp (mcdc_warp.cuh).
 // ------------------------------------------------------------------------------------------------
 struct FissionQueue {             // ring buffer in HBM, structure of arrays, capacity mask+1 (power of two)
-  double *x, *y, *z, *t;
+  double *x, *y, *z, *t, *w;      // w is read and written only when a technique makes weights differ from 1
   unsigned long long *key;
   int4 *meta;                     // {cell, census index k, history id (when events are recorded), batch slot}
   uint32_t *flag;                 // entry i is readable when flag[i & mask] == (uint32)(i + 1)

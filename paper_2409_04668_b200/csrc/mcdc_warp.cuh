@@ -61,7 +61,7 @@ __device__ __noinline__
 __device__ __forceinline__
 #endif
 void general_score(const Tables *gT, double *x_acc_slot, int aggregate, bool active,
-                                           const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d) {
+                                           const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d, double w) {
   // the pre-move state is still in the pool: x y z ux uy uz 1/ux 1/uy 1/uz t, N slots apart
   const double x = pool[gi], y = pool[N + gi], z = pool[2 * N + gi], ux = pool[3 * N + gi], uy = pool[4 * N + gi],
                uz = pool[5 * N + gi], ix = pool[6 * N + gi], iy = pool[7 * N + gi], iz = pool[8 * N + gi], t = pool[9 * N + gi];
@@ -70,19 +70,22 @@ void general_score(const Tables *gT, double *x_acc_slot, int aggregate, bool act
   S.slab = nullptr; S.global_x = x_acc_slot; S.slab_lo = 0; S.slab_bins = 0; S.aggregate = aggregate;
   if (gT->score_fast) {
     PState p;
-    p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = 1.0;
+    p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = w;
     p.key = 0ull; p.ctr = 0u; p.hid = 0u; p.g = g; p.cell = 0; p.last_surf = -1;
     int it = tb.template ld<int>(gT->o_it0_k, pk);
     score_track_fast(tb, S, active, p, it, d);
   } else {
-    score_track(tb, S, active, x, y, z, ux, uy, uz, t, 1.0, g, d);
+    score_track(tb, S, active, x, y, z, ux, uy, uz, t, w, g, d);
   }
 }
 
 __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
 
 // bytes of shared memory per pool slot: x y z ux uy uz 1/ux 1/uy 1/uz t (10 x f64), key, ctr, cell|last, meta, 3 stack entries
-__host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record) { return 10 * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0); }
+// (+ the weight, one more f64, when a technique of Appendix G makes weights differ from 1)
+__host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool weighted) {
+  return (weighted ? 11 : 10) * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
+}
 
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
@@ -90,9 +93,10 @@ struct WarpShared {                // block-wide totals (static shared memory)
   uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
 
-template <bool STAGED, bool RECORD, int NT>
+template <bool STAGED, bool RECORD, bool WEIGHTED, int NT>
 __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   constexpr int NW = NT / 32;
+  constexpr uint32_t ND = WEIGHTED ? 11u : 10u;       // f64 arrays of the pool
   const double INF = CUDART_INF;
   __shared__ WarpShared sh;
   const TB<STAGED> tb(T);
@@ -105,19 +109,21 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   //   u32  ctr, cell|last<<16, meta = g | census index<<8 | batch slot<<20, [history id]  -> PU(k, slot)
   //   u8   stacks F, C, FREE -> PL(k, position)
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
-  const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16);
+  double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16));   // WEIGHTED only
+  const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16) +
+                            (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 + 15) / 16 * 16) : 0u);
 #define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + ((uint32_t)(k) * N + (slot)) * 8u))
-#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (10u * N + (slot)) * 8u))
-#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + 88u * N + ((uint32_t)(k) * N + (slot)) * 4u))
-#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + (RECORD ? 104u : 100u) * N + (uint32_t)(k) * N + (pos)))
-  enum { D_X = 0, D_Y, D_Z, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_T, U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
+#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (ND * N + (slot)) * 8u))
+#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + (ND + 1u) * 8u * N + ((uint32_t)(k) * N + (slot)) * 4u))
+#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + ((ND + 1u) * 8u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
+  enum { D_X = 0, D_Y, D_Z, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_T, D_W, U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
 
   if (STAGED) {
     const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
     uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
     for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
   }
-  for (int k = tid; k < T.K; k += NT) s_popn[k] = 0u;
+  for (int k = tid; k < T.K; k += NT) { s_popn[k] = 0u; if (WEIGHTED) s_popw[k] = 0.0; }
   if (tid == 0) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
     sh.n_coll = sh.n_surf = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
@@ -201,7 +207,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       const bool act = (uint32_t)lane < total;
       const uint32_t i = act ? (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane) : 0u;
       nFree -= total;
-      double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
+      double x = 0.0, y = 0.0, z = 0.0, t = 0.0, w = 1.0;
       unsigned long long key = 0ull;
       uint32_t ctr = 0u, hid = 0u, slot = 0u;
       int cell = 0, pk = 0;
@@ -218,6 +224,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           }
         }
         x = A.q.x[j]; y = A.q.y[j]; z = A.q.z[j]; t = A.q.t[j];
+        if (WEIGHTED) w = A.q.w[j];
         key = A.q.key[j];
         const int4 m = A.q.meta[j];
         cell = ok ? m.x : 0; pk = m.y; hid = (uint32_t)m.z; slot = (uint32_t)m.w;
@@ -261,6 +268,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const uint32_t gi = lb + i;
         PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz; PD(D_T, gi) = t;
         PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+        if (WEIGHTED) PD(D_W, gi) = w;
         PK(gi) = key; PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
         PU(U_META, gi) = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
         if (RECORD) PU(U_HID, gi) = hid;
@@ -345,6 +353,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (u < d_surf) { d_surf = u; which = 6 + j; }
       }
       double t = act ? PD(D_T, gi) : 0.0;
+      double w = 1.0;
+      if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
       const double t_census = tb.census(pk);
       const double d_time = tb.speed(g) * (t_census - t);
       int ev;
@@ -364,11 +374,11 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const int tbin = tb.template ld<int>(T.o_tbin_k, pk);
         const bool one_bin = cbin != NONE32 && tbin >= 0;      // the whole segment lies in one tally bin
         if (__any_sync(MCDC_FULL, act && !one_bin))
-          general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d);
+          general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
         if (__any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
           const long long bin = sc ? (long long)(tbin * G + g) * n_spatial + (long long)cbin : -1;
-          tally_add_converged(S, bin, d);
+          tally_add_converged(S, bin, WEIGHTED ? w * d : d);
         }
       }
       // ---- move (A.3) ----
@@ -396,7 +406,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
         if (bc == 1) {                                 // vacuum: leaks
           alive = false;
-          atomicAdd(&sh.led[LED_LEAK], 1.0);
+          atomicAdd(&sh.led[LED_LEAK], w);
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
           if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
           else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
@@ -420,7 +430,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
             if (idx < 0) idx = (int)tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
             c2 = slow_cross(gT, cell, idx, (int)s_star, x, y, z, ux, uy, uz);
           }
-          if (c2 < 0) { alive = false; lost = true; atomicAdd(&sh.led[LED_LOST], 1.0); }
+          if (c2 < 0) { alive = false; lost = true; atomicAdd(&sh.led[LED_LOST], w); }
           else new_cl = (uint32_t)c2 | (s_star << 16);
         }
       }
@@ -437,7 +447,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
         WCNT(W_CENSUS, (uint32_t)__popc(m_cen));
         const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
-        if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
+        if (WEIGHTED) {
+          if (census_k >= 0) atomicAdd(s_popw + census_k, w);
+          if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
+        } else if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
       }
       {
         const unsigned m_s = __ballot_sync(MCDC_FULL, ev == EV_SURFACE), m_lost = __ballot_sync(MCDC_FULL, lost);
@@ -471,30 +484,61 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       if (born) g = 0;
       const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
       const int mg = mat * G + g;
-      // reaction: scatter, capture, fission in this order (D6)
-      const double yv = draw(key, ctr) * tb.sig_t(mg);
+      // reaction: scatter, capture, fission in this order (D6); with weights, the techniques of Appendix G
+      const double xi_r = draw(key, ctr);
       if (born) ctr = 0u;                              // nothing drawn yet from a new child's stream
       int kind = FI_NONE, n_child = 0;                 // kind of the outgoing flight; children of a fission
       bool alive = false, captured = false, fissioned = false;
       uint32_t c0 = 0u;
+      double w = 1.0, l_cap = 0.0, l_fis = 0.0, l_prod = 0.0, l_gain = 0.0, l_loss = 0.0;   // WEIGHTED only
+      if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
       if (born) { kind = FI_CHILD; alive = true; }
       else if (act) {
-        if (yv < tb.sig_s_tot(mg)) { kind = FI_SCATTER; alive = true; }
-        else if (yv < tb.sig_sc(mg) || tb.sig_f(mg) == 0.0) captured = true;
-        else {
+        const double s_tot = tb.sig_s_tot(mg), sig_f = tb.sig_f(mg);
+        bool scatter = false, dead = false;
+        if (WEIGHTED && T.implicit_capture) {          // G.1: the captured fraction leaves the weight
+          const double w_c = w * tb.cap_frac(mg);
+          l_cap += w_c; w -= w_c;
+          const double s_r = s_tot + sig_f;
+          if (!(s_r > 0.0)) { l_cap += w; w = 0.0; dead = true; }
+          else scatter = (xi_r * s_r < s_tot) || sig_f == 0.0;
+        } else {
+          const double yv = xi_r * tb.sig_t(mg);
+          scatter = yv < s_tot;
+          if (!scatter && (yv < tb.sig_sc(mg) || sig_f == 0.0)) { dead = true; captured = true; l_cap += w; }
+        }
+        if (dead) {
+        } else if (scatter) {
+          if (WEIGHTED && T.wr_threshold > 0.0 && w < T.wr_threshold) {   // G.2 weight roulette
+            const double xi_w = draw(key, ctr);
+            if (xi_w * T.wr_survive < w) { l_gain += T.wr_survive - w; w = T.wr_survive; kind = FI_SCATTER; alive = true; }
+            else l_loss += w;
+          } else { kind = FI_SCATTER; alive = true; }
+        } else {
           const double xi_nu = draw(key, ctr);
           n_child = (int)floor(tb.nu(mg) + xi_nu);
           c0 = ctr;
           fissioned = true;
+          l_fis += w; l_prod += (double)n_child * w;
           if (n_child > 0) { kind = FI_CHILD; alive = true; }
         }
       }
       {
         const unsigned m_cap = __ballot_sync(MCDC_FULL, captured), m_fis = __ballot_sync(MCDC_FULL, fissioned);
-        if (lane == 0 && m_cap) atomicAdd(&sh.led[LED_CAPTURE], (double)__popc(m_cap));
+        if (WEIGHTED) {
+          l_cap = warp_sum(l_cap); l_fis = warp_sum(l_fis); l_prod = warp_sum(l_prod);
+          l_gain = warp_sum(l_gain); l_loss = warp_sum(l_loss);
+          if (lane == 0) {
+            if (l_cap != 0.0) atomicAdd(&sh.led[LED_CAPTURE], l_cap);
+            if (l_fis != 0.0) atomicAdd(&sh.led[LED_FISSION_ABS], l_fis);
+            if (l_prod != 0.0) atomicAdd(&sh.led[LED_PRODUCTION], l_prod);
+            if (l_gain != 0.0) atomicAdd(&sh.led[LED_VR_GAIN], l_gain);
+            if (l_loss != 0.0) atomicAdd(&sh.led[LED_VR_LOSS], l_loss);
+          }
+        } else if (lane == 0 && m_cap) atomicAdd(&sh.led[LED_CAPTURE], (double)__popc(m_cap));
         if (m_fis) {
           const uint32_t kids = __reduce_add_sync(MCDC_FULL, (uint32_t)n_child);
-          if (lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], (double)__popc(m_fis)); atomicAdd(&sh.led[LED_PRODUCTION], (double)kids); }
+          if (!WEIGHTED && lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], (double)__popc(m_fis)); atomicAdd(&sh.led[LED_PRODUCTION], (double)kids); }
           WCNT(W_CHILDREN, kids);
         }
         WCNT(W_COLL, (uint32_t)__popc(__ballot_sync(MCDC_FULL, act && !born)));
@@ -520,6 +564,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
               const uint32_t r = (uint32_t)(pre - n_push + c);
               const uint32_t i2 = (uint32_t)PL(L_FREE, lb + nFree - 1u - r), g2 = lb + i2;
               PD(D_X, g2) = x; PD(D_Y, g2) = y; PD(D_Z, g2) = z; PD(D_T, g2) = t;
+              if (WEIGHTED) PD(D_W, g2) = w;
               PK(g2) = child_key(key, c0, (uint32_t)(c + 1)); PU(U_CTR, g2) = 0u;
               PU(U_CL, g2) = (cl & 0xFFFFu) | (NONE16 << 16);
               PU(U_META, g2) = (meta & ~255u) | 255u;
@@ -544,6 +589,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
             for (int c = 0; c < n_push; ++c) {
               const uint32_t j = (uint32_t)(qb + (unsigned long long)c) & A.q.mask;
               A.q.x[j] = x; A.q.y[j] = y; A.q.z[j] = z; A.q.t[j] = t;
+              if (WEIGHTED) A.q.w[j] = w;
               A.q.key[j] = child_key(key, c0, (uint32_t)(c + 1));
               A.q.meta[j] = qm;
             }
@@ -567,6 +613,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (alive) {
           PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
           PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+          if (WEIGHTED) PD(D_W, gi) = w;
           PK(gi) = key; PU(U_CTR, gi) = ctr;
           PU(U_META, gi) = (meta & ~255u) | (uint32_t)g;
           PU(U_CL, gi) = (cl & 0xFFFFu) | (NONE16 << 16);
@@ -590,7 +637,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   }
   __syncthreads();
   for (int k = tid; k < T.K; k += NT) {
-    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
+    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, WEIGHTED ? s_popw[k] : (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
   }
   if (tid == 0) {
     DevCounters *cnt = A.cnt;

@@ -30,12 +30,14 @@ def M():
     return M
 
 
-def _pair(M, p, tech, **gkw):
+def _pair(M, p, tech, scheduler=0, **gkw):
+    """scheduler 0 = the history kernel k_warp (weighted variant) unless the population control forces the
+    census-stepped scheduler; 1 = census-stepped."""
     from oracle import Oracle
     o = Oracle(p); o.set_technique(**tech)
     o.run(p.n_histories, p.seed, n_batches=p.n_batches, record_history_events=True)
     g = M.Problem(p, **gkw); g.set_technique(**tech)
-    g.run(record_history_events=True)
+    g.run(record_history_events=True, scheduler=scheduler)
     return o, g
 
 
@@ -61,13 +63,16 @@ def _compare(o, g, rtol_bins, frac=0.99999):
     assert np.array_equal(no, ng) and np.allclose(wo, wg, rtol=1e-10)
 
 
+@pytest.mark.parametrize("scheduler", [0, 1])
 @pytest.mark.parametrize("tech", sorted(TECHS))
-def test_config0_with_techniques_matches_the_oracle(M, tech):
+def test_config0_with_techniques_matches_the_oracle(M, tech, scheduler):
     from workloads import configs as W
+    if scheduler == 1 and TECHS[tech].get("population_control"):
+        pytest.skip("the population control always runs census-stepped: covered by scheduler 0")
     p = W.config0_infinite_medium(n_histories=40000, n_batches=20)
     if tech == "ic":                                       # without roulette chains only end by fission: no fission here
         p.sigma_s = np.array([[[0.7]]]); p.sigma_c = np.array([[0.3]]); p.sigma_f = np.array([[0.0]]); p.nu = np.array([[0.0]])
-    o, g = _pair(M, p, TECHS[tech])
+    o, g = _pair(M, p, TECHS[tech], scheduler=scheduler)
     _compare(o, g, rtol_bins=1e-9)
     if tech != "ic":                                       # the closed form through the GPU path as well (pin G-b)
         mg, sg = g.tallies()
@@ -80,13 +85,14 @@ def test_config0_with_techniques_matches_the_oracle(M, tech):
     g.close()
 
 
-@pytest.mark.parametrize("name,N,B,tech", [("config1", 100_000, 20, "all"), ("config1a", 50_000, 10, "ic"),
-                                           ("config3", 40_000, 20, "all"), ("config3", 40_000, 20, "ic_wr"),
-                                           ("config2", 60_000, 12, "ic_wr")])
-def test_larger_configs_with_techniques(M, name, N, B, tech):
+@pytest.mark.parametrize("name,N,B,tech,scheduler", [
+    ("config1", 100_000, 20, "all", 0), ("config1a", 50_000, 10, "ic", 0), ("config1a", 50_000, 10, "ic", 1),
+    ("config3", 40_000, 20, "all", 0), ("config3", 100_000, 20, "ic_wr", 0), ("config3", 40_000, 20, "ic_wr", 1),
+    ("config2", 60_000, 12, "ic_wr", 0), ("config2", 60_000, 12, "ic_wr", 1), ("stress", 120_000, 12, "ic_wr", 0)])
+def test_larger_configs_with_techniques(M, name, N, B, tech, scheduler):
     from workloads import configs as W
-    p = W.get_config(name, n_histories=N, n_batches=B)
-    o, g = _pair(M, p, TECHS[tech])
+    p = W.stress_geometry(n_histories=N, n_batches=B) if name == "stress" else W.get_config(name, n_histories=N, n_batches=B)
+    o, g = _pair(M, p, TECHS[tech], scheduler=scheduler)
     _compare(o, g, rtol_bins=1e-7)
     g.close()
 
