@@ -34,6 +34,13 @@ NCU = {"config3_pin_lattice": {"dram_bytes_per_history": 3.23, "thread_inst_per_
                                "source": "profiles/r01d_k_warp.md"}}
 
 
+# variants of the workload with the techniques of DESIGN.md Appendix G switched on (the headline run is analog)
+TECHNIQUES = {"analog": None,
+              "ic_wr": dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0),
+              "pc": dict(population_control=True),
+              "all": dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0, population_control=True)}
+
+
 def _peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -185,9 +192,13 @@ def bench_gpu(args):
     n_hist, n_b = p.n_histories, p.n_batches
     from paper_2409_04668_b200.sharding import shard_range
 
-    # weak scaling: every rank runs n_hist histories of its own id range; no data-path collective
+    # weak scaling: every rank runs n_hist histories of its own id range; the one exchange of the job is the
+    # sum-reduction of the accumulators at its end, inside the timed region
     first_id = shard_range(n_hist * world, world, rank)[0]
     g = M.Problem(p, device=dev)
+    tech = TECHNIQUES[args.technique]
+    if tech:
+        g.set_technique(**tech)
 
     def barrier():
         torch.cuda.synchronize()
@@ -211,11 +222,13 @@ def bench_gpu(args):
     for _ in range(args.steps):
         g.run(n_hist, p.seed, n_b, first_history_id=first_id)
         ms_tr += g.counters()["ms_transport"]
+    c = g.counters()                                      # this rank's own counts
+    if world > 1:
+        g.all_reduce()                                    # NCCL all-reduce of sum / sumsq / ledger / populations
     ev1.record()
     barrier()
     t_wall1 = time.time()
     ms = ev0.elapsed_time(ev1)
-    c = g.counters()
     if world > 1:
         t = torch.tensor([ms, ms_tr], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -234,7 +247,7 @@ def bench_gpu(args):
                                 n_b * args.steps)
         n_tr = max(1, launches // 2)                       # one k_warp + one k_closeout launch per sub-batch
         ach = alg / (ms_tr * 1e-3) / 1e9
-        ncu = NCU.get(p.name)
+        ncu = NCU.get(p.name) if args.technique == "analog" else None   # the capture is of the analog kernel
         traffic = ncu["dram_bytes_per_history"] * n_hist * args.steps / n_tr if ncu else None
         roofline = {"bound": "hbm", "kernel": "k_warp", "achieved": ach, "peak": peak, "unit": "GB/s",
                     "frac": ach / peak, "traffic": traffic, "peak_kind": peak_kind,
@@ -258,7 +271,9 @@ def bench_gpu(args):
                           "l2": "the path has no input buffers (histories are generated on chip from seed and id); its "
                                 "only global data, the per-batch tally accumulators, are rewritten by the close-out of "
                                 "every step, so no step can reuse a previous step's cache contents",
-                          "parallelism": f"history-range sharding x{world}"},
+                          "parallelism": f"history-range sharding x{world}" +
+                                         (", one NCCL all-reduce of the accumulators at the end" if world > 1 else ""),
+                          "technique": args.technique},
                "segments_per_s": seg_per_s, "segments_per_history": c["segments"] / max(1, c["histories"]),
                "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu}
     # ---- e2e: host buffers in, host buffers out, through the C ABI (create + bind + run + get) ----
@@ -270,6 +285,8 @@ def bench_gpu(args):
     for _ in range(e2e_steps):
         h = M.mcdc_problem_create(p)                      # H2D: the problem description
         M.mcdc_workspace_bind(h, ptr, g.workspace_bytes, g.max_hist, g.max_slots, g._stream.cuda_stream)
+        if tech:
+            M.mcdc_technique_set(h, **tech)
         M.mcdc_run_ex(h, n_hist, p.seed, n_b, first_id)
         mean, sdev = M.mcdc_tallies_get(h, p.n_bins)      # D2H: sum and sumsq
         M.mcdc_problem_destroy(h)
@@ -341,6 +358,8 @@ def main():
     ap.add_argument("--histories", type=float, default=0)
     ap.add_argument("--batches", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--technique", default="analog", choices=sorted(TECHNIQUES),
+                    help="variance-reduction variant of the workload (DESIGN.md Appendix G); the headline is analog")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--sweep", action="store_true", help="also run the config-4 batch-size sweep (adds a 'sweep' key)")
     ap.add_argument("--sweep-max", type=float, default=1e9)
