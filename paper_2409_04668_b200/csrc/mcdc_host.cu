@@ -1018,6 +1018,8 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
   ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;   // in-warp merge of equal bins pays only on tiny meshes
+  ha.step_mode = 0; ha.step_k = 0; ha.step_source = 1; ha.step_single = 1; ha.bank_cap = 0;
+  ha.in = p->bankA; ha.census_out = p->bankB;             // unused outside the census-step mode
   CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
   // consumers' cursor := producers' cursor (drops whatever an aborted launch may have left behind)
   CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
@@ -1054,6 +1056,99 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   return MCDC_OK;
 }
 
+// ---- population control on the history kernel: one k_warp<WEIGHTED> launch per census step (census-step mode),
+// the control kernels between the steps; the host reads the bank counters once per step ----
+int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record) {
+  const uint32_t ns = sb.n_slots, ws_ns = p->ws_slots;
+  uint32_t *counts_dev = p->counts_dev;
+  std::vector<uint32_t> h_counts((size_t)8 * ws_ns);
+  CK(cudaMemsetAsync(counts_dev, 0, (size_t)8 * ws_ns * sizeof(uint32_t), p->stream));
+  Bank A = p->bankA, Bk = p->bankB;
+  const int k_first = step_of(p, p->src_t0), k_last = step_of(p, p->src_t1);
+  HistoryArgs ha;
+  ha.q = p->queue;
+  ha.hist_cursor = p->d_hist_cursor;
+  ha.seed_mixed = mix64(seed + MCDC_GAMMA);
+  ha.first_history = first_history_id + sb.first_local;
+  ha.n_hist = sb.n_hist; ha.hb = sb.hs;
+  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
+  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
+  const bool staged = p->stage_tables;
+  ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
+  ha.pool_slots = p->pool_slots;
+  const int nt = p->hist_threads;
+  const uint64_t per_block = (uint64_t)p->pool_slots * (nt / 32);
+  const int grid_src = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + per_block - 1) / per_block));
+  ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)sb.n_hist / ((uint64_t)grid_src * (nt / 32) * 8)));
+  ha.n_slots = sb.n_slots;
+  ha.step_mode = 1; ha.step_single = (k_first == k_last) ? 1 : 0; ha.bank_cap = p->cap;
+  uint64_t live_total = 0;
+  for (int k = 0; k < p->K; ++k) {
+    const bool src = k >= k_first && k <= k_last;
+    if (!src && live_total == 0) {
+      if (k > k_last) break;
+      continue;
+    }
+    ha.step_k = k; ha.step_source = src ? 1 : 0;
+    ha.n_chunks = src ? sb.n_slots * ((sb.hs + ha.src_chunk - 1) / ha.src_chunk) : 0u;
+    ha.in = A; ha.census_out = Bk;
+    CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
+    CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
+    CK(cudaMemsetAsync(A.cursor, 0, ns * sizeof(uint32_t), p->stream));
+    const uint64_t work = live_total + (src ? sb.n_hist : 0);
+    const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work + per_block - 1) / per_block));
+    cudaEvent_t a, b;
+    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    CK(cudaEventRecord(a, p->stream));
+    warp_launch(staged, record, true, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    CK(cudaEventRecord(b, p->stream));
+    p->ev_pairs.emplace_back(a, b);
+    p->launches++;
+    CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    CK(cudaGetLastError());
+    uint32_t n_max = 0;
+    live_total = 0;
+    {
+      const uint32_t *hc = h_counts.data() + (Bk.count - counts_dev);
+      for (uint32_t s = 0; s < ns; ++s) {
+        if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
+        live_total += hc[s]; n_max = std::max(n_max, hc[s]);
+      }
+    }
+    if (k < p->K - 1 && live_total > 0) {
+      if (p->tech.population_control) {                   // Appendix G.3: census bank Bk -> live bank A
+        PcParams pc;
+        pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs;
+        const dim3 pgrid((n_max + 255) / 256, ns);
+        CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
+        CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
+        k_pc_weight<<<pgrid, 256, 0, p->stream>>>(Bk, p->cap, p->d_wfix);
+        k_pc_apply<<<pgrid, 256, 0, p->stream>>>(Bk, A, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
+        p->launches += 2;
+        CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+        CK(cudaStreamSynchronize(p->stream));
+        CK(cudaGetLastError());
+        const uint32_t *hc = h_counts.data() + (A.count - counts_dev);
+        live_total = 0;
+        for (uint32_t s = 0; s < ns; ++s) {
+          if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
+          live_total += hc[s];
+        }
+      } else std::swap(A, Bk);
+    }
+    CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));
+  }
+  if (sb.closeout) {
+    int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
+    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    p->launches++;
+  }
+  CK(cudaGetLastError());
+  return MCDC_OK;
+}
+
 }  // namespace
 
 extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts) {
@@ -1068,9 +1163,10 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   const bool record = opts->record_history_events != 0;
   if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
   // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
-  // ... and so does the population control, which needs every particle of a batch parked at the census
-  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u ||
-                       p->tech.population_control;
+  const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u;
+  // the population control needs every particle of a batch parked at the census: the history kernel then runs one
+  // launch per census step (census-step mode) with the control kernels in between
+  const bool stepwarp = !stepped && p->tech.population_control;
   if (record) {
     if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
     CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
@@ -1091,7 +1187,7 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       p->blocks_per_sm = occ;
   }
   if (!stepped) {
-    const int rcp = plan_warp_kernel(p, record, p->tech.implicit_capture || p->tech.wr_threshold > 0.0);
+    const int rcp = plan_warp_kernel(p, record, stepwarp || p->tech.implicit_capture || p->tech.wr_threshold > 0.0);
     if (rcp != MCDC_OK) return rcp;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
@@ -1100,8 +1196,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   CK(cudaEventRecord(e_run0, p->stream));
 
   // ---- plan sub-batches ----
-  if (stepped && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
-  const uint64_t slot_max = stepped ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
+  if ((stepped || stepwarp) && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
+  const uint64_t slot_max = (stepped || stepwarp) ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
   int rc = MCDC_OK;
   if (p->tech.population_control && hb > slot_max) return MCDC_ERR_ARG;   // the control acts on whole batches
   if (hb <= slot_max) {                                  // whole batches, one per slot
@@ -1111,7 +1207,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       sb.n_slots = std::min<uint32_t>(per_sub, B - b);
       sb.first_local = (uint64_t)b * hb; sb.n_hist = (uint32_t)(sb.n_slots * hb); sb.hs = (uint32_t)hb; sb.closeout = 1;
       rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
-                   : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+           : stepwarp ? run_subbatch_stepwarp(p, sb, seed, opts->first_history_id, record)
+                      : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
     }
   } else {                                               // one batch = several pieces spread over the slots
     const uint64_t per_sub = std::min<uint64_t>(p->ws_hist, slot_max * p->ws_slots);
@@ -1124,7 +1221,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
         sb.first_local = (uint64_t)b * hb + off; sb.n_hist = (uint32_t)n;
         sb.closeout = (off + n >= hb) ? 2 : 0;
         rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
-                   : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+           : stepwarp ? run_subbatch_stepwarp(p, sb, seed, opts->first_history_id, record)
+                      : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
       }
     }
   }

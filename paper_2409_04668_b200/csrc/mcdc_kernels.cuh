@@ -649,6 +649,12 @@ struct HistoryArgs {
   int aggregate;
   uint32_t smem_tables;           // bytes of dynamic shared memory in front of the census arrays
   uint32_t pool_slots;            // particles held in each warp's shared-memory pool
+  // census-step mode of k_warp<WEIGHTED> (population control, Appendix G.3): one launch transports one census step.
+  // Particles come from the live bank `in` (survivors of the control at the previous census) and from the source
+  // histories born in this step; a particle that reaches the census time is parked in `census_out` instead of going on.
+  int step_mode, step_k, step_source, step_single;   // on/off; census index; sources may be born in this step; all are
+  uint32_t bank_cap;              // bank capacity per batch slot
+  Bank in, census_out;
 };
 
 __device__ __forceinline__ uint32_t ld_acquire_u32(const uint32_t *p) {

@@ -142,6 +142,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
   bool src_exhausted = false;
+  const bool step_mode = WEIGHTED && A.step_mode != 0; // census-step mode (Appendix G.3)
+  bool bank_done = !step_mode;                         // the live bank of this step has been handed out
+  uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
+  if (step_mode && !A.step_source) src_exhausted = true;
   enum { W_COLL = 0, W_SURF, W_CENSUS, W_CHILDREN, W_LOST, W_SRC };
 #define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
@@ -158,6 +162,38 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
     if (phase == 0) {
       // =============== R: acquire work for up to 32 free slots, initialise the new particles (A.3, A.6) ===============
       const uint32_t want = min(32u, nFree);
+      if (WEIGHTED && !bank_done) {
+        // ---- census-step mode: particles of the live bank first (full records: nothing is sampled here) ----
+        uint32_t base = 0u, cnt = 0u;
+        if (lane == 0) { cnt = min(A.in.count[bank_slot], A.bank_cap); base = atomicAdd(A.in.cursor + bank_slot, want); }
+        base = __shfl_sync(MCDC_FULL, base, 0); cnt = __shfl_sync(MCDC_FULL, cnt, 0);
+        if (base >= cnt) {                               // this batch slot is handed out: try the next one
+          bank_slot = (bank_slot + 1u) % A.n_slots;
+          if (++bank_probes >= A.n_slots) bank_done = true;
+          continue;
+        }
+        bank_probes = 0u;
+        const uint32_t nb = min(want, cnt - base);
+        const bool actb = (uint32_t)lane < nb;
+        if (actb) {
+          const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
+          const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
+          const double ux = A.in.ux[j], uy = A.in.uy[j], uz = A.in.uz[j];
+          const int4 m = A.in.meta[j];                   // {cell, last surface, counter, group}
+          PD(D_X, gi) = A.in.x[j]; PD(D_Y, gi) = A.in.y[j]; PD(D_Z, gi) = A.in.z[j]; PD(D_T, gi) = A.in.t[j];
+          PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
+          PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+          PD(D_W, gi) = A.in.w[j];
+          PK(gi) = A.in.key[j]; PU(U_CTR, gi) = (uint32_t)m.z;
+          PU(U_CL, gi) = (uint32_t)m.x | ((m.y < 0 ? NONE16 : (uint32_t)m.y) << 16);
+          PU(U_META, gi) = (uint32_t)m.w | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
+          if (RECORD) PU(U_HID, gi) = A.in.hid[j];
+          PL(L_F, lb + nF + (uint32_t)lane) = (uint8_t)i;
+        }
+        nFree -= nb; nF += nb;
+        __syncwarp();
+        continue;
+      }
       // source histories come from the warp's own chunk of the sub-batch; one global atomic per chunk
       // Chunks are dealt round-robin over the batch slots, so the warps in flight spread their scores over all the
       // slot accumulators instead of contending for the hot bins of one.
@@ -211,7 +247,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       unsigned long long key = 0ull;
       uint32_t ctr = 0u, hid = 0u, slot = 0u;
       int cell = 0, pk = 0;
-      bool ok = act, is_src = false;
+      bool ok = act, is_src = false, skip = false;     // skip: a source born in another census step (census-step mode)
       if (act && (uint32_t)lane >= n_src) {            // a fission child from the global queue (A.6)
         const unsigned long long qi = qbase + (unsigned long long)((uint32_t)lane - n_src);
         const uint32_t j = (uint32_t)qi & A.q.mask;
@@ -241,6 +277,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         z = T.src_lo[2] + xi_z * (T.src_hi[2] - T.src_lo[2]);
         t = T.src_t0 + xi_t * (T.src_t1 - T.src_t0);
         pk = census_index(tb, t);
+        if (WEIGHTED && step_mode && !A.step_single && pk != A.step_k) { skip = true; ok = false; }
       }
       // group: chi of the fission-site material (child) or the source pdf; then the direction
       const double xi_g = draw(key, ctr);
@@ -261,9 +298,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         cell = slow_locate_source(gT, x, y, z, ux, uy, uz);
         if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
       }
-      const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0);
+      const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0 && !skip);
       if (m_lost) { WCNT(W_LOST, (uint32_t)__popc(m_lost)); if (lane == 0) atomicAdd(&sh.led[LED_LOST], (double)__popc(m_lost)); }
-      WCNT(W_SRC, n_src);
+      if (WEIGHTED && step_mode) WCNT(W_SRC, (uint32_t)__popc(__ballot_sync(MCDC_FULL, is_src && !skip)));
+      else WCNT(W_SRC, n_src);
       if (ok) {
         const uint32_t gi = lb + i;
         PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz; PD(D_T, gi) = t;
@@ -390,7 +428,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       if (ev == EV_CENSUS) {                           // A.8: bookkeeping only, then the next interval
         census_k = pk;
         if (d > 0.0) new_cl = (cl & 0xFFFFu) | (NONE16 << 16);
-        if (pk == T.K - 1) alive = false;
+        if (pk == T.K - 1 || step_mode) alive = false;   // census-step mode: parked in the census bank below
         else meta += 1u << 8;
       } else if (ev == EV_SURFACE) {                   // A.5
         const bool is_face = which < 6;
@@ -439,6 +477,25 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (new_cl != cl) PU(U_CL, gi) = new_cl;
         if (ev == EV_CENSUS) PU(U_META, gi) = meta;
         if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
+      }
+      if (WEIGHTED && step_mode) {
+        // ---- census-step mode: park the arrivals of a census that is not the last in their batch's census bank ----
+        const bool park = act && ev == EV_CENSUS && pk != T.K - 1;
+        if (__any_sync(MCDC_FULL, park)) {
+          const int bslot = park ? (int)(meta >> 20) : -1;
+          const uint32_t idx = warp_append_by_slot(A.census_out.count, bslot);
+          if (park) {
+            if (idx >= A.bank_cap) atomicExch(&A.cnt->overflow, 1);
+            else {
+              const size_t j = (size_t)bslot * A.bank_cap + idx;
+              const Bank &O = A.census_out;
+              const uint32_t last2 = new_cl >> 16;
+              O.x[j] = x; O.y[j] = y; O.z[j] = z; O.ux[j] = ux; O.uy[j] = uy; O.uz[j] = uz; O.t[j] = t; O.w[j] = w;
+              O.key[j] = PK(gi); O.hid[j] = RECORD ? PU(U_HID, gi) : 0u;
+              O.meta[j] = make_int4(cell, last2 == NONE16 ? -1 : (int)last2, (int)PU(U_CTR, gi), g);
+            }
+          }
+        }
       }
       // ---- census population (A.8): one shared-memory add per distinct census index in the warp ----
       const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);

@@ -31,8 +31,8 @@ def M():
 
 
 def _pair(M, p, tech, scheduler=0, **gkw):
-    """scheduler 0 = the history kernel k_warp (weighted variant) unless the population control forces the
-    census-stepped scheduler; 1 = census-stepped."""
+    """scheduler 0 = the history kernel k_warp (weighted variant; one launch per census step when the population
+    control is on); 1 = the census-stepped kernel k_transport."""
     from oracle import Oracle
     o = Oracle(p); o.set_technique(**tech)
     o.run(p.n_histories, p.seed, n_batches=p.n_batches, record_history_events=True)
@@ -67,8 +67,6 @@ def _compare(o, g, rtol_bins, frac=0.99999):
 @pytest.mark.parametrize("tech", sorted(TECHS))
 def test_config0_with_techniques_matches_the_oracle(M, tech, scheduler):
     from workloads import configs as W
-    if scheduler == 1 and TECHS[tech].get("population_control"):
-        pytest.skip("the population control always runs census-stepped: covered by scheduler 0")
     p = W.config0_infinite_medium(n_histories=40000, n_batches=20)
     if tech == "ic":                                       # without roulette chains only end by fission: no fission here
         p.sigma_s = np.array([[[0.7]]]); p.sigma_c = np.array([[0.3]]); p.sigma_f = np.array([[0.0]]); p.nu = np.array([[0.0]])
@@ -87,7 +85,8 @@ def test_config0_with_techniques_matches_the_oracle(M, tech, scheduler):
 
 @pytest.mark.parametrize("name,N,B,tech,scheduler", [
     ("config1", 100_000, 20, "all", 0), ("config1a", 50_000, 10, "ic", 0), ("config1a", 50_000, 10, "ic", 1),
-    ("config3", 40_000, 20, "all", 0), ("config3", 100_000, 20, "ic_wr", 0), ("config3", 40_000, 20, "ic_wr", 1),
+    ("config3", 40_000, 20, "all", 0), ("config3", 40_000, 20, "all", 1), ("config3", 100_000, 20, "pc", 0),
+    ("config2", 60_000, 12, "all", 0), ("config3", 100_000, 20, "ic_wr", 0), ("config3", 40_000, 20, "ic_wr", 1),
     ("config2", 60_000, 12, "ic_wr", 0), ("config2", 60_000, 12, "ic_wr", 1), ("stress", 120_000, 12, "ic_wr", 0)])
 def test_larger_configs_with_techniques(M, name, N, B, tech, scheduler):
     from workloads import configs as W
