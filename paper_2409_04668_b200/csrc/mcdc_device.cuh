@@ -107,6 +107,25 @@ __device__ __noinline__ ulonglong2 philox_block(unsigned long long key, uint32_t
   return r;
 }
 
+// the same block function inlined at its call site, so that its dependent chain can overlap independent work there
+__device__ __forceinline__ ulonglong2 philox_block_inl(unsigned long long key, uint32_t block) {
+  uint32_t c0 = block, c1 = 0u, c2 = 0u, c3 = 0u;
+  uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE.U32 each
+    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  ulonglong2 r;
+  r.x = ((unsigned long long)c1 << 32) | c0;
+  r.y = ((unsigned long long)c3 << 32) | c2;
+  return r;
+}
+
 // u = ((x >> 12) + 0.5) * 2^-52, built exactly: [1,2) mantissa trick then one exact subtraction.
 __device__ __forceinline__ double u64_to_unit(unsigned long long x) {
   double d = __longlong_as_double((long long)((x >> 12) | 0x3FF0000000000000ull));
@@ -115,6 +134,12 @@ __device__ __forceinline__ double u64_to_unit(unsigned long long x) {
 
 __device__ __forceinline__ double draw(unsigned long long key, uint32_t &ctr) {
   const ulonglong2 b = philox_block(key, ctr >> 1);
+  const unsigned long long x = (ctr & 1u) ? b.y : b.x;
+  ctr += 1u;
+  return u64_to_unit(x);
+}
+__device__ __forceinline__ double draw_inl(unsigned long long key, uint32_t &ctr) {
+  const ulonglong2 b = philox_block_inl(key, ctr >> 1);
   const unsigned long long x = (ctr & 1u) ? b.y : b.x;
   ctr += 1u;
   return u64_to_unit(x);

@@ -20,6 +20,9 @@
 #ifndef MCDC_STORE_INV
 #define MCDC_STORE_INV 1        // keep 1/direction in the pool (else recomputed every flight)
 #endif
+#ifndef MCDC_F_INLINE_PHILOX
+#define MCDC_F_INLINE_PHILOX 0  // Philox block of the flight phase inlined (its chain may overlap the geometry)
+#endif
 #ifndef MCDC_SCORE_NOINLINE
 #define MCDC_SCORE_NOINLINE 0   // general (multi-bin) scorer out of line
 #endif
@@ -77,6 +80,11 @@ void general_score(const Tables *gT, double *x_acc_slot, int aggregate, bool act
   } else {
     score_track(tb, S, active, x, y, z, ux, uy, uz, t, w, g, d);
   }
+}
+
+// 0 < v < +inf, decided on the bit pattern (two integer instructions instead of two fp64 compares)
+__device__ __forceinline__ bool pos_finite(double v) {
+  return (unsigned long long)(__double_as_longlong(v) - 1ll) < 0x7FEFFFFFFFFFFFFFull;
 }
 
 __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
@@ -138,6 +146,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   const Tables *gT = T.self_dev;
   const int G = T.G;
   const long long n_spatial = (long long)T.mesh_n[0] * T.mesh_n[1] * T.mesh_n[2];
+  const bool bins32 = T.n_bins < 0x7FFFFFFFull;        // tally bin indices fit 32 bits: no 64-bit multiply per score
   // warp-uniform scheduler state
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
@@ -334,7 +343,11 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         unsigned long long key = 0ull;
         uint32_t ctr = 0u;
         if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
+#if MCDC_F_INLINE_PHILOX
+        const double xi = draw_inl(key, ctr);          // always consumed (D3)
+#else
         const double xi = draw(key, ctr);              // always consumed (D3)
+#endif
         if (act) PU(U_CTR, gi) = ctr;
         d_coll = -log(xi);
       }
@@ -355,16 +368,18 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       ix = 1.0 / ux; iy = 1.0 / uy; iz = 1.0 / uz;
 #endif
       // ---- faces: one candidate per axis, picked by the sign of the direction component ----
-      const int fx = (ux > 0.0) ? 1 : 0, fy = (uy > 0.0) ? 3 : 2, fz = (uz > 0.0) ? 5 : 4;
+      // sign bit alone: for a component that is exactly +-0 the face distance is inf or NaN and is rejected below
+      const bool px = __double2hiint(ux) >= 0, py = __double2hiint(uy) >= 0, pz = __double2hiint(uz) >= 0;
+      const int fx = px ? 1 : 0, fy = py ? 3 : 2, fz = pz ? 5 : 4;
       const uint32_t sfx = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fx);
       const uint32_t sfy = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fy);
       const uint32_t sfz = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fz);
-      const double bx = (sfx == NONE16) ? ((ux > 0.0) ? INF : -INF) : tb.surf_q0((int)sfx);
-      const double by = (sfy == NONE16) ? ((uy > 0.0) ? INF : -INF) : tb.surf_q0((int)sfy);
-      const double bz = (sfz == NONE16) ? ((uz > 0.0) ? INF : -INF) : tb.surf_q0((int)sfz);
+      const double bx = (sfx == NONE16) ? (px ? INF : -INF) : tb.surf_q0((int)sfx);
+      const double by = (sfy == NONE16) ? (py ? INF : -INF) : tb.surf_q0((int)sfy);
+      const double bz = (sfz == NONE16) ? (pz ? INF : -INF) : tb.surf_q0((int)sfz);
       const double dx = (bx - x) * ix, dy = (by - y) * iy, dz = (bz - z) * iz;   // 0 * inf = NaN: rejected below
       // nearest face; equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
-      const bool vx = dx > 0.0 && dx < INF, vy = dy > 0.0 && dy < INF, vz = dz > 0.0 && dz < INF;
+      const bool vx = pos_finite(dx), vy = pos_finite(dy), vz = pos_finite(dz);
       double d_surf = vx ? dx : INF;
       int which = vx ? fx : -1;                        // 2*axis + side of the nearest face, 6 + j for other j
       bool ty = vy && dy < d_surf;
@@ -415,7 +430,9 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
         if (__any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
-          const long long bin = sc ? (long long)(tbin * G + g) * n_spatial + (long long)cbin : -1;
+          long long bin = -1;
+          if (sc) bin = bins32 ? (long long)((tbin * G + g) * (int)n_spatial + (int)cbin)
+                               : (long long)(tbin * G + g) * n_spatial + (long long)cbin;
           tally_add_converged(S, bin, WEIGHTED ? w * d : d);
         }
       }
@@ -459,9 +476,9 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           // a certified neighbour holds every point of this surface patch that lies strictly inside the cell's
           // forward faces (mcdc_host.cu); anything else takes the full search of A.5
           const int ax = (which < 6) ? (which >> 1) : -1;
-          const bool in_x = ax == 0 || ((ux > 0.0) ? (x < bx) : ((ux < 0.0) ? (x > bx) : true));
-          const bool in_y = ax == 1 || ((uy > 0.0) ? (y < by) : ((uy < 0.0) ? (y > by) : true));
-          const bool in_z = ax == 2 || ((uz > 0.0) ? (z < bz) : ((uz < 0.0) ? (z > bz) : true));
+          const bool in_x = ax == 0 || (px ? (x < bx) : (x > bx));
+          const bool in_y = ax == 1 || (py ? (y < by) : (y > by));
+          const bool in_z = ax == 2 || (pz ? (z < bz) : (z > bz));
           int c2;
           if (nb != NONE16 && in_x && in_y && in_z) c2 = (int)nb;
           else {
