@@ -95,6 +95,8 @@ def _load():
     L.orc_score_segment.argtypes = [vp, _dp, _dp, C.c_double, C.c_int, C.c_double, C.c_double]
     L.orc_score_segment.restype = C.c_int
     L.orc_close_batch.argtypes = [vp, C.c_uint64]; L.orc_close_batch.restype = C.c_int
+    L.orc_run_eigenvalue.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int32, _dp]
+    L.orc_run_eigenvalue.restype = C.c_int
     L.orc_technique_set.argtypes = [vp, C.POINTER(_Technique)]; L.orc_technique_set.restype = C.c_int
     L.orc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.orc_census_after_get.restype = C.c_int
     L.orc_population_control.argtypes = [vp, C.c_size_t, _dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.c_uint64,
@@ -225,6 +227,14 @@ class Oracle:
         if rc != 0:
             raise RuntimeError(f"orc_run failed: {rc}")
         self._last_n = int(n_histories)
+
+    def run_eigenvalue(self, n_particles, seed, n_inactive, n_active, reverse_order=False):
+        k = np.zeros(int(n_inactive) + int(n_active))
+        rc = self._L.orc_run_eigenvalue(self._h, int(n_particles), int(seed), int(n_inactive), int(n_active),
+                                        int(reverse_order), _d(k))
+        if rc != 0:
+            raise RuntimeError(f"orc_run_eigenvalue failed: {rc}")
+        return k
 
     def tallies(self):
         mean = np.empty(self.n_bins); sdev = np.empty(self.n_bins)

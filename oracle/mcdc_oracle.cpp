@@ -306,8 +306,9 @@ Particle source_particle(orc_problem &P, uint64_t seed, uint64_t h) {
 }
 
 // A.6 init_child: the child's own stream gives group (chi of the fission-site material) and direction
-void init_child(orc_problem &P, Particle &p) {
-  p.ctr = 0;
+// (keep_ctr: the birth record has already drawn from its stream -- the generation control of Appendix H)
+void init_child(orc_problem &P, Particle &p, bool keep_ctr = false) {
+  if (!keep_ctr) p.ctr = 0;
   int m = P.cell_material[p.cell];
   double xi_g = draw(p.key, p.ctr);
   p.g = sample_cdf(&P.chi[(size_t)m * P.G], P.G, xi_g);
@@ -453,7 +454,7 @@ bool transport(orc_problem &P, Particle &p, std::deque<BankItem> &bank, bool sto
 const double FIX40 = 1099511627776.0;   // 2^40
 typedef std::pair<uint64_t, Particle> Owned;
 void population_control(orc_problem &P, const std::vector<Owned> &arrived, uint64_t target, int k,
-                        std::vector<Owned> &out) {
+                        std::vector<Owned> &out, double w_out = 0.0) {   // w_out > 0: weight given to the copies (H.3)
   uint64_t w_fix = 0;
   for (const Owned &a : arrived) w_fix += (uint64_t)(a.second.w * FIX40);
   if (w_fix == 0 || target == 0) return;
@@ -469,10 +470,10 @@ void population_control(orc_problem &P, const std::vector<Owned> &arrived, uint6
     uint32_t c0 = q.ctr;
     for (int j = 0; j < n; ++j) {
       Particle c = q;                                 // same r, Omega, t, g, cell, last_surface, k
-      c.w = w_t;
+      c.w = (w_out > 0.0) ? w_out : w_t;
       if (j > 0) { c.key = child_key(q.key, c0, (uint32_t)j); c.ctr = 0; }
       out.emplace_back(a.first, c);
-      P.pop_w_after[k] += w_t; P.pop_n_after[k] += 1;
+      P.pop_w_after[k] += c.w; P.pop_n_after[k] += 1;
     }
   }
 }
@@ -693,6 +694,54 @@ int orc_run(orc_problem *P, uint64_t n_histories, uint64_t seed, const orc_run_o
     close_batch(*P);
   }
   P->cur_ev = nullptr;
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Appendix H of DESIGN.md: k-eigenvalue mode, power iteration over fission generations.
+//  H.1 generation 0 = the problem's source, N histories of weight 1; a generation transports its particles
+//      until they die; fission children are NOT transported in the generation that made them, they are its
+//      fission bank.  k_g = (weight of the children made in generation g) / (weight that started it).
+//  H.2 tallies: every generation from n_inactive on is one statistical batch of N histories; earlier ones
+//      are discarded.
+//  H.3 the next generation = the population control of G.3 applied to the fission bank (target N, every
+//      birth record draws xi from its own stream at counter 0), the copies taking weight 1; init_child then
+//      goes on from the record's counter.
+// ---------------------------------------------------------------------------------------------
+int orc_run_eigenvalue(orc_problem *P, uint64_t N, uint64_t seed, uint32_t n_inactive, uint32_t n_active,
+                       int32_t reverse_order, double *k_gen) {
+  if (!P || !k_gen || N == 0 || n_active == 0) return -1;
+  if (P->batch_size != 0 && P->batch_size != N) return -1;
+  P->batch_size = N;
+  P->hist_ev.clear(); P->cur_ev = nullptr;
+  std::vector<Owned> cur, next;                           // (is_birth flag in .first, particle)
+  for (uint64_t h = 0; h < N; ++h) {
+    Particle p = source_particle(*P, seed, h);
+    if (p.alive) cur.emplace_back(0u, p);
+  }
+  const uint32_t G_total = n_inactive + n_active;
+  std::deque<BankItem> fis;
+  for (uint32_t g = 0; g < G_total; ++g) {
+    double start_w = 0.0;
+    for (const Owned &c : cur) start_w += c.second.w;
+    const double prod0 = P->cnt.production;
+    fis.clear();
+    for (size_t i = 0; i < cur.size(); ++i) {
+      Owned &c = cur[reverse_order ? cur.size() - 1 - i : i];
+      Particle p = c.second;
+      if (c.first) init_child(*P, p, true);
+      transport(*P, p, fis);                              // children pile up in fis, nobody pops them here
+    }
+    k_gen[g] = start_w > 0.0 ? (P->cnt.production - prod0) / start_w : 0.0;
+    if (g >= n_inactive) { P->cnt.histories += N; close_batch(*P); }
+    else std::fill(P->x.begin(), P->x.end(), 0.0);
+    std::vector<Owned> bank;
+    for (const BankItem &b : fis) bank.emplace_back(1u, b.p);
+    next.clear();
+    population_control(*P, bank, N, 0, next, 1.0);
+    cur.swap(next);
+    if (cur.empty()) { for (uint32_t r = g + 1; r < G_total; ++r) k_gen[r] = 0.0; break; }
+  }
   return 0;
 }
 

@@ -78,6 +78,11 @@ int  orc_technique_set(orc_problem *p, const orc_technique *t);   /* NULL: analo
 void orc_destroy(orc_problem *p);
 void orc_reset(orc_problem *p);
 int  orc_run(orc_problem *p, uint64_t n_histories, uint64_t seed, const orc_run_opts *o);
+/* k-eigenvalue mode (DESIGN.md Appendix H): n_inactive + n_active fission generations of nominally
+ * N particles; k_gen[g] = children weight / starting weight of generation g; active generations are the
+ * statistical batches of the tallies.  reverse_order: process each generation's bank backwards (pin H-d).  */
+int  orc_run_eigenvalue(orc_problem *p, uint64_t N, uint64_t seed, uint32_t n_inactive, uint32_t n_active,
+                        int32_t reverse_order, double *k_gen);
 int  orc_tallies_get(const orc_problem *p, double *mean, double *sdev, size_t n_bins);
 int  orc_tally_sums_get(const orc_problem *p, double *sum, double *sumsq, size_t n_bins);
 int  orc_counters_get(const orc_problem *p, orc_counters *c);

@@ -420,6 +420,32 @@ def infinite_medium_multigroup(material=0, n_histories=200_000, n_batches=20, n_
                      n_histories, n_batches, run_seed(3))
 
 
+def as_eigenvalue(p, t_far=1e30):
+    """The same problem for the k-eigenvalue mode (DESIGN.md Appendix H): time plays no part there, so the tally has
+    one time bin [0, t_far] and the only census is at t_far (never reached); the source is born at t = 0."""
+    import copy
+    q = copy.deepcopy(p)
+    q.name = p.name + "_eigenvalue"
+    q.time_edges = _f64([0.0, t_far]); q.census_times = _f64([t_far])
+    q.src_t0 = 0.0; q.src_t1 = 0.0
+    return q
+
+
+def bare_slab_absorber(thickness=2.0, sigma_t=1.0, sigma_f=0.4, nu=2.5, n_histories=100_000):
+    """One-group slab with vacuum faces, no scattering (pin H-b: first-flight collision probability), uniform
+    isotropic source over the slab, 10 x-bins."""
+    mats, ss = _materials([dict(sigma_t=[sigma_t], sigma_c=[sigma_t - sigma_f], sigma_f=[sigma_f], nu=[nu], chi=[1.0],
+                                sigma_s=[[0.0]])], 1)
+    surfs = [plane_x(0.0), plane_x(thickness)]
+    bcs = [BC_VACUUM, BC_VACUUM]
+    cells = [([(0, +1), (1, -1)], 0)]
+    src = dict(lo=[0.0, 0.0, 0.0], hi=[thickness, 0.0, 0.0], t0=0.0, t1=0.0, pdf=[1.0])
+    mesh = dict(lo=[0.0, -np.inf, -np.inf], hi=[thickness, np.inf, np.inf], n=[10, 1, 1])
+    T = _f64([0.0, 1e30])
+    return _assemble("bare_slab_absorber", mats, ss, [1.0], surfs, bcs, cells, src, mesh, T, T[1:].copy(),
+                     n_histories, 1, run_seed(5))
+
+
 CONFIGS = {
     "config0": config0_infinite_medium,
     "config1": config1_slab,
