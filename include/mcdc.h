@@ -157,6 +157,20 @@ int mcdc_workspace_bind(mcdc_problem *p, void *dev_ptr, size_t bytes, uint64_t m
 int mcdc_run(mcdc_problem *p, uint64_t n_histories, uint64_t seed);
 int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts);
 
+/* k-eigenvalue mode ("k-eigenvalue and fully time-dependent simulation modes"; SURVEY.md 8(f)
+ * NEXT-2; definition in DESIGN.md Appendix H): power iteration over n_inactive + n_active fission
+ * generations of nominally n_particles particles.  Generation 0 is the problem's source; a generation's
+ * fission children are banked, not transported; k_gen[g] = weight of the children made in generation g /
+ * weight that started it; the bank is then brought to n_particles particles of weight 1 by the control
+ * of mcdc_technique (splitting-roulette, each birth record drawing from its own stream).  Every active
+ * generation is one statistical batch of n_particles histories of the tallies; inactive ones are
+ * discarded.  Time plays no part: describe the problem with one time bin and one census far beyond any
+ * flight.  k_gen: HOST array of n_inactive + n_active doubles.  Needs the workspace of
+ * mcdc_workspace_size(n_particles, 1 or more); implicit capture and roulette apply if set;
+ * population_control must be off (MCDC_ERR_ARG).                                                       */
+int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64_t seed, uint32_t n_inactive,
+                        uint32_t n_active, double *k_gen);
+
 /* mean[i] = sum_i / N (cm of track per source history, not divided by bin volume);
  * sdev[i] = batch standard error of the mean (0 with a single batch).  n_bins must equal
  * n_time_bins*G*nz*ny*nx.                                                                          */

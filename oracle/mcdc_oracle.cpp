@@ -735,6 +735,7 @@ int orc_run_eigenvalue(orc_problem *P, uint64_t N, uint64_t seed, uint32_t n_ina
     k_gen[g] = start_w > 0.0 ? (P->cnt.production - prod0) / start_w : 0.0;
     if (g >= n_inactive) { P->cnt.histories += N; close_batch(*P); }
     else std::fill(P->x.begin(), P->x.end(), 0.0);
+    if (g + 1 == G_total) break;                          // the last generation's bank is not needed
     std::vector<Owned> bank;
     for (const BankItem &b : fis) bank.emplace_back(1u, b.p);
     next.clear();

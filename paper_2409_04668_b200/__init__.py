@@ -17,6 +17,7 @@ from .api import (  # noqa: F401
     mcdc_workspace_bind,
     mcdc_run,
     mcdc_run_ex,
+    mcdc_run_eigenvalue,
     mcdc_tallies_get,
     mcdc_tally_sums_get,
     mcdc_counters_get,

@@ -19,7 +19,7 @@ EXPORTED_SYMBOLS = [
     "mcdc_workspace_bind", "mcdc_run", "mcdc_run_ex", "mcdc_tallies_get", "mcdc_tally_sums_get",
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
-    "mcdc_state_size", "mcdc_state_export", "mcdc_state_import",
+    "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -111,6 +111,8 @@ def lib():
     L.mcdc_census_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.mcdc_census_get.restype = C.c_int
     L.mcdc_history_events_get.argtypes = [vp, C.POINTER(C.c_uint32), C.c_size_t]
     L.mcdc_history_events_get.restype = C.c_int
+    L.mcdc_run_eigenvalue.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _dp]
+    L.mcdc_run_eigenvalue.restype = C.c_int
     L.mcdc_technique_set.argtypes = [vp, C.POINTER(Technique)]; L.mcdc_technique_set.restype = C.c_int
     L.mcdc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]
     L.mcdc_census_after_get.restype = C.c_int
@@ -232,6 +234,13 @@ def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_hi
     _check(lib().mcdc_run_ex(h, int(n_histories), int(seed), C.byref(o)), "mcdc_run_ex", h)
 
 
+def mcdc_run_eigenvalue(h, n_particles, seed, n_inactive, n_active):
+    k = np.zeros(int(n_inactive) + int(n_active))
+    _check(lib().mcdc_run_eigenvalue(h, int(n_particles), int(seed), int(n_inactive), int(n_active), _d(k)),
+           "mcdc_run_eigenvalue", h)
+    return k
+
+
 def mcdc_tallies_get(h, n_bins):
     mean = np.empty(n_bins); sdev = np.empty(n_bins)
     _check(lib().mcdc_tallies_get(h, _d(mean), _d(sdev), n_bins), "mcdc_tallies_get", h)
@@ -349,6 +358,11 @@ class Problem:
         b = int(n_batches if n_batches is not None else self.prob.n_batches)
         mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events, scheduler)
         self._last_n = n
+
+    def run_eigenvalue(self, n_particles=None, seed=None, n_inactive=0, n_active=1):
+        n = int(n_particles if n_particles is not None else self.prob.n_histories)
+        s = int(seed if seed is not None else self.prob.seed)
+        return mcdc_run_eigenvalue(self._h, n, s, n_inactive, n_active)
 
     def tallies(self):
         m, s = mcdc_tallies_get(self._h, self.n_bins)

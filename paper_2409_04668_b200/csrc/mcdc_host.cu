@@ -906,7 +906,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
         for (uint32_t s = 0; s < ns; ++s) n_max = std::max(n_max, hc[s]);
       }
       PcParams pc;
-      pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs;
+      pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs; pc.w_out = 0.0;
       const dim3 grid((n_max + 255) / 256, ns);
       CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
       CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
@@ -1120,7 +1120,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
     if (k < p->K - 1 && live_total > 0) {
       if (p->tech.population_control) {                   // Appendix G.3: census bank Bk -> live bank A
         PcParams pc;
-        pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs;
+        pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs; pc.w_out = 0.0;
         const dim3 pgrid((n_max + 255) / 256, ns);
         CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
         CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
@@ -1244,6 +1244,124 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   CK(cudaMemcpy(&overflow, &p->d_cnt->overflow, sizeof(int), cudaMemcpyDeviceToHost));
   if (overflow) return MCDC_ERR_BANK_OVERFLOW;
   p->histories += n_histories; p->batches += B; p->batch_size = hb;
+  return MCDC_OK;
+}
+
+// ---- k-eigenvalue mode (include/mcdc.h mcdc_run_eigenvalue; DESIGN.md Appendix H) ----
+extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64_t seed, uint32_t n_inactive,
+                                   uint32_t n_active, double *k_gen) {
+  if (!p || !k_gen || n_particles == 0 || n_active == 0 || n_particles > 0x7FFFFFF0ull) return MCDC_ERR_ARG;
+  if (p->batch_size != 0 && p->batch_size != n_particles) return MCDC_ERR_ARG;
+  if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
+  if (!p->tab.warp_ok) return MCDC_ERR_ARG;               // this mode exists on the history kernel only
+  if (p->cap == 0 || p->ws_hist < n_particles) return MCDC_ERR_NO_WORKSPACE;
+  if (p->tech.population_control) return MCDC_ERR_ARG;    // there is no census here; the generation has its own control
+  const int rcp = plan_warp_kernel(p, false, true);
+  if (rcp != MCDC_OK) return rcp;
+  const uint32_t ws_ns = p->ws_slots, N = (uint32_t)n_particles;
+  uint32_t *counts_dev = p->counts_dev;
+  std::vector<uint32_t> h_counts((size_t)8 * ws_ns);
+  CK(cudaMemsetAsync(counts_dev, 0, (size_t)8 * ws_ns * sizeof(uint32_t), p->stream));
+  Bank A = p->bankA, Bk = p->bankB;
+  HistoryArgs ha;
+  ha.q = p->queue;
+  ha.hist_cursor = p->d_hist_cursor;
+  ha.seed_mixed = mix64(seed + MCDC_GAMMA);
+  ha.first_history = 0ull;
+  ha.n_hist = N; ha.hb = N;
+  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.ev = nullptr;
+  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
+  const bool staged = p->stage_tables;
+  ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
+  ha.pool_slots = p->pool_slots;
+  const int nt = p->hist_threads;
+  const uint64_t per_block = (uint64_t)p->pool_slots * (nt / 32);
+  ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)N / ((uint64_t)p->n_sm * (nt / 32) * 8)));
+  ha.n_slots = 1;
+  ha.step_mode = 2; ha.step_k = 0; ha.step_single = 1; ha.bank_cap = p->cap;
+  cudaEvent_t e_run0, e_run1;
+  CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1));
+  p->ms_transport = 0.0;
+  CK(cudaEventRecord(e_run0, p->stream));
+  const uint32_t G_total = n_inactive + n_active;
+  double prod_prev = 0.0, lost_prev = 0.0;
+  {
+    DevCounters h;
+    CK(cudaMemcpy(&h, p->d_cnt, sizeof(h), cudaMemcpyDeviceToHost));
+    prod_prev = h.ledger[1]; lost_prev = h.ledger[6];
+  }
+  uint64_t live = 0;
+  int rc = MCDC_OK;
+  for (uint32_t g = 0; g < G_total; ++g) {
+    ha.step_source = (g == 0) ? 1 : 0;
+    ha.n_chunks = (g == 0) ? (N + ha.src_chunk - 1) / ha.src_chunk : 0u;
+    ha.in = A; ha.census_out = Bk;
+    CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
+    CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
+    CK(cudaMemsetAsync(A.cursor, 0, sizeof(uint32_t), p->stream));
+    CK(cudaMemsetAsync(Bk.count, 0, sizeof(uint32_t), p->stream));
+    const uint64_t work = (g == 0) ? N : live;
+    const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work + per_block - 1) / per_block));
+    cudaEvent_t a, b;
+    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    CK(cudaEventRecord(a, p->stream));
+    warp_launch(staged, false, true, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    CK(cudaEventRecord(b, p->stream));
+    p->ev_pairs.emplace_back(a, b);
+    p->launches++;
+    // H.2: an active generation is one statistical batch; an inactive one is discarded
+    if (g >= n_inactive) {
+      int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
+      k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, 1, 0, p->n_bins, p->d_sum, p->d_sumsq);
+      p->launches++;
+    } else CK(cudaMemsetAsync(p->x_acc, 0, p->n_bins * sizeof(double), p->stream));
+    DevCounters h;
+    CK(cudaMemcpyAsync(&h, p->d_cnt, sizeof(h), cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    CK(cudaGetLastError());
+    if (h.overflow) { rc = MCDC_ERR_BANK_OVERFLOW; break; }
+    const double start_w = (g == 0) ? (double)N - (h.ledger[6] - lost_prev) : (double)live;   // unit weights (H.3)
+    k_gen[g] = start_w > 0.0 ? (h.ledger[1] - prod_prev) / start_w : 0.0;
+    prod_prev = h.ledger[1];
+    const uint32_t n_fis = h_counts[Bk.count - counts_dev];
+    if (n_fis > p->cap) { rc = MCDC_ERR_BANK_OVERFLOW; break; }
+    if (g >= n_inactive) { p->histories += N; p->batches += 1; }
+    live = 0;
+    if (n_fis == 0) { for (uint32_t r = g + 1; r < G_total; ++r) k_gen[r] = 0.0; break; }
+    if (g + 1 == G_total) break;
+    // H.3: the fission bank Bk is controlled to N particles of weight 1 -> the next generation's bank A
+    PcParams pc;
+    pc.cap = p->cap; pc.k = 0; pc.target = N; pc.w_out = 1.0;
+    const dim3 pgrid((n_fis + 255) / 256, 1);
+    CK(cudaMemsetAsync(p->d_wfix, 0, sizeof(unsigned long long), p->stream));
+    CK(cudaMemsetAsync(A.count, 0, sizeof(uint32_t), p->stream));
+    k_pc_weight<<<pgrid, 256, 0, p->stream>>>(Bk, p->cap, p->d_wfix);
+    k_pc_apply<<<pgrid, 256, 0, p->stream>>>(Bk, A, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
+    p->launches += 2;
+    CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+    CK(cudaStreamSynchronize(p->stream));
+    CK(cudaGetLastError());
+    live = h_counts[A.count - counts_dev];
+    if (live > p->cap) { rc = MCDC_ERR_BANK_OVERFLOW; break; }
+  }
+  cudaEventRecord(e_run1, p->stream);
+  cudaError_t se = cudaStreamSynchronize(p->stream);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e_run0, e_run1);
+  p->ms_run = ms;
+  for (auto &pr : p->ev_pairs) {
+    float m2 = 0.f;
+    if (se == cudaSuccess && cudaEventElapsedTime(&m2, pr.first, pr.second) == cudaSuccess) p->ms_transport += m2;
+    cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
+  }
+  p->ev_pairs.clear();
+  cudaEventDestroy(e_run0); cudaEventDestroy(e_run1);
+  if (se != cudaSuccess) return cuda_fail(p, se, "cudaStreamSynchronize");
+  if (rc != MCDC_OK) return rc;
+  p->batch_size = n_particles;
+  p->ev_n = 0;
   return MCDC_OK;
 }
 

@@ -564,6 +564,7 @@ struct PcParams {
   uint32_t cap;
   int k;                              // census index
   unsigned long long target;          // particles per batch after the control
+  double w_out;                       // > 0: weight given to every copy (generation control, Appendix H.3); else w_t
 };
 
 __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P, const unsigned long long *wfix,
@@ -576,6 +577,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
   const bool have = i < n_in && W != 0ull;
   const size_t j = (size_t)slot * P.cap + (have ? i : 0u);
   const double w_t = ((double)W / MCDC_FIX40) / (double)P.target;
+  const double w_new = (P.w_out > 0.0) ? P.w_out : w_t;
   double w = 0.0, gain = 0.0, loss = 0.0;
   unsigned long long key = 0ull;
   uint32_t ctr = 0u;
@@ -609,7 +611,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
       if (o >= P.cap) { atomicExch(&cnt->overflow, 1); break; }
       const size_t q = (size_t)slot * P.cap + o;
       out.x[q] = x; out.y[q] = y; out.z[q] = z; out.ux[q] = ux; out.uy[q] = uy; out.uz[q] = uz; out.t[q] = t;
-      out.w[q] = w_t; out.hid[q] = hid;
+      out.w[q] = w_new; out.hid[q] = hid;
       out.key[q] = (c == 0) ? key : child_key(key, ctr, (uint32_t)c);   // copy 0 keeps its stream
       out.meta[q] = make_int4(m.x, m.y, (c == 0) ? (int)ctr : 0, m.w);
     }
@@ -618,7 +620,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
   block_atomic_add(&cnt->ledger[1 + LED_VR_LOSS], loss, scratch);
   block_atomic_add_u64(&cnt->n[7], (have && n == 0) ? 1ull : 0ull, (unsigned long long *)scratch);
   block_atomic_add_u64(&cnt->n[8], (n > 1) ? (unsigned long long)(n - 1) : 0ull, (unsigned long long *)scratch);
-  block_atomic_add(pop_w_after + P.k, (double)n * w_t, scratch);
+  block_atomic_add(pop_w_after + P.k, (double)n * w_new, scratch);
   block_atomic_add_u64(pop_n_after + P.k, (unsigned long long)n, (unsigned long long *)scratch);
 }
 
@@ -652,7 +654,8 @@ struct HistoryArgs {
   // census-step mode of k_warp<WEIGHTED> (population control, Appendix G.3): one launch transports one census step.
   // Particles come from the live bank `in` (survivors of the control at the previous census) and from the source
   // histories born in this step; a particle that reaches the census time is parked in `census_out` instead of going on.
-  int step_mode, step_k, step_source, step_single;   // on/off; census index; sources may be born in this step; all are
+  int step_mode, step_k, step_source, step_single;   // 0 off, 1 census step, 2 generation (Appendix H); census index;
+                                                     // sources may be born in this launch; all of them are
   uint32_t bank_cap;              // bank capacity per batch slot
   Bank in, census_out;
 };

@@ -151,7 +151,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
   bool src_exhausted = false;
-  const bool step_mode = WEIGHTED && A.step_mode != 0; // census-step mode (Appendix G.3)
+  const bool step_mode = WEIGHTED && A.step_mode != 0; // census-step mode (Appendix G.3) or generation mode (H)
+  const bool gen_mode = WEIGHTED && A.step_mode == 2;  // k-eigenvalue: `in` holds birth records, children go to `census_out`
   bool bank_done = !step_mode;                         // the live bank of this step has been handed out
   uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
   if (step_mode && !A.step_source) src_exhausted = true;
@@ -184,7 +185,18 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         bank_probes = 0u;
         const uint32_t nb = min(want, cnt - base);
         const bool actb = (uint32_t)lane < nb;
-        if (actb) {
+        if (actb && gen_mode) {                          // a birth record: group and direction are sampled in the C phase
+          const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
+          const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
+          const int4 m = A.in.meta[j];                   // {cell, -, counter, -}
+          PD(D_X, gi) = A.in.x[j]; PD(D_Y, gi) = A.in.y[j]; PD(D_Z, gi) = A.in.z[j]; PD(D_T, gi) = A.in.t[j];
+          PD(D_W, gi) = A.in.w[j];
+          PK(gi) = A.in.key[j]; PU(U_CTR, gi) = (uint32_t)m.z;
+          PU(U_CL, gi) = (uint32_t)m.x | (NONE16 << 16);
+          PU(U_META, gi) = 255u | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
+          if (RECORD) PU(U_HID, gi) = A.in.hid[j];
+          PL(L_C, lb + nC + (uint32_t)lane) = (uint8_t)i;
+        } else if (actb) {
           const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
           const double ux = A.in.ux[j], uy = A.in.uy[j], uz = A.in.uz[j];
@@ -199,7 +211,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           if (RECORD) PU(U_HID, gi) = A.in.hid[j];
           PL(L_F, lb + nF + (uint32_t)lane) = (uint8_t)i;
         }
-        nFree -= nb; nF += nb;
+        nFree -= nb;
+        if (gen_mode) nC += nb; else nF += nb;
         __syncwarp();
         continue;
       }
@@ -559,8 +572,9 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
       const int mg = mat * G + g;
       // reaction: scatter, capture, fission in this order (D6); with weights, the techniques of Appendix G
+      const uint32_t ctr_in = ctr;
       const double xi_r = draw(key, ctr);
-      if (born) ctr = 0u;                              // nothing drawn yet from a new child's stream
+      if (born) ctr = ctr_in;                          // a new child has no reaction: its stream goes on where it was
       int kind = FI_NONE, n_child = 0;                 // kind of the outgoing flight; children of a fission
       bool alive = false, captured = false, fissioned = false;
       uint32_t c0 = 0u;
@@ -594,7 +608,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           c0 = ctr;
           fissioned = true;
           l_fis += w; l_prod += (double)n_child * w;
-          if (n_child > 0) { kind = FI_CHILD; alive = true; }
+          if (n_child > 0 && !gen_mode) { kind = FI_CHILD; alive = true; }
         }
       }
       {
@@ -622,7 +636,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (n_child > 0) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + 2, (uint32_t)n_child);
       }
       // fission: publish children 1..n-1 to the global queue, continue as child 0
-      const int n_push = (n_child > 1) ? n_child - 1 : 0;
+      // (generation mode: every child goes to the fission bank of the generation and the parent ends here)
+      const int n_push = gen_mode ? n_child : ((n_child > 1) ? n_child - 1 : 0);
       if (__ballot_sync(MCDC_FULL, n_push > 0) != 0u) {
         int pre = n_push;
 #pragma unroll
@@ -631,7 +646,23 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           if (lane >= o) pre += v;
         }
         const int total = __shfl_sync(MCDC_FULL, pre, 31);
-        if ((uint32_t)total <= nFree) {                // the children fit this warp's pool: they join its C stack
+        if (gen_mode) {
+          uint32_t base = 0u;
+          if (lane == 0) base = atomicAdd(A.census_out.count, (uint32_t)total);   // one batch slot in this mode
+          base = __shfl_sync(MCDC_FULL, base, 0) + (uint32_t)(pre - n_push);
+          if (n_push > 0) {
+            const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
+            const Bank &O = A.census_out;
+            for (int c = 0; c < n_push; ++c) {
+              const uint32_t j = base + (uint32_t)c;
+              if (j >= A.bank_cap) { atomicExch(&A.cnt->overflow, 1); break; }
+              O.x[j] = x; O.y[j] = y; O.z[j] = z; O.t[j] = t; O.w[j] = w;
+              O.key[j] = child_key(key, c0, (uint32_t)c);
+              O.meta[j] = make_int4(cell, -1, 0, 0);
+              O.hid[j] = RECORD ? PU(U_HID, gi) : 0u;
+            }
+          }
+        } else if ((uint32_t)total <= nFree) {         // the children fit this warp's pool: they join its C stack
           if (n_push > 0) {
             const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
             for (int c = 0; c < n_push; ++c) {
