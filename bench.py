@@ -305,10 +305,40 @@ def bench_gpu(args):
     g.close()
     if args.sweep and world == 1:
         out["sweep"] = run_sweep(M, args, dev, peak)
+    if args.eigenvalue and world == 1:
+        out["eigenvalue"] = run_eigenvalue(M, args, dev)
     if rank == 0:
         print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
+
+
+def run_eigenvalue(M, args, dev):
+    """Side measurement (not the headline): the k-eigenvalue mode (DESIGN.md Appendix H) on the config-3 lattice,
+    1e6 particles per generation, 5 inactive + 15 active generations."""
+    import torch
+    from workloads import configs as W
+
+    n, n_in, n_act = 1_000_000, 5, 15
+    p = W.as_eigenvalue(W.config3_pin_lattice(n_histories=n, n_batches=1))
+    g = M.Problem(p, max_histories_per_subbatch=n, max_batches_in_flight=1, device=dev, workspace_scale=1.5)
+    g.run_eigenvalue(n, p.seed, 1, 2)                     # warm-up
+    g.reset()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    k = g.run_eigenvalue(n, p.seed, n_in, n_act)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    c = g.counters()
+    out = {"workload": p.name, "particles_per_generation": n, "inactive": n_in, "active": n_act,
+           "k_eff": float(k[n_in:].mean()), "k_sdev": float(k[n_in:].std(ddof=1) / np.sqrt(n_act)),
+           "ms_per_generation": ms / (n_in + n_act), "particles_per_s": n * (n_in + n_act) / (ms * 1e-3),
+           "segments_per_s": c["segments"] / (ms * 1e-3), "ms_transport": c["ms_transport"],
+           "launches": int(c["kernel_launches"])}
+    g.close()
+    return out
 
 
 def run_sweep(M, args, dev, peak):
@@ -363,6 +393,7 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--sweep", action="store_true", help="also run the config-4 batch-size sweep (adds a 'sweep' key)")
     ap.add_argument("--sweep-max", type=float, default=1e9)
+    ap.add_argument("--eigenvalue", action="store_true", help="also time the k-eigenvalue mode (adds an 'eigenvalue' key)")
     args = ap.parse_args()
     if args.impl == "reference":
         bench_reference(args)
