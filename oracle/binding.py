@@ -97,6 +97,8 @@ def _load():
     L.orc_close_batch.argtypes = [vp, C.c_uint64]; L.orc_close_batch.restype = C.c_int
     L.orc_run_eigenvalue.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, C.c_int32, _dp]
     L.orc_run_eigenvalue.restype = C.c_int
+    L.orc_collision_tally_enable.argtypes = [vp, C.c_int]; L.orc_collision_tally_enable.restype = C.c_int
+    L.orc_collision_tallies_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.orc_collision_tallies_get.restype = C.c_int
     L.orc_technique_set.argtypes = [vp, C.POINTER(_Technique)]; L.orc_technique_set.restype = C.c_int
     L.orc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.orc_census_after_get.restype = C.c_int
     L.orc_population_control.argtypes = [vp, C.c_size_t, _dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.c_uint64,
@@ -241,6 +243,17 @@ class Oracle:
         rc = self._L.orc_tallies_get(self._h, _d(mean), _d(sdev), self.n_bins)
         if rc != 0:
             raise RuntimeError(f"orc_tallies_get failed: {rc}")
+        shp = self.prob.tally_shape()
+        return mean.reshape(shp), sdev.reshape(shp)
+
+    def enable_collision_tally(self, on=True):
+        self._L.orc_collision_tally_enable(self._h, int(bool(on)))
+
+    def collision_tallies(self):
+        mean = np.empty(self.n_bins); sdev = np.empty(self.n_bins)
+        rc = self._L.orc_collision_tallies_get(self._h, _d(mean), _d(sdev), self.n_bins)
+        if rc != 0:
+            raise RuntimeError(f"orc_collision_tallies_get failed: {rc}")
         shp = self.prob.tally_shape()
         return mean.reshape(shp), sdev.reshape(shp)
 

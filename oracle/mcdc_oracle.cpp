@@ -100,6 +100,8 @@ struct orc_problem {
   size_t n_bins;
   // results
   std::vector<double> x, sum, sumsq;         // batch accumulator, sum of S_b, sum of S_b^2
+  int col_on;                                // collision-estimator tally (Appendix I) on the same mesh
+  std::vector<double> xc, sumc, sumsqc;
   std::vector<double> pop_w; std::vector<uint64_t> pop_n;
   std::vector<double> pop_w_after; std::vector<uint64_t> pop_n_after;   // after the population control (G.3)
   orc_technique tech;                        // Appendix G of DESIGN.md; all zero = analog
@@ -348,11 +350,34 @@ void surface_event(orc_problem &P, Particle &p, int s_star) {
 // ---------------------------------------------------------------------------------------------
 // A.6 collision event.  Children are appended to `bank` as birth records.
 // ---------------------------------------------------------------------------------------------
+// Appendix I: the collision tally of the paper's Fig. 3 (`add(mcdc.col_tally, part.v, loc2index(part))`),
+// read as the collision estimator of the flux: the bin that holds the collision site (r, t, g) takes w / Sigma_t.
+// loc2index: i_a = floor((r_a - lo_a) / Delta_a) for lo_a <= r_a < hi_a, largest it with T[it] <= t for
+// T[0] <= t < T[Nt]; a site outside the mesh or the time grid scores nothing.
+void score_collision(orc_problem &P, const Particle &p, double sig_t) {
+  const double r[3] = {p.x, p.y, p.z};
+  int idx[3];
+  for (int a = 0; a < 3; ++a) {
+    if (!(P.mesh_lo[a] <= r[a] && r[a] < P.mesh_hi[a])) return;
+    int n = P.mesh_n[a];
+    if (n == 1) { idx[a] = 0; continue; }
+    double delta = (P.mesh_hi[a] - P.mesh_lo[a]) / (double)n;
+    double q = std::floor((r[a] - P.mesh_lo[a]) / delta);
+    idx[a] = (q > (double)(n - 1)) ? n - 1 : (int)q;
+  }
+  if (!(P.T[0] <= p.t && p.t < P.T[P.Nt])) return;
+  int it = 0;
+  for (int j = 0; j < P.Nt; ++j) if (P.T[j] <= p.t) it = j;
+  size_t bin = ((((size_t)it * P.G + p.g) * P.mesh_n[2] + idx[2]) * P.mesh_n[1] + idx[1]) * P.mesh_n[0] + idx[0];
+  P.xc[bin] += p.w / sig_t;
+}
+
 void collision_event(orc_problem &P, Particle &p, std::deque<BankItem> &bank) {
   P.cnt.collisions += 1; bump(P, 0);
   p.last_surface = -1;
   const int m = P.cell_material[p.cell], G = P.G;
   const size_t mg = (size_t)m * G + p.g;
+  if (P.col_on) score_collision(P, p, P.sigma_t[mg]);   // with the weight the particle arrives with
   double xi = draw(p.key, p.ctr);
   double s_tot = P.sigma_s_tot[mg];
   bool scatter;
@@ -483,6 +508,11 @@ void close_batch(orc_problem &P) {                    // A.9
     double s = P.x[i];
     P.sum[i] += s; P.sumsq[i] += s * s; P.x[i] = 0.0;
   }
+  if (P.col_on)
+    for (size_t i = 0; i < P.n_bins; ++i) {
+      double s = P.xc[i];
+      P.sumc[i] += s; P.sumsqc[i] += s * s; P.xc[i] = 0.0;
+    }
   P.cnt.batches += 1;
 }
 
@@ -578,6 +608,7 @@ int orc_create(const orc_desc *d, orc_problem **out) {
   build_boxes(*P);
   P->cur_ev = nullptr;
   std::memset(&P->tech, 0, sizeof(P->tech));
+  P->col_on = 0;
   orc_reset(P);
   *out = P;
   return 0;
@@ -620,6 +651,7 @@ void orc_destroy(orc_problem *p) { delete p; }
 
 void orc_reset(orc_problem *P) {
   P->x.assign(P->n_bins, 0.0); P->sum.assign(P->n_bins, 0.0); P->sumsq.assign(P->n_bins, 0.0);
+  P->xc.assign(P->n_bins, 0.0); P->sumc.assign(P->n_bins, 0.0); P->sumsqc.assign(P->n_bins, 0.0);
   P->pop_w.assign(P->K, 0.0); P->pop_n.assign(P->K, 0);
   P->pop_w_after.assign(P->K, 0.0); P->pop_n_after.assign(P->K, 0);
   std::memset(&P->cnt, 0, sizeof(P->cnt));
@@ -734,7 +766,7 @@ int orc_run_eigenvalue(orc_problem *P, uint64_t N, uint64_t seed, uint32_t n_ina
     }
     k_gen[g] = start_w > 0.0 ? (P->cnt.production - prod0) / start_w : 0.0;
     if (g >= n_inactive) { P->cnt.histories += N; close_batch(*P); }
-    else std::fill(P->x.begin(), P->x.end(), 0.0);
+    else { std::fill(P->x.begin(), P->x.end(), 0.0); std::fill(P->xc.begin(), P->xc.end(), 0.0); }
     if (g + 1 == G_total) break;                          // the last generation's bank is not needed
     std::vector<Owned> bank;
     for (const BankItem &b : fis) bank.emplace_back(1u, b.p);
@@ -764,6 +796,26 @@ int orc_tallies_get(const orc_problem *P, double *mean, double *sdev, size_t n_b
     mean[i] = mu;
     if (B > 1.0) {
       double m2 = P->sumsq[i] / (hb * hb) / B;
+      double var = (m2 - mu * mu) / (B - 1.0);
+      sdev[i] = var > 0.0 ? std::sqrt(var) : 0.0;
+    } else sdev[i] = 0.0;
+  }
+  return 0;
+}
+
+int orc_collision_tally_enable(orc_problem *P, int on) { if (!P) return -1; P->col_on = on ? 1 : 0; return 0; }
+
+// same statistics as orc_tallies_get (A.9), from the collision-estimator accumulators
+int orc_collision_tallies_get(const orc_problem *P, double *mean, double *sdev, size_t n_bins) {
+  if (n_bins != P->n_bins) return -4;
+  double N = (double)P->cnt.histories, B = (double)P->cnt.batches;
+  if (N == 0.0) return -1;
+  double hb = N / B;
+  for (size_t i = 0; i < n_bins; ++i) {
+    double mu = P->sumc[i] / N;
+    mean[i] = mu;
+    if (B > 1.0) {
+      double m2 = P->sumsqc[i] / (hb * hb) / B;
       double var = (m2 - mu * mu) / (B - 1.0);
       sdev[i] = var > 0.0 ? std::sqrt(var) : 0.0;
     } else sdev[i] = 0.0;

@@ -85,6 +85,9 @@ int  orc_run_eigenvalue(orc_problem *p, uint64_t N, uint64_t seed, uint32_t n_in
                         int32_t reverse_order, double *k_gen);
 int  orc_tallies_get(const orc_problem *p, double *mean, double *sdev, size_t n_bins);
 int  orc_tally_sums_get(const orc_problem *p, double *sum, double *sumsq, size_t n_bins);
+/* collision-estimator tally of the paper's Fig. 3 (DESIGN.md Appendix I): off by default */
+int  orc_collision_tally_enable(orc_problem *p, int on);
+int  orc_collision_tallies_get(const orc_problem *p, double *mean, double *sdev, size_t n_bins);
 int  orc_counters_get(const orc_problem *p, orc_counters *c);
 int  orc_census_get(const orc_problem *p, double *pop_w, uint64_t *pop_n, size_t K);
 int  orc_history_events_get(const orc_problem *p, uint32_t *ev /* [n][4] */, size_t n);
