@@ -175,6 +175,15 @@ int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64_t seed, ui
  * sdev[i] = batch standard error of the mean (0 with a single batch).  n_bins must equal
  * n_time_bins*G*nz*ny*nx.                                                                          */
 int mcdc_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
+/* Collision-estimator tally, the paper's one code listing (Fig. 3:
+ * `add(mcdc.col_tally, part.v, loc2index(part))` inside tally_collision_event); SURVEY.md 8(f) NEXT-4;
+ * reading in DESIGN.md Appendix I: at every collision the bin of the SAME mesh that holds the collision
+ * site (r, t, g) takes w / Sigma_t, w the weight the particle arrives with -- an estimate of the same flux
+ * as the track-length tally.  Off by default; enable before the run.  The accumulators are allocated by
+ * the library (one per batch slot of the bound workspace) and are not part of mcdc_state_export.
+ * mcdc_collision_tallies_get has the layout and statistics of mcdc_tallies_get.                        */
+int mcdc_collision_tally_enable(mcdc_problem *p, int on);
+int mcdc_collision_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
 /* Raw accumulators: sum over batches of S_b and of S_b^2.                                          */
 int mcdc_tally_sums_get(const mcdc_problem *p, double *sum, double *sumsq, size_t n_bins);
 int mcdc_counters_get(const mcdc_problem *p, mcdc_counters *c);

@@ -20,6 +20,8 @@ from .api import (  # noqa: F401
     mcdc_run_eigenvalue,
     mcdc_tallies_get,
     mcdc_tally_sums_get,
+    mcdc_collision_tally_enable,
+    mcdc_collision_tallies_get,
     mcdc_counters_get,
     mcdc_census_get,
     mcdc_history_events_get,

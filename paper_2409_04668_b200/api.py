@@ -20,6 +20,7 @@ EXPORTED_SYMBOLS = [
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
     "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
+    "mcdc_collision_tally_enable", "mcdc_collision_tallies_get",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -113,6 +114,8 @@ def lib():
     L.mcdc_history_events_get.restype = C.c_int
     L.mcdc_run_eigenvalue.argtypes = [vp, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, _dp]
     L.mcdc_run_eigenvalue.restype = C.c_int
+    L.mcdc_collision_tally_enable.argtypes = [vp, C.c_int]; L.mcdc_collision_tally_enable.restype = C.c_int
+    L.mcdc_collision_tallies_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_collision_tallies_get.restype = C.c_int
     L.mcdc_technique_set.argtypes = [vp, C.POINTER(Technique)]; L.mcdc_technique_set.restype = C.c_int
     L.mcdc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]
     L.mcdc_census_after_get.restype = C.c_int
@@ -247,6 +250,16 @@ def mcdc_tallies_get(h, n_bins):
     return mean, sdev
 
 
+def mcdc_collision_tally_enable(h, on=True):
+    _check(lib().mcdc_collision_tally_enable(h, int(bool(on))), "mcdc_collision_tally_enable", h)
+
+
+def mcdc_collision_tallies_get(h, n_bins):
+    mean = np.empty(n_bins); sdev = np.empty(n_bins)
+    _check(lib().mcdc_collision_tallies_get(h, _d(mean), _d(sdev), n_bins), "mcdc_collision_tallies_get", h)
+    return mean, sdev
+
+
 def mcdc_tally_sums_get(h, n_bins):
     s = np.empty(n_bins); q = np.empty(n_bins)
     _check(lib().mcdc_tally_sums_get(h, _d(s), _d(q), n_bins), "mcdc_tally_sums_get", h)
@@ -366,6 +379,13 @@ class Problem:
 
     def tallies(self):
         m, s = mcdc_tallies_get(self._h, self.n_bins)
+        return m.reshape(self.shape), s.reshape(self.shape)
+
+    def enable_collision_tally(self, on=True):
+        mcdc_collision_tally_enable(self._h, on)
+
+    def collision_tallies(self):
+        m, s = mcdc_collision_tallies_get(self._h, self.n_bins)
         return m.reshape(self.shape), s.reshape(self.shape)
 
     def tally_sums(self):

@@ -75,6 +75,10 @@ struct mcdc_problem {
   Tables tab;
   double *d_sum = nullptr, *d_sumsq = nullptr, *d_pop_w = nullptr, *d_pop_w_after = nullptr;
   unsigned long long *d_pop_n = nullptr, *d_pop_n_after = nullptr;
+  // collision-estimator tally (Appendix I): handle-owned, allocated when it is switched on
+  int col_on = 0;
+  double *d_xc_acc = nullptr, *d_sumc = nullptr, *d_sumsqc = nullptr;
+  uint32_t xc_slots = 0;
   unsigned long long *d_wfix = nullptr;   // [ws_slots] arriving weight of a batch in 2^-40 fixed point (workspace)
   mcdc_technique tech = {0, 0.0, 0.0, 0, 0ull};
   DevCounters *d_cnt = nullptr;
@@ -107,6 +111,8 @@ struct mcdc_problem {
 };
 
 namespace {
+
+int ensure_collision_buffers(mcdc_problem *p);   // defined with the result calls
 
 int cuda_fail(mcdc_problem *p, cudaError_t e, const char *where) {
   p->cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
@@ -649,6 +655,9 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p) {
   if (!p) return;
   p->arena.release();
   if (p->d_ev) cudaFree(p->d_ev);
+  if (p->d_xc_acc) cudaFree(p->d_xc_acc);
+  if (p->d_sumc) cudaFree(p->d_sumc);
+  if (p->d_sumsqc) cudaFree(p->d_sumsqc);
   delete p;
 }
 
@@ -662,6 +671,11 @@ extern "C" int mcdc_problem_reset(mcdc_problem *p) {
   CK(cudaMemsetAsync(p->d_pop_n_after, 0, p->K * sizeof(unsigned long long), p->stream));
   CK(cudaMemsetAsync(p->d_cnt, 0, sizeof(DevCounters), p->stream));
   if (p->x_acc) CK(cudaMemsetAsync(p->x_acc, 0, (size_t)p->ws_slots * p->n_bins * sizeof(double), p->stream));
+  if (p->d_xc_acc) {
+    CK(cudaMemsetAsync(p->d_xc_acc, 0, (size_t)p->xc_slots * p->n_bins * sizeof(double), p->stream));
+    CK(cudaMemsetAsync(p->d_sumc, 0, p->n_bins * sizeof(double), p->stream));
+    CK(cudaMemsetAsync(p->d_sumsqc, 0, p->n_bins * sizeof(double), p->stream));
+  }
   CK(cudaStreamSynchronize(p->stream));
   p->histories = p->batches = p->batch_size = p->launches = 0;
   p->ms_run = p->ms_transport = 0.0;
@@ -824,7 +838,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   const int k_first = step_of(p, p->src_t0), k_last = step_of(p, p->src_t1);
   const size_t n_spatial_g = p->n_spatial * (size_t)p->G;
   TransportArgs ta;
-  ta.x_acc = p->x_acc; ta.cnt = p->d_cnt; ta.pop_w = p->d_pop_w; ta.pop_n = p->d_pop_n;
+  ta.x_acc = p->x_acc; ta.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ta.cnt = p->d_cnt; ta.pop_w = p->d_pop_w; ta.pop_n = p->d_pop_n;
   ta.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
   const int max_grid = p->n_sm * p->blocks_per_sm;
   uint64_t live_total = 0;
@@ -930,6 +944,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   if (sb.closeout) {
     int grid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
     k_closeout<<<grid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<grid, 256, 0, p->stream>>>(p->d_xc_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   return MCDC_OK;
@@ -1015,7 +1030,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   ha.seed_mixed = mix64(seed + MCDC_GAMMA);
   ha.first_history = first_history_id + sb.first_local;
   ha.n_hist = sb.n_hist; ha.hb = sb.hs;
-  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
   ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;   // in-warp merge of equal bins pays only on tiny meshes
   ha.step_mode = 0; ha.step_k = 0; ha.step_source = 1; ha.step_single = 1; ha.bank_cap = 0;
@@ -1042,7 +1057,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   cudaEvent_t a, b;
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
-  const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0;
+  const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on;
   warp_launch(staged, record, weighted, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
@@ -1050,6 +1065,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   if (sb.closeout) {
     int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
     k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)sb.n_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)sb.n_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   CK(cudaGetLastError());
@@ -1071,7 +1087,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   ha.seed_mixed = mix64(seed + MCDC_GAMMA);
   ha.first_history = first_history_id + sb.first_local;
   ha.n_hist = sb.n_hist; ha.hb = sb.hs;
-  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
   ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
   const bool staged = p->stage_tables;
@@ -1143,6 +1159,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   if (sb.closeout) {
     int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
     k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   CK(cudaGetLastError());
@@ -1160,6 +1177,7 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
   const uint64_t hb = n_histories / B;
   if (p->batch_size != 0 && p->batch_size != hb) return MCDC_ERR_ARG;
   if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
+  { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
   const bool record = opts->record_history_events != 0;
   if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
   // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
@@ -1187,7 +1205,7 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       p->blocks_per_sm = occ;
   }
   if (!stepped) {
-    const int rcp = plan_warp_kernel(p, record, stepwarp || p->tech.implicit_capture || p->tech.wr_threshold > 0.0);
+    const int rcp = plan_warp_kernel(p, record, stepwarp || p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on);
     if (rcp != MCDC_OK) return rcp;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
@@ -1256,6 +1274,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   if (!p->tab.warp_ok) return MCDC_ERR_ARG;               // this mode exists on the history kernel only
   if (p->cap == 0 || p->ws_hist < n_particles) return MCDC_ERR_NO_WORKSPACE;
   if (p->tech.population_control) return MCDC_ERR_ARG;    // there is no census here; the generation has its own control
+  { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
   const int rcp = plan_warp_kernel(p, false, true);
   if (rcp != MCDC_OK) return rcp;
   const uint32_t ws_ns = p->ws_slots, N = (uint32_t)n_particles;
@@ -1269,7 +1288,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   ha.seed_mixed = mix64(seed + MCDC_GAMMA);
   ha.first_history = 0ull;
   ha.n_hist = N; ha.hb = N;
-  ha.x_acc = p->x_acc; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
+  ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = nullptr;
   ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
   const bool staged = p->stage_tables;
@@ -1314,8 +1333,12 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
     if (g >= n_inactive) {
       int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
       k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, 1, 0, p->n_bins, p->d_sum, p->d_sumsq);
+      if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, 1, 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
       p->launches++;
-    } else CK(cudaMemsetAsync(p->x_acc, 0, p->n_bins * sizeof(double), p->stream));
+    } else {
+      CK(cudaMemsetAsync(p->x_acc, 0, p->n_bins * sizeof(double), p->stream));
+      if (p->col_on) CK(cudaMemsetAsync(p->d_xc_acc, 0, p->n_bins * sizeof(double), p->stream));
+    }
     DevCounters h;
     CK(cudaMemcpyAsync(&h, p->d_cnt, sizeof(h), cudaMemcpyDeviceToHost, p->stream));
     CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
@@ -1425,6 +1448,58 @@ extern "C" int mcdc_census_get(const mcdc_problem *cp, double *pop_w, uint64_t *
   CK(cudaMemcpy(pop_w, p->d_pop_w, K * sizeof(double), cudaMemcpyDeviceToHost));
   CK(cudaMemcpy(pop_n, p->d_pop_n, K * sizeof(uint64_t), cudaMemcpyDeviceToHost));
   return MCDC_OK;
+}
+
+namespace {
+// allocate (or re-allocate after a re-bind with more slots) the collision-estimator accumulators
+int ensure_collision_buffers(mcdc_problem *p) {
+  if (!p->col_on) return MCDC_OK;
+  const uint32_t slots = std::max<uint32_t>(1, p->ws_slots);
+  if (p->d_xc_acc && p->xc_slots >= slots) return MCDC_OK;
+  if (p->d_xc_acc) { cudaFree(p->d_xc_acc); p->d_xc_acc = nullptr; }
+  CK(cudaMalloc((void **)&p->d_xc_acc, (size_t)slots * p->n_bins * sizeof(double)));
+  CK(cudaMemset(p->d_xc_acc, 0, (size_t)slots * p->n_bins * sizeof(double)));
+  p->xc_slots = slots;
+  if (!p->d_sumc) {
+    CK(cudaMalloc((void **)&p->d_sumc, p->n_bins * sizeof(double)));
+    CK(cudaMalloc((void **)&p->d_sumsqc, p->n_bins * sizeof(double)));
+    CK(cudaMemset(p->d_sumc, 0, p->n_bins * sizeof(double)));
+    CK(cudaMemset(p->d_sumsqc, 0, p->n_bins * sizeof(double)));
+  }
+  return MCDC_OK;
+}
+
+// A.9 from a pair of device accumulators
+int batch_statistics(mcdc_problem *p, const double *d_sum, const double *d_sumsq, double *mean, double *sdev, size_t n_bins) {
+  CK(cudaMemcpy(mean, d_sum, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(sdev, d_sumsq, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
+  const double N = (double)p->histories, B = (double)p->batches, hb = N / B;
+  for (size_t i = 0; i < n_bins; ++i) {
+    double mu = mean[i] / N;
+    double sd = 0.0;
+    if (B > 1.0) {
+      double m2 = sdev[i] / (hb * hb) / B;
+      double var = (m2 - mu * mu) / (B - 1.0);
+      sd = var > 0.0 ? std::sqrt(var) : 0.0;
+    }
+    mean[i] = mu; sdev[i] = sd;
+  }
+  return MCDC_OK;
+}
+}  // namespace
+
+extern "C" int mcdc_collision_tally_enable(mcdc_problem *p, int on) {
+  if (!p) return MCDC_ERR_ARG;
+  p->col_on = on ? 1 : 0;
+  return MCDC_OK;
+}
+
+extern "C" int mcdc_collision_tallies_get(const mcdc_problem *cp, double *mean, double *sdev, size_t n_bins) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !mean || !sdev) return MCDC_ERR_ARG;
+  if (n_bins != p->n_bins) return MCDC_ERR_SIZE;
+  if (p->histories == 0 || !p->d_sumc) return MCDC_ERR_ARG;
+  return batch_statistics(p, p->d_sumc, p->d_sumsqc, mean, sdev, n_bins);
 }
 
 extern "C" int mcdc_census_after_get(const mcdc_problem *cp, double *pop_w, uint64_t *pop_n, size_t K) {

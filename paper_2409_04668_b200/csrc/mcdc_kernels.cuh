@@ -239,6 +239,34 @@ __device__ __forceinline__ void score_track_fast(const TBT &tb, const TallySink 
 }
 
 // ------------------------------------------------------------------------------------------------
+// Appendix I: loc2index of a collision site for the collision-estimator tally (the paper's Fig. 3): spatial index
+// floor((r - lo) / Delta) inside [lo, hi), largest it with T[it] <= t inside [T[0], T[Nt]); -1 = scores nothing.
+// ------------------------------------------------------------------------------------------------
+template <class TBT>
+__device__ __forceinline__ long long collision_bin(const TBT &tb, double x, double y, double z, double t, int g) {
+  const Tables &T = tb.T;
+  const double r[3] = {x, y, z};
+  int idx[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (!(T.mesh_lo[a] <= r[a] && r[a] < T.mesh_hi[a])) return -1;
+    const int n = T.mesh_n[a];
+    idx[a] = 0;
+    if (n > 1) {
+      const double q = floor((r[a] - T.mesh_lo[a]) / T.mesh_d[a]);
+      idx[a] = (q > (double)(n - 1)) ? n - 1 : (int)q;
+    }
+  }
+  if (!(tb.time_edge(0) <= t && t < tb.time_edge(T.Nt))) return -1;
+  int lo = 0, hi = T.Nt - 1;
+  while (lo < hi) {
+    const int mid = (lo + hi + 1) >> 1;
+    if (tb.time_edge(mid) <= t) lo = mid; else hi = mid - 1;
+  }
+  return ((((long long)lo * T.G + g) * T.mesh_n[2] + idx[2]) * T.mesh_n[1] + idx[1]) * T.mesh_n[0] + idx[0];
+}
+
+// ------------------------------------------------------------------------------------------------
 // match_any-aggregated append for lanes that may target different slots (source kernel)
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t warp_append_by_slot(uint32_t *counters, int slot) {
@@ -387,6 +415,7 @@ __global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank o
 struct TransportArgs {
   Bank in, census_out, sec_out;
   double *x_acc;                 // [n_slots][n_bins] batch accumulators
+  double *xc_acc;                // the same for the collision-estimator tally (Appendix I), nullptr = off
   DevCounters *cnt;
   double *pop_w;                 // [K]
   unsigned long long *pop_n;     // [K]
@@ -481,6 +510,10 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
           have = surface_event(tb, p, i_star, &acc.led[LED_LEAK][tid], &acc.led[LED_LOST][tid], &acc.cnt[CNT_LOST][tid]);
         } else {
           pc_coll += 1u;
+          if (A.xc_acc != nullptr) {                     // Appendix I, with the weight the particle arrives with
+            const long long cb = collision_bin(tb, p.x, p.y, p.z, p.t, p.g);
+            if (cb >= 0) atomicAdd(A.xc_acc + (size_t)slot * T.n_bins + cb, p.w / tb.sig_t(tb.cell_mat(p.cell) * T.G + p.g));
+          }
           int r = collision_event(tb, p, c0, &acc.led[LED_CAPTURE][tid], &acc.led[LED_FISSION_ABS][tid],
                                   &acc.led[LED_PRODUCTION][tid], &acc.led[LED_VR_GAIN][tid], &acc.led[LED_VR_LOSS][tid]);
           if (r == -1) fi = FI_SCATTER; else have = false;
@@ -644,6 +677,7 @@ struct HistoryArgs {
   uint32_t src_chunk;             // source histories a warp reserves per global atomic
   uint32_t n_slots, n_chunks;     // batch slots of the sub-batch; chunks in all = n_slots * ceil(hb / src_chunk)
   double *x_acc;
+  double *xc_acc;                 // collision-estimator accumulators (Appendix I; k_warp<WEIGHTED> only), nullptr = off
   DevCounters *cnt;
   double *pop_w;
   unsigned long long *pop_n;

@@ -580,6 +580,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       uint32_t c0 = 0u;
       double w = 1.0, l_cap = 0.0, l_fis = 0.0, l_prod = 0.0, l_gain = 0.0, l_loss = 0.0;   // WEIGHTED only
       if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
+      if (WEIGHTED && A.xc_acc != nullptr && act && !born) {   // Appendix I: collision estimator, arriving weight
+        const long long cb = collision_bin(tb, PD(D_X, gi), PD(D_Y, gi), PD(D_Z, gi), PD(D_T, gi), g);
+        if (cb >= 0) atomicAdd(A.xc_acc + (size_t)(meta >> 20) * T.n_bins + cb, w / tb.sig_t(mg));
+      }
       if (born) { kind = FI_CHILD; alive = true; }
       else if (act) {
         const double s_tot = tb.sig_s_tot(mg), sig_f = tb.sig_f(mg);
