@@ -113,6 +113,7 @@ struct mcdc_problem {
 namespace {
 
 int ensure_collision_buffers(mcdc_problem *p);   // defined with the result calls
+int batch_statistics(mcdc_problem *p, const double *d_sum, const double *d_sumsq, double *mean, double *sdev, size_t n_bins);
 
 int cuda_fail(mcdc_problem *p, cudaError_t e, const char *where) {
   p->cuda_err = std::string(where) + ": " + cudaGetErrorString(e);
@@ -575,9 +576,9 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   int dev = 0;
   cudaError_t e = cudaGetDevice(&dev);
   if (e != cudaSuccess) { delete p; return MCDC_ERR_CUDA; }
-  cudaDeviceProp prop;
-  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete p; return MCDC_ERR_CUDA; }
-  p->n_sm = prop.multiProcessorCount;
+  int n_sm = 0;                                          // (one attribute: cudaGetDeviceProperties costs ~1 ms)
+  if (cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n_sm <= 0) { delete p; return MCDC_ERR_CUDA; }
+  p->n_sm = n_sm;
   Tables &t = p->tab;
   DeviceArena &ar = p->arena;
   t.G = G; t.M = M; t.S = S; t.C = C; t.K = p->K; t.Nt = p->Nt;
@@ -633,12 +634,24 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
     t.self_dev = dT;
     if (dT && cudaMemcpy(dT, &t, sizeof(Tables), cudaMemcpyHostToDevice) != cudaSuccess) ar.err = cudaErrorUnknown;
   }
-  p->d_sum = ar.zeros<double>(p->n_bins); p->d_sumsq = ar.zeros<double>(p->n_bins);
-  p->d_pop_w = ar.zeros<double>(p->K); p->d_pop_n = ar.zeros<unsigned long long>(p->K);
-  p->d_pop_w_after = ar.zeros<double>(p->K); p->d_pop_n_after = ar.zeros<unsigned long long>(p->K);
-  p->d_cnt = ar.zeros<DevCounters>(1);
-  p->d_hist_cursor = ar.zeros<uint32_t>(1);
-  p->d_head_tail = ar.zeros<unsigned long long>(2);
+  {
+    // every accumulator of the handle in ONE zeroed allocation (each cudaMalloc + cudaMemset pair costs ~0.1 ms)
+    const size_t nb = p->n_bins, K = (size_t)p->K;
+    const size_t words = 2 * nb + 4 * K + (sizeof(DevCounters) + 7) / 8 + 2 + 2;   // 8-byte words
+    unsigned long long *blk = ar.zeros<unsigned long long>(words);
+    if (blk) {
+      size_t o = 0;
+      p->d_sum = (double *)(blk + o); o += nb;
+      p->d_sumsq = (double *)(blk + o); o += nb;
+      p->d_pop_w = (double *)(blk + o); o += K;
+      p->d_pop_n = blk + o; o += K;
+      p->d_pop_w_after = (double *)(blk + o); o += K;
+      p->d_pop_n_after = blk + o; o += K;
+      p->d_cnt = (DevCounters *)(blk + o); o += (sizeof(DevCounters) + 7) / 8;
+      p->d_head_tail = blk + o; o += 2;
+      p->d_hist_cursor = (uint32_t *)(blk + o); o += 2;
+    }
+  }
   if (ar.err != cudaSuccess) {
     ar.release();
     delete p;
@@ -1410,20 +1423,7 @@ extern "C" int mcdc_tallies_get(const mcdc_problem *cp, double *mean, double *sd
   if (!p || !mean || !sdev) return MCDC_ERR_ARG;
   if (n_bins != p->n_bins) return MCDC_ERR_SIZE;
   if (p->histories == 0) return MCDC_ERR_ARG;
-  CK(cudaMemcpy(mean, p->d_sum, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
-  CK(cudaMemcpy(sdev, p->d_sumsq, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
-  const double N = (double)p->histories, B = (double)p->batches, hb = N / B;
-  for (size_t i = 0; i < n_bins; ++i) {
-    double mu = mean[i] / N;
-    double sd = 0.0;
-    if (B > 1.0) {
-      double m2 = sdev[i] / (hb * hb) / B;
-      double var = (m2 - mu * mu) / (B - 1.0);
-      sd = var > 0.0 ? std::sqrt(var) : 0.0;
-    }
-    mean[i] = mu; sdev[i] = sd;
-  }
-  return MCDC_OK;
+  return batch_statistics(p, p->d_sum, p->d_sumsq, mean, sdev, n_bins);
 }
 
 extern "C" int mcdc_counters_get(const mcdc_problem *cp, mcdc_counters *c) {
@@ -1471,6 +1471,23 @@ int ensure_collision_buffers(mcdc_problem *p) {
 
 // A.9 from a pair of device accumulators
 int batch_statistics(mcdc_problem *p, const double *d_sum, const double *d_sumsq, double *mean, double *sdev, size_t n_bins) {
+  if (n_bins >= (size_t)1 << 18) {                        // large mesh: the per-bin arithmetic runs on the device
+    double *tmp = nullptr;
+    if (cudaMalloc((void **)&tmp, 2 * n_bins * sizeof(double)) == cudaSuccess) {
+      const int grid = (int)std::min<size_t>((n_bins + 255) / 256, (size_t)p->n_sm * 16);
+      k_statistics<<<grid, 256, 0, p->stream>>>(d_sum, d_sumsq, n_bins, (double)p->histories, (double)p->batches, tmp, tmp + n_bins);
+      p->launches++;
+      cudaError_t e1 = cudaMemcpyAsync(mean, tmp, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+      cudaError_t e2 = cudaMemcpyAsync(sdev, tmp + n_bins, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+      cudaError_t e3 = cudaStreamSynchronize(p->stream);
+      cudaFree(tmp);
+      if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaMemcpyAsync(mean)");
+      if (e2 != cudaSuccess) return cuda_fail(p, e2, "cudaMemcpyAsync(sdev)");
+      if (e3 != cudaSuccess) return cuda_fail(p, e3, "k_statistics");
+      return MCDC_OK;
+    }
+    cudaGetLastError();                                   // no room for the temporaries: host loop below
+  }
   CK(cudaMemcpy(mean, d_sum, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
   CK(cudaMemcpy(sdev, d_sumsq, n_bins * sizeof(double), cudaMemcpyDeviceToHost));
   const double N = (double)p->histories, B = (double)p->batches, hb = N / B;

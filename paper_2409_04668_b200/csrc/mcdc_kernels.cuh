@@ -727,4 +727,24 @@ __global__ void __launch_bounds__(256) k_closeout(double *__restrict__ x_acc, in
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// A.9 read-out for large meshes: mean = sum / N, sdev = sqrt((sumsq / hb^2 / B - mean^2) / (B - 1)) per bin
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_statistics(const double *__restrict__ sum, const double *__restrict__ sumsq,
+                                                    unsigned long long n_bins, double N, double B,
+                                                    double *__restrict__ mean, double *__restrict__ sdev) {
+  const double hb = N / B;
+  const unsigned long long stride = (unsigned long long)gridDim.x * blockDim.x;
+  for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_bins; i += stride) {
+    const double mu = sum[i] / N;
+    double sd = 0.0;
+    if (B > 1.0) {
+      const double m2 = sumsq[i] / (hb * hb) / B;
+      const double var = (m2 - __dmul_rn(mu, mu)) / (B - 1.0);   // no FMA contraction: same bits as the host loop
+      sd = var > 0.0 ? sqrt(var) : 0.0;
+    }
+    mean[i] = mu; sdev[i] = sd;
+  }
+}
+
 }  // namespace mcdc
