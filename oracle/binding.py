@@ -99,6 +99,7 @@ def _load():
     L.orc_run_eigenvalue.restype = C.c_int
     L.orc_collision_tally_enable.argtypes = [vp, C.c_int]; L.orc_collision_tally_enable.restype = C.c_int
     L.orc_collision_tallies_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.orc_collision_tallies_get.restype = C.c_int
+    L.orc_regions_set.argtypes = [vp, _ip, _ip]; L.orc_regions_set.restype = C.c_int
     L.orc_technique_set.argtypes = [vp, C.POINTER(_Technique)]; L.orc_technique_set.restype = C.c_int
     L.orc_census_after_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.orc_census_after_get.restype = C.c_int
     L.orc_population_control.argtypes = [vp, C.c_size_t, _dp, C.POINTER(C.c_uint64), C.POINTER(C.c_uint32), C.c_uint64,
@@ -186,6 +187,12 @@ class Oracle:
         self._h = h
         self.n_bins = prob.n_bins
         self._last_n = 0
+        rgn = getattr(prob, "meta", {}).get("regions")     # (region_offset, region_rpn) of a general-CSG workload
+        if rgn is not None:
+            ro = np.ascontiguousarray(rgn[0], dtype=np.int32); rt = np.ascontiguousarray(rgn[1], dtype=np.int32)
+            self._keep += [ro, rt]
+            if L.orc_regions_set(h, _i(ro), _i(rt)) != 0:
+                raise RuntimeError("orc_regions_set failed")
 
     def close(self):
         if getattr(self, "_h", None):

@@ -91,6 +91,10 @@ struct orc_problem {
   std::vector<Surface> surf;
   std::vector<int> cell_offset, hs_surface, hs_sense, cell_material;
   std::vector<double> bb_lo, bb_hi;          // per-cell culling boxes [C][3] (A.5 allows culling)
+  // Appendix J: general CSG regions.  Cell c with rgn_off[c] < rgn_off[c+1] is the postfix expression
+  // rgn_tok[rgn_off[c] .. rgn_off[c+1]) over its half-spaces (token t >= 0: half-space t of the cell's list holds;
+  // -1 AND, -2 OR, -3 NOT); an empty range (or no region table) is the plain intersection of A.1.
+  std::vector<int> rgn_off, rgn_tok;
   double src_lo[3], src_hi[3], src_t0, src_t1;
   std::vector<double> src_pdf;
   int src_dir_mode; double src_dir[3];
@@ -169,9 +173,23 @@ int locate(const orc_problem &P, const double r[3], const double o[3], int cross
       if (r[a] < P.bb_lo[3 * c + a] || r[a] > P.bb_hi[3 * c + a]) { out = true; break; }
     if (out) continue;
     bool ok = true;
-    for (int i = P.cell_offset[c]; i < P.cell_offset[c + 1]; ++i) {
-      int s = P.hs_surface[i];
-      if (sense_at(P.surf[s], r, o, s == crossed) != P.hs_sense[i]) { ok = false; break; }
+    if (!P.rgn_off.empty() && P.rgn_off[c] < P.rgn_off[c + 1]) {      // Appendix J: evaluate the postfix expression
+      std::vector<char> st;
+      const int base = P.cell_offset[c];
+      for (int k = P.rgn_off[c]; k < P.rgn_off[c + 1]; ++k) {
+        int t = P.rgn_tok[k];
+        if (t >= 0) {
+          int s = P.hs_surface[base + t];
+          st.push_back(sense_at(P.surf[s], r, o, s == crossed) == P.hs_sense[base + t]);
+        } else if (t == -3) { st.back() = !st.back(); }
+        else { char b = st.back(); st.pop_back(); st.back() = (t == -1) ? (st.back() && b) : (st.back() || b); }
+      }
+      ok = st.back() != 0;
+    } else {
+      for (int i = P.cell_offset[c]; i < P.cell_offset[c + 1]; ++i) {
+        int s = P.hs_surface[i];
+        if (sense_at(P.surf[s], r, o, s == crossed) != P.hs_sense[i]) { ok = false; break; }
+      }
     }
     if (ok) return c;
   }
@@ -522,6 +540,7 @@ void build_boxes(orc_problem &P) {
   // rounding of a bounding surface is never culled (the exact half-space test then decides).
   P.bb_lo.assign((size_t)3 * P.C, -INF); P.bb_hi.assign((size_t)3 * P.C, INF);
   for (int c = 0; c < P.C; ++c) {
+    if (!P.rgn_off.empty() && P.rgn_off[c] < P.rgn_off[c + 1]) continue;   // a general region: no culling box
     for (int i = P.cell_offset[c]; i < P.cell_offset[c + 1]; ++i) {
       const Surface &s = P.surf[P.hs_surface[i]]; int sense = P.hs_sense[i];
       bool quad = s.A != 0 || s.B != 0 || s.C != 0 || s.D != 0 || s.E != 0 || s.F != 0;
@@ -611,6 +630,32 @@ int orc_create(const orc_desc *d, orc_problem **out) {
   P->col_on = 0;
   orc_reset(P);
   *out = P;
+  return 0;
+}
+
+// Appendix J: general CSG regions; validates the postfix expressions (operands in range, stack never underflows,
+// exactly one value left).  NULL pointers: every cell is the plain intersection again.
+int orc_regions_set(orc_problem *P, const int32_t *region_offset, const int32_t *region_rpn) {
+  if (!P) return -1;
+  P->rgn_off.clear(); P->rgn_tok.clear();
+  if (region_offset && region_rpn) {
+    for (int c = 0; c < P->C; ++c) {
+      int depth = 0;
+      const int nh = P->cell_offset[c + 1] - P->cell_offset[c];
+      if (region_offset[c + 1] < region_offset[c]) return -3;
+      for (int k = region_offset[c]; k < region_offset[c + 1]; ++k) {
+        int t = region_rpn[k];
+        if (t >= 0) { if (t >= nh) return -3; depth += 1; }
+        else if (t == -3) { if (depth < 1) return -3; }
+        else if (t == -1 || t == -2) { if (depth < 2) return -3; depth -= 1; }
+        else return -3;
+      }
+      if (region_offset[c + 1] > region_offset[c] && depth != 1) return -3;
+    }
+    P->rgn_off.assign(region_offset, region_offset + P->C + 1);
+    P->rgn_tok.assign(region_rpn, region_rpn + region_offset[P->C]);
+  }
+  build_boxes(*P);
   return 0;
 }
 

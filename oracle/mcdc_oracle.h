@@ -74,6 +74,11 @@ typedef struct {
 } orc_run_opts;
 
 int  orc_create(const orc_desc *d, orc_problem **out);   /* deep copy; 0 or negative error   */
+/* General CSG regions ("full three-dimensional constructive solid geometry"; DESIGN.md Appendix J):
+ * cell c becomes the postfix expression region_rpn[region_offset[c] .. region_offset[c+1]) over its half-spaces
+ * (token t >= 0: "half-space t of the cell's list holds"; -1 AND, -2 OR, -3 NOT); an empty range leaves the cell
+ * the intersection of its half-spaces.  The cell's list still names every surface that bounds it.            */
+int  orc_regions_set(orc_problem *p, const int32_t *region_offset, const int32_t *region_rpn);
 int  orc_technique_set(orc_problem *p, const orc_technique *t);   /* NULL: analog (the default)        */
 void orc_destroy(orc_problem *p);
 void orc_reset(orc_problem *p);

@@ -495,5 +495,61 @@ def stress_geometry(n_histories=60_000, n_batches=12, covering_mesh=False):
 CONFIGS["stress"] = stress_geometry
 
 
+# ----------------------------------------------------------------------------------------
+# General CSG regions (DESIGN.md Appendix J; parity tests only): a vacuum box that holds the UNION of two overlapping
+# spheres (cell 0) and a z-cylinder that does not touch them (cell 1); cell 2 is the box MINUS those: the
+# complement of a union.  Regions are postfix expressions over a cell's half-space list: t >= 0 operand, -1 AND,
+# -2 OR, -3 NOT; they travel in meta["regions"] = (region_offset, region_rpn).
+# ----------------------------------------------------------------------------------------
+RGN_AND, RGN_OR, RGN_NOT = -1, -2, -3
+CSG_SPHERES = ((3.0, 4.0, 4.0, 2.0), (5.5, 4.0, 4.0, 2.0))      # (x0, y0, z0, r): centres 2.5 apart on the x axis
+CSG_CYL = (9.0, 4.0, 1.0)                                        # (x0, y0, r), parallel to z
+CSG_BOX = (12.0, 8.0, 8.0)
+
+
+def csg_union_geometry(n_histories=60_000, n_batches=12, beam=False):
+    G = 2
+    if beam:                                              # pin J-b: absorber in the union, nothing anywhere else
+        mats, ss = _materials([
+            dict(sigma_t=[1.0, 1.0], sigma_c=[1.0, 1.0], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+                 sigma_s=[[0.0, 0.0], [0.0, 0.0]]),
+            dict(sigma_t=[0.0, 0.0], sigma_c=[0.0, 0.0], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+                 sigma_s=[[0.0, 0.0], [0.0, 0.0]])], G)
+        cell_mats = [0, 1, 1]
+    else:
+        mats, ss = _materials([
+            dict(sigma_t=[0.8, 1.2], sigma_c=[0.15, 0.4], sigma_f=[0.05, 0.1], nu=[2.2, 2.5], chi=[0.7, 0.3],
+                 sigma_s=[[0.4, 0.2], [0.0, 0.7]]),
+            dict(sigma_t=[0.3, 0.5], sigma_c=[0.05, 0.1], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+                 sigma_s=[[0.2, 0.05], [0.02, 0.38]])], G)
+        cell_mats = [0, 0, 1]
+    bx, by, bz = CSG_BOX
+    surfs = [plane_x(0.0), plane_x(bx), plane_y(0.0), plane_y(by), plane_z(0.0), plane_z(bz),
+             sphere(*CSG_SPHERES[0]), sphere(*CSG_SPHERES[1]), cylinder_z(*CSG_CYL)]
+    bcs = [BC_VACUUM] * 6 + [BC_TRANSMISSION] * 3
+    cells = [
+        ([(6, -1), (7, -1)], cell_mats[0]),                                           # inside sphere 0 OR sphere 1
+        ([(8, -1), (4, +1), (5, -1)], cell_mats[1]),                                  # the cylinder (plain intersection)
+        ([(0, +1), (1, -1), (2, +1), (3, -1), (4, +1), (5, -1), (6, -1), (7, -1), (8, -1)], cell_mats[2]),
+    ]
+    A, O, N = RGN_AND, RGN_OR, RGN_NOT
+    rpn = [[0, 1, O],
+           [],
+           [0, 1, A, 2, A, 3, A, 4, A, 5, A, 6, 7, O, 8, O, N, A]]                     # box AND NOT (s0 OR s1 OR cyl)
+    off = np.cumsum([0] + [len(r) for r in rpn]).astype(np.int32)
+    tok = np.array([t for r in rpn for t in r], dtype=np.int32)
+    if beam:
+        src = dict(lo=[0.0, 4.0, 4.0], hi=[0.0, 4.0, 4.0], t0=0.0, t1=0.0, pdf=[1.0, 0.0], mode=DIR_FIXED,
+                   dir=[1.0, 0.0, 0.0])
+    else:
+        src = dict(lo=[0.5, 0.5, 0.5], hi=[11.5, 7.5, 7.5], t0=0.0, t1=1.0, pdf=[0.6, 0.4])
+    mesh = dict(lo=[0.0, 0.0, 0.0], hi=[bx, by, bz], n=[12, 4, 2])
+    T = np.array([0.0, 2.0, 5.0, 9.0, 20.0])
+    p = _assemble("csg_union" + ("_beam" if beam else ""), mats, ss, [1.0, 0.4], surfs, bcs, cells, src, mesh, T,
+                  T[1:].copy(), n_histories, n_batches, run_seed(11))
+    p.meta["regions"] = (off, tok)
+    return p
+
+
 def get_config(name: str, **kw) -> Problem:
     return CONFIGS[name](**kw)
