@@ -134,6 +134,18 @@ int mcdc_technique_set(mcdc_problem *p, const mcdc_technique *t);
 /* Validates and deep-copies *d, classifies surfaces, builds cell-neighbour tables and uploads the
  * problem to the current CUDA device.  *out is untouched on error.                                */
 int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out);
+/* General CSG regions ("full three-dimensional constructive solid geometry"; SURVEY.md 8(f)
+ * NEXT-4; DESIGN.md Appendix J).  As mcdc_problem_create, but cell c is the postfix expression
+ * region_rpn[region_offset[c] .. region_offset[c+1]) over its half-spaces: a token t >= 0 stands for
+ * "half-space t of the cell's list holds" (0-based within the cell), MCDC_RGN_AND / _OR / _NOT combine
+ * them; an empty range leaves the cell the intersection of its half-spaces.  The cell's half-space list
+ * must still name every surface that bounds the cell (distances are taken to all of them).  Both
+ * arrays are HOST memory, deep-copied; region_offset has n_cells + 1 entries starting at 0; expressions
+ * deeper than 32 operands or malformed give MCDC_ERR_GEOM.  Problems with regions run on the
+ * census-stepped kernel (the history kernel's cell records describe intersections only).           */
+enum { MCDC_RGN_AND = -1, MCDC_RGN_OR = -2, MCDC_RGN_NOT = -3 };
+int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t *region_offset,
+                            const int32_t *region_rpn, mcdc_problem **out);
 void mcdc_problem_destroy(mcdc_problem *p);
 /* Zero tallies, ledger, census populations and counters (keeps problem and workspace).            */
 int mcdc_problem_reset(mcdc_problem *p);

@@ -9,6 +9,7 @@ from .api import (  # noqa: F401
     lib,
     lib_path,
     mcdc_problem_create,
+    mcdc_problem_create_csg,
     mcdc_problem_destroy,
     mcdc_problem_reset,
     mcdc_problem_info_get,

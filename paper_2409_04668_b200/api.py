@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
     "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
-    "mcdc_collision_tally_enable", "mcdc_collision_tallies_get",
+    "mcdc_collision_tally_enable", "mcdc_collision_tallies_get", "mcdc_problem_create_csg",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -95,6 +95,8 @@ def lib():
     L = C.CDLL(_LIB_PATH)
     vp = C.c_void_p
     L.mcdc_problem_create.argtypes = [C.POINTER(ProblemDesc), C.POINTER(vp)]; L.mcdc_problem_create.restype = C.c_int
+    L.mcdc_problem_create_csg.argtypes = [C.POINTER(ProblemDesc), _ip, _ip, C.POINTER(vp)]
+    L.mcdc_problem_create_csg.restype = C.c_int
     L.mcdc_problem_destroy.argtypes = [vp]; L.mcdc_problem_destroy.restype = None
     L.mcdc_problem_reset.argtypes = [vp]; L.mcdc_problem_reset.restype = C.c_int
     L.mcdc_workspace_size.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
@@ -185,9 +187,21 @@ def _make_desc(prob):
 
 # ---- functions with the names of include/mcdc.h ------------------------------------------------
 def mcdc_problem_create(prob):
+    """prob.meta["regions"] = (region_offset, region_rpn), when present, makes this mcdc_problem_create_csg."""
+    rgn = (getattr(prob, "meta", None) or {}).get("regions")
+    if rgn is not None:
+        return mcdc_problem_create_csg(prob, rgn[0], rgn[1])
     d, keep = _make_desc(prob)
     h = C.c_void_p()
     _check(lib().mcdc_problem_create(C.byref(d), C.byref(h)), "mcdc_problem_create")
+    return h
+
+
+def mcdc_problem_create_csg(prob, region_offset, region_rpn):
+    d, keep = _make_desc(prob)
+    ro = np.ascontiguousarray(region_offset, dtype=np.int32); rt = np.ascontiguousarray(region_rpn, dtype=np.int32)
+    h = C.c_void_p()
+    _check(lib().mcdc_problem_create_csg(C.byref(d), _i(ro), _i(rt), C.byref(h)), "mcdc_problem_create_csg")
     return h
 
 

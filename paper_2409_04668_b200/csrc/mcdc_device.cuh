@@ -285,6 +285,30 @@ template <class TBT>
 __device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed, double x, double y, double z,
                                               double ux, double uy, double uz) {
   const int e = tb.cell_off(c + 1);
+  if (tb.T.has_regions) {                               // Appendix J: the cell may be a postfix expression
+    const int *off = reinterpret_cast<const int *>(tb.T.blob + tb.T.o_rgn_off);
+    const int *tok = reinterpret_cast<const int *>(tb.T.blob + tb.T.o_rgn_tok);
+    const int k1 = off[c + 1];
+    int k = off[c];
+    if (k < k1) {
+      const int base = tb.cell_off(c);
+      uint32_t st = 0u;                                 // bit stack, top = bit 0 (depth <= 32 checked at create)
+      for (; k < k1; ++k) {
+        const int t = tok[k];
+        if (t >= 0) {
+          const int h = tb.hs(base + t);
+          const int s = h >> 6, want = (h & 1) ? 1 : -1;
+          st = (st << 1) | (surf_sense(tb, s, (h >> 1) & 7, s == crossed, x, y, z, ux, uy, uz) == want ? 1u : 0u);
+        } else if (t == -3) st ^= 1u;
+        else {
+          const uint32_t b = st & 1u;
+          st >>= 1;
+          st = (t == -1) ? (st & (0xFFFFFFFEu | b)) : (st | b);
+        }
+      }
+      return (st & 1u) != 0u;
+    }
+  }
   for (int i = tb.cell_off(c); i < e; ++i) {
     const int h = tb.hs(i);                             // packed: surface << 6 | bc << 4 | type << 1 | (sense > 0)
     const int s = h >> 6, want = (h & 1) ? 1 : -1;

@@ -65,6 +65,7 @@ struct mcdc_problem {
   int G, M, S, C, K, Nt;
   std::vector<double> sigma_t, sigma_c, sigma_f, nu, chi, sigma_s, speed, surf_coef, src_pdf, T, census;
   std::vector<int> surf_bc, cell_off, hs_surface, hs_sense, cell_mat;
+  std::vector<int> rgn_off, rgn_tok;   // general CSG regions (Appendix J): postfix expression per cell, empty = intersection
   double src_lo[3], src_hi[3], src_t0, src_t1, src_dir[3];
   int src_dir_mode;
   double mesh_lo[3], mesh_hi[3];
@@ -240,6 +241,7 @@ void classify_surface(const double *c, int &type, double4 &q) {
 Box cell_box(const mcdc_problem &P, const std::vector<int> &type, const std::vector<double4> &q, int c, bool pad = true) {
   Box b;
   for (int a = 0; a < 3; ++a) { b.lo[a] = -HINF; b.hi[a] = HINF; }
+  if (!P.rgn_off.empty() && P.rgn_off[c] < P.rgn_off[c + 1]) return b;   // a general region: its half-spaces bound nothing
   for (int i = P.cell_off[c]; i < P.cell_off[c + 1]; ++i) {
     int s = P.hs_surface[i], sense = P.hs_sense[i];
     if (type[s] <= ST_PLANE_Z) {
@@ -271,9 +273,31 @@ inline bool boxes_touch(const Box &a, const Box &b) {
 // create / destroy / reset
 // =============================================================================================
 extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out) {
+  return mcdc_problem_create_csg(d, nullptr, nullptr, out);
+}
+
+extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t *region_offset, const int32_t *region_rpn,
+                                       mcdc_problem **out) {
   if (!out) return MCDC_ERR_ARG;
   int rc = validate(d);
   if (rc != MCDC_OK) return rc;
+  if ((region_offset == nullptr) != (region_rpn == nullptr)) return MCDC_ERR_ARG;
+  if (region_offset) {                                    // Appendix J: well-formed postfix expressions only
+    if (region_offset[0] != 0) return MCDC_ERR_GEOM;
+    for (int c = 0; c < d->n_cells; ++c) {
+      const int nh = d->cell_offset[c + 1] - d->cell_offset[c];
+      if (region_offset[c + 1] < region_offset[c]) return MCDC_ERR_GEOM;
+      int depth = 0;
+      for (int k = region_offset[c]; k < region_offset[c + 1]; ++k) {
+        const int t = region_rpn[k];
+        if (t >= 0) { if (t >= nh) return MCDC_ERR_GEOM; if (++depth > 32) return MCDC_ERR_GEOM; }
+        else if (t == MCDC_RGN_NOT) { if (depth < 1) return MCDC_ERR_GEOM; }
+        else if (t == MCDC_RGN_AND || t == MCDC_RGN_OR) { if (depth < 2) return MCDC_ERR_GEOM; --depth; }
+        else return MCDC_ERR_GEOM;
+      }
+      if (region_offset[c + 1] > region_offset[c] && depth != 1) return MCDC_ERR_GEOM;
+    }
+  }
   mcdc_problem *p = new (std::nothrow) mcdc_problem();
   if (!p) return MCDC_ERR_NOMEM;
   const int G = d->n_groups, M = d->n_materials, S = d->n_surfaces, C = d->n_cells;
@@ -290,6 +314,12 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   p->hs_surface.assign(d->hs_surface, d->hs_surface + nhs);
   p->hs_sense.assign(d->hs_sense, d->hs_sense + nhs);
   p->cell_mat.assign(d->cell_material, d->cell_material + C);
+  bool has_regions = false;
+  if (region_offset && region_offset[C] > 0) {
+    p->rgn_off.assign(region_offset, region_offset + C + 1);
+    p->rgn_tok.assign(region_rpn, region_rpn + region_offset[C]);
+    has_regions = true;
+  }
   p->src_pdf.assign(d->src_group_pdf, d->src_group_pdf + G);
   p->T.assign(d->time_edges, d->time_edges + d->n_time_bins + 1);
   p->census.assign(d->census_times, d->census_times + d->n_census);
@@ -355,6 +385,9 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
       const std::vector<int> &cand = users[user_key(i) ^ 1];          // same surface, opposite sense
       for (int c2 : cand)
         if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);  // increasing id by construction
+      if (has_regions)                                                // under a NOT the listed sense says nothing
+        for (int c2 : users[user_key(i)])
+          if (c2 != c && boxes_touch(box[c], box[c2])) nb_cell.push_back(c2);
       nb_off[i + 1] = (int)nb_cell.size();
     }
   // ---- typed cells (mcdc_types.h): tightest axis-aligned plane per (axis, side) = face, the rest = other ----
@@ -479,7 +512,8 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
     }
     return -1;
   };
-  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095;
+  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095 &&
+                 !has_regions;                            // k_warp's cell records describe intersections only
   std::vector<unsigned char> cell2((size_t)C * CELL2_BYTES, 0), other2;
   size_t n_cert = 0, n_transm = 0;
   for (int c = 0; c < C && warp_ok; ++c) {
@@ -613,6 +647,9 @@ extern "C" int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **ou
   t.o_nb_off = puti(nb_off); t.o_nb_cell = puti(nb_cell);
   t.o_loc_off = puti(loc_off); t.o_loc_cell = puti(loc_cell);
   t.o_surf_coef = putd(p->surf_coef);
+  t.has_regions = has_regions ? 1 : 0;
+  t.o_rgn_off = 0; t.o_rgn_tok = 0;
+  if (has_regions) { t.o_rgn_off = puti(p->rgn_off); t.o_rgn_tok = puti(p->rgn_tok); }
   t.score_fast = score_fast;
   t.warp_ok = warp_ok ? 1 : 0;
   (void)any_quadric;

@@ -62,6 +62,9 @@ struct Tables {
   uint32_t o_tbin_k;    // [K] int: the one time bin that holds census interval k, -1 if it spans several
   uint32_t o_it0_k;     // [K] int: time bin at the start of census interval k (hint of the general scorer)
   uint32_t o_surf_coef; // [S][10] general form (inside the hot prefix only when a general quadric exists)
+  uint32_t o_rgn_off;   // [C+1] general CSG regions (Appendix J): postfix tokens of cell c, empty range = intersection
+  uint32_t o_rgn_tok;   // tokens: t >= 0 half-space t of the cell's list holds; -1 AND, -2 OR, -3 NOT
+  int has_regions;
   const Tables *self_dev;  // device-memory copy of this struct (slow paths that must not take the parameter's address)
   int score_fast;       // the tally mesh covers the geometry and the time grid covers [t0, C_K]: no clipping needed
   int warp_ok;          // the problem fits the compact tables of k_warp (16-bit surface / cell ids, ...)
