@@ -281,11 +281,14 @@ __device__ __forceinline__ int surf_sense(const TBT &tb, int s, int type, bool f
   return (b < 0.0) ? -1 : 1;
 }
 
-template <class TBT>
+// RGN: the problem may hold general CSG regions (Appendix J).  The history kernel never runs such problems, and its
+// slow paths are instantiated with RGN = false: code it never executes would still cost it instruction-cache room
+// (adding the expression evaluator to them slowed the analog kernel by 5 %, profiles/r01f).
+template <bool RGN, class TBT>
 __device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed, double x, double y, double z,
                                               double ux, double uy, double uz) {
   const int e = tb.cell_off(c + 1);
-  if (tb.T.has_regions) {                               // Appendix J: the cell may be a postfix expression
+  if (RGN && tb.T.has_regions) {                               // Appendix J: the cell may be a postfix expression
     const int *off = reinterpret_cast<const int *>(tb.T.blob + tb.T.o_rgn_off);
     const int *tok = reinterpret_cast<const int *>(tb.T.blob + tb.T.o_rgn_tok);
     const int k1 = off[c + 1];
@@ -319,33 +322,34 @@ __device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed,
 
 // full search in increasing cell id (A.3); slow path.  Not inlined, and it works on the device-memory copy of
 // the tables so that no caller has to take the address of its kernel parameter block.
+template <bool RGN>
 __device__ __noinline__ int locate_all_dev(const Tables *gT, int crossed, double x, double y, double z, double ux,
                                            double uy, double uz) {
   const TB<false> tb(*gT);
   for (int c = 0; c < gT->C; ++c)
-    if (cell_contains(tb, c, crossed, x, y, z, ux, uy, uz)) return c;
+    if (cell_contains<RGN>(tb, c, crossed, x, y, z, ux, uy, uz)) return c;
   return -1;
 }
-template <class TBT>
+template <bool RGN, class TBT>
 __device__ __forceinline__ int locate_all(const TBT &tb, int crossed, double x, double y, double z, double ux, double uy,
                                           double uz) {
-  return locate_all_dev(tb.T.self_dev, crossed, x, y, z, ux, uy, uz);
+  return locate_all_dev<RGN>(tb.T.self_dev, crossed, x, y, z, ux, uy, uz);
 }
 
 // cell after crossing the surface of half-space slot `slot` of the current cell (A.5, transmission)
-template <class TBT>
+template <bool RGN, class TBT>
 __device__ __forceinline__ int locate_neighbour(const TBT &tb, int slot, int s_star, double x, double y, double z,
                                                 double ux, double uy, double uz) {
   const int e = tb.nb_off(slot + 1);
   for (int i = tb.nb_off(slot); i < e; ++i) {
     const int c = tb.nb_cell(i);
-    if (cell_contains(tb, c, s_star, x, y, z, ux, uy, uz)) return c;
+    if (cell_contains<RGN>(tb, c, s_star, x, y, z, ux, uy, uz)) return c;
   }
-  return locate_all(tb, s_star, x, y, z, ux, uy, uz);
+  return locate_all<RGN>(tb, s_star, x, y, z, ux, uy, uz);
 }
 
 // source-particle location through the locator grid over the source box
-template <class TBT>
+template <bool RGN, class TBT>
 __device__ __forceinline__ int locate_source(const TBT &tb, double x, double y, double z, double ux, double uy,
                                              double uz) {
   const Tables &T = tb.T;
@@ -360,9 +364,9 @@ __device__ __forceinline__ int locate_source(const TBT &tb, double x, double y, 
   const int e = tb.loc_off(vox + 1);
   for (int i = tb.loc_off(vox); i < e; ++i) {
     const int c = tb.loc_cell(i);
-    if (cell_contains(tb, c, -1, x, y, z, ux, uy, uz)) return c;
+    if (cell_contains<RGN>(tb, c, -1, x, y, z, ux, uy, uz)) return c;
   }
-  return locate_all(tb, -1, x, y, z, ux, uy, uz);
+  return locate_all<RGN>(tb, -1, x, y, z, ux, uy, uz);
 }
 
 // specular reflection about grad f at the hit point (A.5)

@@ -657,6 +657,28 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
   t.hot_bytes = (uint32_t)hot;
   t.blob = ar.upload(blob);
   t.src_last = src_last; t.src_dir_mode = p->src_dir_mode;
+  // A point source that lies strictly inside exactly one cell (every half-space of the cell holds with a margin, so
+  // the on-surface direction rule of A.3 cannot come into play) needs no per-particle cell search.
+  t.src_cell = -1;
+  if (!has_regions && p->src_lo[0] == p->src_hi[0] && p->src_lo[1] == p->src_hi[1] && p->src_lo[2] == p->src_hi[2]) {
+    const double x = p->src_lo[0], y = p->src_lo[1], z = p->src_lo[2];
+    int found = -1, n_found = 0;
+    bool near_surface = false;
+    for (int c = 0; c < C; ++c) {
+      bool inside = true;
+      for (int i = p->cell_off[c]; i < p->cell_off[c + 1] && inside; ++i) {
+        const double *k = &p->surf_coef[(size_t)10 * p->hs_surface[i]];
+        const double terms[10] = {k[0] * x * x, k[1] * y * y, k[2] * z * z, k[3] * x * y, k[4] * x * z, k[5] * y * z,
+                                  k[6] * x, k[7] * y, k[8] * z, k[9]};
+        double f = 0.0, mag = 0.0;
+        for (int j = 0; j < 10; ++j) { f += terms[j]; mag += std::fabs(terms[j]); }
+        if (std::fabs(f) <= 1e-9 * (mag + 1e-300)) { near_surface = true; inside = false; }
+        else if ((f > 0.0) != (p->hs_sense[i] > 0)) inside = false;
+      }
+      if (inside) { found = c; ++n_found; }
+    }
+    if (!near_surface && n_found == 1) t.src_cell = found;
+  }
   t.src_t0 = p->src_t0; t.src_t1 = p->src_t1;
   for (int a = 0; a < 3; ++a) {
     t.src_lo[a] = p->src_lo[a]; t.src_hi[a] = p->src_hi[a]; t.src_dir[a] = p->src_dir[a];
@@ -672,21 +694,21 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     if (dT && cudaMemcpy(dT, &t, sizeof(Tables), cudaMemcpyHostToDevice) != cudaSuccess) ar.err = cudaErrorUnknown;
   }
   {
-    // every accumulator of the handle in ONE zeroed allocation (each cudaMalloc + cudaMemset pair costs ~0.1 ms)
+    // every accumulator of the handle in ONE zeroed allocation (each cudaMalloc + cudaMemset pair costs ~0.1 ms);
+    // the counters the kernels poll or hit with atomics (ledger, queue cursors, source cursor) get 256 bytes each
     const size_t nb = p->n_bins, K = (size_t)p->K;
-    const size_t words = 2 * nb + 4 * K + (sizeof(DevCounters) + 7) / 8 + 2 + 2;   // 8-byte words
+    auto up32 = [](size_t w) { return (w + 31) / 32 * 32; };               // 8-byte words, rounded to 256 bytes
+    const size_t words = up32(2 * nb) + up32(4 * K) + up32((sizeof(DevCounters) + 7) / 8) + 32 + 32;
     unsigned long long *blk = ar.zeros<unsigned long long>(words);
     if (blk) {
       size_t o = 0;
       p->d_sum = (double *)(blk + o); o += nb;
-      p->d_sumsq = (double *)(blk + o); o += nb;
-      p->d_pop_w = (double *)(blk + o); o += K;
-      p->d_pop_n = blk + o; o += K;
-      p->d_pop_w_after = (double *)(blk + o); o += K;
-      p->d_pop_n_after = blk + o; o += K;
-      p->d_cnt = (DevCounters *)(blk + o); o += (sizeof(DevCounters) + 7) / 8;
-      p->d_head_tail = blk + o; o += 2;
-      p->d_hist_cursor = (uint32_t *)(blk + o); o += 2;
+      p->d_sumsq = (double *)(blk + o); o = up32(2 * nb);
+      p->d_pop_w = (double *)(blk + o); p->d_pop_n = blk + o + K;
+      p->d_pop_w_after = (double *)(blk + o + 2 * K); p->d_pop_n_after = blk + o + 3 * K; o += up32(4 * K);
+      p->d_cnt = (DevCounters *)(blk + o); o += up32((sizeof(DevCounters) + 7) / 8);
+      p->d_head_tail = blk + o; o += 32;
+      p->d_hist_cursor = (uint32_t *)(blk + o); o += 32;
     }
   }
   if (ar.err != cudaSuccess) {
@@ -1002,51 +1024,68 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 
 // ---- k_warp instantiations: (tables staged, per-history events recorded, threads per block) ----
 #ifndef MCDC_WARP_CASES
-#define MCDC_WARP_CASES(X) X(256) X(512) X(1024)
+#define MCDC_WARP_CASES(X) X(512)          // threads per block compiled in (tuning builds: -DMCDC_WARP_CASES(X)="X(256) X(512) X(1024)")
 #endif
-template <bool STAGED, bool RECORD, bool WEIGHTED>
+enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
+template <bool STAGED, bool RECORD, int VARIANT>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
-#define X(N) case N: k_warp<STAGED, RECORD, WEIGHTED, N><<<grid, N, smem, st>>>(T, A); break;
+#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, N><<<grid, N, smem, st>>>(T, A); break;
     MCDC_WARP_CASES(X)
 #undef X
   }
 }
-template <bool STAGED, bool RECORD, bool WEIGHTED>
+template <bool STAGED, bool RECORD, int VARIANT>
 cudaError_t warp_set_smem_nt(int nt, int bytes) {
   switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, WEIGHTED, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     MCDC_WARP_CASES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <bool WEIGHTED>
-void warp_launch_w(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (record) warp_launch_nt<true, true, WEIGHTED>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, WEIGHTED>(nt, grid, smem, st, T, A); }
-  else        { if (record) warp_launch_nt<false, true, WEIGHTED>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, WEIGHTED>(nt, grid, smem, st, T, A); }
+template <int VARIANT>
+void warp_launch_v(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  if (staged) { if (record) warp_launch_nt<true, true, VARIANT>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT>(nt, grid, smem, st, T, A); }
+  else        { if (record) warp_launch_nt<false, true, VARIANT>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT>(nt, grid, smem, st, T, A); }
 }
-void warp_launch(bool staged, bool record, bool weighted, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (weighted) warp_launch_w<true>(staged, record, nt, grid, smem, st, T, A);
-  else warp_launch_w<false>(staged, record, nt, grid, smem, st, T, A);
+void warp_launch(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  switch (variant) {
+    case KW_ANALOG: warp_launch_v<KW_ANALOG>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP>(staged, record, nt, grid, smem, st, T, A); break;
+    default: warp_launch_v<KW_GENERATION>(staged, record, nt, grid, smem, st, T, A); break;
+  }
 }
-template <bool WEIGHTED>
-cudaError_t warp_set_smem_w(bool staged, bool record, int nt, int bytes) {
-  if (staged) return record ? warp_set_smem_nt<true, true, WEIGHTED>(nt, bytes) : warp_set_smem_nt<true, false, WEIGHTED>(nt, bytes);
-  return record ? warp_set_smem_nt<false, true, WEIGHTED>(nt, bytes) : warp_set_smem_nt<false, false, WEIGHTED>(nt, bytes);
+template <int VARIANT>
+cudaError_t warp_set_smem_v(bool staged, bool record, int nt, int bytes) {
+  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT>(nt, bytes);
+  return record ? warp_set_smem_nt<false, true, VARIANT>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT>(nt, bytes);
 }
-cudaError_t warp_set_smem(bool staged, bool record, bool weighted, int nt, int bytes) {
-  return weighted ? warp_set_smem_w<true>(staged, record, nt, bytes) : warp_set_smem_w<false>(staged, record, nt, bytes);
+cudaError_t warp_set_smem(bool staged, bool record, int variant, int nt, int bytes) {
+  switch (variant) {
+    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG>(staged, record, nt, bytes);
+    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED>(staged, record, nt, bytes);
+    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP>(staged, record, nt, bytes);
+    default: return warp_set_smem_v<KW_GENERATION>(staged, record, nt, bytes);
+  }
 }
 
 // shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
-int plan_warp_kernel(mcdc_problem *p, bool record, bool weighted) {
+int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
+  const bool weighted = variant != KW_ANALOG;
   int dev = 0, max_optin = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   int nt = 512;
   if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
-  if (nt != 256 && nt != 512 && nt != 1024) nt = 512;
+  {
+    bool compiled = false;
+#define X(N) compiled = compiled || nt == N;
+    MCDC_WARP_CASES(X)
+#undef X
+    if (!compiled) nt = 512;
+  }
   const int nw = nt / 32;
   const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8, 16) : 0);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
@@ -1066,7 +1105,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record, bool weighted) {
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
-  cudaError_t e1 = warp_set_smem(staged, record, weighted, nt, (int)p->pool_smem);
+  cudaError_t e1 = warp_set_smem(staged, record, variant, nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
   return MCDC_OK;
 }
@@ -1111,7 +1150,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
   CK(cudaEventRecord(a, p->stream));
   const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on;
-  warp_launch(staged, record, weighted, nt, grid, smem, p->stream, p->tab, ha);
+  warp_launch(staged, record, weighted ? KW_WEIGHTED : KW_ANALOG, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->ev_pairs.emplace_back(a, b);
   p->launches++;
@@ -1170,7 +1209,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
     cudaEvent_t a, b;
     CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
     CK(cudaEventRecord(a, p->stream));
-    warp_launch(staged, record, true, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    warp_launch(staged, record, KW_CENSUS_STEP, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
     p->ev_pairs.emplace_back(a, b);
     p->launches++;
@@ -1258,7 +1297,8 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
       p->blocks_per_sm = occ;
   }
   if (!stepped) {
-    const int rcp = plan_warp_kernel(p, record, stepwarp || p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on);
+    const int rcp = plan_warp_kernel(p, record, stepwarp ? KW_CENSUS_STEP
+                                     : (p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on) ? KW_WEIGHTED : KW_ANALOG);
     if (rcp != MCDC_OK) return rcp;
   }
   cudaEvent_t e_run0, e_run1, ev0, ev1;
@@ -1328,7 +1368,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   if (p->cap == 0 || p->ws_hist < n_particles) return MCDC_ERR_NO_WORKSPACE;
   if (p->tech.population_control) return MCDC_ERR_ARG;    // there is no census here; the generation has its own control
   { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
-  const int rcp = plan_warp_kernel(p, false, true);
+  const int rcp = plan_warp_kernel(p, false, KW_GENERATION);
   if (rcp != MCDC_OK) return rcp;
   const uint32_t ws_ns = p->ws_slots, N = (uint32_t)n_particles;
   uint32_t *counts_dev = p->counts_dev;
@@ -1378,7 +1418,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
     cudaEvent_t a, b;
     CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
     CK(cudaEventRecord(a, p->stream));
-    warp_launch(staged, false, true, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    warp_launch(staged, false, KW_GENERATION, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
     p->ev_pairs.emplace_back(a, b);
     p->launches++;

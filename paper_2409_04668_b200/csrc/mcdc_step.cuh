@@ -62,7 +62,7 @@ __device__ __forceinline__ bool flight_init(const TBT &tb, PState &p, int kind) 
   p.ix = 1.0 / p.ux; p.iy = 1.0 / p.uy; p.iz = 1.0 / p.uz;
   p.last_surf = -1;
   if (kind == FI_SOURCE) {
-    p.cell = locate_source(tb, p.x, p.y, p.z, p.ux, p.uy, p.uz);
+    p.cell = locate_source<true>(tb, p.x, p.y, p.z, p.ux, p.uy, p.uz);
     return p.cell >= 0;
   }
   return true;
@@ -130,7 +130,7 @@ __device__ __forceinline__ bool surface_event(const TBT &tb, PState &p, int i_st
   const int bc = tb.surf_bc(s_star);
   if (bc == 1) { *led_leak += p.w; return false; }
   if (bc == 2) { reflect(tb, s_star, (h >> 1) & 7, p.x, p.y, p.z, p.ux, p.uy, p.uz); return true; }
-  const int c = locate_neighbour(tb, i_star, s_star, p.x, p.y, p.z, p.ux, p.uy, p.uz);
+  const int c = locate_neighbour<true>(tb, i_star, s_star, p.x, p.y, p.z, p.ux, p.uy, p.uz);
   if (c < 0) { *led_lost += p.w; *cnt_lost += 1u; return false; }
   p.cell = c;
   return true;

@@ -75,6 +75,7 @@ struct Tables {
   double src_lo[3], src_hi[3], src_t0, src_t1;
   int src_last;
   int src_dir_mode;
+  int src_cell;         // point source strictly inside one cell (proved at create): that cell, else -1 (locate per particle)
   double src_dir[3];
   int loc_n[3];
   double loc_lo[3], loc_inv_d[3];

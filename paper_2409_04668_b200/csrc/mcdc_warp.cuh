@@ -36,7 +36,7 @@ __device__ __noinline__ int slow_cross(const Tables *gT, int cell, int idx, int 
                                        double ux, double uy, double uz) {
   const TB<false> tb(*gT);
   const int slot = tb.cell_off(cell) + idx;
-  return locate_neighbour(tb, slot, s_star, x, y, z, ux, uy, uz);
+  return locate_neighbour<false>(tb, slot, s_star, x, y, z, ux, uy, uz);
 }
 // A.5 reflection off a surface that is not an axis-aligned plane
 __device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, double x, double y, double z, double *u) {
@@ -47,7 +47,7 @@ __device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, dou
 __device__ __noinline__ int slow_locate_source(const Tables *gT, double x, double y, double z, double ux, double uy,
                                                double uz) {
   const TB<false> tb(*gT);
-  return locate_source(tb, x, y, z, ux, uy, uz);
+  return locate_source<false>(tb, x, y, z, ux, uy, uz);
 }
 // A.4 distance to a surface that is neither an axis-aligned plane face nor a z-cylinder
 __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, bool on, double x, double y, double z,
@@ -101,8 +101,12 @@ struct WarpShared {                // block-wide totals (static shared memory)
   uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
 
-template <bool STAGED, bool RECORD, bool WEIGHTED, int NT>
+// VARIANT: 0 analog (unit weights, not stored); 1 weighted (Appendix G.1 / G.2, collision tally); 2 weighted, census-step
+// mode (G.3); 3 weighted, generation mode (H).  Separate instantiations: every variant carries only its own code --
+// the kernel is sensitive to its instruction-cache footprint (profiles/r01e, r01f).
+template <bool STAGED, bool RECORD, int VARIANT, int NT>
 __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
+  constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
   constexpr uint32_t ND = WEIGHTED ? 11u : 10u;       // f64 arrays of the pool
   const double INF = CUDART_INF;
@@ -151,8 +155,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
   bool src_exhausted = false;
-  const bool step_mode = WEIGHTED && A.step_mode != 0; // census-step mode (Appendix G.3) or generation mode (H)
-  const bool gen_mode = WEIGHTED && A.step_mode == 2;  // k-eigenvalue: `in` holds birth records, children go to `census_out`
+  constexpr bool step_mode = VARIANT >= 2;             // census-step mode (Appendix G.3) or generation mode (H)
+  constexpr bool gen_mode = VARIANT == 3;              // k-eigenvalue: `in` holds birth records, children go to `census_out`
   bool bank_done = !step_mode;                         // the live bank of this step has been handed out
   uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
   if (step_mode && !A.step_source) src_exhausted = true;
@@ -172,7 +176,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
     if (phase == 0) {
       // =============== R: acquire work for up to 32 free slots, initialise the new particles (A.3, A.6) ===============
       const uint32_t want = min(32u, nFree);
-      if (WEIGHTED && !bank_done) {
+      if (step_mode && !bank_done) {
         // ---- census-step mode: particles of the live bank first (full records: nothing is sampled here) ----
         uint32_t base = 0u, cnt = 0u;
         if (lane == 0) { cnt = min(A.in.count[bank_slot], A.bank_cap); base = atomicAdd(A.in.cursor + bank_slot, want); }
@@ -299,7 +303,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         z = T.src_lo[2] + xi_z * (T.src_hi[2] - T.src_lo[2]);
         t = T.src_t0 + xi_t * (T.src_t1 - T.src_t0);
         pk = census_index(tb, t);
-        if (WEIGHTED && step_mode && !A.step_single && pk != A.step_k) { skip = true; ok = false; }
+        if (step_mode && !A.step_single && pk != A.step_k) { skip = true; ok = false; }
       }
       // group: chi of the fission-site material (child) or the source pdf; then the direction
       const double xi_g = draw(key, ctr);
@@ -317,12 +321,13 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         isotropic(xi_mu, xi_phi, ux, uy, uz);
       }
       if (is_src) {
-        cell = slow_locate_source(gT, x, y, z, ux, uy, uz);
+        // (a point source proved to lie strictly inside one cell at create time skips the search: warp-uniform)
+        cell = (T.src_cell >= 0) ? T.src_cell : slow_locate_source(gT, x, y, z, ux, uy, uz);
         if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
       }
       const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0 && !skip);
       if (m_lost) { WCNT(W_LOST, (uint32_t)__popc(m_lost)); if (lane == 0) atomicAdd(&sh.led[LED_LOST], (double)__popc(m_lost)); }
-      if (WEIGHTED && step_mode) WCNT(W_SRC, (uint32_t)__popc(__ballot_sync(MCDC_FULL, is_src && !skip)));
+      if (step_mode) WCNT(W_SRC, (uint32_t)__popc(__ballot_sync(MCDC_FULL, is_src && !skip)));
       else WCNT(W_SRC, n_src);
       if (ok) {
         const uint32_t gi = lb + i;
@@ -508,7 +513,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (ev == EV_CENSUS) PU(U_META, gi) = meta;
         if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
       }
-      if (WEIGHTED && step_mode) {
+      if (step_mode) {
         // ---- census-step mode: park the arrivals of a census that is not the last in their batch's census bank ----
         const bool park = act && ev == EV_CENSUS && pk != T.K - 1;
         if (__any_sync(MCDC_FULL, park)) {
