@@ -652,6 +652,11 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
   if (has_regions) { t.o_rgn_off = puti(p->rgn_off); t.o_rgn_tok = puti(p->rgn_tok); }
   t.score_fast = score_fast;
   t.warp_ok = warp_ok ? 1 : 0;
+  {
+    bool all1 = p->n_one_bin == (size_t)C;
+    for (int k = 0; k < p->K; ++k) all1 = all1 && tbin_k[k] >= 0;
+    t.all_one_bin = all1 ? 1 : 0;
+  }
   (void)any_quadric;
   blob.resize((blob.size() + 15) / 16 * 16, 0);
   t.hot_bytes = (uint32_t)hot;
@@ -1027,48 +1032,58 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 #define MCDC_WARP_CASES(X) X(512)          // threads per block compiled in (tuning builds: -DMCDC_WARP_CASES(X)="X(256) X(512) X(1024)")
 #endif
 enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
-template <bool STAGED, bool RECORD, int VARIANT>
+template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
-#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, N><<<grid, N, smem, st>>>(T, A); break;
+#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, ONEBIN, N><<<grid, N, smem, st>>>(T, A); break;
     MCDC_WARP_CASES(X)
 #undef X
   }
 }
-template <bool STAGED, bool RECORD, int VARIANT>
+template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN>
 cudaError_t warp_set_smem_nt(int nt, int bytes) {
   switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, ONEBIN, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     MCDC_WARP_CASES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-template <int VARIANT>
+// one table of the instantiations: F is a functor template taking <STAGED, RECORD, VARIANT, ONEBIN>
+template <int VARIANT, bool ONEBIN>
 void warp_launch_v(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (record) warp_launch_nt<true, true, VARIANT>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT>(nt, grid, smem, st, T, A); }
-  else        { if (record) warp_launch_nt<false, true, VARIANT>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT>(nt, grid, smem, st, T, A); }
+  if (staged) { if (record) warp_launch_nt<true, true, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); }
+  else        { if (record) warp_launch_nt<false, true, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); }
+}
+template <bool ONEBIN>
+void warp_launch_o(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
+  switch (variant) {
+    case KW_ANALOG: warp_launch_v<KW_ANALOG, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
+    default: warp_launch_v<KW_GENERATION, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
+  }
 }
 void warp_launch(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  switch (variant) {
-    case KW_ANALOG: warp_launch_v<KW_ANALOG>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP>(staged, record, nt, grid, smem, st, T, A); break;
-    default: warp_launch_v<KW_GENERATION>(staged, record, nt, grid, smem, st, T, A); break;
-  }
+  if (T.all_one_bin) warp_launch_o<true>(staged, record, variant, nt, grid, smem, st, T, A);
+  else warp_launch_o<false>(staged, record, variant, nt, grid, smem, st, T, A);
 }
-template <int VARIANT>
+template <int VARIANT, bool ONEBIN>
 cudaError_t warp_set_smem_v(bool staged, bool record, int nt, int bytes) {
-  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT>(nt, bytes);
-  return record ? warp_set_smem_nt<false, true, VARIANT>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT>(nt, bytes);
+  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT, ONEBIN>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT, ONEBIN>(nt, bytes);
+  return record ? warp_set_smem_nt<false, true, VARIANT, ONEBIN>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT, ONEBIN>(nt, bytes);
 }
-cudaError_t warp_set_smem(bool staged, bool record, int variant, int nt, int bytes) {
+template <bool ONEBIN>
+cudaError_t warp_set_smem_o(bool staged, bool record, int variant, int nt, int bytes) {
   switch (variant) {
-    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG>(staged, record, nt, bytes);
-    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED>(staged, record, nt, bytes);
-    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP>(staged, record, nt, bytes);
-    default: return warp_set_smem_v<KW_GENERATION>(staged, record, nt, bytes);
+    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG, ONEBIN>(staged, record, nt, bytes);
+    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED, ONEBIN>(staged, record, nt, bytes);
+    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP, ONEBIN>(staged, record, nt, bytes);
+    default: return warp_set_smem_v<KW_GENERATION, ONEBIN>(staged, record, nt, bytes);
   }
+}
+cudaError_t warp_set_smem(bool staged, bool record, int variant, bool onebin, int nt, int bytes) {
+  return onebin ? warp_set_smem_o<true>(staged, record, variant, nt, bytes) : warp_set_smem_o<false>(staged, record, variant, nt, bytes);
 }
 
 // shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
@@ -1105,7 +1120,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
-  cudaError_t e1 = warp_set_smem(staged, record, variant, nt, (int)p->pool_smem);
+  cudaError_t e1 = warp_set_smem(staged, record, variant, p->tab.all_one_bin != 0, nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
   return MCDC_OK;
 }

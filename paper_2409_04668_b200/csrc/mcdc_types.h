@@ -67,6 +67,7 @@ struct Tables {
   int has_regions;
   const Tables *self_dev;  // device-memory copy of this struct (slow paths that must not take the parameter's address)
   int score_fast;       // the tally mesh covers the geometry and the time grid covers [t0, C_K]: no clipping needed
+  int all_one_bin;      // every cell lies in one spatial tally bin and every census interval in one time bin
   int warp_ok;          // the problem fits the compact tables of k_warp (16-bit surface / cell ids, ...)
   // techniques (include/mcdc.h mcdc_technique, DESIGN.md Appendix G); all zero = analog
   int implicit_capture;

@@ -56,6 +56,14 @@ __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, 
   return surf_distance(tb, s, type, on, x, y, z, ux, uy, uz, 1.0 / ux, 1.0 / uy, 1.0 / uz);
 }
 
+// Appendix I: one collision-estimator score (only runs that enabled the tally come here)
+__device__ __noinline__ void slow_score_collision(const Tables *gT, double *xc_slot, double x, double y, double z, double t,
+                                                  int g, double w, int mg) {
+  const TB<false> tb(*gT);
+  const long long cb = collision_bin(tb, x, y, z, t, g);
+  if (cb >= 0) atomicAdd(xc_slot + cb, w / tb.sig_t(mg));
+}
+
 // A.7 for segments that may touch several tally bins (4-D DDA).  Warp-converged: every lane calls it.
 template <bool STAGED>
 #if MCDC_SCORE_NOINLINE
@@ -104,7 +112,10 @@ struct WarpShared {                // block-wide totals (static shared memory)
 // VARIANT: 0 analog (unit weights, not stored); 1 weighted (Appendix G.1 / G.2, collision tally); 2 weighted, census-step
 // mode (G.3); 3 weighted, generation mode (H).  Separate instantiations: every variant carries only its own code --
 // the kernel is sensitive to its instruction-cache footprint (profiles/r01e, r01f).
-template <bool STAGED, bool RECORD, int VARIANT, int NT>
+// ONEBIN: every cell lies in one spatial tally bin and every census interval in one time bin (Tables::all_one_bin, found
+// at create): every score is a single RED and the 4-D DDA scorer is not compiled in.  It is ~1000 instructions that
+// such problems never execute, in the middle of the flight phase: leaving it out is worth 8 % on config 3 (r01f).
+template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN, int NT>
 __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
@@ -443,10 +454,12 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         S.aggregate = A.aggregate;
         const uint32_t cbin = tb.template ldb<uint32_t>(rec + C2_BIN);
         const int tbin = tb.template ld<int>(T.o_tbin_k, pk);
-        const bool one_bin = cbin != NONE32 && tbin >= 0;      // the whole segment lies in one tally bin
-        if (__any_sync(MCDC_FULL, act && !one_bin))
-          general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
-        if (__any_sync(MCDC_FULL, act && one_bin)) {
+        const bool one_bin = ONEBIN || (cbin != NONE32 && tbin >= 0);   // the whole segment lies in one tally bin
+        if (!ONEBIN) {
+          if (__any_sync(MCDC_FULL, act && !one_bin))
+            general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
+        }
+        if (ONEBIN || __any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
           long long bin = -1;
           if (sc) bin = bins32 ? (long long)((tbin * G + g) * (int)n_spatial + (int)cbin)
@@ -585,10 +598,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       uint32_t c0 = 0u;
       double w = 1.0, l_cap = 0.0, l_fis = 0.0, l_prod = 0.0, l_gain = 0.0, l_loss = 0.0;   // WEIGHTED only
       if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
-      if (WEIGHTED && A.xc_acc != nullptr && act && !born) {   // Appendix I: collision estimator, arriving weight
-        const long long cb = collision_bin(tb, PD(D_X, gi), PD(D_Y, gi), PD(D_Z, gi), PD(D_T, gi), g);
-        if (cb >= 0) atomicAdd(A.xc_acc + (size_t)(meta >> 20) * T.n_bins + cb, w / tb.sig_t(mg));
-      }
+      // Appendix I: collision estimator, arriving weight.  Out of line: inlined, its ~150 instructions sat in the middle
+      // of the C phase and cost runs that never enable the tally 8 % (profiles/r01f)
+      if (WEIGHTED && A.xc_acc != nullptr && act && !born)
+        slow_score_collision(gT, A.xc_acc + (size_t)(meta >> 20) * T.n_bins, PD(D_X, gi), PD(D_Y, gi), PD(D_Z, gi), PD(D_T, gi), g, w, mg);
       if (born) { kind = FI_CHILD; alive = true; }
       else if (act) {
         const double s_tot = tb.sig_s_tot(mg), sig_f = tb.sig_f(mg);
