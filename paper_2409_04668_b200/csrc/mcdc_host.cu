@@ -1032,61 +1032,76 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 #define MCDC_WARP_CASES(X) X(512)          // threads per block compiled in (tuning builds: -DMCDC_WARP_CASES(X)="X(256) X(512) X(1024)")
 #endif
 enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
-template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN>
+template <bool STAGED, bool RECORD, int VARIANT, int SCORE>
 void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (nt) {
-#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, ONEBIN, N><<<grid, N, smem, st>>>(T, A); break;
+#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, SCORE, N><<<grid, N, smem, st>>>(T, A); break;
     MCDC_WARP_CASES(X)
 #undef X
   }
 }
-template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN>
+template <bool STAGED, bool RECORD, int VARIANT, int SCORE>
 cudaError_t warp_set_smem_nt(int nt, int bytes) {
   switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, ONEBIN, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, SCORE, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
     MCDC_WARP_CASES(X)
 #undef X
   }
   return cudaErrorInvalidValue;
 }
-// one table of the instantiations: F is a functor template taking <STAGED, RECORD, VARIANT, ONEBIN>
-template <int VARIANT, bool ONEBIN>
+// one table of the instantiations: F is a functor template taking <STAGED, RECORD, VARIANT, SCORE>
+template <int VARIANT, int SCORE>
 void warp_launch_v(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (record) warp_launch_nt<true, true, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); }
-  else        { if (record) warp_launch_nt<false, true, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT, ONEBIN>(nt, grid, smem, st, T, A); }
+  if (staged) { if (record) warp_launch_nt<true, true, VARIANT, SCORE>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT, SCORE>(nt, grid, smem, st, T, A); }
+  else        { if (record) warp_launch_nt<false, true, VARIANT, SCORE>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT, SCORE>(nt, grid, smem, st, T, A); }
 }
-template <bool ONEBIN>
+template <int SCORE>
 void warp_launch_o(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   switch (variant) {
-    case KW_ANALOG: warp_launch_v<KW_ANALOG, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
-    default: warp_launch_v<KW_GENERATION, ONEBIN>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_ANALOG: warp_launch_v<KW_ANALOG, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
+    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
+    default: warp_launch_v<KW_GENERATION, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
   }
 }
+// SCORE of k_warp for a problem and its merge choice (mcdc_warp.cuh)
+int score_mode(const Tables &T, int aggregate) { return T.all_one_bin ? (aggregate ? 2 : 1) : 0; }
 void warp_launch(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (T.all_one_bin) warp_launch_o<true>(staged, record, variant, nt, grid, smem, st, T, A);
-  else warp_launch_o<false>(staged, record, variant, nt, grid, smem, st, T, A);
+  switch (score_mode(T, A.aggregate)) {
+    case 0: warp_launch_o<0>(staged, record, variant, nt, grid, smem, st, T, A); break;
+    case 1: warp_launch_o<1>(staged, record, variant, nt, grid, smem, st, T, A); break;
+    default: warp_launch_o<2>(staged, record, variant, nt, grid, smem, st, T, A); break;
+  }
 }
-template <int VARIANT, bool ONEBIN>
+template <int VARIANT, int SCORE>
 cudaError_t warp_set_smem_v(bool staged, bool record, int nt, int bytes) {
-  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT, ONEBIN>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT, ONEBIN>(nt, bytes);
-  return record ? warp_set_smem_nt<false, true, VARIANT, ONEBIN>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT, ONEBIN>(nt, bytes);
+  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT, SCORE>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT, SCORE>(nt, bytes);
+  return record ? warp_set_smem_nt<false, true, VARIANT, SCORE>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT, SCORE>(nt, bytes);
 }
-template <bool ONEBIN>
+template <int SCORE>
 cudaError_t warp_set_smem_o(bool staged, bool record, int variant, int nt, int bytes) {
   switch (variant) {
-    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG, ONEBIN>(staged, record, nt, bytes);
-    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED, ONEBIN>(staged, record, nt, bytes);
-    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP, ONEBIN>(staged, record, nt, bytes);
-    default: return warp_set_smem_v<KW_GENERATION, ONEBIN>(staged, record, nt, bytes);
+    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG, SCORE>(staged, record, nt, bytes);
+    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED, SCORE>(staged, record, nt, bytes);
+    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP, SCORE>(staged, record, nt, bytes);
+    default: return warp_set_smem_v<KW_GENERATION, SCORE>(staged, record, nt, bytes);
   }
 }
-cudaError_t warp_set_smem(bool staged, bool record, int variant, bool onebin, int nt, int bytes) {
-  return onebin ? warp_set_smem_o<true>(staged, record, variant, nt, bytes) : warp_set_smem_o<false>(staged, record, variant, nt, bytes);
+cudaError_t warp_set_smem(bool staged, bool record, int variant, int score, int nt, int bytes) {
+  switch (score) {
+    case 0: return warp_set_smem_o<0>(staged, record, variant, nt, bytes);
+    case 1: return warp_set_smem_o<1>(staged, record, variant, nt, bytes);
+    default: return warp_set_smem_o<2>(staged, record, variant, nt, bytes);
+  }
 }
 
 // shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
+// in-warp merge of equal tally addresses pays only on tiny meshes (profiles/r01d); MCDC_AGGREGATE overrides for tuning
+int problem_aggregate(const mcdc_problem *p) {
+  if (const char *e = getenv("MCDC_AGGREGATE")) return atoi(e) ? 1 : 0;
+  return ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
+}
+
 int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
   const bool weighted = variant != KW_ANALOG;
   int dev = 0, max_optin = 0;
@@ -1120,7 +1135,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
-  cudaError_t e1 = warp_set_smem(staged, record, variant, p->tab.all_one_bin != 0, nt, (int)p->pool_smem);
+  cudaError_t e1 = warp_set_smem(staged, record, variant, score_mode(p->tab, problem_aggregate(p)), nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
   return MCDC_OK;
 }
@@ -1136,7 +1151,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   ha.n_hist = sb.n_hist; ha.hb = sb.hs;
   ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
-  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;   // in-warp merge of equal bins pays only on tiny meshes
+  ha.aggregate = problem_aggregate(p);   // in-warp merge of equal bins pays only on tiny meshes
   ha.step_mode = 0; ha.step_k = 0; ha.step_source = 1; ha.step_single = 1; ha.bank_cap = 0;
   ha.in = p->bankA; ha.census_out = p->bankB;             // unused outside the census-step mode
   CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
@@ -1145,7 +1160,6 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
   ha.pool_slots = p->pool_slots;
-  if (const char *e3 = getenv("MCDC_AGGREGATE")) ha.aggregate = atoi(e3);
   const size_t smem = p->pool_smem;
   const int nt = p->hist_threads;
   // one block per SM; fewer only when the sub-batch cannot give every warp one full round of 32 histories (small
@@ -1196,7 +1210,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   ha.n_hist = sb.n_hist; ha.hb = sb.hs;
   ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = record ? p->d_ev + (size_t)sb.first_local * 4 : nullptr;
-  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
+  ha.aggregate = problem_aggregate(p);
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
   ha.pool_slots = p->pool_slots;
@@ -1398,7 +1412,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   ha.n_hist = N; ha.hb = N;
   ha.x_acc = p->x_acc; ha.xc_acc = p->col_on ? p->d_xc_acc : nullptr; ha.cnt = p->d_cnt; ha.pop_w = p->d_pop_w; ha.pop_n = p->d_pop_n;
   ha.ev = nullptr;
-  ha.aggregate = ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
+  ha.aggregate = problem_aggregate(p);
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
   ha.pool_slots = p->pool_slots;

@@ -115,8 +115,11 @@ struct WarpShared {                // block-wide totals (static shared memory)
 // ONEBIN: every cell lies in one spatial tally bin and every census interval in one time bin (Tables::all_one_bin, found
 // at create): every score is a single RED and the 4-D DDA scorer is not compiled in.  It is ~1000 instructions that
 // such problems never execute, in the middle of the flight phase: leaving it out is worth 8 % on config 3 (r01f).
-template <bool STAGED, bool RECORD, int VARIANT, bool ONEBIN, int NT>
+// SCORE: 0 = general (DDA scorer compiled in, one-bin shortcut and in-warp merge chosen at run time); 1 = ONEBIN, one RED
+// per score; 2 = ONEBIN on a tiny mesh, equal addresses merged inside the warp before the RED.
+template <bool STAGED, bool RECORD, int VARIANT, int SCORE, int NT>
 __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
+  constexpr bool ONEBIN = SCORE != 0;
   constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
   constexpr uint32_t ND = WEIGHTED ? 11u : 10u;       // f64 arrays of the pool
@@ -451,7 +454,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const uint32_t slot = meta >> 20;
         TallySink S;
         S.slab = nullptr; S.global_x = A.x_acc + (size_t)slot * T.n_bins; S.slab_lo = 0; S.slab_bins = 0;
-        S.aggregate = A.aggregate;
+        S.aggregate = (SCORE == 0) ? A.aggregate : (SCORE == 2 ? 1 : 0);
         const uint32_t cbin = tb.template ldb<uint32_t>(rec + C2_BIN);
         const int tbin = tb.template ld<int>(T.o_tbin_k, pk);
         const bool one_bin = ONEBIN || (cbin != NONE32 && tbin >= 0);   // the whole segment lies in one tally bin
@@ -464,7 +467,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           long long bin = -1;
           if (sc) bin = bins32 ? (long long)((tbin * G + g) * (int)n_spatial + (int)cbin)
                                : (long long)(tbin * G + g) * n_spatial + (long long)cbin;
-          tally_add_converged(S, bin, WEIGHTED ? w * d : d);
+          if (SCORE == 1) { if (bin >= 0) atomicAdd(S.global_x + bin, WEIGHTED ? w * d : d); }
+          else tally_add_converged(S, bin, WEIGHTED ? w * d : d);
         }
       }
       // ---- move (A.3) ----
