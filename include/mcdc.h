@@ -214,6 +214,10 @@ int mcdc_history_events_get(const mcdc_problem *p, uint32_t *ev, size_t n_histor
 typedef struct {
   uint64_t transmission_halfspaces, certified_halfspaces, cells, one_bin_cells, hot_table_bytes;
   int32_t warp_kernel_ok, score_fast;
+  int32_t all_one_bin;   /* every cell in one spatial tally bin and every census interval in one time bin: the
+                            history kernel without the 4-D DDA scorer is used                               */
+  int32_t source_cell;   /* >= 0: a point source proved to lie strictly inside this cell (no per-particle
+                            search); -1 otherwise                                                          */
 } mcdc_problem_info;
 int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
 

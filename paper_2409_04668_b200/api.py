@@ -77,7 +77,8 @@ _lib = None
 
 class ProblemInfo(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("transmission_halfspaces", "certified_halfspaces", "cells", "one_bin_cells",
-                                          "hot_table_bytes")] + [("warp_kernel_ok", C.c_int32), ("score_fast", C.c_int32)]
+                                          "hot_table_bytes")] + [("warp_kernel_ok", C.c_int32), ("score_fast", C.c_int32),
+                                                                     ("all_one_bin", C.c_int32), ("source_cell", C.c_int32)]
 
 
 def lib_path() -> str:

@@ -1726,6 +1726,7 @@ extern "C" int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *i
   info->transmission_halfspaces = p->n_transm; info->certified_halfspaces = p->n_cert;
   info->cells = (uint64_t)p->C; info->one_bin_cells = p->n_one_bin; info->hot_table_bytes = p->tab.hot_bytes;
   info->warp_kernel_ok = p->tab.warp_ok; info->score_fast = p->tab.score_fast;
+  info->all_one_bin = p->tab.all_one_bin; info->source_cell = p->tab.src_cell;
   return MCDC_OK;
 }
 

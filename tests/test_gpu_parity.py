@@ -235,6 +235,14 @@ def test_certificates_one_bin_cells_and_async_only_workspace(M):
     assert i3["transmission_halfspaces"] == 289 * 6 - 68 and i3["certified_halfspaces"] == i3["transmission_halfspaces"]
     assert i3["cells"] == 578 and i3["one_bin_cells"] == 578 and i3["warp_kernel_ok"] == 1 and i3["score_fast"] == 1
     assert i3["hot_table_bytes"] < 64 * 1024
+    # every pin / moderator cell lies in one pin bin and census = time edges: the kernel without the DDA scorer;
+    # the point source at the lattice centre sits strictly inside the centre pin (cell 288)
+    assert i3["all_one_bin"] == 1 and i3["source_cell"] == 288
+    for cfg, one_bin, src_cell in (("config0", 1, -1), ("config1", 0, -1), ("config1a", 0, -1), ("config2", 0, -1)):
+        q = M.Problem(W.get_config(cfg, n_histories=1000, n_batches=1))
+        iq = q.info()
+        assert (iq["all_one_bin"], iq["source_cell"]) == (one_bin, src_cell), (cfg, iq)   # config1a: the beam starts ON a surface
+        q.close()
     full = M.mcdc_workspace_size(g._h, 4000, 4)
     assert g.workspace_bytes < full
     g.run(record_history_events=True)
