@@ -216,8 +216,9 @@ typedef struct {
   int32_t warp_kernel_ok, score_fast;
   int32_t all_one_bin;   /* every cell in one spatial tally bin and every census interval in one time bin: the
                             history kernel without the 4-D DDA scorer is used                               */
-  int32_t source_cell;   /* >= 0: a point source proved to lie strictly inside this cell (no per-particle
-                            search); -1 otherwise                                                          */
+  int32_t source_cell;   /* >= 0: the cell source particles are born in without a search -- a point source
+                            proved strictly inside it, or a source box inside the closure of this axis-aligned
+                            box cell (particles drawn strictly inside its bounds); -1: search per particle    */
 } mcdc_problem_info;
 int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
 

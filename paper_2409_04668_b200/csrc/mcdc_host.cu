@@ -684,6 +684,23 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     }
     if (!near_surface && n_found == 1) t.src_cell = found;
   }
+  t.src_chk = 0;
+  for (int a = 0; a < 3; ++a) { t.src_clo[a] = -HINF; t.src_chi[a] = HINF; }
+  if (t.src_cell < 0 && !has_regions) {
+    // A source box inside the closure of ONE cell bounded by axis-aligned planes only: a particle drawn strictly inside
+    // that cell's bounds is in it (a draw that rounds onto a face still takes the search, where the direction decides)
+    for (int c = 0; c < C && t.src_cell < 0; ++c) {
+      bool planes_only = p->cell_off[c + 1] > p->cell_off[c];
+      for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) planes_only = planes_only && type[p->hs_surface[i]] <= ST_PLANE_Z;
+      if (!planes_only) continue;
+      const Box b = cell_box(*p, type, q, c, false);
+      bool inside = true;
+      for (int a = 0; a < 3; ++a) inside = inside && p->src_lo[a] >= b.lo[a] && p->src_hi[a] <= b.hi[a];
+      if (!inside) continue;
+      t.src_cell = c; t.src_chk = 1;
+      for (int a = 0; a < 3; ++a) { t.src_clo[a] = b.lo[a]; t.src_chi[a] = b.hi[a]; }
+    }
+  }
   t.src_t0 = p->src_t0; t.src_t1 = p->src_t1;
   for (int a = 0; a < 3; ++a) {
     t.src_lo[a] = p->src_lo[a]; t.src_hi[a] = p->src_hi[a]; t.src_dir[a] = p->src_dir[a];

@@ -76,7 +76,11 @@ struct Tables {
   double src_lo[3], src_hi[3], src_t0, src_t1;
   int src_last;
   int src_dir_mode;
-  int src_cell;         // point source strictly inside one cell (proved at create): that cell, else -1 (locate per particle)
+  int src_cell;         // >= 0: the cell of every source particle, proved at create (else -1: locate per particle):
+                        //   a point source strictly inside one cell (src_chk = 0), or a source box inside the closure of
+                        //   one axis-aligned box cell (src_chk = 1: valid for particles strictly inside src_clo..src_chi)
+  int src_chk;
+  double src_clo[3], src_chi[3];
   double src_dir[3];
   int loc_n[3];
   double loc_lo[3], loc_inv_d[3];

@@ -71,19 +71,21 @@ __device__ __noinline__
 #else
 __device__ __forceinline__
 #endif
-void general_score(const Tables *gT, double *x_acc_slot, int aggregate, bool active,
+void general_score(const Tables &Tg, double *x_acc_slot, int aggregate, bool active,
                                            const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d, double w) {
   // the pre-move state is still in the pool: x y z ux uy uz 1/ux 1/uy 1/uz t, N slots apart
   const double x = pool[gi], y = pool[N + gi], z = pool[2 * N + gi], ux = pool[3 * N + gi], uy = pool[4 * N + gi],
                uz = pool[5 * N + gi], ix = pool[6 * N + gi], iy = pool[7 * N + gi], iz = pool[8 * N + gi], t = pool[9 * N + gi];
-  const TB<STAGED> tb(*gT);
+  // Tg is the kernel's parameter block (constant bank) when this is inlined -- reading the mesh constants through the
+  // device-memory copy of the tables made every DDA step wait on global loads (config 2: long_scoreboard 3.2 per issue)
+  const TB<STAGED> tb(Tg);
   TallySink S;
   S.slab = nullptr; S.global_x = x_acc_slot; S.slab_lo = 0; S.slab_bins = 0; S.aggregate = aggregate;
-  if (gT->score_fast) {
+  if (Tg.score_fast) {
     PState p;
     p.x = x; p.y = y; p.z = z; p.ux = ux; p.uy = uy; p.uz = uz; p.ix = ix; p.iy = iy; p.iz = iz; p.t = t; p.w = w;
     p.key = 0ull; p.ctr = 0u; p.hid = 0u; p.g = g; p.cell = 0; p.last_surf = -1;
-    int it = tb.template ld<int>(gT->o_it0_k, pk);
+    int it = tb.template ld<int>(Tg.o_it0_k, pk);
     score_track_fast(tb, S, active, p, it, d);
   } else {
     score_track(tb, S, active, x, y, z, ux, uy, uz, t, w, g, d);
@@ -336,7 +338,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       }
       if (is_src) {
         // (a point source proved to lie strictly inside one cell at create time skips the search: warp-uniform)
-        cell = (T.src_cell >= 0) ? T.src_cell : slow_locate_source(gT, x, y, z, ux, uy, uz);
+        const bool known = T.src_cell >= 0 &&
+                           (!T.src_chk || (x > T.src_clo[0] && x < T.src_chi[0] && y > T.src_clo[1] && y < T.src_chi[1] &&
+                                           z > T.src_clo[2] && z < T.src_chi[2]));
+        cell = known ? T.src_cell : slow_locate_source(gT, x, y, z, ux, uy, uz);
         if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
       }
       const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0 && !skip);
@@ -460,7 +465,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const bool one_bin = ONEBIN || (cbin != NONE32 && tbin >= 0);   // the whole segment lies in one tally bin
         if (!ONEBIN) {
           if (__any_sync(MCDC_FULL, act && !one_bin))
-            general_score<STAGED>(gT, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
+            general_score<STAGED>(MCDC_SCORE_NOINLINE ? *gT : T, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
         }
         if (ONEBIN || __any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
