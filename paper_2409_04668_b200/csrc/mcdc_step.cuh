@@ -29,6 +29,7 @@ struct PState {
 // first index with xi < cdf[i]; fallback `last`.  cdf(i) is any callable.
 template <class F>
 __device__ __forceinline__ int sample_cdf(F cdf, int n, int last, double xi) {
+#pragma unroll 1
   for (int i = 0; i < n; ++i)
     if (xi < cdf(i)) return i;
   return last;
@@ -89,6 +90,7 @@ __device__ __forceinline__ void source_position(const Tables &T, unsigned long l
 // smallest k with C[k] > t, else K-1 (D15)
 template <class TBT>
 __device__ __forceinline__ int census_index(const TBT &tb, double t) {
+#pragma unroll 1
   for (int k = 0; k < tb.T.K; ++k)
     if (tb.census(k) > t) return k;
   return tb.T.K - 1;

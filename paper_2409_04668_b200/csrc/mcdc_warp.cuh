@@ -56,6 +56,41 @@ __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, 
   return surf_distance(tb, s, type, on, x, y, z, ux, uy, uz, 1.0 / ux, 1.0 / uy, 1.0 / uz);
 }
 
+// A.6 fission children that do not fit their parent's pool go to the global ring queue (SoA entries, per-entry
+// sequence flags published with st.release).  Warp-converged: every lane calls it; lanes without children pass
+// n_push = 0.  Out of line: it runs in under 1 % of the collision rounds and its ~470 instructions sat in the middle
+// of the C phase (profiles/r01g).
+__device__ __noinline__ void slow_publish_children(FissionQueue q, DevCounters *cnt, bool weighted, double x, double y,
+                                                   double z, double t, double w, unsigned long long key, uint32_t c0,
+                                                   int n_push, int pre, int total, int4 qm) {
+  const int lane = threadIdx.x & 31;
+  unsigned long long *q_head = q.head_tail, *q_tail = q.head_tail + 1;
+  const unsigned long long q_cap = (unsigned long long)q.mask + 1ull;
+  unsigned long long qb = 0ull;
+  int okq = 1;
+  if (lane == 0) {
+    qb = atomicAdd(q_tail, (unsigned long long)total);
+    if (qb + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) okq = 0;
+  }
+  qb = __shfl_sync(MCDC_FULL, qb, 0) + (unsigned long long)(pre - n_push);
+  okq = __shfl_sync(MCDC_FULL, okq, 0);
+  if (!okq && lane == 0) atomicExch(&cnt->overflow, 1);
+  if (n_push > 0 && okq) {
+    for (int c = 0; c < n_push; ++c) {
+      const uint32_t j = (uint32_t)(qb + (unsigned long long)c) & q.mask;
+      q.x[j] = x; q.y[j] = y; q.z[j] = z; q.t[j] = t;
+      if (weighted) q.w[j] = w;
+      q.key[j] = child_key(key, c0, (uint32_t)(c + 1));
+      q.meta[j] = qm;
+    }
+    __threadfence();
+    for (int c = 0; c < n_push; ++c) {
+      const unsigned long long qi = qb + (unsigned long long)c;
+      st_release_u32(q.flag + ((uint32_t)qi & q.mask), (uint32_t)(qi + 1ull));
+    }
+  }
+}
+
 // Appendix I: one collision-estimator score (only runs that enabled the tally come here)
 __device__ __noinline__ void slow_score_collision(const Tables *gT, double *xc_slot, double x, double y, double z, double t,
                                                   int g, double w, int mg) {
@@ -427,6 +462,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       if (tz) { d_surf = dz; which = fz; }
       // ---- other half-spaces (cylinders, general quadrics, redundant planes), list order, strict < ----
       const uint32_t orec = T.o_other2 + (info >> 16) * OTHER2_BYTES;
+#pragma unroll 1                                       // (peeled, the loop left a second, cold copy of its body in the flight phase)
       for (int j = 0; j < n_other; ++j) {
         const uint2 e = tb.template ldb<uint2>(orec + (uint32_t)j * OTHER2_BYTES);
         const uint32_t s = e.x & 0xFFFFu;
@@ -696,6 +732,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         } else if ((uint32_t)total <= nFree) {         // the children fit this warp's pool: they join its C stack
           if (n_push > 0) {
             const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
+#pragma unroll 1
             for (int c = 0; c < n_push; ++c) {
               const uint32_t r = (uint32_t)(pre - n_push + c);
               const uint32_t i2 = (uint32_t)PL(L_FREE, lb + nFree - 1u - r), g2 = lb + i2;
@@ -709,32 +746,14 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
             }
           }
           nFree -= (uint32_t)total; nC += (uint32_t)total;
-        } else {                                       // pool full: publish them to the global queue
-          unsigned long long qb = 0ull;
-          int okq = 1;
-          if (lane == 0) {
-            qb = atomicAdd(q_tail, (unsigned long long)total);
-            if (qb + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) okq = 0;
+        } else {                                       // pool full: publish them to the global queue (rare: out of line)
+          double x = 0.0, y = 0.0, z = 0.0, t = 0.0;
+          int4 qm = make_int4(0, 0, 0, 0);
+          if (n_push > 0) {
+            x = PD(D_X, gi); y = PD(D_Y, gi); z = PD(D_Z, gi); t = PD(D_T, gi);
+            qm = make_int4(cell, (int)((meta >> 8) & 4095u), RECORD ? (int)PU(U_HID, gi) : 0, (int)(meta >> 20));
           }
-          qb = __shfl_sync(MCDC_FULL, qb, 0) + (unsigned long long)(pre - n_push);
-          okq = __shfl_sync(MCDC_FULL, okq, 0);
-          if (!okq && lane == 0) atomicExch(&A.cnt->overflow, 1);
-          if (n_push > 0 && okq) {
-            const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
-            const int4 qm = make_int4(cell, (int)((meta >> 8) & 4095u), RECORD ? (int)PU(U_HID, gi) : 0, (int)(meta >> 20));
-            for (int c = 0; c < n_push; ++c) {
-              const uint32_t j = (uint32_t)(qb + (unsigned long long)c) & A.q.mask;
-              A.q.x[j] = x; A.q.y[j] = y; A.q.z[j] = z; A.q.t[j] = t;
-              if (WEIGHTED) A.q.w[j] = w;
-              A.q.key[j] = child_key(key, c0, (uint32_t)(c + 1));
-              A.q.meta[j] = qm;
-            }
-            __threadfence();
-            for (int c = 0; c < n_push; ++c) {
-              const unsigned long long qi = qb + (unsigned long long)c;
-              st_release_u32(A.q.flag + ((uint32_t)qi & A.q.mask), (uint32_t)(qi + 1ull));
-            }
-          }
+          slow_publish_children(A.q, A.cnt, WEIGHTED, x, y, z, t, w, key, c0, n_push, pre, total, qm);
         }
       }
       if (fissioned && n_child > 0) { key = child_key(key, c0, 0u); ctr = 0u; }   // fission parent -> its first child, in place
