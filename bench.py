@@ -28,10 +28,10 @@ import numpy as np  # noqa: E402
 METRIC = "histories/s"
 N_SM = 148
 ISSUE_LANES_PER_SM = 128        # 4 warp schedulers x 32 lanes: one warp instruction per scheduler per cycle
-# From the committed ncu capture of k_warp on this workload (profiles/r01g_k_warp_onebin.md): per launch of 1e7 config-3
+# From the committed ncu capture of k_warp on this workload (profiles/r01h_k_warp_final.md): per launch of 1e7 config-3
 # histories, dram__bytes_read.sum + dram__bytes_write.sum, and thread instructions per track segment.
-NCU = {"config3_pin_lattice": {"dram_bytes_per_history": 3.23, "thread_inst_per_segment": 915.0,
-                               "source": "profiles/r01g_k_warp_onebin.md"}}
+NCU = {"config3_pin_lattice": {"dram_bytes_per_history": 3.23, "thread_inst_per_segment": 879.0,
+                               "source": "profiles/r01h_k_warp_final.md"}}
 
 
 # variants of the workload with the techniques of DESIGN.md Appendix G switched on (the headline run is analog)
