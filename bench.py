@@ -102,6 +102,56 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+class NvmlSampler:
+    """The same samples through NVML (pynvml), polled every 5 ms from a thread: the timed region of the default run
+    is ~90 ms, too short for nvidia-smi's 100 ms loop to see more than a couple of samples."""
+
+    def __init__(self, gpu_index=0):
+        import pynvml
+        self.nv = pynvml
+        pynvml.nvmlInit()
+        self.h = pynvml.nvmlDeviceGetHandleByIndex(gpu_index)
+        self.mx = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        self.rows = []
+        self.run = False
+
+    def start(self):
+        self.run = True
+        self.t = threading.Thread(target=self._poll, daemon=True)
+        self.t.start()
+
+    def _poll(self):
+        nv = self.nv
+        while self.run:
+            try:
+                self.rows.append((time.time(), float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)),
+                                  int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))))
+            except Exception:
+                pass
+            time.sleep(0.005)
+
+    def stop(self, t0, t1):
+        self.run = False
+        self.t.join(timeout=1)
+        nv = self.nv
+        rows = [r for r in self.rows if t0 <= r[0] <= t1] or self.rows
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksEventReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksEventReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksEventReasonSwPowerCap", 0x4)}
+        reasons = sorted(n for n, bit in names.items() if any(r[2] & bit for r in rows))
+        sm = [r[1] for r in rows]
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": self.mx, "reasons": reasons,
+                "samples": len(sm), "source": "nvml, 5 ms poll"}
+
+
+def make_sampler(gpu_index):
+    try:
+        return NvmlSampler(gpu_index)
+    except Exception:
+        return ClockSampler(gpu_index)
+
+
 def _problem(args):
     from workloads import configs as W
 
@@ -209,7 +259,7 @@ def bench_gpu(args):
     for _ in range(args.warmup):
         g.reset(); g.run(n_hist, p.seed, n_b, first_history_id=first_id)
     barrier()
-    sampler = ClockSampler(local)
+    sampler = make_sampler(local)
     if rank == 0:
         sampler.start()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
