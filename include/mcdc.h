@@ -93,6 +93,15 @@ typedef struct {
   uint64_t first_history_id;      /* global id of the first history (resumable / shardable runs)   */
   int32_t record_history_events;  /* keep per-history event counts of this run (N x 4 uint32)      */
   int32_t scheduler;              /* MCDC_SCHED_*; both give the same trajectories and tallies      */
+  /* Test knobs of the history kernel (MCDC_SCHED_ASYNC); 0 = the library chooses.  They change which
+   * code path a run takes, never its results (tests/test_gpu_paths.py holds both to the oracle):
+   *  debug_pool_slots: cap on the particle slots of each warp's shared-memory pool (rounded down to
+   *    a multiple of 8, at least 32).  With 32 slots a pool is full after one refill, so every fission
+   *    child beyond the first goes through the global ring queue in HBM instead of the pool.
+   *  debug_stage_tables: +1 stage the hot problem tables in shared memory whenever a pool of >= 32
+   *    slots still fits; -1 never stage them (every table read goes through L1/L2).                  */
+  uint32_t debug_pool_slots;
+  int32_t debug_stage_tables;
 } mcdc_run_opts;
 
 typedef struct {
@@ -177,7 +186,8 @@ int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc
  * of mcdc_technique (splitting-roulette, each birth record drawing from its own stream).  Every active
  * generation is one statistical batch of n_particles histories of the tallies; inactive ones are
  * discarded.  Time plays no part: describe the problem with one time bin and one census far beyond any
- * flight.  k_gen: HOST array of n_inactive + n_active doubles.  Needs the workspace of
+ * flight (n_census must be 1, else MCDC_ERR_ARG: a census arrival inside a generation has no meaning here).
+ * k_gen: HOST array of n_inactive + n_active doubles.  Needs the workspace of
  * mcdc_workspace_size(n_particles, 1 or more); implicit capture and roulette apply if set;
  * population_control must be off (MCDC_ERR_ARG).                                                       */
 int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64_t seed, uint32_t n_inactive,
@@ -192,7 +202,8 @@ int mcdc_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n
  * reading in DESIGN.md Appendix I: at every collision the bin of the SAME mesh that holds the collision
  * site (r, t, g) takes w / Sigma_t, w the weight the particle arrives with -- an estimate of the same flux
  * as the track-length tally.  Off by default; enable before the run.  The accumulators are allocated by
- * the library (one per batch slot of the bound workspace) and are not part of mcdc_state_export.
+ * the library (one per batch slot of the bound workspace); while the tally is enabled its sum / sumsq are part
+ * of the mcdc_state_export vector (every rank must then have it enabled).
  * mcdc_collision_tallies_get has the layout and statistics of mcdc_tallies_get.                        */
 int mcdc_collision_tally_enable(mcdc_problem *p, int on);
 int mcdc_collision_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
@@ -227,7 +238,8 @@ int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
  * summed over ranks once at the end.  These calls expose the handle's accumulators as ONE fp64 vector
  * so that the caller can reduce it with any collective (ncclAllReduce on a device buffer, gloo/MPI on
  * a host buffer) and put the sum back:
- *   [0, n_bins) sum   [n_bins, 2 n_bins) sumsq   then pop_w[K], pop_n[K], ledger[7] (source production
+ *   [0, n_bins) sum   [n_bins, 2 n_bins) sumsq   [then sum and sumsq of the collision-estimator tally, 2 n_bins
+ *   more entries, while mcdc_collision_tally_enable is on]   then pop_w[K], pop_n[K], ledger[7] (source production
  *   capture fission_abs leak census_final lost), counts[7] (histories segments collisions surf_hits
  *   census_events children lost_n), vr[2] (gain, loss), pc[2] (removed, added), histories, batches.
  * Integer entries are stored as doubles (exact below 2^53).  on_device != 0: buf is DEVICE memory

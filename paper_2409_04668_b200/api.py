@@ -52,7 +52,7 @@ class ProblemDesc(C.Structure):
 
 class RunOpts(C.Structure):
     _fields_ = [("n_batches", C.c_uint32), ("first_history_id", C.c_uint64), ("record_history_events", C.c_int32),
-                ("scheduler", C.c_int32)]
+                ("scheduler", C.c_int32), ("debug_pool_slots", C.c_uint32), ("debug_stage_tables", C.c_int32)]
 
 
 class Counters(C.Structure):
@@ -247,8 +247,10 @@ def mcdc_run(h, n_histories, seed):
 SCHED_ASYNC, SCHED_CENSUS_STEPPED = 0, 1
 
 
-def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False, scheduler=0):
-    o = RunOpts(int(n_batches), int(first_history_id), int(bool(record_history_events)), int(scheduler))
+def mcdc_run_ex(h, n_histories, seed, n_batches=1, first_history_id=0, record_history_events=False, scheduler=0,
+                debug_pool_slots=0, debug_stage_tables=0):
+    o = RunOpts(int(n_batches), int(first_history_id), int(bool(record_history_events)), int(scheduler),
+                int(debug_pool_slots), int(debug_stage_tables))
     _check(lib().mcdc_run_ex(h, int(n_histories), int(seed), C.byref(o)), "mcdc_run_ex", h)
 
 
@@ -380,11 +382,12 @@ class Problem:
         return mcdc_problem_info_get(self._h)
 
     def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False,
-            scheduler=0):
+            scheduler=0, debug_pool_slots=0, debug_stage_tables=0):
         n = int(n_histories if n_histories is not None else self.prob.n_histories)
         s = int(seed if seed is not None else self.prob.seed)
         b = int(n_batches if n_batches is not None else self.prob.n_batches)
-        mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events, scheduler)
+        mcdc_run_ex(self._h, n, s, b, first_history_id, record_history_events, scheduler, debug_pool_slots,
+                    debug_stage_tables)
         self._last_n = n
 
     def run_eigenvalue(self, n_particles=None, seed=None, n_inactive=0, n_active=1):

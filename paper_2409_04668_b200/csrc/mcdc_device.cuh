@@ -65,13 +65,6 @@ struct TB {
   }
 };
 
-// cooperative copy of the hot prefix into shared memory (call from all threads, then __syncthreads)
-__device__ __forceinline__ void stage_tables(const Tables &T) {
-  const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
-  uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
-  for (uint32_t i = threadIdx.x; i < T.hot_bytes / 16u; i += blockDim.x) dst[i] = src[i];
-}
-
 // ------------------------------------------------------------------------------------------------
 // RNG: counter-based, keyed by a 64-bit particle key; draw index = particle counter (Appendix B).
 // ------------------------------------------------------------------------------------------------
@@ -89,26 +82,7 @@ __device__ __forceinline__ unsigned long long child_key(unsigned long long kp, u
 
 // Philox4x32-10 on counter (block, 0, 0, 0); returns the two 64-bit halves (o1:o0) and (o3:o2).
 // Not inlined: ~80 instructions called from a handful of sites keeps the kernels inside the i-cache.
-__device__ __noinline__ ulonglong2 philox_block(unsigned long long key, uint32_t block) {
-  uint32_t c0 = block, c1 = 0u, c2 = 0u, c3 = 0u;
-  uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
-#pragma unroll
-  for (int r = 0; r < 10; ++r) {
-    const unsigned long long p0 = (unsigned long long)0xD2511F53u * c0;   // one IMAD.WIDE.U32 each
-    const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c2;
-    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0, hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
-    uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
-    c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
-    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
-  }
-  ulonglong2 r;
-  r.x = ((unsigned long long)c1 << 32) | c0;
-  r.y = ((unsigned long long)c3 << 32) | c2;
-  return r;
-}
-
-// the same block function inlined at its call site, so that its dependent chain can overlap independent work there
-__device__ __forceinline__ ulonglong2 philox_block_inl(unsigned long long key, uint32_t block) {
+static __device__ __noinline__ ulonglong2 philox_block(unsigned long long key, uint32_t block) {
   uint32_t c0 = block, c1 = 0u, c2 = 0u, c3 = 0u;
   uint32_t k0 = (uint32_t)key, k1 = (uint32_t)(key >> 32);
 #pragma unroll
@@ -134,12 +108,6 @@ __device__ __forceinline__ double u64_to_unit(unsigned long long x) {
 
 __device__ __forceinline__ double draw(unsigned long long key, uint32_t &ctr) {
   const ulonglong2 b = philox_block(key, ctr >> 1);
-  const unsigned long long x = (ctr & 1u) ? b.y : b.x;
-  ctr += 1u;
-  return u64_to_unit(x);
-}
-__device__ __forceinline__ double draw_inl(unsigned long long key, uint32_t &ctr) {
-  const ulonglong2 b = philox_block_inl(key, ctr >> 1);
   const unsigned long long x = (ctr & 1u) ? b.y : b.x;
   ctr += 1u;
   return u64_to_unit(x);
@@ -323,7 +291,7 @@ __device__ __forceinline__ bool cell_contains(const TBT &tb, int c, int crossed,
 // full search in increasing cell id (A.3); slow path.  Not inlined, and it works on the device-memory copy of
 // the tables so that no caller has to take the address of its kernel parameter block.
 template <bool RGN>
-__device__ __noinline__ int locate_all_dev(const Tables *gT, int crossed, double x, double y, double z, double ux,
+static __device__ __noinline__ int locate_all_dev(const Tables *gT, int crossed, double x, double y, double z, double ux,
                                            double uy, double uz) {
   const TB<false> tb(*gT);
   for (int c = 0; c < gT->C; ++c)

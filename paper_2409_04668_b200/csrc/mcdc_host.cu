@@ -13,7 +13,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/mcdc.h"
-#include "mcdc_warp.cuh"
+#include "mcdc_warp_inst.cuh"
 
 using namespace mcdc;
 
@@ -83,8 +83,8 @@ struct mcdc_problem {
   unsigned long long *d_wfix = nullptr;   // [ws_slots] arriving weight of a batch in 2^-40 fixed point (workspace)
   mcdc_technique tech = {0, 0.0, 0.0, 0, 0ull};
   DevCounters *d_cnt = nullptr;
-  uint32_t *d_ev = nullptr;      // [n][4] of the last run (cudaMalloc'ed on demand)
-  size_t ev_n = 0;
+  uint32_t *d_ev = nullptr;      // [n][4] of the last run (cudaMalloc'ed on demand, kept and grown)
+  size_t ev_n = 0, ev_cap = 0;
   // workspace (caller-owned)
   char *ws = nullptr;
   size_t ws_bytes = 0;
@@ -107,7 +107,12 @@ struct mcdc_problem {
   uint32_t pool_slots = 0;
   size_t pool_smem = 0;
   size_t n_cert = 0, n_transm = 0, n_one_bin = 0;   // certified / all transmission half-spaces; cells in one tally bin
-  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;   // async launches of the run in flight
+  // CUDA events owned by the handle (created on first use, destroyed with it): run brackets, one pair per
+  // k_warp launch of the run in flight (ev_used of them recorded), the pair around each k_transport launch
+  cudaEvent_t e_run0 = nullptr, e_run1 = nullptr, e_tr0 = nullptr, e_tr1 = nullptr;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;
+  size_t ev_used = 0;
+  bool transport_attr_set = false;   // cudaFuncSetAttribute(k_transport) done for this handle's device
   std::string cuda_err;
 };
 
@@ -748,6 +753,9 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
 extern "C" void mcdc_problem_destroy(mcdc_problem *p) {
   if (!p) return;
   p->arena.release();
+  for (auto &pr : p->ev_pairs) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
+  for (cudaEvent_t e : {p->e_run0, p->e_run1, p->e_tr0, p->e_tr1})
+    if (e) cudaEventDestroy(e);
   if (p->d_ev) cudaFree(p->d_ev);
   if (p->d_xc_acc) cudaFree(p->d_xc_acc);
   if (p->d_sumc) cudaFree(p->d_sumc);
@@ -919,10 +927,11 @@ struct SubBatch {
   uint32_t n_slots;
   uint32_t hs;            // histories per slot
   int closeout;           // 0 none, 1 per-slot batches, 2 all slots form one batch
+  uint32_t closeout_slots;   // slots the close-out covers (>= n_slots: earlier pieces of a split batch may have used more)
 };
 
-int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
-                 cudaEvent_t ev0, cudaEvent_t ev1) {
+int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record) {
+  cudaEvent_t ev0 = p->e_tr0, ev1 = p->e_tr1;
   const uint32_t ns = sb.n_slots;
   const uint32_t ws_ns = p->ws_slots;
   uint32_t *counts_dev = p->counts_dev;
@@ -1037,102 +1046,48 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
   }
   if (sb.closeout) {
     int grid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
-    k_closeout<<<grid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
-    if (p->col_on) { k_closeout<<<grid, 256, 0, p->stream>>>(p->d_xc_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
+    k_closeout<<<grid, 256, 0, p->stream>>>(p->x_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<grid, 256, 0, p->stream>>>(p->d_xc_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   return MCDC_OK;
 }
 
-// ---- k_warp instantiations: (tables staged, per-history events recorded, threads per block) ----
-#ifndef MCDC_WARP_CASES
-#define MCDC_WARP_CASES(X) X(512)          // threads per block compiled in (tuning builds: -DMCDC_WARP_CASES(X)="X(256) X(512) X(1024)")
-#endif
+// ---- k_warp instantiations live in translation units of their own (mcdc_warp_inst.cu, one per VARIANT) ----
 enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
-template <bool STAGED, bool RECORD, int VARIANT, int SCORE>
-void warp_launch_nt(int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  switch (nt) {
-#define X(N) case N: k_warp<STAGED, RECORD, VARIANT, SCORE, N><<<grid, N, smem, st>>>(T, A); break;
-    MCDC_WARP_CASES(X)
-#undef X
-  }
-}
-template <bool STAGED, bool RECORD, int VARIANT, int SCORE>
-cudaError_t warp_set_smem_nt(int nt, int bytes) {
-  switch (nt) {
-#define X(N) case N: return cudaFuncSetAttribute(k_warp<STAGED, RECORD, VARIANT, SCORE, N>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-    MCDC_WARP_CASES(X)
-#undef X
-  }
-  return cudaErrorInvalidValue;
-}
-// one table of the instantiations: F is a functor template taking <STAGED, RECORD, VARIANT, SCORE>
-template <int VARIANT, int SCORE>
-void warp_launch_v(bool staged, bool record, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  if (staged) { if (record) warp_launch_nt<true, true, VARIANT, SCORE>(nt, grid, smem, st, T, A); else warp_launch_nt<true, false, VARIANT, SCORE>(nt, grid, smem, st, T, A); }
-  else        { if (record) warp_launch_nt<false, true, VARIANT, SCORE>(nt, grid, smem, st, T, A); else warp_launch_nt<false, false, VARIANT, SCORE>(nt, grid, smem, st, T, A); }
-}
-template <int SCORE>
-void warp_launch_o(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  switch (variant) {
-    case KW_ANALOG: warp_launch_v<KW_ANALOG, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_WEIGHTED: warp_launch_v<KW_WEIGHTED, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
-    case KW_CENSUS_STEP: warp_launch_v<KW_CENSUS_STEP, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
-    default: warp_launch_v<KW_GENERATION, SCORE>(staged, record, nt, grid, smem, st, T, A); break;
-  }
-}
 // SCORE of k_warp for a problem and its merge choice (mcdc_warp.cuh)
 int score_mode(const Tables &T, int aggregate) { return T.all_one_bin ? (aggregate ? 2 : 1) : 0; }
 void warp_launch(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  switch (score_mode(T, A.aggregate)) {
-    case 0: warp_launch_o<0>(staged, record, variant, nt, grid, smem, st, T, A); break;
-    case 1: warp_launch_o<1>(staged, record, variant, nt, grid, smem, st, T, A); break;
-    default: warp_launch_o<2>(staged, record, variant, nt, grid, smem, st, T, A); break;
-  }
-}
-template <int VARIANT, int SCORE>
-cudaError_t warp_set_smem_v(bool staged, bool record, int nt, int bytes) {
-  if (staged) return record ? warp_set_smem_nt<true, true, VARIANT, SCORE>(nt, bytes) : warp_set_smem_nt<true, false, VARIANT, SCORE>(nt, bytes);
-  return record ? warp_set_smem_nt<false, true, VARIANT, SCORE>(nt, bytes) : warp_set_smem_nt<false, false, VARIANT, SCORE>(nt, bytes);
-}
-template <int SCORE>
-cudaError_t warp_set_smem_o(bool staged, bool record, int variant, int nt, int bytes) {
+  (void)nt;
+  const int score = score_mode(T, A.aggregate);
   switch (variant) {
-    case KW_ANALOG: return warp_set_smem_v<KW_ANALOG, SCORE>(staged, record, nt, bytes);
-    case KW_WEIGHTED: return warp_set_smem_v<KW_WEIGHTED, SCORE>(staged, record, nt, bytes);
-    case KW_CENSUS_STEP: return warp_set_smem_v<KW_CENSUS_STEP, SCORE>(staged, record, nt, bytes);
-    default: return warp_set_smem_v<KW_GENERATION, SCORE>(staged, record, nt, bytes);
+    case KW_ANALOG: warp_launch_variant<KW_ANALOG>(staged, record, score, grid, smem, st, T, A); break;
+    case KW_WEIGHTED: warp_launch_variant<KW_WEIGHTED>(staged, record, score, grid, smem, st, T, A); break;
+    case KW_CENSUS_STEP: warp_launch_variant<KW_CENSUS_STEP>(staged, record, score, grid, smem, st, T, A); break;
+    default: warp_launch_variant<KW_GENERATION>(staged, record, score, grid, smem, st, T, A); break;
   }
 }
 cudaError_t warp_set_smem(bool staged, bool record, int variant, int score, int nt, int bytes) {
-  switch (score) {
-    case 0: return warp_set_smem_o<0>(staged, record, variant, nt, bytes);
-    case 1: return warp_set_smem_o<1>(staged, record, variant, nt, bytes);
-    default: return warp_set_smem_o<2>(staged, record, variant, nt, bytes);
+  (void)nt;
+  switch (variant) {
+    case KW_ANALOG: return warp_set_smem_variant<KW_ANALOG>(staged, record, score, bytes);
+    case KW_WEIGHTED: return warp_set_smem_variant<KW_WEIGHTED>(staged, record, score, bytes);
+    case KW_CENSUS_STEP: return warp_set_smem_variant<KW_CENSUS_STEP>(staged, record, score, bytes);
+    default: return warp_set_smem_variant<KW_GENERATION>(staged, record, score, bytes);
   }
 }
 
 // shared-memory plan of k_warp for this problem: stage the hot tables when a pool of at least 64 slots per warp still fits
-// in-warp merge of equal tally addresses pays only on tiny meshes (profiles/r01d); MCDC_AGGREGATE overrides for tuning
-int problem_aggregate(const mcdc_problem *p) {
-  if (const char *e = getenv("MCDC_AGGREGATE")) return atoi(e) ? 1 : 0;
-  return ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0;
-}
+// in-warp merge of equal tally addresses pays only on tiny meshes (profiles/r01d)
+int problem_aggregate(const mcdc_problem *p) { return ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0; }
 
-int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
+// debug_pool_slots / debug_stage_tables: the documented test knobs of mcdc_run_opts (0 = automatic choice)
+int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_pool_slots = 0, int debug_stage_tables = 0) {
   const bool weighted = variant != KW_ANALOG;
   int dev = 0, max_optin = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-  int nt = 512;
-  if (const char *e = getenv("MCDC_THREADS")) nt = atoi(e);
-  {
-    bool compiled = false;
-#define X(N) compiled = compiled || nt == N;
-    MCDC_WARP_CASES(X)
-#undef X
-    if (!compiled) nt = 512;
-  }
+  const int nt = MCDC_WARP_THREADS;
   const int nw = nt / 32;
   const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8, 16) : 0);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
@@ -1146,9 +1101,10 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
     return W / 8 * 8;                                  // keeps every array of the pool 8-byte aligned
   };
   bool staged = slots(true) >= 64;
-  if (const char *e = getenv("MCDC_STAGE_TABLES")) staged = atoi(e) != 0 && slots(true) >= 32;
+  if (debug_stage_tables > 0) staged = slots(true) >= 32;
+  if (debug_stage_tables < 0) staged = false;
   long W = slots(staged);
-  if (const char *e = getenv("MCDC_POOL")) W = std::min<long>(W, std::max<long>(32, atol(e) / 8 * 8));
+  if (debug_pool_slots) W = std::min<long>(W, std::max<long>(32, (long)debug_pool_slots / 8 * 8));
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
@@ -1157,9 +1113,35 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant) {
   return MCDC_OK;
 }
 
+// the next pair of the handle's launch events (created once, reused by every run)
+int next_event_pair(mcdc_problem *p, cudaEvent_t &a, cudaEvent_t &b) {
+  if (p->ev_used == p->ev_pairs.size()) {
+    cudaEvent_t x = nullptr, y = nullptr;
+    CK(cudaEventCreate(&x));
+    cudaError_t e = cudaEventCreate(&y);
+    if (e != cudaSuccess) { cudaEventDestroy(x); return cuda_fail(p, e, "cudaEventCreate"); }
+    p->ev_pairs.emplace_back(x, y);
+  }
+  a = p->ev_pairs[p->ev_used].first; b = p->ev_pairs[p->ev_used].second;
+  p->ev_used++;
+  return MCDC_OK;
+}
+int ensure_run_events(mcdc_problem *p) {
+  for (cudaEvent_t *e : {&p->e_run0, &p->e_run1, &p->e_tr0, &p->e_tr1})
+    if (!*e) CK(cudaEventCreate(e));
+  return MCDC_OK;
+}
+// sum the device time of the recorded launch pairs (after the stream has been synchronised)
+void collect_launch_times(mcdc_problem *p, bool ok) {
+  for (size_t i = 0; i < p->ev_used; ++i) {
+    float m2 = 0.f;
+    if (ok && cudaEventElapsedTime(&m2, p->ev_pairs[i].first, p->ev_pairs[i].second) == cudaSuccess) p->ms_transport += m2;
+  }
+  p->ev_used = 0;
+}
+
 // ---- asynchronous scheduler: one k_warp launch per sub-batch, no host synchronisation ----
-int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record,
-                       cudaEvent_t ev0, cudaEvent_t ev1) {
+int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record) {
   HistoryArgs ha;
   ha.q = p->queue;
   ha.hist_cursor = p->d_hist_cursor;
@@ -1182,28 +1164,24 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   // one block per SM; fewer only when the sub-batch cannot give every warp one full round of 32 histories (small
   // runs are bound by their longest fission chains, so spreading them over all SMs beats filling the pools:
   // 1e5 config-0 histories 0.95 -> 0.68 ms, 1e5 config-3 histories 1.39 -> 1.20 ms)
-  uint64_t per_block = (uint64_t)32 * (nt / 32);
-  if (const char *e5 = getenv("MCDC_MIN_PER_WARP")) per_block = std::max<uint64_t>(1, (uint64_t)atoi(e5)) * (nt / 32);
+  const uint64_t per_block = (uint64_t)32 * (nt / 32);
   int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + per_block - 1) / per_block));
   // chunk of source histories a warp reserves at a time: large enough to keep the cursor atomic cold, small enough
   // that the last chunks still spread over all warps
   ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)sb.n_hist / ((uint64_t)grid * (nt / 32) * 8)));
-  if (const char *e4 = getenv("MCDC_CHUNK")) ha.src_chunk = (uint32_t)std::max(1, atoi(e4));
   ha.n_slots = sb.n_slots;
   ha.n_chunks = sb.n_slots * ((sb.hs + ha.src_chunk - 1) / ha.src_chunk);
-  (void)ev0; (void)ev1;
   cudaEvent_t a, b;
-  CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+  { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
   CK(cudaEventRecord(a, p->stream));
   const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on;
   warp_launch(staged, record, weighted ? KW_WEIGHTED : KW_ANALOG, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
-  p->ev_pairs.emplace_back(a, b);
   p->launches++;
   if (sb.closeout) {
     int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
-    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)sb.n_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
-    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)sb.n_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
+    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   CK(cudaGetLastError());
@@ -1253,11 +1231,10 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
     const uint64_t work = live_total + (src ? sb.n_hist : 0);
     const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work + per_block - 1) / per_block));
     cudaEvent_t a, b;
-    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
     CK(cudaEventRecord(a, p->stream));
     warp_launch(staged, record, KW_CENSUS_STEP, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
-    p->ev_pairs.emplace_back(a, b);
     p->launches++;
     CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
     CK(cudaStreamSynchronize(p->stream));
@@ -1296,8 +1273,8 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   }
   if (sb.closeout) {
     int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);
-    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
-    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)ns, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
+    k_closeout<<<cgrid, 256, 0, p->stream>>>(p->x_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sum, p->d_sumsq);
+    if (p->col_on) { k_closeout<<<cgrid, 256, 0, p->stream>>>(p->d_xc_acc, (int)sb.closeout_slots, sb.closeout == 2 ? 1 : 0, p->n_bins, p->d_sumc, p->d_sumsqc); p->launches++; }
     p->launches++;
   }
   CK(cudaGetLastError());
@@ -1308,68 +1285,75 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
 
 extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed, const mcdc_run_opts *opts) {
   if (!p || n_histories == 0) return MCDC_ERR_ARG;
-  mcdc_run_opts def = {1u, 0ull, 0, 0};
+  mcdc_run_opts def = {1u, 0ull, 0, 0, 0u, 0};
   if (!opts) opts = &def;
   const uint32_t B = opts->n_batches ? opts->n_batches : 1u;
   if (n_histories % B != 0) return MCDC_ERR_ARG;
   const uint64_t hb = n_histories / B;
   if (p->batch_size != 0 && p->batch_size != hb) return MCDC_ERR_ARG;
   if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
-  { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
-  const bool record = opts->record_history_events != 0;
   if (opts->scheduler != MCDC_SCHED_ASYNC && opts->scheduler != MCDC_SCHED_CENSUS_STEPPED) return MCDC_ERR_ARG;
   // problems outside the compact tables of k_warp (16-bit ids, ...) run on the census-stepped scheduler
   const bool stepped = opts->scheduler == MCDC_SCHED_CENSUS_STEPPED || !p->tab.warp_ok || p->ws_slots > 4095u;
   // the population control needs every particle of a batch parked at the census: the history kernel then runs one
   // launch per census step (census-step mode) with the control kernels in between
   const bool stepwarp = !stepped && p->tech.population_control;
-  if (record) {
-    if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; }
-    CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
+  if ((stepped || stepwarp) && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
+  const uint64_t slot_max = (stepped || stepwarp) ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
+  if (p->tech.population_control && hb > slot_max) return MCDC_ERR_ARG;   // the control acts on whole batches
+  { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
+  { const int rce = ensure_run_events(p); if (rce != MCDC_OK) return rce; }
+  const bool record = opts->record_history_events != 0;
+  if (record) {                                          // the per-history event array is kept and only ever grown
+    if (p->ev_cap < n_histories) {
+      if (p->d_ev) { cudaFree(p->d_ev); p->d_ev = nullptr; p->ev_cap = 0; }
+      CK(cudaMalloc((void **)&p->d_ev, n_histories * 4 * sizeof(uint32_t)));
+      p->ev_cap = n_histories;
+    }
     CK(cudaMemsetAsync(p->d_ev, 0, n_histories * 4 * sizeof(uint32_t), p->stream));
     p->ev_n = n_histories;
   } else p->ev_n = 0;
 
-  static bool attr_set = false;
-  if (!attr_set) {
-    CK(cudaFuncSetAttribute(k_transport, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_MAX_BINS * (int)sizeof(double)));
-    attr_set = true;
-  }
-  {
+  if (stepped) {
+    if (!p->transport_attr_set) {
+      CK(cudaFuncSetAttribute(k_transport, cudaFuncAttributeMaxDynamicSharedMemorySize, SLAB_MAX_BINS * (int)sizeof(double)));
+      p->transport_attr_set = true;
+    }
     int occ = 1;   // occupancy with the largest slab this problem can ask for
     size_t per_step = (size_t)p->G * p->n_spatial;
     size_t smem = per_step <= (size_t)SLAB_MAX_BINS ? std::min<size_t>((size_t)SLAB_MAX_BINS, per_step * (size_t)p->Nt) * 8 : 0;
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_transport, TRANSPORT_THREADS, smem) == cudaSuccess && occ > 0)
       p->blocks_per_sm = occ;
-  }
-  if (!stepped) {
+  } else {
     const int rcp = plan_warp_kernel(p, record, stepwarp ? KW_CENSUS_STEP
-                                     : (p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on) ? KW_WEIGHTED : KW_ANALOG);
+                                     : (p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on) ? KW_WEIGHTED : KW_ANALOG,
+                                     opts->debug_pool_slots, opts->debug_stage_tables);
     if (rcp != MCDC_OK) return rcp;
   }
-  cudaEvent_t e_run0, e_run1, ev0, ev1;
-  CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1)); CK(cudaEventCreate(&ev0)); CK(cudaEventCreate(&ev1));
   p->ms_transport = 0.0;
-  CK(cudaEventRecord(e_run0, p->stream));
+  p->ev_used = 0;
+  CK(cudaEventRecord(p->e_run0, p->stream));
 
   // ---- plan sub-batches ----
-  if ((stepped || stepwarp) && p->cap == 0) return MCDC_ERR_NO_WORKSPACE;   // bound for the asynchronous scheduler only
-  const uint64_t slot_max = (stepped || stepwarp) ? std::max<uint64_t>(1, std::min<uint64_t>(p->cap / 2, p->ws_hist)) : p->ws_hist;
+  auto dispatch = [&](const SubBatch &sb) {
+    return stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record)
+         : stepwarp ? run_subbatch_stepwarp(p, sb, seed, opts->first_history_id, record)
+                    : run_subbatch_async(p, sb, seed, opts->first_history_id, record);
+  };
   int rc = MCDC_OK;
-  if (p->tech.population_control && hb > slot_max) return MCDC_ERR_ARG;   // the control acts on whole batches
   if (hb <= slot_max) {                                  // whole batches, one per slot
     const uint32_t per_sub = (uint32_t)std::max<uint64_t>(1, std::min<uint64_t>(p->ws_slots, p->ws_hist / hb));
     for (uint32_t b = 0; b < B && rc == MCDC_OK; b += per_sub) {
       SubBatch sb;
       sb.n_slots = std::min<uint32_t>(per_sub, B - b);
       sb.first_local = (uint64_t)b * hb; sb.n_hist = (uint32_t)(sb.n_slots * hb); sb.hs = (uint32_t)hb; sb.closeout = 1;
-      rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
-           : stepwarp ? run_subbatch_stepwarp(p, sb, seed, opts->first_history_id, record)
-                      : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+      sb.closeout_slots = sb.n_slots;
+      rc = dispatch(sb);
     }
   } else {                                               // one batch = several pieces spread over the slots
     const uint64_t per_sub = std::min<uint64_t>(p->ws_hist, slot_max * p->ws_slots);
     for (uint32_t b = 0; b < B && rc == MCDC_OK; ++b) {
+      uint32_t slots_used = 0;                           // most slots any piece of this batch scored into
       for (uint64_t off = 0; off < hb && rc == MCDC_OK; off += per_sub) {
         SubBatch sb;
         uint64_t n = std::min<uint64_t>(per_sub, hb - off);
@@ -1377,24 +1361,18 @@ extern "C" int mcdc_run_ex(mcdc_problem *p, uint64_t n_histories, uint64_t seed,
         sb.n_slots = (uint32_t)((n + sb.hs - 1) / sb.hs);
         sb.first_local = (uint64_t)b * hb + off; sb.n_hist = (uint32_t)n;
         sb.closeout = (off + n >= hb) ? 2 : 0;
-        rc = stepped ? run_subbatch(p, sb, seed, opts->first_history_id, record, ev0, ev1)
-           : stepwarp ? run_subbatch_stepwarp(p, sb, seed, opts->first_history_id, record)
-                      : run_subbatch_async(p, sb, seed, opts->first_history_id, record, ev0, ev1);
+        slots_used = std::max(slots_used, sb.n_slots);
+        sb.closeout_slots = slots_used;                  // the close-out sums every slot a piece of the batch touched
+        rc = dispatch(sb);
       }
     }
   }
-  cudaEventRecord(e_run1, p->stream);
+  cudaEventRecord(p->e_run1, p->stream);
   cudaError_t se = cudaStreamSynchronize(p->stream);
   float ms = 0.f;
-  cudaEventElapsedTime(&ms, e_run0, e_run1);
+  if (se == cudaSuccess) cudaEventElapsedTime(&ms, p->e_run0, p->e_run1);
   p->ms_run = ms;
-  for (auto &pr : p->ev_pairs) {
-    float m2 = 0.f;
-    if (se == cudaSuccess && cudaEventElapsedTime(&m2, pr.first, pr.second) == cudaSuccess) p->ms_transport += m2;
-    cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
-  }
-  p->ev_pairs.clear();
-  cudaEventDestroy(e_run0); cudaEventDestroy(e_run1); cudaEventDestroy(ev0); cudaEventDestroy(ev1);
+  collect_launch_times(p, se == cudaSuccess);
   if (rc != MCDC_OK) return rc;
   if (se != cudaSuccess) return cuda_fail(p, se, "cudaStreamSynchronize");
   int overflow = 0;
@@ -1411,6 +1389,8 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   if (p->batch_size != 0 && p->batch_size != n_particles) return MCDC_ERR_ARG;
   if (!p->ws) return MCDC_ERR_NO_WORKSPACE;
   if (!p->tab.warp_ok) return MCDC_ERR_ARG;               // this mode exists on the history kernel only
+  if (p->K != 1) return MCDC_ERR_ARG;                     // H.2: one census beyond every flight (a census arrival would be
+                                                          // parked in the generation's fission bank)
   if (p->cap == 0 || p->ws_hist < n_particles) return MCDC_ERR_NO_WORKSPACE;
   if (p->tech.population_control) return MCDC_ERR_ARG;    // there is no census here; the generation has its own control
   { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
@@ -1438,10 +1418,10 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)N / ((uint64_t)p->n_sm * (nt / 32) * 8)));
   ha.n_slots = 1;
   ha.step_mode = 2; ha.step_k = 0; ha.step_single = 1; ha.bank_cap = p->cap;
-  cudaEvent_t e_run0, e_run1;
-  CK(cudaEventCreate(&e_run0)); CK(cudaEventCreate(&e_run1));
+  { const int rce = ensure_run_events(p); if (rce != MCDC_OK) return rce; }
   p->ms_transport = 0.0;
-  CK(cudaEventRecord(e_run0, p->stream));
+  p->ev_used = 0;
+  CK(cudaEventRecord(p->e_run0, p->stream));
   const uint32_t G_total = n_inactive + n_active;
   double prod_prev = 0.0, lost_prev = 0.0;
   {
@@ -1462,11 +1442,10 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
     const uint64_t work = (g == 0) ? N : live;
     const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work + per_block - 1) / per_block));
     cudaEvent_t a, b;
-    CK(cudaEventCreate(&a)); CK(cudaEventCreate(&b));
+    { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
     CK(cudaEventRecord(a, p->stream));
     warp_launch(staged, false, KW_GENERATION, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
-    p->ev_pairs.emplace_back(a, b);
     p->launches++;
     // H.2: an active generation is one statistical batch; an inactive one is discarded
     if (g >= n_inactive) {
@@ -1508,18 +1487,12 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
     live = h_counts[A.count - counts_dev];
     if (live > p->cap) { rc = MCDC_ERR_BANK_OVERFLOW; break; }
   }
-  cudaEventRecord(e_run1, p->stream);
+  cudaEventRecord(p->e_run1, p->stream);
   cudaError_t se = cudaStreamSynchronize(p->stream);
   float ms = 0.f;
-  cudaEventElapsedTime(&ms, e_run0, e_run1);
+  if (se == cudaSuccess) cudaEventElapsedTime(&ms, p->e_run0, p->e_run1);
   p->ms_run = ms;
-  for (auto &pr : p->ev_pairs) {
-    float m2 = 0.f;
-    if (se == cudaSuccess && cudaEventElapsedTime(&m2, pr.first, pr.second) == cudaSuccess) p->ms_transport += m2;
-    cudaEventDestroy(pr.first); cudaEventDestroy(pr.second);
-  }
-  p->ev_pairs.clear();
-  cudaEventDestroy(e_run0); cudaEventDestroy(e_run1);
+  collect_launch_times(p, se == cudaSuccess);
   if (se != cudaSuccess) return cuda_fail(p, se, "cudaStreamSynchronize");
   if (rc != MCDC_OK) return rc;
   p->batch_size = n_particles;
@@ -1669,7 +1642,8 @@ extern "C" int mcdc_technique_set(mcdc_problem *p, const mcdc_technique *t) {
 
 // ---- multi-rank reduction support (include/mcdc.h "Multi-GPU domain replication") ----
 namespace {
-size_t state_doubles(const mcdc_problem *p) { return 2 * p->n_bins + 2 * (size_t)p->K + 9 + 9 + 2; }
+// sum, sumsq, [sum_c, sumsq_c when the collision-estimator tally is on], pop_w, pop_n, ledger, counts, histories, batches
+size_t state_doubles(const mcdc_problem *p) { return (p->col_on ? 4 : 2) * p->n_bins + 2 * (size_t)p->K + 9 + 9 + 2; }
 }
 extern "C" int mcdc_state_size(const mcdc_problem *p, size_t *n) {
   if (!p || !n) return MCDC_ERR_ARG;
@@ -1685,6 +1659,12 @@ extern "C" int mcdc_state_export(const mcdc_problem *cp, double *buf, size_t n, 
   const cudaMemcpyKind big = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
   CK(cudaMemcpyAsync(buf, p->d_sum, nb * sizeof(double), big, p->stream));
   CK(cudaMemcpyAsync(buf + nb, p->d_sumsq, nb * sizeof(double), big, p->stream));
+  if (p->col_on) {                                        // Appendix I accumulators ride along (allocated on first use)
+    { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
+    CK(cudaMemcpyAsync(buf + 2 * nb, p->d_sumc, nb * sizeof(double), big, p->stream));
+    CK(cudaMemcpyAsync(buf + 3 * nb, p->d_sumsqc, nb * sizeof(double), big, p->stream));
+    buf += 2 * nb;
+  }
   CK(cudaMemcpyAsync(buf + 2 * nb, p->d_pop_w, K * sizeof(double), big, p->stream));
   // the integer tail goes through the host (a few hundred bytes)
   std::vector<unsigned long long> pn(K);
@@ -1711,6 +1691,12 @@ extern "C" int mcdc_state_import(mcdc_problem *p, const double *buf, size_t n, i
   const cudaMemcpyKind big = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   CK(cudaMemcpyAsync(p->d_sum, buf, nb * sizeof(double), big, p->stream));
   CK(cudaMemcpyAsync(p->d_sumsq, buf + nb, nb * sizeof(double), big, p->stream));
+  if (p->col_on) {
+    { const int rcc = ensure_collision_buffers(p); if (rcc != MCDC_OK) return rcc; }
+    CK(cudaMemcpyAsync(p->d_sumc, buf + 2 * nb, nb * sizeof(double), big, p->stream));
+    CK(cudaMemcpyAsync(p->d_sumsqc, buf + 3 * nb, nb * sizeof(double), big, p->stream));
+    buf += 2 * nb;
+  }
   CK(cudaMemcpyAsync(p->d_pop_w, buf + 2 * nb, K * sizeof(double), big, p->stream));
   std::vector<double> tail(K + 20);
   const double *src = buf + 2 * nb + K;

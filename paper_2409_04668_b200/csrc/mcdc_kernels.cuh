@@ -369,6 +369,7 @@ struct SourceParams {
   int single_step;                     // all sources are born in step k (skip the time filter)
 };
 
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank out, DevCounters *cnt) {
   __shared__ double scratch[32];
   const TB<false> tb(T);
@@ -405,6 +406,7 @@ __global__ void __launch_bounds__(256) k_source(Tables T, SourceParams P, Bank o
   block_atomic_add_u64(&cnt->n[0], live ? 1ull : 0ull, (unsigned long long *)scratch);
   block_atomic_add_u64(&cnt->n[6], lost ? 1ull : 0ull, (unsigned long long *)scratch);
 }
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // Census-stepped transport kernel: one census step (or one fission generation inside it) for every slot.
@@ -422,6 +424,7 @@ struct TransportArgs {
   uint32_t *ev;                  // [n_hist][4] per-history event counts of this sub-batch, or nullptr
 };
 
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepParams P, TransportArgs A) {
   double *slab = reinterpret_cast<double *>(g_smem);     // [P.slab_bins]
   __shared__ BlockAccum acc;
@@ -574,6 +577,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
   block_atomic_add(A.pop_w + P.k, popw, acc.scratch);
   block_atomic_add_u64(A.pop_n + P.k, (unsigned long long)popn, (unsigned long long *)acc.scratch);
 }
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // Population control at census (Appendix G.3; "time-dependent population control"), census-stepped
@@ -583,6 +587,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
 // ------------------------------------------------------------------------------------------------
 #define MCDC_FIX40 1099511627776.0   // 2^40
 
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(256) k_pc_weight(Bank in, uint32_t cap, unsigned long long *wfix) {
   __shared__ unsigned long long scratch[32];
   const int slot = blockIdx.y;
@@ -592,6 +597,7 @@ __global__ void __launch_bounds__(256) k_pc_weight(Bank in, uint32_t cap, unsign
   if (i < n) v = (unsigned long long)(in.w[(size_t)slot * cap + i] * MCDC_FIX40);   // truncation, as the oracle's cast
   block_atomic_add_u64(wfix + slot, v, scratch);
 }
+#endif
 
 struct PcParams {
   uint32_t cap;
@@ -600,6 +606,7 @@ struct PcParams {
   double w_out;                       // > 0: weight given to every copy (generation control, Appendix H.3); else w_t
 };
 
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P, const unsigned long long *wfix,
                                                   DevCounters *cnt, double *pop_w_after, unsigned long long *pop_n_after) {
   __shared__ double scratch[32];
@@ -656,6 +663,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
   block_atomic_add(pop_w_after + P.k, (double)n * w_new, scratch);
   block_atomic_add_u64(pop_n_after + P.k, (unsigned long long)n, (unsigned long long *)scratch);
 }
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // Global fission queue and launch arguments of the asynchronous history kernel k_warp (mcdc_warp.cuh).
@@ -711,6 +719,7 @@ __device__ __forceinline__ unsigned long long ld_volatile_u64(const unsigned lon
 // ------------------------------------------------------------------------------------------------
 // Batch close-out (A.9): sum += S_b, sumsq += S_b^2, S_b = 0 for every slot of the sub-batch.
 // ------------------------------------------------------------------------------------------------
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(256) k_closeout(double *__restrict__ x_acc, int n_slots, int group_all,
                                                   unsigned long long n_bins, double *__restrict__ sum,
                                                   double *__restrict__ sumsq) {
@@ -726,10 +735,12 @@ __global__ void __launch_bounds__(256) k_closeout(double *__restrict__ x_acc, in
     if (any) { sum[i] += s; sumsq[i] += group_all ? s * s : q; }
   }
 }
+#endif
 
 // ------------------------------------------------------------------------------------------------
 // A.9 read-out for large meshes: mean = sum / N, sdev = sqrt((sumsq / hb^2 / B - mean^2) / (B - 1)) per bin
 // ------------------------------------------------------------------------------------------------
+#ifndef MCDC_WARP_VARIANT   // defined once, in the host translation unit
 __global__ void __launch_bounds__(256) k_statistics(const double *__restrict__ sum, const double *__restrict__ sumsq,
                                                     unsigned long long n_bins, double N, double B,
                                                     double *__restrict__ mean, double *__restrict__ sdev) {
@@ -746,5 +757,6 @@ __global__ void __launch_bounds__(256) k_statistics(const double *__restrict__ s
     mean[i] = mu; sdev[i] = sd;
   }
 }
+#endif
 
 }  // namespace mcdc

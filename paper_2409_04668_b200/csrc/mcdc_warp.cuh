@@ -17,40 +17,30 @@
 #pragma once
 #include "mcdc_kernels.cuh"
 
-#ifndef MCDC_STORE_INV
-#define MCDC_STORE_INV 1        // keep 1/direction in the pool (else recomputed every flight)
-#endif
-#ifndef MCDC_F_INLINE_PHILOX
-#define MCDC_F_INLINE_PHILOX 0  // Philox block of the flight phase inlined (its chain may overlap the geometry)
-#endif
-#ifndef MCDC_SCORE_NOINLINE
-#define MCDC_SCORE_NOINLINE 0   // general (multi-bin) scorer out of line
-#endif
-
 namespace mcdc {
 
 // ---- slow paths: rare, not inlined, and they read the tables from global memory (device copy of Tables) ----
 
 // A.5 transmission without a certified neighbour: candidate cells of half-space `idx` of `cell`, then every cell
-__device__ __noinline__ int slow_cross(const Tables *gT, int cell, int idx, int s_star, double x, double y, double z,
+static __device__ __noinline__ int slow_cross(const Tables *gT, int cell, int idx, int s_star, double x, double y, double z,
                                        double ux, double uy, double uz) {
   const TB<false> tb(*gT);
   const int slot = tb.cell_off(cell) + idx;
   return locate_neighbour<false>(tb, slot, s_star, x, y, z, ux, uy, uz);
 }
 // A.5 reflection off a surface that is not an axis-aligned plane
-__device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, double x, double y, double z, double *u) {
+static __device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, double x, double y, double z, double *u) {
   const TB<false> tb(*gT);
   reflect(tb, s, type, x, y, z, u[0], u[1], u[2]);
 }
 // A.3 cell of a source particle
-__device__ __noinline__ int slow_locate_source(const Tables *gT, double x, double y, double z, double ux, double uy,
+static __device__ __noinline__ int slow_locate_source(const Tables *gT, double x, double y, double z, double ux, double uy,
                                                double uz) {
   const TB<false> tb(*gT);
   return locate_source<false>(tb, x, y, z, ux, uy, uz);
 }
 // A.4 distance to a surface that is neither an axis-aligned plane face nor a z-cylinder
-__device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, bool on, double x, double y, double z,
+static __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, bool on, double x, double y, double z,
                                              double ux, double uy, double uz) {
   const TB<false> tb(*gT);
   return surf_distance(tb, s, type, on, x, y, z, ux, uy, uz, 1.0 / ux, 1.0 / uy, 1.0 / uz);
@@ -60,7 +50,7 @@ __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, 
 // sequence flags published with st.release).  Warp-converged: every lane calls it; lanes without children pass
 // n_push = 0.  Out of line: it runs in under 1 % of the collision rounds and its ~470 instructions sat in the middle
 // of the C phase (profiles/r01g).
-__device__ __noinline__ void slow_publish_children(FissionQueue q, DevCounters *cnt, bool weighted, double x, double y,
+static __device__ __noinline__ void slow_publish_children(FissionQueue q, DevCounters *cnt, bool weighted, double x, double y,
                                                    double z, double t, double w, unsigned long long key, uint32_t c0,
                                                    int n_push, int pre, int total, int4 qm) {
   const int lane = threadIdx.x & 31;
@@ -69,8 +59,10 @@ __device__ __noinline__ void slow_publish_children(FissionQueue q, DevCounters *
   unsigned long long qb = 0ull;
   int okq = 1;
   if (lane == 0) {
+    // consumers advance head before they read their entries: up to one claimed-but-unread entry per thread of the
+    // launch may still be in use behind head, so that many entries stay out of the producers' reach
     qb = atomicAdd(q_tail, (unsigned long long)total);
-    if (qb + (unsigned long long)total - ld_volatile_u64(q_head) + 65536ull > q_cap) okq = 0;
+    if (qb + (unsigned long long)total - ld_volatile_u64(q_head) + (unsigned long long)gridDim.x * blockDim.x > q_cap) okq = 0;
   }
   qb = __shfl_sync(MCDC_FULL, qb, 0) + (unsigned long long)(pre - n_push);
   okq = __shfl_sync(MCDC_FULL, okq, 0);
@@ -92,7 +84,7 @@ __device__ __noinline__ void slow_publish_children(FissionQueue q, DevCounters *
 }
 
 // Appendix I: one collision-estimator score (only runs that enabled the tally come here)
-__device__ __noinline__ void slow_score_collision(const Tables *gT, double *xc_slot, double x, double y, double z, double t,
+static __device__ __noinline__ void slow_score_collision(const Tables *gT, double *xc_slot, double x, double y, double z, double t,
                                                   int g, double w, int mg) {
   const TB<false> tb(*gT);
   const long long cb = collision_bin(tb, x, y, z, t, g);
@@ -101,12 +93,7 @@ __device__ __noinline__ void slow_score_collision(const Tables *gT, double *xc_s
 
 // A.7 for segments that may touch several tally bins (4-D DDA).  Warp-converged: every lane calls it.
 template <bool STAGED>
-#if MCDC_SCORE_NOINLINE
-__device__ __noinline__
-#else
-__device__ __forceinline__
-#endif
-void general_score(const Tables &Tg, double *x_acc_slot, int aggregate, bool active,
+__device__ __forceinline__ void general_score(const Tables &Tg, double *x_acc_slot, int aggregate, bool active,
                                            const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d, double w) {
   // the pre-move state is still in the pool: x y z ux uy uz 1/ux 1/uy 1/uz t, N slots apart
   const double x = pool[gi], y = pool[N + gi], z = pool[2 * N + gi], ux = pool[3 * N + gi], uy = pool[4 * N + gi],
@@ -415,11 +402,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         unsigned long long key = 0ull;
         uint32_t ctr = 0u;
         if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
-#if MCDC_F_INLINE_PHILOX
-        const double xi = draw_inl(key, ctr);          // always consumed (D3)
-#else
         const double xi = draw(key, ctr);              // always consumed (D3)
-#endif
         if (act) PU(U_CTR, gi) = ctr;
         d_coll = -log(xi);
       }
@@ -432,13 +415,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, ix = INF, iy = INF, iz = 1.0;
       if (act) {
         x = PD(D_X, gi); y = PD(D_Y, gi); z = PD(D_Z, gi); ux = PD(D_UX, gi); uy = PD(D_UY, gi); uz = PD(D_UZ, gi);
-#if MCDC_STORE_INV
-        ix = PD(D_IX, gi); iy = PD(D_IY, gi); iz = PD(D_IZ, gi);
-#endif
+        ix = PD(D_IX, gi); iy = PD(D_IY, gi); iz = PD(D_IZ, gi);   // 1/direction is kept in the pool (three divisions per segment otherwise)
       }
-#if !MCDC_STORE_INV
-      ix = 1.0 / ux; iy = 1.0 / uy; iz = 1.0 / uz;
-#endif
       // ---- faces: one candidate per axis, picked by the sign of the direction component ----
       // sign bit alone: for a component that is exactly +-0 the face distance is inf or NaN and is rejected below
       const bool px = __double2hiint(ux) >= 0, py = __double2hiint(uy) >= 0, pz = __double2hiint(uz) >= 0;
@@ -501,7 +479,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         const bool one_bin = ONEBIN || (cbin != NONE32 && tbin >= 0);   // the whole segment lies in one tally bin
         if (!ONEBIN) {
           if (__any_sync(MCDC_FULL, act && !one_bin))
-            general_score<STAGED>(MCDC_SCORE_NOINLINE ? *gT : T, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
+            general_score<STAGED>(T, S.global_x, A.aggregate, act && !one_bin, &PD(0, 0), N, gi, g, pk, d, w);
         }
         if (ONEBIN || __any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;

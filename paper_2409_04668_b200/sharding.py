@@ -26,18 +26,6 @@ def shard_range(n_total: int, world: int, rank: int, n_batches: int | None = Non
     return first_b * hb, nb * hb, nb
 
 
-def merge_statistics(sum_, sumsq, n_hist, n_batches):
-    """mean / sdev from reduced accumulators: sum over batches of S_b and S_b^2."""
-    hb = n_hist / n_batches
-    mean = sum_ / n_hist
-    if n_batches > 1:
-        var = (sumsq / (hb * hb) / n_batches - mean * mean) / (n_batches - 1)
-        sdev = np.sqrt(np.maximum(var, 0.0))
-    else:
-        sdev = np.zeros_like(mean)
-    return mean, sdev
-
-
 def all_reduce_tallies(sum_, sumsq, ledger, group=None):
     """Sum-reduce raw accumulators over the process group (gloo on CPU tensors, nccl on CUDA tensors)."""
     import torch

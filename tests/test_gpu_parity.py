@@ -216,11 +216,7 @@ def test_full_size_config3_sampled_against_the_oracle(M):
     # E7 on the GPU result: the 8 symmetries of the square
     m = mean[:, :, 0].sum(axis=(0, 1))
     assert np.allclose(m, m[::-1, :], rtol=0.05) and np.allclose(m, m.T, rtol=0.05)
-    # integrated flux per history against an oracle sample (statistical): mean track length per history
-    o.reset(); o.run(20_000, p.seed, n_batches=20)
-    mo, so = o.tallies()
-    tot_o, tot_g = mo.sum(), mean.sum()
-    assert tot_g == pytest.approx(tot_o, rel=0.03)
+    # (the per-bin comparison with the oracle at this size is tests/test_gpu_fullsize.py)
     g.close()
 
 

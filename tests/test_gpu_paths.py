@@ -1,0 +1,175 @@
+"""GPU parity on the paths the history kernel takes only under pressure, forced with the documented test knobs of
+mcdc_run_opts (include/mcdc.h): 32-slot pools send every fission child beyond the first through the global ring
+queue in HBM; debug_stage_tables = -1 runs the instantiations that read the tables through L1/L2.  Same bars as
+tests/test_gpu_parity.py: per-history event counts equal for >= 99.999 % of histories, every bin 1e-9 (config 0) /
+1e-7, exact ledger and census populations.  Also: a batch split into uneven pieces."""
+import numpy as np
+import pytest
+
+pytestmark = [pytest.mark.gpu, pytest.mark.timeout(600)]
+
+LEDGER = ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost")
+COUNTS = ("histories", "segments", "collisions", "surf_hits", "census_events", "children", "lost_n", "batches")
+
+
+@pytest.fixture(scope="module")
+def M():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_2409_04668_b200 as M
+    M.lib()
+    return M
+
+
+def _oracle(p, record=True, **tech):
+    from oracle import Oracle
+    o = Oracle(p)
+    if tech:
+        o.set_technique(**tech)
+    o.run(p.n_histories, p.seed, n_batches=p.n_batches, record_history_events=record)
+    return o
+
+
+def _compare(o, g, rtol):
+    co, cg = o.counters(), g.counters()
+    for k in LEDGER + COUNTS:
+        assert cg[k] == co[k], (k, cg[k], co[k])
+    assert cg["source"] + cg["production"] == cg["capture"] + cg["fission_abs"] + cg["leak"] + cg["census_final"] + cg["lost"]
+    eo, eg = o.history_events(), g.history_events()
+    assert np.all(eo == eg, axis=1).mean() >= 0.99999
+    mo, so = o.tallies(); mg, sg = g.tallies()
+    scale = np.abs(mo).max()
+    assert np.all(np.abs(mg - mo) <= rtol * np.maximum(np.abs(mo), np.abs(mg)) + 1e-13 * scale)
+    assert np.allclose(sg, so, rtol=1e-6, atol=1e-12 * scale)
+    err = np.sqrt(so ** 2 + sg ** 2) + 1e-12 * scale
+    assert np.all(np.abs(mg - mo) <= 4.0 * err) and mg.sum() == pytest.approx(mo.sum(), rel=1e-3)
+    wo, no = o.census(); wg, ng = g.census()
+    assert np.array_equal(no, ng) and np.allclose(wo, wg, rtol=1e-14)
+
+
+CASES = [("config0", 100_000, 20, 1e-9), ("config3", 100_000, 20, 1e-7), ("config1", 100_000, 10, 1e-7),
+         ("config2", 100_000, 10, 1e-7)]
+
+
+@pytest.mark.parametrize("name,N,B,rtol", CASES)
+def test_small_pools_send_fission_children_through_the_global_queue(M, name, N, B, rtol):
+    from workloads import configs as W
+    p = W.get_config(name, n_histories=N, n_batches=B)
+    o = _oracle(p)
+    g = M.Problem(p)
+    g.run(record_history_events=True, debug_pool_slots=32)
+    _compare(o, g, rtol)
+    if name in ("config0", "config3"):
+        # the knob did what it is for: with 32-slot pools the run cannot have held its children in the pools.  The
+        # queue cursors are the evidence: mcdc_counters has no field for them, so run the default pool as the control
+        # and require identical results -- queue or pool, the trajectories are the same
+        ev_q = g.history_events()
+        g.reset(); g.run(record_history_events=True)
+        assert np.array_equal(g.history_events(), ev_q)
+    g.close()
+
+
+@pytest.mark.parametrize("name,N,B,rtol", CASES + [("stress", 120_000, 12, 1e-9)])
+@pytest.mark.parametrize("pool", [0, 32])
+def test_unstaged_tables_instantiation_matches_the_oracle(M, name, N, B, rtol, pool):
+    from workloads import configs as W
+    p = W.stress_geometry(n_histories=N, n_batches=B) if name == "stress" else W.get_config(name, n_histories=N, n_batches=B)
+    o = _oracle(p)
+    g = M.Problem(p)
+    g.run(record_history_events=True, debug_stage_tables=-1, debug_pool_slots=pool)
+    _compare(o, g, rtol)
+    g.close()
+
+
+def test_weighted_kernel_with_small_pools_and_unstaged_tables(M):
+    """The weighted instantiation carries the weight through the queue (q.w): implicit capture + roulette, collision
+    tally on, forced queue, both table modes."""
+    from oracle import Oracle
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=60_000, n_batches=12)
+    tech = dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0)
+    o = Oracle(p); o.set_technique(**tech); o.enable_collision_tally(True)
+    o.run(p.n_histories, p.seed, n_batches=p.n_batches, record_history_events=True)
+    mo, _ = o.tallies(); mco, _ = o.collision_tallies()
+    for stage in (0, -1):
+        g = M.Problem(p); g.set_technique(**tech); g.enable_collision_tally(True)
+        g.run(record_history_events=True, debug_pool_slots=32, debug_stage_tables=stage)
+        co, cg = o.counters(), g.counters()
+        for k in COUNTS:
+            assert cg[k] == co[k], (k, cg[k], co[k])
+        for k in LEDGER + ("vr_gain", "vr_loss"):
+            assert cg[k] == pytest.approx(co[k], rel=1e-10), k
+        assert np.all(o.history_events() == g.history_events(), axis=1).mean() >= 0.99999
+        mg, _ = g.tallies(); mcg, _ = g.collision_tallies()
+        assert np.allclose(mg, mo, rtol=1e-7, atol=1e-13 * np.abs(mo).max())
+        assert np.allclose(mcg, mco, rtol=1e-7, atol=1e-13 * np.abs(mco).max())
+        g.close()
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_uneven_pieces_of_a_split_batch_are_all_closed_out(M, scheduler):
+    """hb = 1005 with 1000 histories per sub-batch and 4 slots: piece 1 scores into 4 slots (250 each), piece 2 (5
+    histories) into 3.  The close-out must cover every slot any piece of the batch used."""
+    from oracle import Oracle
+    from workloads import configs as W
+    p = W.config1_slab(n_histories=3 * 1005, n_batches=3)
+    o = Oracle(p); o.run(p.n_histories, p.seed, n_batches=3, record_history_events=True)
+    so, qo = o.tally_sums()
+    for nh, ns in ((1000, 4), (1000, 3), (400, 7)):
+        g = M.Problem(p, max_histories_per_subbatch=nh, max_batches_in_flight=ns)
+        g.run(record_history_events=True, scheduler=scheduler)
+        s, q = g.tally_sums()
+        assert np.allclose(s, so, rtol=1e-12, atol=1e-14 * np.abs(so).max()), (nh, ns)
+        assert np.allclose(q, qo, rtol=1e-11, atol=1e-14 * np.abs(qo).max()), (nh, ns)
+        assert np.array_equal(g.history_events(), o.history_events())
+        # nothing may be left behind in an accumulator: a second, identical run doubles the sums exactly like the oracle's
+        g.run(record_history_events=False, scheduler=scheduler)
+        s2, _ = g.tally_sums()
+        assert np.allclose(s2, 2.0 * so, rtol=1e-12, atol=1e-14 * np.abs(so).max()), (nh, ns)
+        g.close()
+
+
+def test_state_vector_carries_the_collision_tally(M):
+    """Two handles run the two halves of a job with the collision-estimator tally on; their exported state vectors are
+    added and imported into a third handle, which must answer like the single run (tallies AND collision tallies)."""
+    import torch
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=40_000, n_batches=8)
+    whole = M.Problem(p); whole.enable_collision_tally(True); whole.run()
+    mw, sw = whole.tallies(); mcw, scw = whole.collision_tallies()
+    n0 = whole.state_size()
+    assert n0 == 4 * p.n_bins + 2 * p.n_census + 20
+    halves = []
+    for first, n, nb in ((0, 20_000, 4), (20_000, 20_000, 4)):
+        h = M.Problem(p); h.enable_collision_tally(True)
+        h.run(n, p.seed, nb, first_history_id=first)
+        for dev in ("cuda:0", "cpu"):
+            buf = torch.empty(n0, dtype=torch.float64, device=dev)
+            h.state_export(buf)
+            halves.append((dev, buf.cpu()))
+        h.close()
+    dev_sum = halves[0][1] + halves[2][1]
+    assert torch.equal(halves[0][1], halves[1][1]) and torch.equal(halves[2][1], halves[3][1])   # device and host exports agree
+    t = M.Problem(p); t.enable_collision_tally(True)
+    t.state_import(dev_sum.to("cuda:0"))
+    mt, st = t.tallies(); mct, sct = t.collision_tallies()
+    assert np.allclose(mt, mw, rtol=1e-12, atol=0) and np.allclose(st, sw, rtol=1e-8, atol=1e-16)
+    assert np.allclose(mct, mcw, rtol=1e-12, atol=0) and np.allclose(sct, scw, rtol=1e-8, atol=1e-16)
+    assert t.counters()["histories"] == 40_000 and t.counters()["collisions"] == whole.counters()["collisions"]
+    # a handle without the tally refuses the longer vector instead of mis-reading it
+    u = M.Problem(p)
+    with pytest.raises(M.McdcError) as e:
+        u.state_import(dev_sum)
+    assert e.value.code == -4
+    for x in (whole, t, u):
+        x.close()
+
+
+def test_eigenvalue_mode_refuses_more_than_one_census(M):
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=2000, n_batches=1)        # 20 census times
+    g = M.Problem(p)
+    with pytest.raises(M.McdcError) as e:
+        g.run_eigenvalue(2000, p.seed, 1, 2)
+    assert e.value.code == -1
+    g.close()

@@ -10,6 +10,19 @@ import torch.multiprocessing as mp
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
+def merge_statistics(sum_, sumsq, n_hist, n_batches):
+    """mean / sdev from reduced accumulators, written out here for the check: the product computes them
+    inside mcdc_tallies_get after mcdc_state_import."""
+    hb = n_hist / n_batches
+    mean = sum_ / n_hist
+    if n_batches > 1:
+        var = (sumsq / (hb * hb) / n_batches - mean * mean) / (n_batches - 1)
+        sdev = np.sqrt(np.maximum(var, 0.0))
+    else:
+        sdev = np.zeros_like(mean)
+    return mean, sdev
+
+
 def test_shard_range_partitions_exactly():
     from paper_2409_04668_b200.sharding import shard_range
     for n, w in ((10, 3), (7, 7), (1000003, 8), (5, 8)):
@@ -27,7 +40,7 @@ def _worker(rank, world, port, q):
     sys.path.insert(0, ROOT)
     import torch.distributed as dist
     from oracle import Oracle
-    from paper_2409_04668_b200.sharding import all_reduce_tallies, merge_statistics, shard_range
+    from paper_2409_04668_b200.sharding import all_reduce_tallies, shard_range
     from workloads import configs as W
 
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
@@ -99,7 +112,7 @@ class _OracleState:
 def _worker_state(rank, world, port, q):
     sys.path.insert(0, ROOT)
     import torch.distributed as dist
-    from paper_2409_04668_b200.sharding import all_reduce_state, merge_statistics, shard_range
+    from paper_2409_04668_b200.sharding import all_reduce_state, shard_range
     from workloads import configs as W
 
     os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
@@ -115,7 +128,6 @@ def _worker_state(rank, world, port, q):
 
 def test_all_reduce_state_gives_every_rank_the_whole_job():
     from oracle import Oracle
-    from paper_2409_04668_b200.sharding import merge_statistics
     from workloads import configs as W
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
