@@ -256,8 +256,9 @@ def bench_gpu(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    dbg = dict(debug_pool_slots=args.debug_pool_slots, debug_stage_tables=args.debug_stage_tables)
     for _ in range(args.warmup):
-        g.reset(); g.run(n_hist, p.seed, n_b, first_history_id=first_id)
+        g.reset(); g.run(n_hist, p.seed, n_b, first_history_id=first_id, **dbg)
     barrier()
     sampler = make_sampler(local)
     if rank == 0:
@@ -270,7 +271,7 @@ def bench_gpu(args):
     t_wall0 = time.time()
     ev0.record()
     for _ in range(args.steps):
-        g.run(n_hist, p.seed, n_b, first_history_id=first_id)
+        g.run(n_hist, p.seed, n_b, first_history_id=first_id, **dbg)
         ms_tr += g.counters()["ms_transport"]
     c = g.counters()                                      # this rank's own counts
     if world > 1:
@@ -441,6 +442,8 @@ def main():
     ap.add_argument("--technique", default="analog", choices=sorted(TECHNIQUES),
                     help="variance-reduction variant of the workload (DESIGN.md Appendix G); the headline is analog")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--debug-pool-slots", type=int, default=0, help="mcdc_run_opts.debug_pool_slots (test knob; 0 = automatic)")
+    ap.add_argument("--debug-stage-tables", type=int, default=0, help="mcdc_run_opts.debug_stage_tables (test knob; 0 = automatic)")
     ap.add_argument("--sweep", action="store_true", help="also run the config-4 batch-size sweep (adds a 'sweep' key)")
     ap.add_argument("--sweep-max", type=float, default=1e9)
     ap.add_argument("--eigenvalue", action="store_true", help="also time the k-eigenvalue mode (adds an 'eigenvalue' key)")

@@ -104,7 +104,7 @@ struct mcdc_problem {
   int n_sm = 148, blocks_per_sm = 1, blocks_per_sm_hist = 1;
   bool stage_tables = false;
   int hist_threads = 512;
-  uint32_t pool_slots = 0;
+  uint32_t pool_slots = 0, pool_reserve = 0;
   size_t pool_smem = 0;
   size_t n_cert = 0, n_transm = 0, n_one_bin = 0;   // certified / all transmission half-spaces; cells in one tally bin
   // CUDA events owned by the handle (created on first use, destroyed with it): run brackets, one pair per
@@ -1081,12 +1081,18 @@ cudaError_t warp_set_smem(bool staged, bool record, int variant, int score, int 
 // in-warp merge of equal tally addresses pays only on tiny meshes (profiles/r01d)
 int problem_aggregate(const mcdc_problem *p) { return ((size_t)p->G * p->n_spatial <= 64) ? 1 : 0; }
 
+#ifndef MCDC_POOL_RESERVE
+#define MCDC_POOL_RESERVE 8u
+#endif
 // debug_pool_slots / debug_stage_tables: the documented test knobs of mcdc_run_opts (0 = automatic choice)
 int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_pool_slots = 0, int debug_stage_tables = 0) {
   const bool weighted = variant != KW_ANALOG;
   int dev = 0, max_optin = 0;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+#ifdef MCDC_WARP_SMEM_CAP
+  max_optin = std::min(max_optin, MCDC_WARP_SMEM_CAP);
+#endif
   const int nt = MCDC_WARP_THREADS;
   const int nw = nt / 32;
   const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8, 16) : 0);
@@ -1107,6 +1113,8 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_p
   if (debug_pool_slots) W = std::min<long>(W, std::max<long>(32, (long)debug_pool_slots / 8 * 8));
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
+  // slots a refill leaves free for fission children (mcdc_warp.cuh); the debug knob asks for pools that overflow
+  p->pool_reserve = debug_pool_slots ? 0u : MCDC_POOL_RESERVE;
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
   cudaError_t e1 = warp_set_smem(staged, record, variant, score_mode(p->tab, problem_aggregate(p)), nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
@@ -1158,7 +1166,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
-  ha.pool_slots = p->pool_slots;
+  ha.pool_slots = p->pool_slots; ha.pool_reserve = p->pool_reserve;
   const size_t smem = p->pool_smem;
   const int nt = p->hist_threads;
   // one block per SM; fewer only when the sub-batch cannot give every warp one full round of 32 histories (small
@@ -1208,7 +1216,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   ha.aggregate = problem_aggregate(p);
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
-  ha.pool_slots = p->pool_slots;
+  ha.pool_slots = p->pool_slots; ha.pool_reserve = p->pool_reserve;
   const int nt = p->hist_threads;
   const uint64_t per_block = (uint64_t)p->pool_slots * (nt / 32);
   const int grid_src = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, ((uint64_t)sb.n_hist + per_block - 1) / per_block));
@@ -1412,7 +1420,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
   ha.aggregate = problem_aggregate(p);
   const bool staged = p->stage_tables;
   ha.smem_tables = staged ? (uint32_t)align_up(p->tab.hot_bytes, 16) : 0u;
-  ha.pool_slots = p->pool_slots;
+  ha.pool_slots = p->pool_slots; ha.pool_reserve = p->pool_reserve;
   const int nt = p->hist_threads;
   const uint64_t per_block = (uint64_t)p->pool_slots * (nt / 32);
   ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)N / ((uint64_t)p->n_sm * (nt / 32) * 8)));

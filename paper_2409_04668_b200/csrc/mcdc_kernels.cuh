@@ -693,6 +693,7 @@ struct HistoryArgs {
   int aggregate;
   uint32_t smem_tables;           // bytes of dynamic shared memory in front of the census arrays
   uint32_t pool_slots;            // particles held in each warp's shared-memory pool
+  uint32_t pool_reserve;          // slots a refill leaves free for the children of fissions
   // census-step mode of k_warp<WEIGHTED> (population control, Appendix G.3): one launch transports one census step.
   // Particles come from the live bank `in` (survivors of the control at the previous census) and from the source
   // histories born in this step; a particle that reaches the census time is parked in `census_out` instead of going on.

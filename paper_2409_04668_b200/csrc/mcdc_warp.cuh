@@ -121,10 +121,11 @@ __device__ __forceinline__ bool pos_finite(double v) {
 
 __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
 
-// bytes of shared memory per pool slot: x y z ux uy uz 1/ux 1/uy 1/uz t (10 x f64), key, ctr, cell|last, meta, 3 stack entries
+// bytes of shared memory per pool slot: x y z ux uy uz 1/ux 1/uy 1/uz t (10 x f64), key, the unused half of the last
+// Philox block (u64), ctr, cell|last, meta, 3 stack entries
 // (+ the weight, one more f64, when a technique of Appendix G makes weights differ from 1)
 __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool weighted) {
-  return (weighted ? 11 : 10) * 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
+  return (weighted ? 11 : 10) * 8 + 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
 }
 
 struct WarpShared {                // block-wide totals (static shared memory)
@@ -141,8 +142,13 @@ struct WarpShared {                // block-wide totals (static shared memory)
 // such problems never execute, in the middle of the flight phase: leaving it out is worth 8 % on config 3 (r01f).
 // SCORE: 0 = general (DDA scorer compiled in, one-bin shortcut and in-warp merge chosen at run time); 1 = ONEBIN, one RED
 // per score; 2 = ONEBIN on a tiny mesh, equal addresses merged inside the warp before the RED.
+#ifdef MCDC_WARP_MAXNREG
+#define MCDC_WARP_BOUNDS __maxnreg__(MCDC_WARP_MAXNREG)
+#else
+#define MCDC_WARP_BOUNDS __launch_bounds__(NT, 1)
+#endif
 template <bool STAGED, bool RECORD, int VARIANT, int SCORE, int NT>
-__global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
+__global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   constexpr bool ONEBIN = SCORE != 0;
   constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
@@ -156,6 +162,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   // ---- carve the dynamic shared memory: [staged tables][census populations][pool arrays][stacks] ----
   // One offset and the stride N address every array (pointers would cost two registers each):
   //   f64  x y z ux uy uz 1/ux 1/uy 1/uz t  -> PD(k, slot), k = 0..9        u64  key       -> PK(slot)
+  //   u64  second half of Philox block ctr >> 1, valid while ctr is odd (Appendix B: "may cache the half-block") -> PC(slot)
   //   u32  ctr, cell|last<<16, meta = g | census index<<8 | batch slot<<20, [history id]  -> PU(k, slot)
   //   u8   stacks F, C, FREE -> PL(k, position)
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
@@ -164,8 +171,9 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
                             (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 + 15) / 16 * 16) : 0u);
 #define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + ((uint32_t)(k) * N + (slot)) * 8u))
 #define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (ND * N + (slot)) * 8u))
-#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + (ND + 1u) * 8u * N + ((uint32_t)(k) * N + (slot)) * 4u))
-#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + ((ND + 1u) * 8u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
+#define PC(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + ((ND + 1u) * N + (slot)) * 8u))
+#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + (ND + 2u) * 8u * N + ((uint32_t)(k) * N + (slot)) * 4u))
+#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + ((ND + 2u) * 8u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
   enum { D_X = 0, D_Y, D_Z, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_T, D_W, U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
 
   if (STAGED) {
@@ -184,7 +192,6 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
   __syncthreads();
 
   unsigned long long *q_head = A.q.head_tail, *q_tail = A.q.head_tail + 1;
-  const unsigned long long q_cap = (unsigned long long)A.q.mask + 1ull;
   const Tables *gT = T.self_dev;
   const int G = T.G;
   const long long n_spatial = (long long)T.mesh_n[0] * T.mesh_n[1] * T.mesh_n[2];
@@ -202,10 +209,15 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
 #define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
   for (;;) {
+    // A refill leaves `pool_reserve` slots free: fission children are born into the parent's pool, and a pool that
+    // refills to the brim sends them through the global queue in HBM instead (measured: 16 warps x 88 slots filled
+    // completely ran 1.7x slower than 104 slots, 64 slots 6x slower -- profiles/r02b).  A refill that cannot fill
+    // half a warp waits while the pool has other work.
+    const uint32_t room = nFree > A.pool_reserve ? nFree - A.pool_reserve : 0u;
     int phase;                                         // 0 = R, 1 = F, 2 = C
     if (nF >= 32u) phase = 1;
     else if (nC >= 32u) phase = 2;
-    else if (nFree > 0u && dry == 0u) phase = 0;
+    else if (room >= 16u && dry == 0u) phase = 0;
     else if (nF > 0u && nF >= nC) phase = 1;
     else if (nC > 0u) phase = 2;
     else phase = 0;
@@ -213,7 +225,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
 
     if (phase == 0) {
       // =============== R: acquire work for up to 32 free slots, initialise the new particles (A.3, A.6) ===============
-      const uint32_t want = min(32u, nFree);
+      const uint32_t want = min(32u, max(room, 1u));   // (room = 0 only with an empty pool smaller than the reserve)
       if (step_mode && !bank_done) {
         // ---- census-step mode: particles of the live bank first (full records: nothing is sampled here) ----
         uint32_t base = 0u, cnt = 0u;
@@ -227,6 +239,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         bank_probes = 0u;
         const uint32_t nb = min(want, cnt - base);
         const bool actb = (uint32_t)lane < nb;
+        unsigned long long bkey = 0ull;
+        uint32_t bctr = 0u, bgi = 0u;
         if (actb && gen_mode) {                          // a birth record: group and direction are sampled in the C phase
           const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
@@ -238,6 +252,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           PU(U_META, gi) = 255u | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
           if (RECORD) PU(U_HID, gi) = A.in.hid[j];
           PL(L_C, lb + nC + (uint32_t)lane) = (uint8_t)i;
+          bkey = A.in.key[j]; bctr = (uint32_t)m.z; bgi = gi;
         } else if (actb) {
           const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
@@ -252,6 +267,12 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           PU(U_META, gi) = (uint32_t)m.w | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
           if (RECORD) PU(U_HID, gi) = A.in.hid[j];
           PL(L_F, lb + nF + (uint32_t)lane) = (uint8_t)i;
+          bkey = A.in.key[j]; bctr = (uint32_t)m.z; bgi = gi;
+        }
+        // a record that comes back with an odd counter needs the second half of its current block again
+        if (__any_sync(MCDC_FULL, (bctr & 1u) != 0u)) {
+          const ulonglong2 blk = philox_block(bkey, bctr >> 1);
+          if (bctr & 1u) PC(bgi) = blk.y;
         }
         nFree -= nb;
         if (gen_mode) nC += nb; else nF += nb;
@@ -333,9 +354,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         hid = src_base + (uint32_t)lane;
         slot = hid / A.hb;
         key = mix64(A.seed_mixed ^ (A.first_history + (unsigned long long)hid));
-        double xi_x, xi_y, xi_z, xi_t;
-        draw2(key, ctr, xi_x, xi_y);
-        draw2(key, ctr, xi_z, xi_t);
+        // xi_x, xi_y = block 0, xi_z, xi_t = block 1
+        const ulonglong2 b0 = philox_block(key, 0u), b1 = philox_block(key, 1u);
+        const double xi_x = u64_to_unit(b0.x), xi_y = u64_to_unit(b0.y), xi_z = u64_to_unit(b1.x), xi_t = u64_to_unit(b1.y);
+        ctr = 4u;
         x = T.src_lo[0] + xi_x * (T.src_hi[0] - T.src_lo[0]);
         y = T.src_lo[1] + xi_y * (T.src_hi[1] - T.src_lo[1]);
         z = T.src_lo[2] + xi_z * (T.src_hi[2] - T.src_lo[2]);
@@ -343,8 +365,12 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         pk = census_index(tb, t);
         if (step_mode && !A.step_single && pk != A.step_k) { skip = true; ok = false; }
       }
-      // group: chi of the fission-site material (child) or the source pdf; then the direction
-      const double xi_g = draw(key, ctr);
+      // group: chi of the fission-site material (child) or the source pdf; then the direction.  The counter is even here
+      // (4 after a source position, 0 for a child): xi_g, xi_mu = one block, xi_phi = the first half of the next, whose
+      // second half is kept for the particle's next draw
+      const ulonglong2 ba = philox_block(key, ctr >> 1), bb = philox_block(key, (ctr >> 1) + 1u);
+      const double xi_g = u64_to_unit(ba.x);
+      unsigned long long half = ba.y;                  // second half of the block the next draw falls in
       int g;
       if (is_src) g = sample_cdf([&](int q) { return tb.src_cdf(q); }, G, T.src_last, xi_g);
       else {
@@ -352,11 +378,10 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         g = sample_cdf([&](int q) { return tb.cdf_chi(mat * G + q); }, G, tb.last_chi(mat), xi_g);
       }
       double ux, uy, uz;
-      if (is_src && T.src_dir_mode != 0) { ux = T.src_dir[0]; uy = T.src_dir[1]; uz = T.src_dir[2]; }
+      if (is_src && T.src_dir_mode != 0) { ux = T.src_dir[0]; uy = T.src_dir[1]; uz = T.src_dir[2]; ctr += 1u; }
       else {
-        double xi_mu, xi_phi;
-        draw2(key, ctr, xi_mu, xi_phi);
-        isotropic(xi_mu, xi_phi, ux, uy, uz);
+        isotropic(u64_to_unit(ba.y), u64_to_unit(bb.x), ux, uy, uz);
+        ctr += 3u; half = bb.y;
       }
       if (is_src) {
         // (a point source proved to lie strictly inside one cell at create time skips the search: warp-uniform)
@@ -375,15 +400,14 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz; PD(D_T, gi) = t;
         PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
         if (WEIGHTED) PD(D_W, gi) = w;
-        PK(gi) = key; PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
+        PK(gi) = key; PC(gi) = half; PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
         PU(U_META, gi) = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
         if (RECORD) PU(U_HID, gi) = hid;
       }
       const unsigned m_ok = __ballot_sync(MCDC_FULL, ok), m_bad = __ballot_sync(MCDC_FULL, act && !ok);
       if (ok) PL(L_F, lb + nF + lanes_below(m_ok, lane)) = (uint8_t)i;
-      nF += (uint32_t)__popc(m_ok);
       if (act && !ok) PL(L_FREE, lb + nFree + lanes_below(m_bad, lane)) = (uint8_t)i;
-      nFree += (uint32_t)__popc(m_bad);
+      nF += (uint32_t)__popc(m_ok); nFree += (uint32_t)__popc(m_bad);
       __syncwarp();
       continue;
     }
@@ -402,8 +426,13 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         unsigned long long key = 0ull;
         uint32_t ctr = 0u;
         if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
-        const double xi = draw(key, ctr);              // always consumed (D3)
-        if (act) PU(U_CTR, gi) = ctr;
+        // always consumed (D3).  Draw 2b is the first half of block b and leaves the second half in the pool for
+        // draw 2b + 1, wherever that one is made (the collision phase reads it; here the block is computed for the
+        // even lanes of the round anyway)
+        const ulonglong2 blk = philox_block(key, ctr >> 1);
+        const bool odd = (ctr & 1u) != 0u;
+        const double xi = u64_to_unit(odd ? blk.y : blk.x);
+        if (act) { PU(U_CTR, gi) = ctr + 1u; if (!odd) PC(gi) = blk.y; }
         d_coll = -log(xi);
       }
       const int cell = (int)(cl & 0xFFFFu), g = (int)(meta & 255u), pk = (int)((meta >> 8) & 4095u);
@@ -612,12 +641,23 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
       if (born) g = 0;
       const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
       const int mg = mat * G + g;
-      // reaction: scatter, capture, fission in this order (D6); with weights, the techniques of Appendix G
-      const uint32_t ctr_in = ctr;
-      const double xi_r = draw(key, ctr);
-      if (born) ctr = ctr_in;                          // a new child has no reaction: its stream goes on where it was
+      // The random numbers of this round.  A collision consumes at most four draws from the counter c it arrives with
+      // (reaction, group, mu, phi; a fission: reaction, nu -- its children draw from streams of their own in a later
+      // round; a child: group, mu, phi), five with a weight roulette.  Draws c .. c+3 lie in the blocks b0 = (c+1) >> 1
+      // and b0 + 1, plus -- when c is odd -- the half block the pool kept from the draw before (PC): two Philox blocks
+      // per round whatever the lanes do (Appendix B allows caching the unused half block; the draws are the same).
+      const bool odd = (ctr & 1u) != 0u;
+      const uint32_t b0 = (ctr + 1u) >> 1;
+      unsigned long long r0 = 0ull, r1, r2, r3, r4 = 0ull;
+      if (act && odd) r0 = PC(gi);
+      {
+        const ulonglong2 ba = philox_block(key, b0), bb = philox_block(key, b0 + 1u);
+        r1 = odd ? ba.x : ba.y; r2 = odd ? ba.y : bb.x; r3 = odd ? bb.x : bb.y;
+        if (!odd) r0 = ba.x; else r4 = bb.y;
+      }
+      const double xi_r = u64_to_unit(r0);
       int kind = FI_NONE, n_child = 0;                 // kind of the outgoing flight; children of a fission
-      bool alive = false, captured = false, fissioned = false;
+      bool alive = false, captured = false, fissioned = false, reborn = false, rouletted = false;
       uint32_t c0 = 0u;
       double w = 1.0, l_cap = 0.0, l_fis = 0.0, l_prod = 0.0, l_gain = 0.0, l_loss = 0.0;   // WEIGHTED only
       if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
@@ -643,17 +683,18 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         if (dead) {
         } else if (scatter) {
           if (WEIGHTED && T.wr_threshold > 0.0 && w < T.wr_threshold) {   // G.2 weight roulette
-            const double xi_w = draw(key, ctr);
+            const double xi_w = u64_to_unit(r1);
+            rouletted = true;
             if (xi_w * T.wr_survive < w) { l_gain += T.wr_survive - w; w = T.wr_survive; kind = FI_SCATTER; alive = true; }
             else l_loss += w;
           } else { kind = FI_SCATTER; alive = true; }
         } else {
-          const double xi_nu = draw(key, ctr);
+          const double xi_nu = u64_to_unit(r1);
           n_child = (int)floor(tb.nu(mg) + xi_nu);
-          c0 = ctr;
+          c0 = ctr + 2u;
           fissioned = true;
           l_fis += w; l_prod += (double)n_child * w;
-          if (n_child > 0 && !gen_mode) { kind = FI_CHILD; alive = true; }
+          if (n_child > 0 && !gen_mode) reborn = true;   // the parent's slot goes on as its first child (below)
         }
       }
       {
@@ -680,7 +721,8 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
         atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + 0, 1u);
         if (n_child > 0) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + 2, (uint32_t)n_child);
       }
-      // fission: publish children 1..n-1 to the global queue, continue as child 0
+      // fission: children 1..n-1 go to free slots of this pool (or the global queue), the parent's slot becomes child 0;
+      // all of them are "born" entries of the C stack: a later round samples their group and direction
       // (generation mode: every child goes to the fission bank of the generation and the parent ends here)
       const int n_push = gen_mode ? n_child : ((n_child > 1) ? n_child - 1 : 0);
       if (__ballot_sync(MCDC_FULL, n_push > 0) != 0u) {
@@ -734,28 +776,45 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
           slow_publish_children(A.q, A.cnt, WEIGHTED, x, y, z, t, w, key, c0, n_push, pre, total, qm);
         }
       }
-      if (fissioned && n_child > 0) { key = child_key(key, c0, 0u); ctr = 0u; }   // fission parent -> its first child, in place
+      if (reborn) {                                    // fission parent -> its first child, in place, born next round
+        PK(gi) = child_key(key, c0, 0u); PU(U_CTR, gi) = 0u;
+        PU(U_CL, gi) = (cl & 0xFFFFu) | (NONE16 << 16);
+        PU(U_META, gi) = meta | 255u;
+        if (WEIGHTED) PD(D_W, gi) = w;
+      }
       // group and direction of the outgoing flight (A.6): one draw for the group, two for the direction
       if (__any_sync(MCDC_FULL, alive)) {
-        const double xi_g = draw(key, ctr);
+        // a scattered particle is past the reaction draw: group, mu, phi = draws c+1 .. c+3, and an odd c leaves draw
+        // c+4 (r4, the second half of block b0+1) for later; a child starts at its counter: draws c .. c+2, an even c
+        // leaves c+3 (r3)
+        unsigned long long q_g = r1, q_mu = r2, q_phi = r3, half = r4;
+        uint32_t used = 4u;
+        if (born) { q_g = r0; q_mu = r1; q_phi = r2; half = r3; used = 3u; }
+        if (WEIGHTED && __any_sync(MCDC_FULL, rouletted && alive)) {   // the roulette took draw c+1: one draw further
+          const ulonglong2 bc = philox_block(key, b0 + 2u);
+          if (rouletted) { q_g = r2; q_mu = r3; q_phi = odd ? r4 : bc.x; half = bc.y; used = 5u; }
+        }
+        const double xi_g = u64_to_unit(q_g);
         if (kind == FI_SCATTER) g = sample_cdf([&](int q) { return tb.cdf_s(mg * G + q); }, G, tb.last_s(mg), xi_g * tb.sig_s_tot(mg));
         else g = sample_cdf([&](int q) { return tb.cdf_chi(mat * G + q); }, G, tb.last_chi(mat), xi_g);
-        double xi_mu, xi_phi, ux, uy, uz;
-        draw2(key, ctr, xi_mu, xi_phi);
-        isotropic(xi_mu, xi_phi, ux, uy, uz);
+        double ux, uy, uz;
+        isotropic(u64_to_unit(q_mu), u64_to_unit(q_phi), ux, uy, uz);
         if (alive) {
           PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
           PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
           if (WEIGHTED) PD(D_W, gi) = w;
-          PK(gi) = key; PU(U_CTR, gi) = ctr;
+          const uint32_t ctr_out = ctr + used;
+          PU(U_CTR, gi) = ctr_out;
+          if (ctr_out & 1u) PC(gi) = half;             // in the middle of a block: keep its second half for the next draw
           PU(U_META, gi) = (meta & ~255u) | (uint32_t)g;
           PU(U_CL, gi) = (cl & 0xFFFFu) | (NONE16 << 16);
         }
       }
-      const unsigned mF = __ballot_sync(MCDC_FULL, alive), mD = __ballot_sync(MCDC_FULL, act && !alive);
+      const unsigned mF = __ballot_sync(MCDC_FULL, alive), mC = __ballot_sync(MCDC_FULL, reborn), mD = __ballot_sync(MCDC_FULL, act && !alive && !reborn);
       if (alive) PL(L_F, lb + nF + lanes_below(mF, lane)) = (uint8_t)i;
-      if (act && !alive) PL(L_FREE, lb + nFree + lanes_below(mD, lane)) = (uint8_t)i;
-      nF += (uint32_t)__popc(mF); nFree += (uint32_t)__popc(mD);
+      if (reborn) PL(L_C, lb + nC + lanes_below(mC, lane)) = (uint8_t)i;
+      if (act && !alive && !reborn) PL(L_FREE, lb + nFree + lanes_below(mD, lane)) = (uint8_t)i;
+      nF += (uint32_t)__popc(mF); nC += (uint32_t)__popc(mC); nFree += (uint32_t)__popc(mD);
       __syncwarp();
     }
   }
@@ -789,6 +848,7 @@ __global__ void __launch_bounds__(NT, 1) k_warp(Tables T, HistoryArgs A) {
 
 #undef PD
 #undef PK
+#undef PC
 #undef PU
 #undef PL
 #undef WCNT
