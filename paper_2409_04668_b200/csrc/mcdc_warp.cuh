@@ -95,9 +95,10 @@ static __device__ __noinline__ void slow_score_collision(const Tables *gT, doubl
 template <bool STAGED>
 __device__ __forceinline__ void general_score(const Tables &Tg, double *x_acc_slot, int aggregate, bool active,
                                            const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d, double w) {
-  // the pre-move state is still in the pool: x y z ux uy uz 1/ux 1/uy 1/uz t, N slots apart
-  const double x = pool[gi], y = pool[N + gi], z = pool[2 * N + gi], ux = pool[3 * N + gi], uy = pool[4 * N + gi],
-               uz = pool[5 * N + gi], ix = pool[6 * N + gi], iy = pool[7 * N + gi], iz = pool[8 * N + gi], t = pool[9 * N + gi];
+  // the pre-move state is still in the pool, as pairs (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz), pair arrays N slots apart
+  const double2 *pp = reinterpret_cast<const double2 *>(pool);
+  const double2 xy = pp[gi], zt = pp[N + gi], u01 = pp[2 * N + gi], u2i0 = pp[3 * N + gi], i12 = pp[4 * N + gi];
+  const double x = xy.x, y = xy.y, z = zt.x, t = zt.y, ux = u01.x, uy = u01.y, uz = u2i0.x, ix = u2i0.y, iy = i12.x, iz = i12.y;
   // Tg is the kernel's parameter block (constant bank) when this is inlined -- reading the mesh constants through the
   // device-memory copy of the tables made every DDA step wait on global loads (config 2: long_scoreboard 3.2 per issue)
   const TB<STAGED> tb(Tg);
@@ -125,7 +126,7 @@ __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (
 // Philox block (u64), ctr, cell|last, meta, 3 stack entries
 // (+ the weight, one more f64, when a technique of Appendix G makes weights differ from 1)
 __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool weighted) {
-  return (weighted ? 11 : 10) * 8 + 8 + 8 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
+  return (weighted ? 7 : 6) * 16 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
 }
 
 struct WarpShared {                // block-wide totals (static shared memory)
@@ -152,7 +153,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   constexpr bool ONEBIN = SCORE != 0;
   constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
-  constexpr uint32_t ND = WEIGHTED ? 11u : 10u;       // f64 arrays of the pool
+  constexpr uint32_t NPAIR = WEIGHTED ? 7u : 6u;      // 16-byte pair arrays of the pool
   const double INF = CUDART_INF;
   __shared__ WarpShared sh;
   const TB<STAGED> tb(T);
@@ -161,20 +162,26 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   const uint32_t N = W * (uint32_t)NW;
   // ---- carve the dynamic shared memory: [staged tables][census populations][pool arrays][stacks] ----
   // One offset and the stride N address every array (pointers would cost two registers each):
-  //   f64  x y z ux uy uz 1/ux 1/uy 1/uz t  -> PD(k, slot), k = 0..9        u64  key       -> PK(slot)
-  //   u64  second half of Philox block ctr >> 1, valid while ctr is odd (Appendix B: "may cache the half-block") -> PC(slot)
+  //   16-byte pairs (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz)(key, half block)[(w, -)] -> PP(pair, slot), one LDS.128 each:
+  //     32 lanes gather 32 arbitrary slots, and a 16-byte gather costs fewer shared-memory wavefronts per byte than an
+  //     8-byte one (8 bank groups instead of 16: ~7 wavefronts per 16 B against ~5 per 8 B, profiles/r02c)
+  //   single fields of a pair -> PD(k, slot), k = D_X .. D_W;  key -> PK(slot)
+  //   half block = second half of Philox block ctr >> 1, valid while ctr is odd (Appendix B: "may cache the half-block") -> PC(slot)
   //   u32  ctr, cell|last<<16, meta = g | census index<<8 | batch slot<<20, [history id]  -> PU(k, slot)
   //   u8   stacks F, C, FREE -> PL(k, position)
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
   double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16));   // WEIGHTED only
   const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16) +
                             (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 + 15) / 16 * 16) : 0u);
-#define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + ((uint32_t)(k) * N + (slot)) * 8u))
-#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (ND * N + (slot)) * 8u))
-#define PC(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + ((ND + 1u) * N + (slot)) * 8u))
-#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + (ND + 2u) * 8u * N + ((uint32_t)(k) * N + (slot)) * 4u))
-#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + ((ND + 2u) * 8u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
-  enum { D_X = 0, D_Y, D_Z, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_T, D_W, U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
+#define PP(pr, slot) (*reinterpret_cast<double2 *>(g_smem + pool_off + ((uint32_t)(pr) * N + (slot)) * 16u))
+#define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + (((uint32_t)(k) >> 1) * N + (slot)) * 16u + ((uint32_t)(k) & 1u) * 8u))
+#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (5u * N + (slot)) * 16u))
+#define PC(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (5u * N + (slot)) * 16u + 8u))
+#define PKC(slot) (*reinterpret_cast<ulonglong2 *>(g_smem + pool_off + (5u * N + (slot)) * 16u))
+#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + NPAIR * 16u * N + ((uint32_t)(k) * N + (slot)) * 4u))
+#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + (NPAIR * 16u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
+  enum { D_X = 0, D_Y, D_Z, D_T, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_W = 12, P_XY = 0, P_ZT, P_U01, P_U2I0, P_I12, P_KEY, P_W,
+         U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
 
   if (STAGED) {
     const uint4 *src = reinterpret_cast<const uint4 *>(T.blob);
@@ -397,10 +404,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       else WCNT(W_SRC, n_src);
       if (ok) {
         const uint32_t gi = lb + i;
-        PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz; PD(D_T, gi) = t;
-        PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+        PP(P_XY, gi) = make_double2(x, y); PP(P_ZT, gi) = make_double2(z, t); PP(P_U01, gi) = make_double2(ux, uy);
+        PP(P_U2I0, gi) = make_double2(uz, 1.0 / ux); PP(P_I12, gi) = make_double2(1.0 / uy, 1.0 / uz);
         if (WEIGHTED) PD(D_W, gi) = w;
-        PK(gi) = key; PC(gi) = half; PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
+        PKC(gi) = make_ulonglong2(key, half); PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
         PU(U_META, gi) = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
         if (RECORD) PU(U_HID, gi) = hid;
       }
@@ -442,9 +449,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const int n_other = (int)(info & 255u), mg = (int)((info >> 8) & 255u) * G + g;
       d_coll = (tb.sig_t(mg) > 0.0) ? d_coll * tb.inv_sig_t(mg) : INF;
       double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, ix = INF, iy = INF, iz = 1.0;
-      if (act) {
-        x = PD(D_X, gi); y = PD(D_Y, gi); z = PD(D_Z, gi); ux = PD(D_UX, gi); uy = PD(D_UY, gi); uz = PD(D_UZ, gi);
-        ix = PD(D_IX, gi); iy = PD(D_IY, gi); iz = PD(D_IZ, gi);   // 1/direction is kept in the pool (three divisions per segment otherwise)
+      double t = 0.0;
+      if (act) {                                       // 1/direction is kept in the pool (three divisions per segment otherwise)
+        const double2 xy = PP(P_XY, gi), zt = PP(P_ZT, gi), u01 = PP(P_U01, gi), u2i0 = PP(P_U2I0, gi), i12 = PP(P_I12, gi);
+        x = xy.x; y = xy.y; z = zt.x; t = zt.y; ux = u01.x; uy = u01.y; uz = u2i0.x; ix = u2i0.y; iy = i12.x; iz = i12.y;
       }
       // ---- faces: one candidate per axis, picked by the sign of the direction component ----
       // sign bit alone: for a component that is exactly +-0 the face distance is inf or NaN and is rejected below
@@ -485,7 +493,6 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         }
         if (u < d_surf) { d_surf = u; which = 6 + j; }
       }
-      double t = act ? PD(D_T, gi) : 0.0;
       double w = 1.0;
       if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
       const double t_census = tb.census(pk);
@@ -573,7 +580,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         }
       }
       if (act) {
-        PD(D_X, gi) = x; PD(D_Y, gi) = y; PD(D_Z, gi) = z; PD(D_T, gi) = t;
+        PP(P_XY, gi) = make_double2(x, y); PP(P_ZT, gi) = make_double2(z, t);
         if (new_cl != cl) PU(U_CL, gi) = new_cl;
         if (ev == EV_CENSUS) PU(U_META, gi) = meta;
         if (RECORD && ev != EV_COLLISION) atomicAdd(A.ev + (size_t)PU(U_HID, gi) * 4 + (ev == EV_CENSUS ? 3 : 1), 1u);
@@ -634,7 +641,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const uint32_t gi = lb + i;
       unsigned long long key = 0ull;
       uint32_t ctr = 0u, cl = 0u, meta = 0u;
-      if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
+      unsigned long long r0 = 0ull;                    // the half block the pool kept (used when the counter is odd)
+      if (act) { const ulonglong2 kc = PKC(gi); key = kc.x; r0 = kc.y; ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
       const int cell = (int)(cl & 0xFFFFu);
       int g = (int)(meta & 255u);
       const bool born = g == 255;                      // a fission child placed in this pool: only its flight is sampled
@@ -648,8 +656,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // per round whatever the lanes do (Appendix B allows caching the unused half block; the draws are the same).
       const bool odd = (ctr & 1u) != 0u;
       const uint32_t b0 = (ctr + 1u) >> 1;
-      unsigned long long r0 = 0ull, r1, r2, r3, r4 = 0ull;
-      if (act && odd) r0 = PC(gi);
+      unsigned long long r1, r2, r3, r4 = 0ull;
       {
         const ulonglong2 ba = philox_block(key, b0), bb = philox_block(key, b0 + 1u);
         r1 = odd ? ba.x : ba.y; r2 = odd ? ba.y : bb.x; r3 = odd ? bb.x : bb.y;
@@ -751,12 +758,12 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           }
         } else if ((uint32_t)total <= nFree) {         // the children fit this warp's pool: they join its C stack
           if (n_push > 0) {
-            const double x = PD(D_X, gi), y = PD(D_Y, gi), z = PD(D_Z, gi), t = PD(D_T, gi);
+            const double2 xy = PP(P_XY, gi), zt = PP(P_ZT, gi);
 #pragma unroll 1
             for (int c = 0; c < n_push; ++c) {
               const uint32_t r = (uint32_t)(pre - n_push + c);
               const uint32_t i2 = (uint32_t)PL(L_FREE, lb + nFree - 1u - r), g2 = lb + i2;
-              PD(D_X, g2) = x; PD(D_Y, g2) = y; PD(D_Z, g2) = z; PD(D_T, g2) = t;
+              PP(P_XY, g2) = xy; PP(P_ZT, g2) = zt;
               if (WEIGHTED) PD(D_W, g2) = w;
               PK(g2) = child_key(key, c0, (uint32_t)(c + 1)); PU(U_CTR, g2) = 0u;
               PU(U_CL, g2) = (cl & 0xFFFFu) | (NONE16 << 16);
@@ -800,8 +807,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         double ux, uy, uz;
         isotropic(u64_to_unit(q_mu), u64_to_unit(q_phi), ux, uy, uz);
         if (alive) {
-          PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
-          PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
+          PP(P_U01, gi) = make_double2(ux, uy); PP(P_U2I0, gi) = make_double2(uz, 1.0 / ux);
+          PP(P_I12, gi) = make_double2(1.0 / uy, 1.0 / uz);
           if (WEIGHTED) PD(D_W, gi) = w;
           const uint32_t ctr_out = ctr + used;
           PU(U_CTR, gi) = ctr_out;
@@ -849,6 +856,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
 #undef PD
 #undef PK
 #undef PC
+#undef PP
+#undef PKC
 #undef PU
 #undef PL
 #undef WCNT
