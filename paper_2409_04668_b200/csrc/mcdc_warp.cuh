@@ -131,7 +131,7 @@ __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool wei
 
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
-  unsigned long long n_coll, n_surf, n_census, n_children, n_lost, n_src;
+  unsigned long long n_coll, n_seg, n_census, n_children, n_lost, n_src;
   uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
 
@@ -191,7 +191,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   for (int k = tid; k < T.K; k += NT) { s_popn[k] = 0u; if (WEIGHTED) s_popw[k] = 0.0; }
   if (tid == 0) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
-    sh.n_coll = sh.n_surf = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
+    sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
   }
   if (lane < 8) sh.wcnt[wid][lane] = 0u;
   const uint32_t lb = (uint32_t)wid * W;               // first slot of this warp
@@ -212,7 +212,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   bool bank_done = !step_mode;                         // the live bank of this step has been handed out
   uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
   if (step_mode && !A.step_source) src_exhausted = true;
-  enum { W_COLL = 0, W_SURF, W_CENSUS, W_CHILDREN, W_LOST, W_SRC };
+  uint32_t n_seg = 0u;                                 // segments of this warp (warp-uniform)
+  enum { W_COLL = 0, W_CHILDREN, W_LOST, W_SRC };
 #define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
   for (;;) {
@@ -423,6 +424,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // =============== F: one segment -- distances, event choice, score, move, census / surface event ===============
       const uint32_t n = min(32u, nF);
       nF -= n;
+      n_seg += n;                                      // every lane of a flight round makes one segment
       const bool act = (uint32_t)lane < n;
       const uint32_t i = act ? (uint32_t)PL(L_F, lb + nF + (uint32_t)lane) : 0u;
       const uint32_t gi = lb + i;
@@ -609,18 +611,14 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       if (m_cen) {
         const unsigned peers = __match_any_sync(MCDC_FULL, census_k);
         if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
-        WCNT(W_CENSUS, (uint32_t)__popc(m_cen));
         const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
         if (WEIGHTED) {
           if (census_k >= 0) atomicAdd(s_popw + census_k, w);
           if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
         } else if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
       }
-      {
-        const unsigned m_s = __ballot_sync(MCDC_FULL, ev == EV_SURFACE), m_lost = __ballot_sync(MCDC_FULL, lost);
-        WCNT(W_SURF, (uint32_t)__popc(m_s));
-        WCNT(W_LOST, (uint32_t)__popc(m_lost));
-      }
+      // (surface events are not counted here: segments - collisions - census events, at the end of the block)
+      if (__any_sync(MCDC_FULL, lost)) WCNT(W_LOST, (uint32_t)__popc(__ballot_sync(MCDC_FULL, lost)));
       // ---- hand the slots on: F again, C, or FREE ----
       const bool toF = alive && ev != EV_COLLISION, toC = alive && ev == EV_COLLISION, dead = act && !alive;
       const unsigned mF = __ballot_sync(MCDC_FULL, toF), mC = __ballot_sync(MCDC_FULL, toC), mD = __ballot_sync(MCDC_FULL, dead);
@@ -830,23 +828,27 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   __syncwarp();
   if (lane == 0) {
     const uint32_t *wc = sh.wcnt[wid];
-    atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_surf, (unsigned long long)wc[W_SURF]);
-    atomicAdd(&sh.n_census, (unsigned long long)wc[W_CENSUS]); atomicAdd(&sh.n_children, (unsigned long long)wc[W_CHILDREN]);
+    atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_seg, (unsigned long long)n_seg);
+    atomicAdd(&sh.n_children, (unsigned long long)wc[W_CHILDREN]);
     atomicAdd(&sh.n_lost, (unsigned long long)wc[W_LOST]); atomicAdd(&sh.n_src, (unsigned long long)wc[W_SRC]);
   }
   __syncthreads();
   for (int k = tid; k < T.K; k += NT) {
-    if (s_popn[k] != 0u) { atomicAdd(A.pop_w + k, WEIGHTED ? s_popw[k] : (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]); }
+    if (s_popn[k] != 0u) {
+      atomicAdd(A.pop_w + k, WEIGHTED ? s_popw[k] : (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]);
+      atomicAdd(&sh.n_census, (unsigned long long)s_popn[k]);   // census events of the block = its population counts
+    }
   }
+  __syncthreads();
   if (tid == 0) {
     DevCounters *cnt = A.cnt;
     for (int e = 0; e < LED_N; ++e)
       if (sh.led[e] != 0.0) atomicAdd(&cnt->ledger[1 + e], sh.led[e]);
     atomicAdd(&cnt->ledger[0], (double)sh.n_src);
     atomicAdd(&cnt->n[0], sh.n_src);
-    atomicAdd(&cnt->n[1], sh.n_coll + sh.n_surf + sh.n_census);
+    atomicAdd(&cnt->n[1], sh.n_seg);
     atomicAdd(&cnt->n[2], sh.n_coll);
-    atomicAdd(&cnt->n[3], sh.n_surf);
+    atomicAdd(&cnt->n[3], sh.n_seg - sh.n_coll - sh.n_census);   // a segment ends in a collision, a census or a surface event
     atomicAdd(&cnt->n[4], sh.n_census);
     atomicAdd(&cnt->n[5], sh.n_children);
     atomicAdd(&cnt->n[6], sh.n_lost);
