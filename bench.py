@@ -28,10 +28,28 @@ import numpy as np  # noqa: E402
 METRIC = "histories/s"
 N_SM = 148
 ISSUE_LANES_PER_SM = 128        # 4 warp schedulers x 32 lanes: one warp instruction per scheduler per cycle
-# From the committed ncu capture of k_warp on this workload (profiles/r01h_k_warp_final.md): per launch of 1e7 config-3
-# histories, dram__bytes_read.sum + dram__bytes_write.sum, and thread instructions per track segment.
-NCU = {"config3_pin_lattice": {"dram_bytes_per_history": 3.23, "thread_inst_per_segment": 879.0,
-                               "source": "profiles/r01h_k_warp_final.md"}}
+# ncu-derived constants (DRAM bytes per history, thread instructions per segment) come from the committed
+# profiles/ncu_constants.json, keyed by kernel instantiation + workload and stamped with the revision of the kernel
+# sources the capture was made from; they are printed only when the running library reports the same revision
+# (mcdc_kernel_info_get), so a figure from another build never sits beside this run's timing.
+NCU_JSON = os.path.join(ROOT, "profiles", "ncu_constants.json")
+
+
+def ncu_constants(kernel_info, workload, technique):
+    """-> (entry or None, note).  kernel_info: 'k_warp<1,0,0,1,512> rev=abc grid=148 ...'"""
+    try:
+        with open(NCU_JSON) as f:
+            table = json.load(f)
+    except (OSError, ValueError):
+        return None, "profiles/ncu_constants.json missing"
+    name = kernel_info.split(" ")[0] if kernel_info else ""
+    rev = next((t[4:] for t in kernel_info.split() if t.startswith("rev=")), "")
+    for e in table.get("captures", []):
+        if e.get("kernel") == name and e.get("workload") == workload and e.get("technique", "analog") == technique:
+            if e.get("rev") != rev:
+                return None, f"stale: {e.get('source')} was captured at kernel rev {e.get('rev')}, this library is rev {rev}"
+            return e, e.get("source")
+    return None, f"no capture of {name} on {workload} ({technique}) in profiles/ncu_constants.json"
 
 
 # variants of the workload with the techniques of DESIGN.md Appendix G switched on (the headline run is analog)
@@ -172,10 +190,11 @@ def _desc_bytes(p):
     return n + 31 * 8
 
 
-def algorithmic_bytes(p, c, n_hist, n_batches):
-    """176 B per segment + 112 B per fission child + 88 B per source history + close-out."""
-    closeout = 3 * 16 * p.n_bins * n_batches
-    return 176.0 * c["segments"] + 112.0 * c["children"] + 88.0 * n_hist + closeout
+def algorithmic_bytes(p, c, n_hist, n_batches=0):
+    """SURVEY.md 8(d), the history kernel's part: 176 B per segment + 112 B per fission child + 88 B per source history.
+    The close-out (3 x 16 B per bin per batch) is k_closeout's work, not k_warp's: it is NOT in this figure, which is
+    divided by k_warp's device time alone."""
+    return 176.0 * c["segments"] + 112.0 * c["children"] + 88.0 * n_hist
 
 
 # ------------------------------------------------------------------------------------------------
@@ -193,9 +212,48 @@ def run_cpu_sample(p, seconds_target=15.0, first_history_id=0):
     t0 = time.perf_counter(); o.run(n2, p.seed, n_batches=1, first_history_id=first_history_id)
     dt = time.perf_counter() - t0
     c = o.counters()
-    return {"value": n2 / dt, "unit": METRIC, "cores": 1, "kind": "oracle",
+    return {"value": n2 / dt, "unit": METRIC, "cores": 1, "kind": "oracle", "n": n2,
             "sample": f"first {n2} histories of {p.name} (seed {p.seed}), single thread, {dt:.1f} s",
             "segments_per_s": c["segments"] / dt}
+
+
+def _cpu_part(job):
+    """One oracle process: `n` histories of the workload from history id `first` (a range of its own)."""
+    name, kw, seed, first, n = job
+    from oracle import Oracle
+    from workloads import configs as W
+    p = W.get_config(name, **kw)
+    o = Oracle(p)
+    t0 = time.perf_counter()
+    o.run(n, seed, n_batches=1, first_history_id=first)
+    dt = time.perf_counter() - t0
+    seg = o.counters()["segments"]
+    o.close()
+    return n, dt, seg
+
+
+def run_cpu_all_cores(args, p, per_core_rate, seconds_target=12.0):
+    """the oracle as it stands on ALL host cores -- P = nproc independent processes over disjoint
+    history-id ranges of the same workload (histories are independent; no tuning, no threads inside)."""
+    import multiprocessing as mp
+    P = os.cpu_count() or 1
+    n = int(max(1000, min(p.n_histories // P, per_core_rate * seconds_target)))
+    kw = {}
+    if args.histories:
+        kw["n_histories"] = int(args.histories)
+    if args.batches:
+        kw["n_batches"] = int(args.batches)
+    jobs = [(args.workload, kw, p.seed, i * n, n) for i in range(P)]
+    ctx = mp.get_context("spawn")
+    with ctx.Pool(P) as pool:
+        pool.map(_cpu_part, [(args.workload, kw, p.seed, 0, 200)] * P)      # start every process, load the checker
+        t0 = time.perf_counter()
+        res = pool.map(_cpu_part, jobs, chunksize=1)
+        wall = time.perf_counter() - t0
+    tot = sum(r[0] for r in res)
+    return {"value": tot / wall, "unit": METRIC, "cores": P, "kind": "oracle",
+            "sample": f"{P} processes x {n} histories of {p.name} (disjoint id ranges from 0, seed {p.seed}), {wall:.1f} s wall",
+            "segments_per_s": sum(r[2] for r in res) / wall}
 
 
 def bench_reference(args):
@@ -204,7 +262,7 @@ def bench_reference(args):
         return
     p = _problem(args)
     vals = []
-    per_step = max(3.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    per_step = args.ref_seconds or max(3.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
     for _ in range(args.warmup):
         run_cpu_sample(p, seconds_target=min(2.0, per_step))
     t0 = time.perf_counter()
@@ -212,11 +270,15 @@ def bench_reference(args):
         vals.append(run_cpu_sample(p, seconds_target=per_step, first_history_id=0))
     dt = time.perf_counter() - t0
     v = float(np.mean([x["value"] for x in vals]))
-    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": METRIC, "n_gpus": args.gpus, "steps": args.steps,
+    n_sample = int(np.mean([x["n"] for x in vals]))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    out = {"impl": "reference", "metric": METRIC, "value": v, "unit": METRIC, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps), "higher_is_better": True,
            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": p.name, "histories_per_step": p.n_histories, "n_batches": p.n_batches,
-                      "note": "oracle timed on a bounded sample of the workload per step"},
+           "config": {"workload": p.name, "histories_per_step": n_sample, "workload_histories": p.n_histories,
+                      "n_batches": 1, "seed": p.seed,
+                      "note": f"each step is a bounded SAMPLE of the workload: the oracle (one host thread, rank 0) runs the "
+                              f"first {n_sample} of its {p.n_histories} histories; ms_per_step is the time of that sample"},
            "cpu_baseline": {"value": v, "unit": METRIC, "cores": 1, "kind": "oracle", "sample": vals[-1]["sample"]},
            "e2e": {"value": v, "unit": METRIC, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "gpu_launches": 0}
@@ -294,27 +356,35 @@ def bench_gpu(args):
         clocks = sampler.stop(t_wall0, t_wall1)
         peak, peak_kind, sm_max = _peaks()
         # dominant kernel: k_warp.  Algorithmic bytes of the steps it processed / its device time.
-        alg = algorithmic_bytes(p, {"segments": c["segments"], "children": c["children"]}, n_hist * args.steps,
-                                n_b * args.steps)
+        alg = algorithmic_bytes(p, {"segments": c["segments"], "children": c["children"]}, n_hist * args.steps)
         n_tr = max(1, launches // 2)                       # one k_warp + one k_closeout launch per sub-batch
         ach = alg / (ms_tr * 1e-3) / 1e9
-        ncu = NCU.get(p.name) if args.technique == "analog" else None   # the capture is of the analog kernel
+        kinfo = g.kernel_info()
+        ncu, ncu_note = ncu_constants(kinfo, p.name, args.technique)
         traffic = ncu["dram_bytes_per_history"] * n_hist * args.steps / n_tr if ncu else None
-        roofline = {"bound": "hbm", "kernel": "k_warp", "achieved": ach, "peak": peak, "unit": "GB/s",
+        roofline = {"bound": "hbm", "kernel": kinfo, "achieved": ach, "peak": peak, "unit": "GB/s",
                     "frac": ach / peak, "traffic": traffic, "peak_kind": peak_kind,
-                    "note": "achieved = SURVEY 8(d) algorithmic bytes (176 B/segment + 112 B/child + 88 B/history + "
-                            "close-out) / summed k_warp device time (CUDA events on the library's stream); particle "
-                            "state lives in shared memory, so the DRAM traffic (bytes per launch, from the ncu capture "
-                            "in profiles/) is far below this figure and the kernel is issue-bound: see roofline_alu",
+                    "frac_measured_dram": (traffic * n_tr / (ms_tr * 1e-3) / 1e9 / peak) if traffic else None,
+                    "ncu_source": ncu_note,
+                    "note": "achieved = SURVEY 8(d) algorithmic-bytes equivalent of the history kernel (176 B/segment + "
+                            "112 B/child + 88 B/history) / summed k_warp device time (CUDA events on the library's "
+                            "stream); particle state lives in shared memory, so the measured DRAM traffic (bytes per "
+                            "launch from the ncu capture, frac_measured_dram) is far below this figure and the kernel "
+                            "is issue-bound: see roofline_alu",
                     "launches": int(n_tr), "ms_kernel_total": ms_tr}
         roofline_alu = None
         if ncu:
             ti = ncu["thread_inst_per_segment"] * c["segments"] / (ms_tr * 1e-3)
             pk = N_SM * ISSUE_LANES_PER_SM * sm_max * 1e6
-            roofline_alu = {"bound": "alu", "kernel": "k_warp", "achieved": ti / 1e12, "peak": pk / 1e12,
+            roofline_alu = {"bound": "alu", "kernel": kinfo.split(" ")[0], "achieved": ti / 1e12, "peak": pk / 1e12,
                             "unit": "T thread-inst/s", "frac": ti / pk,
+                            "issue_active_pct": ncu.get("issue_active_pct"),
+                            "l2_red_sectors_per_s": (ncu["l2_atom_red_sectors_per_segment"] * c["segments"] / (ms_tr * 1e-3))
+                            if ncu.get("l2_atom_red_sectors_per_segment") else None,
+                            "l2_hit_rate_pct": ncu.get("l2_hit_rate_pct"),
                             "note": "instruction issue: thread instructions per segment from the ncu capture x segments/s, "
-                                    "against 148 SMs x 4 schedulers x 32 lanes x max SM clock (DESIGN.md section 6)"}
+                                    "against 148 SMs x 4 schedulers x 32 lanes x max SM clock (DESIGN.md section 6); "
+                                    "l2_red_sectors_per_s = fp64 RED/atomic sectors at L2 per second (atomic throughput)"}
         out = {"metric": METRIC, "value": value, "unit": METRIC, "n_gpus": world, "steps": args.steps,
                "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -353,8 +423,10 @@ def bench_gpu(args):
                       "note": "mcdc_problem_create (host arrays) + workspace_bind + run_ex + tallies_get (host) per step"}
         if world == 1 and not args.no_cpu:
             out["cpu_baseline"] = run_cpu_sample(p, seconds_target=args.cpu_seconds)
+            out["cpu_baseline_all_cores"] = run_cpu_all_cores(args, p, out["cpu_baseline"]["value"],
+                                                              seconds_target=min(12.0, args.cpu_seconds))
     g.close()
-    if args.sweep and world == 1:
+    if not args.no_sweep and world == 1 and args.workload == "config3" and not args.histories and args.technique == "analog":
         out["sweep"] = run_sweep(M, args, dev, peak)
     if args.eigenvalue and world == 1:
         out["eigenvalue"] = run_eigenvalue(M, args, dev)
@@ -393,7 +465,8 @@ def run_eigenvalue(M, args, dev):
 
 
 def run_sweep(M, args, dev, peak):
-    """BASELINE config 4: the config-3 problem at 1e5 .. 1e9 histories (1e9 as device-sized sub-batches)."""
+    """BASELINE config 4: the config-3 problem at 1e5 .. 1e9 histories (1e9 as device-sized sub-batches): histories/s,
+    segments/s and algorithmic HBM GB/s vs batch size.  Outside the timed region of the headline, same JSON line."""
     import torch
     from workloads import configs as W
 
@@ -420,13 +493,26 @@ def run_sweep(M, args, dev, peak):
         torch.cuda.synchronize()
         ms = e0.elapsed_time(e1)
         c = g.counters()
-        alg = algorithmic_bytes(p, c, n * reps, nb * reps)
+        alg = algorithmic_bytes(p, c, n * reps)
         rows.append({"histories": n, "n_batches": nb, "histories_per_s": n * reps / (ms * 1e-3),
                      "segments_per_s": c["segments"] / (ms * 1e-3), "ms_per_run": ms / reps,
-                     "alg_GBps": alg / (ms_k * 1e-3) / 1e9, "frac_of_hbm_peak": alg / (ms_k * 1e-3) / 1e9 / peak,
+                     "hbm_GBps_algorithmic": alg / (ms_k * 1e-3) / 1e9, "frac_of_hbm_peak": alg / (ms_k * 1e-3) / 1e9 / peak,
                      "launches_per_run": (c["kernel_launches"]) // reps, "workspace_bytes": g.workspace_bytes})
         g.close()
     return rows
+
+
+def launch_ranks(n):
+    """`python bench.py --gpus N` outside a launcher: start N ranks of this command line itself, one per GPU, the way the
+    driver does (torch.distributed.run, rendezvous on 127.0.0.1), and become that launcher."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={n}", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    sys.stdout.flush()
+    os.execv(sys.executable, cmd)
 
 
 def main():
@@ -444,10 +530,15 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
     ap.add_argument("--debug-pool-slots", type=int, default=0, help="mcdc_run_opts.debug_pool_slots (test knob; 0 = automatic)")
     ap.add_argument("--debug-stage-tables", type=int, default=0, help="mcdc_run_opts.debug_stage_tables (test knob; 0 = automatic)")
-    ap.add_argument("--sweep", action="store_true", help="also run the config-4 batch-size sweep (adds a 'sweep' key)")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the config-4 batch-size sweep (the 'sweep' key of the "
+                    "default config-3 line: 1e5 .. 1e9 histories, a few seconds of GPU time)")
+    ap.add_argument("--sweep", action="store_true", help="(default now; kept for old command lines)")
     ap.add_argument("--sweep-max", type=float, default=1e9)
+    ap.add_argument("--ref-seconds", type=float, default=0.0, help="--impl reference: CPU seconds per step (0 = automatic)")
     ap.add_argument("--eigenvalue", action="store_true", help="also time the k-eigenvalue mode (adds an 'eigenvalue' key)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        launch_ranks(args.gpus)                            # does not return
     if args.impl == "reference":
         bench_reference(args)
     else:

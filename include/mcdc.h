@@ -249,6 +249,15 @@ int mcdc_state_size(const mcdc_problem *p, size_t *n_doubles);
 int mcdc_state_export(const mcdc_problem *p, double *buf, size_t n_doubles, int on_device);
 int mcdc_state_import(mcdc_problem *p, const double *buf, size_t n_doubles, int on_device);
 
+/* Which transport kernel the LAST run of this handle launched, as text: the k_warp instantiation
+ * "k_warp<STAGED,RECORD,VARIANT,SCORE,threads>", the revision of the kernel sources it was built from (first
+ * 12 hex digits of their SHA-1, set by the build), the grid, the pool slots per warp and the dynamic shared
+ * memory -- or "k_transport ..." for the census-stepped scheduler; empty before the first run.  Measurement
+ * aid: bench.py keys the ncu-derived constants of profiles/ by this string, so a figure
+ * captured from another kernel build is never printed beside this one's timing.  buf: HOST, n bytes,
+ * always NUL-terminated; MCDC_ERR_ARG on NULL / n == 0.                                              */
+int mcdc_kernel_info_get(const mcdc_problem *p, char *buf, size_t n);
+
 const char *mcdc_strerror(int code);
 const char *mcdc_last_cuda_error(const mcdc_problem *p);
 /* "major.minor sm_XX" of the build; never fails.                                                  */

@@ -13,6 +13,7 @@ from .api import (  # noqa: F401
     mcdc_problem_destroy,
     mcdc_problem_reset,
     mcdc_problem_info_get,
+    mcdc_kernel_info_get,
     mcdc_workspace_size,
     mcdc_workspace_size_async,
     mcdc_workspace_bind,

@@ -20,7 +20,7 @@ EXPORTED_SYMBOLS = [
     "mcdc_counters_get", "mcdc_census_get", "mcdc_history_events_get", "mcdc_strerror",
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
     "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
-    "mcdc_collision_tally_enable", "mcdc_collision_tallies_get", "mcdc_problem_create_csg",
+    "mcdc_collision_tally_enable", "mcdc_collision_tallies_get", "mcdc_problem_create_csg", "mcdc_kernel_info_get",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -125,6 +125,7 @@ def lib():
     L.mcdc_state_size.argtypes = [vp, C.POINTER(C.c_size_t)]; L.mcdc_state_size.restype = C.c_int
     L.mcdc_state_export.argtypes = [vp, vp, C.c_size_t, C.c_int]; L.mcdc_state_export.restype = C.c_int
     L.mcdc_state_import.argtypes = [vp, vp, C.c_size_t, C.c_int]; L.mcdc_state_import.restype = C.c_int
+    L.mcdc_kernel_info_get.argtypes = [vp, C.c_char_p, C.c_size_t]; L.mcdc_kernel_info_get.restype = C.c_int
     L.mcdc_strerror.argtypes = [C.c_int]; L.mcdc_strerror.restype = C.c_char_p
     L.mcdc_last_cuda_error.argtypes = [vp]; L.mcdc_last_cuda_error.restype = C.c_char_p
     L.mcdc_version.argtypes = []; L.mcdc_version.restype = C.c_char_p
@@ -225,6 +226,12 @@ def mcdc_problem_info_get(h) -> dict:
     info = ProblemInfo()
     _check(lib().mcdc_problem_info_get(h, C.byref(info)), "mcdc_problem_info_get", h)
     return {n: int(getattr(info, n)) for n, _ in ProblemInfo._fields_}
+
+
+def mcdc_kernel_info_get(h) -> str:
+    buf = C.create_string_buffer(256)
+    _check(lib().mcdc_kernel_info_get(h, buf, 256), "mcdc_kernel_info_get", h)
+    return buf.value.decode()
 
 
 def mcdc_workspace_size_async(h, max_histories_per_subbatch, max_batches_in_flight) -> int:
@@ -380,6 +387,9 @@ class Problem:
 
     def info(self):
         return mcdc_problem_info_get(self._h)
+
+    def kernel_info(self):
+        return mcdc_kernel_info_get(self._h)
 
     def run(self, n_histories=None, seed=None, n_batches=None, first_history_id=0, record_history_events=False,
             scheduler=0, debug_pool_slots=0, debug_stage_tables=0):

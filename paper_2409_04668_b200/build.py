@@ -23,6 +23,17 @@ NVCC_FLAGS = ARCH + ["-O3", "-lineinfo", "-std=c++17", "--compiler-options", "-f
 LINK_FLAGS = ARCH + ["-shared", "-cudart", "static", "--compiler-options", "-fPIC"]
 
 
+def kernel_rev() -> str:
+    """First 12 hex digits of the SHA-1 over the kernel sources (headers + instantiation unit): the library reports it
+    through mcdc_kernel_info_get, and profiles/ncu_constants.json records the revision each capture was made from."""
+    import hashlib
+    h = hashlib.sha1()
+    for f in HEADERS + ["mcdc_warp_inst.cu"]:
+        with open(os.path.join(CSRC, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:12]
+
+
 def lib_path() -> str:
     return LIB
 
@@ -42,10 +53,11 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
     os.makedirs(OBJ, exist_ok=True)
+    rev = [f'-DMCDC_KERNEL_REV="{kernel_rev()}"']
 
     def compile_unit(u):
         src, obj, defs = u
-        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(defs) + list(defines) + \
+        cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(defs) + rev + list(defines) + \
               ["-c", os.path.join(CSRC, src), "-o", os.path.join(OBJ, obj)]
         r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
         return u, r

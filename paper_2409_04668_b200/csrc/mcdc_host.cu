@@ -60,6 +60,10 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
 }  // namespace
 
+#ifndef MCDC_KERNEL_REV
+#define MCDC_KERNEL_REV "unknown"      // build.py: first 12 hex digits of the SHA-1 over the kernel sources
+#endif
+
 struct mcdc_problem {
   // host copy of the description (deep)
   int G, M, S, C, K, Nt;
@@ -113,6 +117,7 @@ struct mcdc_problem {
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;
   size_t ev_used = 0;
   bool transport_attr_set = false;   // cudaFuncSetAttribute(k_transport) done for this handle's device
+  std::string last_kernel;           // transport kernel instantiation + launch shape of the last run (mcdc_kernel_info_get)
   std::string cuda_err;
 };
 
@@ -988,6 +993,7 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
       CK(cudaMemsetAsync(sec.count, 0, ns * sizeof(uint32_t), p->stream));
       int grid = (int)std::min<uint64_t>((uint64_t)max_grid, std::max<uint64_t>(1, (n_in + TRANSPORT_THREADS - 1) / TRANSPORT_THREADS));
       CK(cudaEventRecord(ev0, p->stream));
+      if (p->last_kernel.compare(0, 11, "k_transport") != 0) p->last_kernel = std::string("k_transport rev=") + MCDC_KERNEL_REV;
       k_transport<<<grid, TRANSPORT_THREADS, smem, p->stream>>>(p->tab, st, ta);
       CK(cudaEventRecord(ev1, p->stream));
       p->launches++;
@@ -1057,9 +1063,12 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
 // SCORE of k_warp for a problem and its merge choice (mcdc_warp.cuh)
 int score_mode(const Tables &T, int aggregate) { return T.all_one_bin ? (aggregate ? 2 : 1) : 0; }
-void warp_launch(bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
-  (void)nt;
+void warp_launch(mcdc_problem *p, bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   const int score = score_mode(T, A.aggregate);
+  char name[160];
+  snprintf(name, sizeof name, "k_warp<%d,%d,%d,%d,%d> rev=%s grid=%d pool_slots=%u smem=%zu", staged ? 1 : 0, record ? 1 : 0, variant,
+           score, nt, MCDC_KERNEL_REV, grid, A.pool_slots, smem);
+  p->last_kernel = name;
   switch (variant) {
     case KW_ANALOG: warp_launch_variant<KW_ANALOG>(staged, record, score, grid, smem, st, T, A); break;
     case KW_WEIGHTED: warp_launch_variant<KW_WEIGHTED>(staged, record, score, grid, smem, st, T, A); break;
@@ -1183,7 +1192,7 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
   { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
   CK(cudaEventRecord(a, p->stream));
   const bool weighted = p->tech.implicit_capture || p->tech.wr_threshold > 0.0 || p->col_on;
-  warp_launch(staged, record, weighted ? KW_WEIGHTED : KW_ANALOG, nt, grid, smem, p->stream, p->tab, ha);
+  warp_launch(p, staged, record, weighted ? KW_WEIGHTED : KW_ANALOG, nt, grid, smem, p->stream, p->tab, ha);
   CK(cudaEventRecord(b, p->stream));
   p->launches++;
   if (sb.closeout) {
@@ -1241,7 +1250,7 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
     cudaEvent_t a, b;
     { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
     CK(cudaEventRecord(a, p->stream));
-    warp_launch(staged, record, KW_CENSUS_STEP, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    warp_launch(p, staged, record, KW_CENSUS_STEP, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
     p->launches++;
     CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
@@ -1452,7 +1461,7 @@ extern "C" int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64
     cudaEvent_t a, b;
     { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
     CK(cudaEventRecord(a, p->stream));
-    warp_launch(staged, false, KW_GENERATION, nt, grid, p->pool_smem, p->stream, p->tab, ha);
+    warp_launch(p, staged, false, KW_GENERATION, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
     p->launches++;
     // H.2: an active generation is one statistical batch; an inactive one is discarded
@@ -1759,4 +1768,10 @@ extern "C" const char *mcdc_strerror(int code) {
 
 extern "C" const char *mcdc_last_cuda_error(const mcdc_problem *p) { return p ? p->cuda_err.c_str() : ""; }
 
-extern "C" const char *mcdc_version(void) { return "0.1 sm_100a"; }
+extern "C" const char *mcdc_version(void) { return "0.2 sm_100a"; }
+
+extern "C" int mcdc_kernel_info_get(const mcdc_problem *p, char *buf, size_t n) {
+  if (!p || !buf || n == 0) return MCDC_ERR_ARG;
+  snprintf(buf, n, "%s", p->last_kernel.c_str());
+  return MCDC_OK;
+}
