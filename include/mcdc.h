@@ -150,8 +150,9 @@ int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out);
  * them; an empty range leaves the cell the intersection of its half-spaces.  The cell's half-space list
  * must still name every surface that bounds the cell (distances are taken to all of them).  Both
  * arrays are HOST memory, deep-copied; region_offset has n_cells + 1 entries starting at 0; expressions
- * deeper than 32 operands or malformed give MCDC_ERR_GEOM.  Problems with regions run on the
- * census-stepped kernel (the history kernel's cell records describe intersections only).           */
+ * deeper than 32 operands or malformed give MCDC_ERR_GEOM.  Both schedulers run such problems; on the
+ * history kernel a region cell has no typed faces and no certified neighbours (every crossing of one
+ * of its surfaces takes the cell search of A.5 with the expression evaluator).                       */
 enum { MCDC_RGN_AND = -1, MCDC_RGN_OR = -2, MCDC_RGN_NOT = -3 };
 int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t *region_offset,
                             const int32_t *region_rpn, mcdc_problem **out);

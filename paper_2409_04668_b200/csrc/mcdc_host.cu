@@ -406,7 +406,9 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
   std::vector<std::vector<int>> others(C);
   for (int c = 0; c < C; ++c) {
     for (int a = 0; a < 3; ++a) { bound[c][2 * a] = -HINF; bound[c][2 * a + 1] = HINF; face[c][2 * a] = face[c][2 * a + 1] = -1; }
-    for (int i = p->cell_off[c]; i < p->cell_off[c + 1]; ++i) {
+    // (a general region has no faces: under OR / NOT a listed plane bounds nothing, so all its surfaces are "others")
+    const bool is_region = has_regions && p->rgn_off[c] < p->rgn_off[c + 1];
+    for (int i = p->cell_off[c]; i < p->cell_off[c + 1] && !is_region; ++i) {
       const int s = p->hs_surface[i];
       if (type[s] > ST_PLANE_Z) continue;
       const int a = type[s] - ST_PLANE_X;
@@ -490,9 +492,11 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     }
     return true;
   };
+  auto region_cell = [&](int c) { return has_regions && p->rgn_off[c] < p->rgn_off[c + 1]; };
   auto certified = [&](int c, int i) -> int {                                // neighbour across half-space slot i of cell c
     const int s = p->hs_surface[i];
     if (p->surf_bc[s] != MCDC_BC_TRANSMISSION) return -1;
+    if (region_cell(c)) return -1;                                           // its surface patches are not bounded by its box
     Box R = ubox[c];
     int axis = -1, f = -1;
     if (type[s] <= ST_PLANE_Z) {
@@ -508,6 +512,7 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     } else return -1;
     for (int k = nb_off[i]; k < nb_off[i + 1]; ++k) {
       const int n = nb_cell[k];
+      if (region_cell(n)) continue;                                          // membership of a region is never proved here
       if (axis >= 0) {
         const int fo = f ^ 1;
         if (face[n][fo] < 0 || p->hs_surface[face[n][fo]] != s) continue;
@@ -522,8 +527,7 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     }
     return -1;
   };
-  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095 &&
-                 !has_regions;                            // k_warp's cell records describe intersections only
+  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095;
   std::vector<unsigned char> cell2((size_t)C * CELL2_BYTES, 0), other2;
   size_t n_cert = 0, n_transm = 0;
   for (int c = 0; c < C && warp_ok; ++c) {
@@ -1062,12 +1066,13 @@ int run_subbatch(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t fi
 // ---- k_warp instantiations live in translation units of their own (mcdc_warp_inst.cu, one per VARIANT) ----
 enum { KW_ANALOG = 0, KW_WEIGHTED = 1, KW_CENSUS_STEP = 2, KW_GENERATION = 3 };   // VARIANT of k_warp
 // SCORE of k_warp for a problem and its merge choice (mcdc_warp.cuh)
-int score_mode(const Tables &T, int aggregate) { return T.all_one_bin ? (aggregate ? 2 : 1) : 0; }
+// (-1: the instantiation for general CSG regions, Appendix J)
+int score_mode(const Tables &T, int aggregate) { return T.has_regions ? -1 : T.all_one_bin ? (aggregate ? 2 : 1) : 0; }
 void warp_launch(mcdc_problem *p, bool staged, bool record, int variant, int nt, int grid, size_t smem, cudaStream_t st, const Tables &T, const HistoryArgs &A) {
   const int score = score_mode(T, A.aggregate);
   char name[160];
-  snprintf(name, sizeof name, "k_warp<%d,%d,%d,%d,%d> rev=%s grid=%d pool_slots=%u smem=%zu", staged ? 1 : 0, record ? 1 : 0, variant,
-           score, nt, MCDC_KERNEL_REV, grid, A.pool_slots, smem);
+  snprintf(name, sizeof name, "k_warp<%d,%d,%d,%d,%d%s> rev=%s grid=%d pool_slots=%u smem=%zu", staged ? 1 : 0, record ? 1 : 0, variant,
+           score < 0 ? 0 : score, nt, score < 0 ? ",rgn" : "", MCDC_KERNEL_REV, grid, A.pool_slots, smem);
   p->last_kernel = name;
   switch (variant) {
     case KW_ANALOG: warp_launch_variant<KW_ANALOG>(staged, record, score, grid, smem, st, T, A); break;

@@ -22,11 +22,14 @@ namespace mcdc {
 // ---- slow paths: rare, not inlined, and they read the tables from global memory (device copy of Tables) ----
 
 // A.5 transmission without a certified neighbour: candidate cells of half-space `idx` of `cell`, then every cell
+// (RGN: the problem holds general CSG regions, Appendix J -- instantiations of their own, so that the expression
+// evaluator is no part of the kernels that never run it)
+template <bool RGN>
 static __device__ __noinline__ int slow_cross(const Tables *gT, int cell, int idx, int s_star, double x, double y, double z,
                                        double ux, double uy, double uz) {
   const TB<false> tb(*gT);
   const int slot = tb.cell_off(cell) + idx;
-  return locate_neighbour<false>(tb, slot, s_star, x, y, z, ux, uy, uz);
+  return locate_neighbour<RGN>(tb, slot, s_star, x, y, z, ux, uy, uz);
 }
 // A.5 reflection off a surface that is not an axis-aligned plane
 static __device__ __noinline__ void slow_reflect(const Tables *gT, int s, int type, double x, double y, double z, double *u) {
@@ -34,10 +37,11 @@ static __device__ __noinline__ void slow_reflect(const Tables *gT, int s, int ty
   reflect(tb, s, type, x, y, z, u[0], u[1], u[2]);
 }
 // A.3 cell of a source particle
+template <bool RGN>
 static __device__ __noinline__ int slow_locate_source(const Tables *gT, double x, double y, double z, double ux, double uy,
                                                double uz) {
   const TB<false> tb(*gT);
-  return locate_source<false>(tb, x, y, z, ux, uy, uz);
+  return locate_source<RGN>(tb, x, y, z, ux, uy, uz);
 }
 // A.4 distance to a surface that is neither an axis-aligned plane face nor a z-cylinder
 static __device__ __noinline__ double slow_distance(const Tables *gT, int s, int type, bool on, double x, double y, double z,
@@ -143,12 +147,15 @@ struct WarpShared {                // block-wide totals (static shared memory)
 // such problems never execute, in the middle of the flight phase: leaving it out is worth 8 % on config 3 (r01f).
 // SCORE: 0 = general (DDA scorer compiled in, one-bin shortcut and in-warp merge chosen at run time); 1 = ONEBIN, one RED
 // per score; 2 = ONEBIN on a tiny mesh, equal addresses merged inside the warp before the RED.
+// RGN: cells may be general CSG regions (Appendix J).  A region cell has no faces and no certified neighbours: every one of
+// its surfaces is an "other" entry, every crossing takes the search of A.5 with the expression evaluator (slow_cross<true>),
+// and source particles are located with it; everything else of the kernel is unchanged.  Always with SCORE = 0.
 #ifdef MCDC_WARP_MAXNREG
 #define MCDC_WARP_BOUNDS __maxnreg__(MCDC_WARP_MAXNREG)
 #else
 #define MCDC_WARP_BOUNDS __launch_bounds__(NT, 1)
 #endif
-template <bool STAGED, bool RECORD, int VARIANT, int SCORE, int NT>
+template <bool STAGED, bool RECORD, int VARIANT, int SCORE, int NT, bool RGN = false>
 __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   constexpr bool ONEBIN = SCORE != 0;
   constexpr bool WEIGHTED = VARIANT != 0;
@@ -396,7 +403,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const bool known = T.src_cell >= 0 &&
                            (!T.src_chk || (x > T.src_clo[0] && x < T.src_chi[0] && y > T.src_clo[1] && y < T.src_chi[1] &&
                                            z > T.src_clo[2] && z < T.src_chi[2]));
-        cell = known ? T.src_cell : slow_locate_source(gT, x, y, z, ux, uy, uz);
+        cell = known ? T.src_cell : slow_locate_source<RGN>(gT, x, y, z, ux, uy, uz);
         if (cell < 0) ok = false;                      // a source particle outside every cell is lost (A.3)
       }
       const unsigned m_lost = __ballot_sync(MCDC_FULL, is_src && cell < 0 && !skip);
@@ -575,7 +582,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           if (nb != NONE16 && in_x && in_y && in_z) c2 = (int)nb;
           else {
             if (idx < 0) idx = (int)tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
-            c2 = slow_cross(gT, cell, idx, (int)s_star, x, y, z, ux, uy, uz);
+            c2 = slow_cross<RGN>(gT, cell, idx, (int)s_star, x, y, z, ux, uy, uz);
           }
           if (c2 < 0) { alive = false; lost = true; atomicAdd(&sh.led[LED_LOST], w); }
           else new_cl = (uint32_t)c2 | (s_star << 16);

@@ -19,19 +19,23 @@ def M():
     return M
 
 
-@pytest.mark.parametrize("tech", [None, dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0, population_control=True)])
-def test_union_and_complement_cells_match_the_oracle(M, tech):
+@pytest.mark.parametrize("scheduler", [0, 1])
+@pytest.mark.parametrize("tech", [None, dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0),
+                                  dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0, population_control=True)])
+def test_union_and_complement_cells_match_the_oracle(M, tech, scheduler):
     from oracle import Oracle
     from workloads import configs as W
     N, B = 120_000, 12
     p = W.csg_union_geometry(n_histories=N, n_batches=B)
     o = Oracle(p); g = M.Problem(p)
-    assert g.info()["warp_kernel_ok"] == 0                 # regions run on the census-stepped kernel
+    assert g.info()["warp_kernel_ok"] == 1                 # regions run on the history kernel too (its RGN instantiations)
     o.enable_collision_tally(); g.enable_collision_tally()
     if tech:
         o.set_technique(**tech); g.set_technique(**tech)
     o.run(N, p.seed, n_batches=B, record_history_events=True)
-    g.run(record_history_events=True)
+    g.run(record_history_events=True, scheduler=scheduler)
+    assert g.kernel_info().startswith("k_transport" if scheduler else "k_warp<1,1,%d,0,512,rgn>" %
+                                      (2 if tech and tech.get("population_control") else 1))
     co, cg = o.counters(), g.counters()
     for k in COUNTS:
         assert cg[k] == co[k], (k, cg[k], co[k])
@@ -51,6 +55,7 @@ def test_beam_through_the_union_closed_form_on_the_gpu(M):
     N = 200_000
     p = W.csg_union_geometry(n_histories=N, n_batches=10, beam=True)
     g = M.Problem(p); g.run()
+    assert g.kernel_info().startswith("k_warp<1,0,0,0,512,rgn>")
     c = g.counters()
     t_exact = np.exp(-6.5)                                 # union of the two spheres along the axis: x = 1 .. 7.5
     assert c["leak"] / N == pytest.approx(t_exact, abs=4.5 * np.sqrt(t_exact * (1 - t_exact) / N))
