@@ -160,6 +160,9 @@ class Oracle:
     def __init__(self, prob):
         L = _load()
         self._L = L
+        if getattr(prob, "meta", {}).get("lattice") is not None:   # universes / lattices: expanded here (oracle/lattice.py)
+            from .lattice import flat_problem
+            prob = flat_problem(prob)
         self.prob = prob
         d = _Desc()
         d.G, d.M, d.S, d.C = prob.n_groups, prob.n_materials, prob.n_surfaces, prob.n_cells

@@ -551,5 +551,90 @@ def csg_union_geometry(n_histories=60_000, n_batches=12, beam=False):
     return p
 
 
+# ----------------------------------------------------------------------------------------
+# Universes and lattices (DESIGN.md Appendix K): geometry given as a rectangular array of elements, each filled with
+# a universe -- surfaces and cells in coordinates local to the element (origin at its centre in x and y, z unshifted).
+# A universe cell lists half-spaces of the universe's own surfaces (index >= 0) or of the element's six faces
+# (LAT_XLO .. LAT_ZHI).  The description travels in meta["lattice"]; the flat arrays of the Problem stay empty and
+# the library / the oracle each expand it themselves.  Input tables only: no arithmetic of the method.
+# ----------------------------------------------------------------------------------------
+LAT_XLO, LAT_XHI, LAT_YLO, LAT_YHI, LAT_ZLO, LAT_ZHI = -1, -2, -3, -4, -5, -6
+
+
+def _lattice_problem(name, mats, ss, speed, lattice, src, mesh, time_edges, census, n_histories, n_batches, seed, meta=None):
+    p = _assemble(name, mats, ss, speed, [np.zeros(10)], [0], [], src, mesh, time_edges, census, n_histories, n_batches,
+                  seed, meta=dict(meta or {}, lattice=lattice))
+    p.surf_coef = np.zeros((0, 10)); p.surf_bc = _i32([])                   # no flat geometry: see meta["lattice"]
+    return p
+
+
+def config3_lattice(n_histories=10_000_000, n_batches=100, n_pins=17):
+    """Config 3 written as a 17 x 17 lattice of two pin-cell universes (fuel A / fuel B in a checkerboard) instead of
+    578 hand-written cells; the expansion must give config3_pin_lattice's tables exactly."""
+    p, r, H = 1.26, 0.54, 10.0
+    n = n_pins
+    mats, ss, speed, k0 = config3_xs(p, r)
+
+    def pin_universe(fuel):
+        return dict(surf=[cylinder_z(0.0, 0.0, r)],
+                    cells=[([(0, -1), (LAT_ZLO, +1), (LAT_ZHI, -1)], fuel),
+                           ([(LAT_XLO, +1), (LAT_XHI, -1), (LAT_YLO, +1), (LAT_YHI, -1), (0, +1), (LAT_ZLO, +1),
+                             (LAT_ZHI, -1)], 2)])
+    lattice = dict(universes=[pin_universe(0), pin_universe(1)], nx=n, ny=n, x0=0.0, y0=0.0, pitch_x=p, pitch_y=p,
+                   z_lo=0.0, z_hi=H, fill=[[(i + j) % 2 for i in range(n)] for j in range(n)],
+                   bc=[BC_REFLECTIVE, BC_REFLECTIVE, BC_REFLECTIVE, BC_REFLECTIVE, BC_VACUUM, BC_VACUUM])
+    c = 0.5 * n * p
+    src = dict(lo=[c, c, 0.5 * H], hi=[c, c, 0.5 * H], t0=0.0, t1=0.0, pdf=mats["chi"][0].copy())
+    mesh = dict(lo=[0.0, 0.0, 0.0], hi=[n * p, n * p, H], n=[n, n, 1])
+    T = np.array([k * 5e-7 for k in range(21)], dtype=np.float64)
+    return _lattice_problem("config3_lattice", mats, ss, speed, lattice, src, mesh, T, T[1:].copy(), n_histories,
+                            n_batches, run_seed(3), meta=dict(k0=k0, pitch=p, radius=r))
+
+
+LATTICE_MIXED = dict(nx=4, ny=3, x0=-2.5, y0=1.0, pitch_x=1.5, pitch_y=2.0, z_lo=-1.0, z_hi=3.0,
+                     r_fuel=0.4, r_clad=0.55, ball=(0.1, -0.2, 1.0, 0.45))   # ball: local centre and radius
+
+
+def lattice_mixed(n_histories=60_000, n_batches=12):
+    """Parity / pin workload: a 4 x 3 lattice that does not start at the origin, with unequal pitches and three
+    universes -- a clad pin (two concentric z-cylinders, three cells), a bare moderator box (one cell, no surface) and
+    a box holding an off-centre ball (a translated general quadric); vacuum in x, reflective in y and at the bottom,
+    vacuum on top; two groups; a source box over the whole lattice; a mesh that does not follow the elements."""
+    G = 2
+    L = LATTICE_MIXED
+    mats, ss = _materials([
+        dict(sigma_t=[0.8, 1.2], sigma_c=[0.15, 0.4], sigma_f=[0.05, 0.1], nu=[2.2, 2.5], chi=[0.7, 0.3],
+             sigma_s=[[0.4, 0.2], [0.0, 0.7]]),                                  # fuel
+        dict(sigma_t=[0.3, 0.5], sigma_c=[0.05, 0.1], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+             sigma_s=[[0.2, 0.05], [0.02, 0.38]]),                               # clad
+        dict(sigma_t=[0.6, 0.9], sigma_c=[0.1, 0.2], sigma_f=[0.0, 0.0], nu=[0.0, 0.0], chi=[0.0, 0.0],
+             sigma_s=[[0.3, 0.2], [0.1, 0.6]]),                                  # moderator
+    ], G)
+    box = [(LAT_XLO, +1), (LAT_XHI, -1), (LAT_YLO, +1), (LAT_YHI, -1), (LAT_ZLO, +1), (LAT_ZHI, -1)]
+    u_pin = dict(surf=[cylinder_z(0.0, 0.0, L["r_fuel"]), cylinder_z(0.0, 0.0, L["r_clad"])],
+                 cells=[([(0, -1), (LAT_ZLO, +1), (LAT_ZHI, -1)], 0),
+                        ([(0, +1), (1, -1), (LAT_ZLO, +1), (LAT_ZHI, -1)], 1),
+                        (box + [(1, +1)], 2)])
+    u_box = dict(surf=[], cells=[(box, 2)])
+    u_ball = dict(surf=[sphere(*L["ball"])], cells=[([(0, -1)], 0), (box + [(0, +1)], 2)])
+    fill = [[0, 1, 2, 0],
+            [2, 0, 0, 1],
+            [0, 2, 1, 0]]
+    lattice = dict(universes=[u_pin, u_box, u_ball], nx=L["nx"], ny=L["ny"], x0=L["x0"], y0=L["y0"],
+                   pitch_x=L["pitch_x"], pitch_y=L["pitch_y"], z_lo=L["z_lo"], z_hi=L["z_hi"], fill=fill,
+                   bc=[BC_VACUUM, BC_VACUUM, BC_REFLECTIVE, BC_REFLECTIVE, BC_REFLECTIVE, BC_VACUUM])
+    x1 = L["x0"] + L["nx"] * L["pitch_x"]; y1 = L["y0"] + L["ny"] * L["pitch_y"]
+    src = dict(lo=[L["x0"], L["y0"], L["z_lo"]], hi=[x1, y1, L["z_hi"]], t0=0.0, t1=1.0, pdf=[0.6, 0.4])
+    mesh = dict(lo=[L["x0"], L["y0"], L["z_lo"]], hi=[x1, y1, L["z_hi"]], n=[5, 4, 2])
+    T = np.array([0.0, 1.0, 2.5, 5.0, 9.0])
+    return _lattice_problem("lattice_mixed", mats, ss, [1.0, 0.4], lattice, src, mesh, T, np.array([2.0, 4.5, 9.0]),
+                            n_histories, n_batches, run_seed(13))
+
+
+CONFIGS["csg_union"] = csg_union_geometry
+CONFIGS["config3_lattice"] = config3_lattice
+CONFIGS["lattice_mixed"] = lattice_mixed
+
+
 def get_config(name: str, **kw) -> Problem:
     return CONFIGS[name](**kw)
