@@ -156,6 +156,43 @@ int mcdc_problem_create(const mcdc_problem_desc *d, mcdc_problem **out);
 enum { MCDC_RGN_AND = -1, MCDC_RGN_OR = -2, MCDC_RGN_NOT = -3 };
 int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t *region_offset,
                             const int32_t *region_rpn, mcdc_problem **out);
+/* Universes and lattices ("full three-dimensional constructive solid geometry" is all the paper says;
+ * SURVEY.md 8(f) NEXT-4; definition in DESIGN.md Appendix K).  A lattice is an nx x ny array of box elements of size
+ * pitch_x x pitch_y with corner (x0, y0), all spanning z_lo .. z_hi; element (i, j) is filled with universe
+ * fill[j * nx + i].  Universe u owns the quadric surfaces usurf_coef[usurf_offset[u] .. usurf_offset[u+1])[10],
+ * given in coordinates LOCAL to an element (origin at the element's centre in x and y; z is not shifted), and the
+ * cells ucell_offset[u] .. ucell_offset[u+1); universe cell c is the intersection of the half-spaces
+ * uhs_offset[c] .. uhs_offset[c+1): uhs_surface >= 0 names a surface of the same universe (0-based within it), a
+ * negative value one of the element's faces (MCDC_LAT_*), uhs_sense is +1 / -1 as in mcdc_problem_desc.
+ * The flat geometry, in this order: surfaces = planes x = x0 + i pitch_x (i = 0..nx), planes y = y0 + j pitch_y
+ * (j = 0..ny), z = z_lo, z = z_hi -- outer ones with bc[MCDC_LAT face order: x-lo x-hi y-lo y-hi z-lo z-hi], inner ones
+ * transmission -- then element by element (j outer, i inner) the universe's surfaces translated to the element's
+ * centre (f(r - c), all transmission); cells = element by element in the same order, the universe's cells in their
+ * order, half-space lists in their order.  All arrays are HOST memory, deep-copied.
+ *  mcdc_lattice_expand_size / mcdc_lattice_expand: the flat arrays themselves (no device needed), into caller
+ *    buffers of surf_coef[S][10], surf_bc[S], cell_offset[C+1], hs_surface[H], hs_sense[H], cell_material[C].
+ *  mcdc_problem_create_lattice: mcdc_problem_create on *d with its geometry fields (n_surfaces, n_cells, surf_*,
+ *    cell_offset, hs_*, cell_material: ignored, may be 0 / NULL) replaced by the expansion.
+ * A malformed description (universe id or local surface out of range, unknown face code, empty cell, sense not
+ * +-1, non-positive pitch, z_hi <= z_lo, bc out of range) gives MCDC_ERR_GEOM.                            */
+enum { MCDC_LAT_XLO = -1, MCDC_LAT_XHI = -2, MCDC_LAT_YLO = -3, MCDC_LAT_YHI = -4, MCDC_LAT_ZLO = -5, MCDC_LAT_ZHI = -6 };
+typedef struct {
+  int32_t n_universes;
+  const int32_t *usurf_offset;             /* [U+1]                                                  */
+  const double *usurf_coef;                /* [usurf_offset[U]][10], local coordinates               */
+  const int32_t *ucell_offset;             /* [U+1]                                                  */
+  const int32_t *uhs_offset;               /* [ucell_offset[U] + 1]                                  */
+  const int32_t *uhs_surface, *uhs_sense;  /* [uhs_offset[ucell_offset[U]]]                          */
+  const int32_t *ucell_material;           /* [ucell_offset[U]]                                      */
+  int32_t nx, ny;
+  double x0, y0, pitch_x, pitch_y, z_lo, z_hi;
+  const int32_t *fill;                     /* [ny][nx] universe of element (i, j)                    */
+  int32_t bc[6];                           /* MCDC_BC_* of the outer faces                           */
+} mcdc_lattice_desc;
+int mcdc_lattice_expand_size(const mcdc_lattice_desc *lat, int32_t *n_surfaces, int32_t *n_cells, int32_t *n_halfspaces);
+int mcdc_lattice_expand(const mcdc_lattice_desc *lat, double *surf_coef, int32_t *surf_bc, int32_t *cell_offset,
+                        int32_t *hs_surface, int32_t *hs_sense, int32_t *cell_material);
+int mcdc_problem_create_lattice(const mcdc_problem_desc *d, const mcdc_lattice_desc *lat, mcdc_problem **out);
 void mcdc_problem_destroy(mcdc_problem *p);
 /* Zero tallies, ledger, census populations and counters (keeps problem and workspace).            */
 int mcdc_problem_reset(mcdc_problem *p);

@@ -21,6 +21,7 @@ EXPORTED_SYMBOLS = [
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
     "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
     "mcdc_collision_tally_enable", "mcdc_collision_tallies_get", "mcdc_problem_create_csg", "mcdc_kernel_info_get",
+    "mcdc_lattice_expand_size", "mcdc_lattice_expand", "mcdc_problem_create_lattice",
 ]
 
 _dp = C.POINTER(C.c_double)
@@ -48,6 +49,13 @@ class ProblemDesc(C.Structure):
         ("mesh_lo", C.c_double * 3), ("mesh_hi", C.c_double * 3), ("mesh_n", C.c_int32 * 3),
         ("n_time_bins", C.c_int32), ("time_edges", _dp), ("n_census", C.c_int32), ("census_times", _dp),
     ]
+
+
+class LatticeDesc(C.Structure):
+    _fields_ = [("n_universes", C.c_int32), ("usurf_offset", _ip), ("usurf_coef", _dp), ("ucell_offset", _ip),
+                ("uhs_offset", _ip), ("uhs_surface", _ip), ("uhs_sense", _ip), ("ucell_material", _ip),
+                ("nx", C.c_int32), ("ny", C.c_int32), ("x0", C.c_double), ("y0", C.c_double), ("pitch_x", C.c_double),
+                ("pitch_y", C.c_double), ("z_lo", C.c_double), ("z_hi", C.c_double), ("fill", _ip), ("bc", C.c_int32 * 6)]
 
 
 class RunOpts(C.Structure):
@@ -98,6 +106,11 @@ def lib():
     L.mcdc_problem_create.argtypes = [C.POINTER(ProblemDesc), C.POINTER(vp)]; L.mcdc_problem_create.restype = C.c_int
     L.mcdc_problem_create_csg.argtypes = [C.POINTER(ProblemDesc), _ip, _ip, C.POINTER(vp)]
     L.mcdc_problem_create_csg.restype = C.c_int
+    i32p = C.POINTER(C.c_int32)
+    L.mcdc_lattice_expand_size.argtypes = [C.POINTER(LatticeDesc), i32p, i32p, i32p]; L.mcdc_lattice_expand_size.restype = C.c_int
+    L.mcdc_lattice_expand.argtypes = [C.POINTER(LatticeDesc), _dp, _ip, _ip, _ip, _ip, _ip]; L.mcdc_lattice_expand.restype = C.c_int
+    L.mcdc_problem_create_lattice.argtypes = [C.POINTER(ProblemDesc), C.POINTER(LatticeDesc), C.POINTER(vp)]
+    L.mcdc_problem_create_lattice.restype = C.c_int
     L.mcdc_problem_destroy.argtypes = [vp]; L.mcdc_problem_destroy.restype = None
     L.mcdc_problem_reset.argtypes = [vp]; L.mcdc_problem_reset.restype = C.c_int
     L.mcdc_workspace_size.argtypes = [vp, C.c_uint64, C.c_uint32, C.POINTER(C.c_size_t)]
@@ -187,9 +200,72 @@ def _make_desc(prob):
     return d, keep
 
 
+def _make_lattice(lat):
+    """The lattice dict of workloads.configs (universes = [{surf: [coef10, ...], cells: [([(surface, sense), ...],
+    material), ...]}, ...], nx, ny, x0, y0, pitch_x, pitch_y, z_lo, z_hi, fill [ny][nx], bc [6]) -> (LatticeDesc, keep-alive)."""
+    us_off, uc_off, uh_off, coef, hs_s, hs_n, mat = [0], [0], [0], [], [], [], []
+    for u in lat["universes"]:
+        coef += [np.asarray(c, dtype=np.float64).reshape(10) for c in u["surf"]]
+        us_off.append(len(coef))
+        for hs, m in u["cells"]:
+            for s, sense in hs:
+                hs_s.append(int(s)); hs_n.append(int(sense))
+            uh_off.append(len(hs_s)); mat.append(int(m))
+        uc_off.append(len(mat))
+    arr = dict(us_off=np.asarray(us_off, dtype=np.int32), uc_off=np.asarray(uc_off, dtype=np.int32),
+               uh_off=np.asarray(uh_off, dtype=np.int32), hs_s=np.asarray(hs_s, dtype=np.int32),
+               hs_n=np.asarray(hs_n, dtype=np.int32), mat=np.asarray(mat, dtype=np.int32),
+               coef=np.ascontiguousarray(np.stack(coef) if coef else np.zeros((1, 10)), dtype=np.float64),
+               fill=np.ascontiguousarray(np.asarray(lat["fill"], dtype=np.int32).reshape(-1)))
+    d = LatticeDesc()
+    d.n_universes = len(lat["universes"])
+    d.usurf_offset, d.usurf_coef, d.ucell_offset, d.uhs_offset = _i(arr["us_off"]), _d(arr["coef"]), _i(arr["uc_off"]), _i(arr["uh_off"])
+    d.uhs_surface, d.uhs_sense, d.ucell_material = _i(arr["hs_s"]), _i(arr["hs_n"]), _i(arr["mat"])
+    d.nx, d.ny = int(lat["nx"]), int(lat["ny"])
+    if arr["fill"].size != d.nx * d.ny:
+        raise McdcError(-3, "mcdc_lattice", "fill must be [ny][nx]")
+    d.x0, d.y0, d.pitch_x, d.pitch_y = float(lat["x0"]), float(lat["y0"]), float(lat["pitch_x"]), float(lat["pitch_y"])
+    d.z_lo, d.z_hi = float(lat["z_lo"]), float(lat["z_hi"])
+    d.fill = _i(arr["fill"])
+    d.bc = (C.c_int32 * 6)(*[int(b) for b in lat["bc"]])
+    return d, arr
+
+
+def mcdc_lattice_expand(lat) -> dict:
+    """The flat geometry of a lattice description (mcdc_lattice_expand_size + mcdc_lattice_expand; no device needed)."""
+    d, keep = _make_lattice(lat)
+    nS, nC, nH = C.c_int32(), C.c_int32(), C.c_int32()
+    _check(lib().mcdc_lattice_expand_size(C.byref(d), C.byref(nS), C.byref(nC), C.byref(nH)), "mcdc_lattice_expand_size")
+    out = dict(surf_coef=np.empty((nS.value, 10)), surf_bc=np.empty(nS.value, dtype=np.int32),
+               cell_offset=np.empty(nC.value + 1, dtype=np.int32), hs_surface=np.empty(nH.value, dtype=np.int32),
+               hs_sense=np.empty(nH.value, dtype=np.int32), cell_material=np.empty(nC.value, dtype=np.int32))
+    _check(lib().mcdc_lattice_expand(C.byref(d), _d(out["surf_coef"]), _i(out["surf_bc"]), _i(out["cell_offset"]),
+                                     _i(out["hs_surface"]), _i(out["hs_sense"]), _i(out["cell_material"])), "mcdc_lattice_expand")
+    return out
+
+
+def mcdc_lattice_expand_size(lat):
+    d, keep = _make_lattice(lat)
+    nS, nC, nH = C.c_int32(), C.c_int32(), C.c_int32()
+    _check(lib().mcdc_lattice_expand_size(C.byref(d), C.byref(nS), C.byref(nC), C.byref(nH)), "mcdc_lattice_expand_size")
+    return nS.value, nC.value, nH.value
+
+
+def mcdc_problem_create_lattice(prob, lat):
+    d, keep = _make_desc(prob)
+    ld, keep2 = _make_lattice(lat)
+    h = C.c_void_p()
+    _check(lib().mcdc_problem_create_lattice(C.byref(d), C.byref(ld), C.byref(h)), "mcdc_problem_create_lattice")
+    return h
+
+
 # ---- functions with the names of include/mcdc.h ------------------------------------------------
 def mcdc_problem_create(prob):
-    """prob.meta["regions"] = (region_offset, region_rpn), when present, makes this mcdc_problem_create_csg."""
+    """prob.meta["regions"] = (region_offset, region_rpn), when present, makes this mcdc_problem_create_csg;
+    prob.meta["lattice"] makes it mcdc_problem_create_lattice."""
+    lat = (getattr(prob, "meta", None) or {}).get("lattice")
+    if lat is not None:
+        return mcdc_problem_create_lattice(prob, lat)
     rgn = (getattr(prob, "meta", None) or {}).get("regions")
     if rgn is not None:
         return mcdc_problem_create_csg(prob, rgn[0], rgn[1])

@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(CSRC, "_obj")
 LIB = os.path.join(HERE, "libmcdc.so")
 # (source, object name, extra defines)
-UNITS = [("mcdc_host.cu", "mcdc_host.o", [])] + \
+UNITS = [("mcdc_host.cu", "mcdc_host.o", []), ("mcdc_lattice.cu", "mcdc_lattice.o", [])] + \
         [("mcdc_warp_inst.cu", f"mcdc_warp_v{v}.o", [f"-DMCDC_WARP_VARIANT={v}"]) for v in range(4)]
 HEADERS = ["mcdc_types.h", "mcdc_device.cuh", "mcdc_step.cuh", "mcdc_kernels.cuh", "mcdc_warp.cuh", "mcdc_warp_inst.cuh"]
 
@@ -42,7 +42,7 @@ def _stale() -> bool:
     if not os.path.exists(LIB):
         return True
     t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in [u[0] for u in UNITS] + HEADERS]
+    deps = [os.path.join(CSRC, f) for f in sorted(set(u[0] for u in UNITS)) + HEADERS]
     deps.append(os.path.join(os.path.dirname(HERE), "include", "mcdc.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
