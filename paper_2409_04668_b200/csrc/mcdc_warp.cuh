@@ -220,6 +220,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
   if (step_mode && !A.step_source) src_exhausted = true;
   uint32_t n_seg = 0u;                                 // segments of this warp (warp-uniform)
+  double acc_popw = 0.0;                               // census-step mode: weight this lane saw arrive at census A.step_k
   enum { W_COLL = 0, W_CHILDREN, W_LOST, W_SRC };
 #define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
@@ -538,7 +539,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // ---- move (A.3) ----
       x += d * ux; y += d * uy; z += d * uz;
       t = (ev == EV_CENSUS) ? t_census : t + d * tb.inv_speed(g);
-      bool alive = act, lost = false;
+      bool alive = act, lost = false, leaked = false;
       uint32_t new_cl = cl;
       int census_k = -1;
       if (ev == EV_CENSUS) {                           // A.8: bookkeeping only, then the next interval
@@ -558,9 +559,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const int type = is_face ? (which >> 1) : (int)((e.y >> 9) & 7u);   // faces: ST_PLANE_X/Y/Z = axis
         int idx = is_face ? -1 : (int)(e.y & 255u);
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
-        if (bc == 1) {                                 // vacuum: leaks
-          alive = false;
-          atomicAdd(&sh.led[LED_LEAK], w);
+        if (bc == 1) {                                 // vacuum: leaks (summed over the warp below)
+          alive = false; leaked = true;
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
           if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
           else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
@@ -613,16 +613,27 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           }
         }
       }
-      // ---- census population (A.8): one shared-memory add per distinct census index in the warp ----
+      // ---- census population (A.8): one shared-memory count per distinct census index in the warp ----
       const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
       if (m_cen) {
         const unsigned peers = __match_any_sync(MCDC_FULL, census_k);
         if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
         const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
         if (WEIGHTED) {
-          if (census_k >= 0) atomicAdd(s_popw + census_k, w);
-          if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
+          // Lanes that add to the same shared-memory double serialise in a compare-and-swap loop, and in census-step
+          // mode every census event of the launch carries the same index, A.step_k: that one add was 56 % of the samples
+          // of a census-step launch (profiles/r02c).  There the weight is summed in a register and leaves at the end.
+          if (step_mode) { if (census_k >= 0) acc_popw += w; }
+          else {
+            if (census_k >= 0) atomicAdd(s_popw + census_k, w);
+            if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
+          }
         } else if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
+      }
+      if (WEIGHTED) { if (leaked) atomicAdd(&sh.led[LED_LEAK], w); }   // (few lanes leak in one round)
+      else {                                           // unit weights: one shared-memory add per warp
+        const unsigned m_leak = __ballot_sync(MCDC_FULL, leaked);
+        if (m_leak && lane == 0) atomicAdd(&sh.led[LED_LEAK], (double)__popc(m_leak));
       }
       // (surface events are not counted here: segments - collisions - census events, at the end of the block)
       if (__any_sync(MCDC_FULL, lost)) WCNT(W_LOST, (uint32_t)__popc(__ballot_sync(MCDC_FULL, lost)));
@@ -833,6 +844,13 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
 
   // ---- warp totals -> block totals -> global ----
   __syncwarp();
+  if (WEIGHTED && step_mode) {
+    const double s = warp_sum(acc_popw);
+    if (lane == 0 && s != 0.0) {
+      atomicAdd(s_popw + A.step_k, s);
+      if (A.step_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], s);
+    }
+  }
   if (lane == 0) {
     const uint32_t *wc = sh.wcnt[wid];
     atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_seg, (unsigned long long)n_seg);
