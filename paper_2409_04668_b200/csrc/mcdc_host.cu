@@ -1211,11 +1211,13 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
 }
 
 // ---- population control on the history kernel: one k_warp<WEIGHTED> launch per census step (census-step mode),
-// the control kernels between the steps; the host reads the bank counters once per step ----
+// the control kernels between the steps.  Nothing comes back to the host inside the loop: the launches of all census
+// steps are queued back to back ("mid-run host <-> device copies" are the cost the paper itself names).
+// What the host used to read per step is decided on the device instead: grids are sized for the bank capacity and
+// blocks without work leave at once; a bank overflow sets the device flag that mcdc_run_ex checks after the run.
 int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record) {
   const uint32_t ns = sb.n_slots, ws_ns = p->ws_slots;
   uint32_t *counts_dev = p->counts_dev;
-  std::vector<uint32_t> h_counts((size_t)8 * ws_ns);
   CK(cudaMemsetAsync(counts_dev, 0, (size_t)8 * ws_ns * sizeof(uint32_t), p->stream));
   Bank A = p->bankA, Bk = p->bankB;
   const int k_first = step_of(p, p->src_t0), k_last = step_of(p, p->src_t1);
@@ -1237,58 +1239,36 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   ha.src_chunk = (uint32_t)std::max<uint64_t>(32, std::min<uint64_t>(128, (uint64_t)sb.n_hist / ((uint64_t)grid_src * (nt / 32) * 8)));
   ha.n_slots = sb.n_slots;
   ha.step_mode = 1; ha.step_single = (k_first == k_last) ? 1 : 0; ha.bank_cap = p->cap;
-  uint64_t live_total = 0;
-  for (int k = 0; k < p->K; ++k) {
-    const bool src = k >= k_first && k <= k_last;
-    if (!src && live_total == 0) {
-      if (k > k_last) break;
-      continue;
-    }
+  // the population in flight is not known here: as many blocks as the banks could feed (a run of a few thousand
+  // histories does not wake every SM), every SM otherwise
+  const uint64_t work_max = std::max<uint64_t>((uint64_t)sb.n_hist, (uint64_t)std::min<uint64_t>((uint64_t)p->cap * ns, (uint64_t)4 * sb.n_hist));
+  const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work_max + per_block - 1) / per_block));
+  for (int k = k_first; k < p->K; ++k) {
+    const bool src = k <= k_last;
     ha.step_k = k; ha.step_source = src ? 1 : 0;
     ha.n_chunks = src ? sb.n_slots * ((sb.hs + ha.src_chunk - 1) / ha.src_chunk) : 0u;
     ha.in = A; ha.census_out = Bk;
     CK(cudaMemsetAsync(p->d_hist_cursor, 0, sizeof(uint32_t), p->stream));
     CK(cudaMemcpyAsync(p->d_head_tail, p->d_head_tail + 1, sizeof(unsigned long long), cudaMemcpyDeviceToDevice, p->stream));
     CK(cudaMemsetAsync(A.cursor, 0, ns * sizeof(uint32_t), p->stream));
-    const uint64_t work = live_total + (src ? sb.n_hist : 0);
-    const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work + per_block - 1) / per_block));
     cudaEvent_t a, b;
     { const int rce = next_event_pair(p, a, b); if (rce != MCDC_OK) return rce; }
     CK(cudaEventRecord(a, p->stream));
     warp_launch(p, staged, record, KW_CENSUS_STEP, nt, grid, p->pool_smem, p->stream, p->tab, ha);
     CK(cudaEventRecord(b, p->stream));
     p->launches++;
-    CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
-    CK(cudaStreamSynchronize(p->stream));
-    CK(cudaGetLastError());
-    uint32_t n_max = 0;
-    live_total = 0;
-    {
-      const uint32_t *hc = h_counts.data() + (Bk.count - counts_dev);
-      for (uint32_t s = 0; s < ns; ++s) {
-        if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
-        live_total += hc[s]; n_max = std::max(n_max, hc[s]);
-      }
-    }
-    if (k < p->K - 1 && live_total > 0) {
+    if (k < p->K - 1) {
       if (p->tech.population_control) {                   // Appendix G.3: census bank Bk -> live bank A
         PcParams pc;
         pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs; pc.w_out = 0.0;
-        const dim3 pgrid((n_max + 255) / 256, ns);
+        // (a batch holds at most 4x its source count here unless the caller bound a larger bank: blocks past a
+        // slot's count leave at once)
+        const dim3 pgrid((p->cap + 255) / 256, ns);
         CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
         CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
         k_pc_weight<<<pgrid, 256, 0, p->stream>>>(Bk, p->cap, p->d_wfix);
         k_pc_apply<<<pgrid, 256, 0, p->stream>>>(Bk, A, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
         p->launches += 2;
-        CK(cudaMemcpyAsync(h_counts.data(), counts_dev, (size_t)8 * ws_ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
-        CK(cudaStreamSynchronize(p->stream));
-        CK(cudaGetLastError());
-        const uint32_t *hc = h_counts.data() + (A.count - counts_dev);
-        live_total = 0;
-        for (uint32_t s = 0; s < ns; ++s) {
-          if (hc[s] > p->cap) return MCDC_ERR_BANK_OVERFLOW;
-          live_total += hc[s];
-        }
       } else std::swap(A, Bk);
     }
     CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));

@@ -592,6 +592,7 @@ __global__ void __launch_bounds__(256) k_pc_weight(Bank in, uint32_t cap, unsign
   __shared__ unsigned long long scratch[32];
   const int slot = blockIdx.y;
   const uint32_t n = min(in.count[slot], cap);
+  if (blockIdx.x * blockDim.x >= n) return;              // (grids are sized for the bank capacity: no host read of the counts)
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   unsigned long long v = 0ull;
   if (i < n) v = (unsigned long long)(in.w[(size_t)slot * cap + i] * MCDC_FIX40);   // truncation, as the oracle's cast
@@ -612,6 +613,7 @@ __global__ void __launch_bounds__(256) k_pc_apply(Bank in, Bank out, PcParams P,
   __shared__ double scratch[32];
   const int slot = blockIdx.y, lane = lane_id();
   const uint32_t n_in = min(in.count[slot], P.cap);
+  if (blockIdx.x * blockDim.x >= n_in) return;
   const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
   const unsigned long long W = wfix[slot];
   const bool have = i < n_in && W != 0ull;
