@@ -65,6 +65,8 @@ struct TB {
   }
 };
 
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ------------------------------------------------------------------------------------------------
 // RNG: counter-based, keyed by a 64-bit particle key; draw index = particle counter (Appendix B).
 // ------------------------------------------------------------------------------------------------

@@ -218,6 +218,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   constexpr bool gen_mode = VARIANT == 3;              // k-eigenvalue: `in` holds birth records, children go to `census_out`
   bool bank_done = !step_mode;                         // the live bank of this step has been handed out
   uint32_t bank_slot = (blockIdx.x * (uint32_t)NW + (uint32_t)wid) % max(A.n_slots, 1u), bank_probes = 0u;
+  uint32_t res_next = 0u, res_end = 0u;                // records of bank_slot's bank reserved by this warp, not yet taken
+  enum { BANK_CHUNK = 128 };
   if (step_mode && !A.step_source) src_exhausted = true;
   uint32_t n_seg = 0u;                                 // segments of this warp (warp-uniform)
   double acc_popw = 0.0;                               // census-step mode: weight this lane saw arrive at census A.step_k
@@ -244,16 +246,30 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const uint32_t want = min(32u, max(room, 1u));   // (room = 0 only with an empty pool smaller than the reserve)
       if (step_mode && !bank_done) {
         // ---- census-step mode: particles of the live bank first (full records: nothing is sampled here) ----
-        uint32_t base = 0u, cnt = 0u;
-        if (lane == 0) { cnt = min(A.in.count[bank_slot], A.bank_cap); base = atomicAdd(A.in.cursor + bank_slot, want); }
-        base = __shfl_sync(MCDC_FULL, base, 0); cnt = __shfl_sync(MCDC_FULL, cnt, 0);
-        if (base >= cnt) {                               // this batch slot is handed out: try the next one
-          bank_slot = (bank_slot + 1u) % A.n_slots;
-          if (++bank_probes >= A.n_slots) bank_done = true;
-          continue;
+        // The warp reserves BANK_CHUNK records of the current batch slot's bank with one global atomic and asks for them
+        // in L2; its refills then take up to 32 of them at a time.  (One returning atomic and one trip to DRAM per
+        // refill were a quarter of the warp time of a census-step launch, profiles/r02d.)
+        if (res_next == res_end) {
+          uint32_t rb = 0u, cnt = 0u;
+          if (lane == 0) { cnt = min(A.in.count[bank_slot], A.bank_cap); rb = atomicAdd(A.in.cursor + bank_slot, (uint32_t)BANK_CHUNK); }
+          rb = __shfl_sync(MCDC_FULL, rb, 0); cnt = __shfl_sync(MCDC_FULL, cnt, 0);
+          if (rb >= cnt) {                               // this batch slot is handed out: try the next one
+            bank_slot = (bank_slot + 1u) % A.n_slots;
+            if (++bank_probes >= A.n_slots) bank_done = true;
+            continue;
+          }
+          bank_probes = 0u;
+          res_next = rb; res_end = min(rb + (uint32_t)BANK_CHUNK, cnt);
+          for (uint32_t r = res_next + 32u + (uint32_t)lane; r < res_end; r += 32u) {   // (the first 32 are loaded right below)
+            const size_t j = (size_t)bank_slot * A.bank_cap + r;
+            prefetch_l2(A.in.x + j); prefetch_l2(A.in.y + j); prefetch_l2(A.in.z + j); prefetch_l2(A.in.t + j);
+            prefetch_l2(A.in.w + j); prefetch_l2(A.in.key + j); prefetch_l2(A.in.meta + j);
+            if (!gen_mode) { prefetch_l2(A.in.ux + j); prefetch_l2(A.in.uy + j); prefetch_l2(A.in.uz + j); }
+          }
         }
-        bank_probes = 0u;
-        const uint32_t nb = min(want, cnt - base);
+        const uint32_t base = res_next;
+        const uint32_t nb = min(want, res_end - res_next);
+        res_next += nb;
         const bool actb = (uint32_t)lane < nb;
         unsigned long long bkey = 0ull;
         uint32_t bctr = 0u, bgi = 0u;
@@ -513,6 +529,20 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       else if (d_surf <= d_coll) { d = d_surf; ev = EV_SURFACE; }
       else { d = d_coll; ev = EV_COLLISION; }
       if (!act) { ev = -1; d = 0.0; }
+      // census-step mode: the arrivals of this round will be appended to their batch's census bank further down; the
+      // counter is bumped here, one atomic per batch slot in the warp, so that its round trip overlaps the rest of the round
+      unsigned park_peers = 0u;
+      int park_leader = 0;
+      uint32_t park_base = 0u;
+      if (step_mode) {
+        const bool park = act && ev == EV_CENSUS && pk != T.K - 1;
+        if (__any_sync(MCDC_FULL, park)) {
+          const int bslot = park ? (int)(meta >> 20) : -1;
+          park_peers = __match_any_sync(MCDC_FULL, bslot);
+          park_leader = __ffs(park_peers) - 1;
+          if (park && lane == park_leader) park_base = atomicAdd(A.census_out.count + bslot, (uint32_t)__popc(park_peers));
+        }
+      }
 
       // ---- track-length score (A.7) from the pre-move state ----
       {
@@ -539,7 +569,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // ---- move (A.3) ----
       x += d * ux; y += d * uy; z += d * uz;
       t = (ev == EV_CENSUS) ? t_census : t + d * tb.inv_speed(g);
-      bool alive = act, lost = false, leaked = false;
+      bool alive = act, lost = false;
       uint32_t new_cl = cl;
       int census_k = -1;
       if (ev == EV_CENSUS) {                           // A.8: bookkeeping only, then the next interval
@@ -559,8 +589,9 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const int type = is_face ? (which >> 1) : (int)((e.y >> 9) & 7u);   // faces: ST_PLANE_X/Y/Z = axis
         int idx = is_face ? -1 : (int)(e.y & 255u);
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
-        if (bc == 1) {                                 // vacuum: leaks (summed over the warp below)
-          alive = false; leaked = true;
+        if (bc == 1) {                                 // vacuum: leaks
+          alive = false;
+          atomicAdd(&sh.led[LED_LEAK], w);
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
           if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
           else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
@@ -599,7 +630,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const bool park = act && ev == EV_CENSUS && pk != T.K - 1;
         if (__any_sync(MCDC_FULL, park)) {
           const int bslot = park ? (int)(meta >> 20) : -1;
-          const uint32_t idx = warp_append_by_slot(A.census_out.count, bslot);
+          const uint32_t idx = __shfl_sync(MCDC_FULL, park_base, park_leader) + lanes_below(park_peers, lane);
           if (park) {
             if (idx >= A.bank_cap) atomicExch(&A.cnt->overflow, 1);
             else {
@@ -629,11 +660,6 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
             if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
           }
         } else if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
-      }
-      if (WEIGHTED) { if (leaked) atomicAdd(&sh.led[LED_LEAK], w); }   // (few lanes leak in one round)
-      else {                                           // unit weights: one shared-memory add per warp
-        const unsigned m_leak = __ballot_sync(MCDC_FULL, leaked);
-        if (m_leak && lane == 0) atomicAdd(&sh.led[LED_LEAK], (double)__popc(m_leak));
       }
       // (surface events are not counted here: segments - collisions - census events, at the end of the block)
       if (__any_sync(MCDC_FULL, lost)) WCNT(W_LOST, (uint32_t)__popc(__ballot_sync(MCDC_FULL, lost)));
