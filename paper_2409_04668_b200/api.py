@@ -344,8 +344,16 @@ def mcdc_run_eigenvalue(h, n_particles, seed, n_inactive, n_active):
     return k
 
 
-def mcdc_tallies_get(h, n_bins):
-    mean = np.empty(n_bins); sdev = np.empty(n_bins)
+def mcdc_tallies_get(h, n_bins, out=None):
+    """out = (mean, sdev): caller-owned contiguous float64 arrays of n_bins elements to fill (e.g. views of pinned
+    host memory, which the device-to-host copy then reaches at full PCIe rate); default: fresh arrays."""
+    if out is None:
+        mean = np.empty(n_bins); sdev = np.empty(n_bins)
+    else:
+        mean, sdev = out
+        if mean.size != n_bins or sdev.size != n_bins or mean.dtype != np.float64 or sdev.dtype != np.float64 or \
+                not mean.flags.c_contiguous or not sdev.flags.c_contiguous:
+            raise McdcError(-4, "mcdc_tallies_get", "out arrays must be contiguous float64 of n_bins elements")
     _check(lib().mcdc_tallies_get(h, _d(mean), _d(sdev), n_bins), "mcdc_tallies_get", h)
     return mean, sdev
 

@@ -1573,15 +1573,20 @@ int ensure_collision_buffers(mcdc_problem *p) {
 // A.9 from a pair of device accumulators
 int batch_statistics(mcdc_problem *p, const double *d_sum, const double *d_sumsq, double *mean, double *sdev, size_t n_bins) {
   if (n_bins >= (size_t)1 << 18) {                        // large mesh: the per-bin arithmetic runs on the device
+    // temporaries: two batch accumulators of the bound workspace when it has them (they are zero between runs and are
+    // zeroed again here), else a transient allocation
     double *tmp = nullptr;
-    if (cudaMalloc((void **)&tmp, 2 * n_bins * sizeof(double)) == cudaSuccess) {
+    const bool in_ws = p->x_acc && p->ws_slots >= 2;
+    if (in_ws) tmp = p->x_acc;
+    if (in_ws || cudaMalloc((void **)&tmp, 2 * n_bins * sizeof(double)) == cudaSuccess) {
       const int grid = (int)std::min<size_t>((n_bins + 255) / 256, (size_t)p->n_sm * 16);
       k_statistics<<<grid, 256, 0, p->stream>>>(d_sum, d_sumsq, n_bins, (double)p->histories, (double)p->batches, tmp, tmp + n_bins);
       p->launches++;
       cudaError_t e1 = cudaMemcpyAsync(mean, tmp, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
       cudaError_t e2 = cudaMemcpyAsync(sdev, tmp + n_bins, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+      if (in_ws) cudaMemsetAsync(tmp, 0, 2 * n_bins * sizeof(double), p->stream);
       cudaError_t e3 = cudaStreamSynchronize(p->stream);
-      cudaFree(tmp);
+      if (!in_ws) cudaFree(tmp);
       if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaMemcpyAsync(mean)");
       if (e2 != cudaSuccess) return cuda_fail(p, e2, "cudaMemcpyAsync(sdev)");
       if (e3 != cudaSuccess) return cuda_fail(p, e3, "k_statistics");
