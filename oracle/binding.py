@@ -8,7 +8,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "mcdc_oracle.cpp")
-_LIB = os.path.join(_HERE, "libmcdc_oracle.so")
+# ORACLE_SANITIZE=1: a second build with AddressSanitizer + UBSan (-O1 -g, same -ffp-contract=off), loaded instead of
+# the plain one; run the suite with LD_PRELOAD=$(gcc -print-file-name=libasan.so) (profiles/r02_sanitizers.md)
+_SANITIZE = os.environ.get("ORACLE_SANITIZE", "") not in ("", "0")
+_LIB = os.path.join(_HERE, "libmcdc_oracle_asan.so" if _SANITIZE else "libmcdc_oracle.so")
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -59,7 +62,9 @@ def build(force: bool = False) -> str:
     if (not force and os.path.exists(_LIB)
             and os.path.getmtime(_LIB) >= max(os.path.getmtime(_SRC), os.path.getmtime(hdr))):
         return _LIB
-    cmd = ["g++", "-O2", "-ffp-contract=off", "-std=c++17", "-fPIC", "-shared", "-Wall", "-o", _LIB, _SRC]
+    opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] \
+        if _SANITIZE else ["-O2"]
+    cmd = ["g++"] + opt + ["-ffp-contract=off", "-std=c++17", "-fPIC", "-shared", "-Wall", "-o", _LIB, _SRC]
     subprocess.check_call(cmd)
     return _LIB
 
