@@ -354,7 +354,7 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     }
     s_tot[mg] = run;
     s_sc[mg] = run + p->sigma_c[mg];
-    inv_sig_t[mg] = p->sigma_t[mg] > 0.0 ? 1.0 / p->sigma_t[mg] : 0.0;
+    inv_sig_t[mg] = p->sigma_t[mg] > 0.0 ? 1.0 / p->sigma_t[mg] : HINF;   // void: -log(xi) * inf = no collision (A.2)
   }
   for (int m = 0; m < M; ++m) {
     double run = 0.0;
@@ -527,7 +527,7 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     }
     return -1;
   };
-  bool warp_ok = S < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095;
+  bool warp_ok = S + 2 < (int)NONE16 && C < (int)NONE16 && M <= 255 && G <= 254 && p->K <= 4095;
   std::vector<unsigned char> cell2((size_t)C * CELL2_BYTES, 0), other2;
   size_t n_cert = 0, n_transm = 0;
   for (int c = 0; c < C && warp_ok; ++c) {
@@ -536,7 +536,9 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
     uint16_t fs[6], fn[6], fbc = 0;
     uint8_t fi[6];
     for (int f = 0; f < 6; ++f) {
-      fs[f] = fn[f] = (uint16_t)NONE16; fi[f] = 0;
+      // a side without a face names one of the two sentinel entries behind the surface table: position +inf (upper
+      // side) or -inf (lower side), so that the kernel reads every face position without a test
+      fs[f] = (uint16_t)(S + ((f & 1) ? 0 : 1)); fn[f] = (uint16_t)NONE16; fi[f] = 0;
       const int i = face[c][f];
       if (i < 0) continue;
       const int s = p->hs_surface[i];
@@ -651,7 +653,11 @@ extern "C" int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t
   }
   t.implicit_capture = 0; t.wr_threshold = 0.0; t.wr_survive = 0.0;
   t.o_tbin_k = puti(tbin_k); t.o_it0_k = puti(it0_k);
-  t.o_surf_q = put(q.data(), q.size() * sizeof(double4));
+  {                                                      // + the two sentinel positions of sides without a face
+    std::vector<double4> qs(q);
+    qs.push_back(make_double4(HINF, 0.0, 0.0, 0.0)); qs.push_back(make_double4(-HINF, 0.0, 0.0, 0.0));
+    t.o_surf_q = put(qs.data(), qs.size() * sizeof(double4));
+  }
   t.o_cell2 = put(cell2.data(), cell2.size()); t.o_other2 = put(other2.data(), other2.size());
   bool any_quadric = false;
   for (int s = 0; s < S; ++s) any_quadric = any_quadric || type[s] == ST_QUADRIC;

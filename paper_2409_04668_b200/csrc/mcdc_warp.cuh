@@ -450,15 +450,17 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       nF -= n;
       n_seg += n;                                      // every lane of a flight round makes one segment
       const bool act = (uint32_t)lane < n;
-      const uint32_t i = act ? (uint32_t)PL(L_F, lb + nF + (uint32_t)lane) : 0u;
+      // (a round is almost always full; the idle lanes of a partial one read the slot of its last active lane, so that
+      // no load below needs a guard or a default -- their results are dropped: ev = -1, stores and scores keep `act`)
+      const uint32_t i = (uint32_t)PL(L_F, lb + nF + min((uint32_t)lane, n - 1u));
       const uint32_t gi = lb + i;
       // distance to collision first: the random-number state is dead before the geometry needs its registers
-      uint32_t cl = NONE16 << 16, meta = 0u;
+      uint32_t cl, meta;
       double d_coll;
       {
-        unsigned long long key = 0ull;
-        uint32_t ctr = 0u;
-        if (act) { key = PK(gi); ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
+        const unsigned long long key = PK(gi);
+        const uint32_t ctr = PU(U_CTR, gi);
+        cl = PU(U_CL, gi); meta = PU(U_META, gi);
         // always consumed (D3).  Draw 2b is the first half of block b and leaves the second half in the pool for
         // draw 2b + 1, wherever that one is made (the collision phase reads it; here the block is computed for the
         // even lanes of the round anyway)
@@ -473,13 +475,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const uint32_t rec = T.o_cell2 + (uint32_t)cell * CELL2_BYTES;
       const uint32_t info = tb.template ldb<uint32_t>(rec + C2_INFO);
       const int n_other = (int)(info & 255u), mg = (int)((info >> 8) & 255u) * G + g;
-      d_coll = (tb.sig_t(mg) > 0.0) ? d_coll * tb.inv_sig_t(mg) : INF;
-      double x = 0.0, y = 0.0, z = 0.0, ux = 0.0, uy = 0.0, uz = 1.0, ix = INF, iy = INF, iz = 1.0;
-      double t = 0.0;
-      if (act) {                                       // 1/direction is kept in the pool (three divisions per segment otherwise)
-        const double2 xy = PP(P_XY, gi), zt = PP(P_ZT, gi), u01 = PP(P_U01, gi), u2i0 = PP(P_U2I0, gi), i12 = PP(P_I12, gi);
-        x = xy.x; y = xy.y; z = zt.x; t = zt.y; ux = u01.x; uy = u01.y; uz = u2i0.x; ix = u2i0.y; iy = i12.x; iz = i12.y;
-      }
+      d_coll *= tb.inv_sig_t(mg);                      // (1 / Sigma_t is +inf in a void: no collision)
+      // 1/direction is kept in the pool (three divisions per segment otherwise)
+      const double2 xy = PP(P_XY, gi), zt = PP(P_ZT, gi), u01 = PP(P_U01, gi), u2i0 = PP(P_U2I0, gi), i12 = PP(P_I12, gi);
+      double x = xy.x, y = xy.y, z = zt.x, t = zt.y, ux = u01.x, uy = u01.y, uz = u2i0.x, ix = u2i0.y, iy = i12.x, iz = i12.y;
       // ---- faces: one candidate per axis, picked by the sign of the direction component ----
       // sign bit alone: for a component that is exactly +-0 the face distance is inf or NaN and is rejected below
       const bool px = __double2hiint(ux) >= 0, py = __double2hiint(uy) >= 0, pz = __double2hiint(uz) >= 0;
@@ -487,9 +486,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const uint32_t sfx = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fx);
       const uint32_t sfy = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fy);
       const uint32_t sfz = tb.template ldb<uint16_t>(rec + C2_FACE_SURF + 2u * fz);
-      const double bx = (sfx == NONE16) ? (px ? INF : -INF) : tb.surf_q0((int)sfx);
-      const double by = (sfy == NONE16) ? (py ? INF : -INF) : tb.surf_q0((int)sfy);
-      const double bz = (sfz == NONE16) ? (pz ? INF : -INF) : tb.surf_q0((int)sfz);
+      // (a side without a face names a sentinel entry of the surface table: +inf above, -inf below)
+      const double bx = tb.surf_q0((int)sfx), by = tb.surf_q0((int)sfy), bz = tb.surf_q0((int)sfz);
       const double dx = (bx - x) * ix, dy = (by - y) * iy, dz = (bz - z) * iz;   // 0 * inf = NaN: rejected below
       // nearest face; equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
       const bool vx = pos_finite(dx), vy = pos_finite(dy), vz = pos_finite(dz);
@@ -679,16 +677,17 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const uint32_t n = min(32u, nC);
       nC -= n;
       const bool act = (uint32_t)lane < n;
-      const uint32_t i = act ? (uint32_t)PL(L_C, lb + nC + (uint32_t)lane) : 0u;
+      // (idle lanes of a partial round read the slot of its last active lane, as in the flight phase: no guarded loads)
+      const uint32_t i = (uint32_t)PL(L_C, lb + nC + min((uint32_t)lane, n - 1u));
       const uint32_t gi = lb + i;
-      unsigned long long key = 0ull;
-      uint32_t ctr = 0u, cl = 0u, meta = 0u;
-      unsigned long long r0 = 0ull;                    // the half block the pool kept (used when the counter is odd)
-      if (act) { const ulonglong2 kc = PKC(gi); key = kc.x; r0 = kc.y; ctr = PU(U_CTR, gi); cl = PU(U_CL, gi); meta = PU(U_META, gi); }
+      const ulonglong2 kc = PKC(gi);
+      const unsigned long long key = kc.x;
+      unsigned long long r0 = kc.y;                    // the half block the pool kept (used when the counter is odd)
+      const uint32_t ctr = PU(U_CTR, gi), cl = PU(U_CL, gi), meta = PU(U_META, gi);
       const int cell = (int)(cl & 0xFFFFu);
       int g = (int)(meta & 255u);
-      const bool born = g == 255;                      // a fission child placed in this pool: only its flight is sampled
-      if (born) g = 0;
+      const bool born = act && g == 255;               // a fission child placed in this pool: only its flight is sampled
+      if (g == 255) g = 0;
       const int mat = (int)((tb.template ldb<uint32_t>(T.o_cell2 + (uint32_t)cell * CELL2_BYTES + C2_INFO) >> 8) & 255u);
       const int mg = mat * G + g;
       // The random numbers of this round.  A collision consumes at most four draws from the counter c it arrives with
