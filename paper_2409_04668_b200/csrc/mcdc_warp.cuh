@@ -99,9 +99,10 @@ static __device__ __noinline__ void slow_score_collision(const Tables *gT, doubl
 template <bool STAGED>
 __device__ __forceinline__ void general_score(const Tables &Tg, double *x_acc_slot, int aggregate, bool active,
                                            const double *pool, uint32_t N, uint32_t gi, int g, int pk, double d, double w) {
-  // the pre-move state is still in the pool, as pairs (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz), pair arrays N slots apart
-  const double2 *pp = reinterpret_cast<const double2 *>(pool);
-  const double2 xy = pp[gi], zt = pp[N + gi], u01 = pp[2 * N + gi], u2i0 = pp[3 * N + gi], i12 = pp[4 * N + gi];
+  // the pre-move state is still in the pool: five pairs (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz) per slot
+  (void)N;
+  const double2 *pp = reinterpret_cast<const double2 *>(pool) + 5u * gi;
+  const double2 xy = pp[0], zt = pp[1], u01 = pp[2], u2i0 = pp[3], i12 = pp[4];
   const double x = xy.x, y = xy.y, z = zt.x, t = zt.y, ux = u01.x, uy = u01.y, uz = u2i0.x, ix = u2i0.y, iy = i12.x, iz = i12.y;
   // Tg is the kernel's parameter block (constant bank) when this is inlined -- reading the mesh constants through the
   // device-memory copy of the tables made every DDA step wait on global loads (config 2: long_scoreboard 3.2 per issue)
@@ -126,11 +127,11 @@ __device__ __forceinline__ bool pos_finite(double v) {
 
 __device__ __forceinline__ uint32_t lanes_below(unsigned m, int lane) { return (uint32_t)__popc(m & ((1u << lane) - 1u)); }
 
-// bytes of shared memory per pool slot: x y z ux uy uz 1/ux 1/uy 1/uz t (10 x f64), key, the unused half of the last
-// Philox block (u64), ctr, cell|last, meta, 3 stack entries
+// bytes of shared memory per pool slot: the flight record x y z t ux uy uz 1/ux 1/uy 1/uz (10 x f64, contiguous), the key and
+// the unused half of the last Philox block (2 x u64), ctr, cell | last, meta [, history id] (u32 each), 3 stack entries
 // (+ the weight, one more f64, when a technique of Appendix G makes weights differ from 1)
 __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool weighted) {
-  return (weighted ? 7 : 6) * 16 + 4 + 4 + 4 + 3 + (record ? 4 : 0);
+  return 80 + 16 + 12 + 3 + (record ? 4 : 0) + (weighted ? 8 : 0);
 }
 
 struct WarpShared {                // block-wide totals (static shared memory)
@@ -160,7 +161,6 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   constexpr bool ONEBIN = SCORE != 0;
   constexpr bool WEIGHTED = VARIANT != 0;
   constexpr int NW = NT / 32;
-  constexpr uint32_t NPAIR = WEIGHTED ? 7u : 6u;      // 16-byte pair arrays of the pool
   const double INF = CUDART_INF;
   __shared__ WarpShared sh;
   const TB<STAGED> tb(T);
@@ -168,26 +168,30 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   const uint32_t W = A.pool_slots;                    // slots per warp
   const uint32_t N = W * (uint32_t)NW;
   // ---- carve the dynamic shared memory: [staged tables][census populations][pool arrays][stacks] ----
-  // One offset and the stride N address every array (pointers would cost two registers each):
-  //   16-byte pairs (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz)(key, half block)[(w, -)] -> PP(pair, slot), one LDS.128 each:
-  //     32 lanes gather 32 arbitrary slots, and a 16-byte gather costs fewer shared-memory wavefronts per byte than an
-  //     8-byte one (8 bank groups instead of 16: ~7 wavefronts per 16 B against ~5 per 8 B, profiles/r02c)
-  //   single fields of a pair -> PD(k, slot), k = D_X .. D_W;  key -> PK(slot)
-  //   half block = second half of Philox block ctr >> 1, valid while ctr is odd (Appendix B: "may cache the half-block") -> PC(slot)
-  //   u32  ctr, cell|last<<16, meta = g | census index<<8 | batch slot<<20, [history id]  -> PU(k, slot)
-  //   u8   stacks F, C, FREE -> PL(k, position)
+  // Offsets from pool_off (N = slots of the block):
+  //   flight records, 80 bytes per slot: (x y)(z t)(ux uy)(uz 1/ux)(1/uy 1/uz) as five 16-byte pairs -> PP(pair, slot), one
+  //     LDS.128 each at a constant offset from the slot's address (one multiply per round instead of one per array; 5
+  //     pairs per slot keep a 32-slot gather spread over the bank groups as the slot index itself: 5 is odd);
+  //     single fields -> PD(k, slot), k = D_X .. D_IZ
+  //   N * 80:  (key, half block) per slot -> PKC / PK / PC; half block = second half of Philox block ctr >> 1, valid while
+  //     ctr is odd (Appendix B: "may cache the half-block")
+  //   N * 96:  [weight, f64 per slot -> PW(slot)]   (WEIGHTED)
+  //   then u32 arrays ctr, cell | last << 16, meta = g | census index << 8 | batch slot << 20, [history id] -> PU(k, slot)
+  //     (4-byte stride: the counter store of every flight round stays free of bank conflicts)
+  //   then the u8 stacks F, C, FREE -> PL(k, position)
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
   double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16));   // WEIGHTED only
   const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16) +
                             (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 + 15) / 16 * 16) : 0u);
-#define PP(pr, slot) (*reinterpret_cast<double2 *>(g_smem + pool_off + ((uint32_t)(pr) * N + (slot)) * 16u))
-#define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + (((uint32_t)(k) >> 1) * N + (slot)) * 16u + ((uint32_t)(k) & 1u) * 8u))
-#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (5u * N + (slot)) * 16u))
-#define PC(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + (5u * N + (slot)) * 16u + 8u))
-#define PKC(slot) (*reinterpret_cast<ulonglong2 *>(g_smem + pool_off + (5u * N + (slot)) * 16u))
-#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + NPAIR * 16u * N + ((uint32_t)(k) * N + (slot)) * 4u))
-#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + (NPAIR * 16u + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
-  enum { D_X = 0, D_Y, D_Z, D_T, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, D_W = 12, P_XY = 0, P_ZT, P_U01, P_U2I0, P_I12, P_KEY, P_W,
+#define PP(pr, slot) (*reinterpret_cast<double2 *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(pr) * 16u))
+#define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(k) * 8u))
+#define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + N * 80u + (slot) * 16u))
+#define PC(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + N * 80u + (slot) * 16u + 8u))
+#define PKC(slot) (*reinterpret_cast<ulonglong2 *>(g_smem + pool_off + N * 80u + (slot) * 16u))
+#define PW(slot) (*reinterpret_cast<double *>(g_smem + pool_off + N * 96u + (slot) * 8u))
+#define PU(k, slot) (*reinterpret_cast<uint32_t *>(g_smem + pool_off + N * (WEIGHTED ? 104u : 96u) + ((uint32_t)(k) * N + (slot)) * 4u))
+#define PL(k, pos) (*reinterpret_cast<uint8_t *>(g_smem + pool_off + ((WEIGHTED ? 104u : 96u) + (RECORD ? 16u : 12u)) * N + (uint32_t)(k) * N + (pos)))
+  enum { D_X = 0, D_Y, D_Z, D_T, D_UX, D_UY, D_UZ, D_IX, D_IY, D_IZ, P_XY = 0, P_ZT, P_U01, P_U2I0, P_I12,
          U_CTR = 0, U_CL, U_META, U_HID, L_F = 0, L_C, L_FREE };
 
   if (STAGED) {
@@ -278,7 +282,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
           const int4 m = A.in.meta[j];                   // {cell, -, counter, -}
           PD(D_X, gi) = A.in.x[j]; PD(D_Y, gi) = A.in.y[j]; PD(D_Z, gi) = A.in.z[j]; PD(D_T, gi) = A.in.t[j];
-          PD(D_W, gi) = A.in.w[j];
+          PW(gi) = A.in.w[j];
           PK(gi) = A.in.key[j]; PU(U_CTR, gi) = (uint32_t)m.z;
           PU(U_CL, gi) = (uint32_t)m.x | (NONE16 << 16);
           PU(U_META, gi) = 255u | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
@@ -293,7 +297,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           PD(D_X, gi) = A.in.x[j]; PD(D_Y, gi) = A.in.y[j]; PD(D_Z, gi) = A.in.z[j]; PD(D_T, gi) = A.in.t[j];
           PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
           PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
-          PD(D_W, gi) = A.in.w[j];
+          PW(gi) = A.in.w[j];
           PK(gi) = A.in.key[j]; PU(U_CTR, gi) = (uint32_t)m.z;
           PU(U_CL, gi) = (uint32_t)m.x | ((m.y < 0 ? NONE16 : (uint32_t)m.y) << 16);
           PU(U_META, gi) = (uint32_t)m.w | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
@@ -431,8 +435,9 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const uint32_t gi = lb + i;
         PP(P_XY, gi) = make_double2(x, y); PP(P_ZT, gi) = make_double2(z, t); PP(P_U01, gi) = make_double2(ux, uy);
         PP(P_U2I0, gi) = make_double2(uz, 1.0 / ux); PP(P_I12, gi) = make_double2(1.0 / uy, 1.0 / uz);
-        if (WEIGHTED) PD(D_W, gi) = w;
-        PKC(gi) = make_ulonglong2(key, half); PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
+        if (WEIGHTED) PW(gi) = w;
+        PKC(gi) = make_ulonglong2(key, half);
+        PU(U_CTR, gi) = ctr; PU(U_CL, gi) = (uint32_t)cell | (NONE16 << 16);
         PU(U_META, gi) = (uint32_t)g | ((uint32_t)pk << 8) | (slot << 20);
         if (RECORD) PU(U_HID, gi) = hid;
       }
@@ -518,7 +523,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         if (u < d_surf) { d_surf = u; which = 6 + j; }
       }
       double w = 1.0;
-      if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
+      if (WEIGHTED) w = act ? PW(gi) : 0.0;
       const double t_census = tb.census(pk);
       const double d_time = tb.speed(g) * (t_census - t);
       int ev;
@@ -708,7 +713,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       bool alive = false, captured = false, fissioned = false, reborn = false, rouletted = false;
       uint32_t c0 = 0u;
       double w = 1.0, l_cap = 0.0, l_fis = 0.0, l_prod = 0.0, l_gain = 0.0, l_loss = 0.0;   // WEIGHTED only
-      if (WEIGHTED) w = act ? PD(D_W, gi) : 0.0;
+      if (WEIGHTED) w = act ? PW(gi) : 0.0;
       // Appendix I: collision estimator, arriving weight.  Out of line: inlined, its ~150 instructions sat in the middle
       // of the C phase and cost runs that never enable the tally 8 % (profiles/r01f)
       if (WEIGHTED && A.xc_acc != nullptr && act && !born)
@@ -805,7 +810,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
               const uint32_t r = (uint32_t)(pre - n_push + c);
               const uint32_t i2 = (uint32_t)PL(L_FREE, lb + nFree - 1u - r), g2 = lb + i2;
               PP(P_XY, g2) = xy; PP(P_ZT, g2) = zt;
-              if (WEIGHTED) PD(D_W, g2) = w;
+              if (WEIGHTED) PW(g2) = w;
               PK(g2) = child_key(key, c0, (uint32_t)(c + 1)); PU(U_CTR, g2) = 0u;
               PU(U_CL, g2) = (cl & 0xFFFFu) | (NONE16 << 16);
               PU(U_META, g2) = (meta & ~255u) | 255u;
@@ -828,7 +833,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         PK(gi) = child_key(key, c0, 0u); PU(U_CTR, gi) = 0u;
         PU(U_CL, gi) = (cl & 0xFFFFu) | (NONE16 << 16);
         PU(U_META, gi) = meta | 255u;
-        if (WEIGHTED) PD(D_W, gi) = w;
+        if (WEIGHTED) PW(gi) = w;
       }
       // group and direction of the outgoing flight (A.6): one draw for the group, two for the direction
       if (__any_sync(MCDC_FULL, alive)) {
@@ -850,7 +855,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         if (alive) {
           PP(P_U01, gi) = make_double2(ux, uy); PP(P_U2I0, gi) = make_double2(uz, 1.0 / ux);
           PP(P_I12, gi) = make_double2(1.0 / uy, 1.0 / uz);
-          if (WEIGHTED) PD(D_W, gi) = w;
+          if (WEIGHTED) PW(gi) = w;
           const uint32_t ctr_out = ctr + used;
           PU(U_CTR, gi) = ctr_out;
           if (ctr_out & 1u) PC(gi) = half;             // in the middle of a block: keep its second half for the next draw
@@ -910,6 +915,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
 #undef PC
 #undef PP
 #undef PKC
+#undef PW
 #undef PU
 #undef PL
 #undef WCNT
