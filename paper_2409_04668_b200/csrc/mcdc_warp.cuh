@@ -213,7 +213,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   const Tables *gT = T.self_dev;
   const int G = T.G;
   const long long n_spatial = (long long)T.mesh_n[0] * T.mesh_n[1] * T.mesh_n[2];
-  const bool bins32 = T.n_bins < 0x7FFFFFFFull;        // tally bin indices fit 32 bits: no 64-bit multiply per score
+  // indices into all the batch accumulators fit 32 bits: no 64-bit multiplies per score
+  const bool bins32 = T.n_bins * (unsigned long long)max(A.n_slots, 1u) < 0x7FFFFFFFull;
   // warp-uniform scheduler state
   uint32_t nF = 0u, nC = 0u, nFree = W, dry = 0u, r_calls = 0u;
   uint32_t src_next = 0u, src_end = 0u;                // the warp's chunk of source histories
@@ -495,15 +496,21 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       const double bx = tb.surf_q0((int)sfx), by = tb.surf_q0((int)sfy), bz = tb.surf_q0((int)sfz);
       const double dx = (bx - x) * ix, dy = (by - y) * iy, dz = (bz - z) * iz;   // 0 * inf = NaN: rejected below
       // nearest face; equal distances (an edge hit): the earlier half-space of the cell's list wins (D5)
-      const bool vx = pos_finite(dx), vy = pos_finite(dy), vz = pos_finite(dz);
+      const bool vx = dx > 0.0 && dx < INF, vy = dy > 0.0 && dy < INF, vz = dz > 0.0 && dz < INF;
       double d_surf = vx ? dx : INF;
       int which = vx ? fx : -1;                        // 2*axis + side of the nearest face, 6 + j for other j
-      bool ty = vy && dy < d_surf;
-      if (vy && dy == d_surf) ty = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fy) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
-      if (ty) { d_surf = dy; which = fy; }
-      bool tz = vz && dz < d_surf;
-      if (vz && dz == d_surf) tz = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fz) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
-      if (tz) { d_surf = dz; which = fz; }
+      if (vy && dy < d_surf) { d_surf = dy; which = fy; }
+      if (vz && dz < d_surf) { d_surf = dz; which = fz; }
+      // two faces at exactly the same finite distance: rare enough for a branch the whole warp takes or skips
+      if (__any_sync(MCDC_FULL, (vx && vy && dx == dy) || (vz && (dz == dx || dz == dy) && (vx || vy)))) {
+        d_surf = vx ? dx : INF; which = vx ? fx : -1;
+        bool ty = vy && dy < d_surf;
+        if (vy && dy == d_surf) ty = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fy) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
+        if (ty) { d_surf = dy; which = fy; }
+        bool tz = vz && dz < d_surf;
+        if (vz && dz == d_surf) tz = tb.template ldb<uint8_t>(rec + C2_FACE_IDX + fz) < tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
+        if (tz) { d_surf = dz; which = fz; }
+      }
       // ---- other half-spaces (cylinders, general quadrics, redundant planes), list order, strict < ----
       const uint32_t orec = T.o_other2 + (info >> 16) * OTHER2_BYTES;
 #pragma unroll 1                                       // (peeled, the loop left a second, cold copy of its body in the flight phase)
@@ -562,11 +569,16 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         }
         if (ONEBIN || __any_sync(MCDC_FULL, act && one_bin)) {
           const bool sc = act && one_bin && d > 0.0;
-          long long bin = -1;
-          if (sc) bin = bins32 ? (long long)((tbin * G + g) * (int)n_spatial + (int)cbin)
-                               : (long long)(tbin * G + g) * n_spatial + (long long)cbin;
-          if (SCORE == 1) { if (bin >= 0) atomicAdd(S.global_x + bin, WEIGHTED ? w * d : d); }
-          else tally_add_converged(S, bin, WEIGHTED ? w * d : d);
+          if (SCORE == 1) {                            // one RED; the usual case indexes all accumulators with 32 bits
+            if (sc) {
+              if (bins32) atomicAdd(A.x_acc + (slot * (uint32_t)T.n_bins + (uint32_t)((tbin * G + g) * (int)n_spatial + (int)cbin)), WEIGHTED ? w * d : d);
+              else atomicAdd(S.global_x + ((long long)(tbin * G + g) * n_spatial + (long long)cbin), WEIGHTED ? w * d : d);
+            }
+          } else {
+            long long bin = -1;
+            if (sc) bin = (long long)(tbin * G + g) * n_spatial + (long long)cbin;
+            tally_add_converged(S, bin, WEIGHTED ? w * d : d);
+          }
         }
       }
       // ---- move (A.3) ----
