@@ -584,7 +584,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // ---- move (A.3) ----
       x += d * ux; y += d * uy; z += d * uz;
       t = (ev == EV_CENSUS) ? t_census : t + d * tb.inv_speed(g);
-      bool alive = act, lost = false;
+      bool alive = act;
       uint32_t new_cl = cl;
       int census_k = -1;
       if (ev == EV_CENSUS) {                           // A.8: bookkeeping only, then the next interval
@@ -630,7 +630,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
             if (idx < 0) idx = (int)tb.template ldb<uint8_t>(rec + C2_FACE_IDX + which);
             c2 = slow_cross<RGN>(gT, cell, idx, (int)s_star, x, y, z, ux, uy, uz);
           }
-          if (c2 < 0) { alive = false; lost = true; atomicAdd(&sh.led[LED_LOST], w); }
+          if (c2 < 0) { alive = false; atomicAdd(&sh.led[LED_LOST], w); atomicAdd(&sh.wcnt[wid][W_LOST], 1u); }   // (never, in a sound geometry)
           else new_cl = (uint32_t)c2 | (s_star << 16);
         }
       }
@@ -659,25 +659,25 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           }
         }
       }
-      // ---- census population (A.8): one shared-memory count per distinct census index in the warp ----
-      const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
-      if (m_cen) {
-        const unsigned peers = __match_any_sync(MCDC_FULL, census_k);
-        if (census_k >= 0 && lane == __ffs(peers) - 1) atomicAdd(s_popn + census_k, (uint32_t)__popc(peers));
-        const unsigned m_fin = __ballot_sync(MCDC_FULL, census_k == T.K - 1);
+      // ---- census population (A.8) ----
+      // Asynchronous modes: one native shared-memory add per arriving lane (the hardware serialises equal addresses; a
+      // __match_any_sync to merge them first cost more than it saved).  Census-step mode: every arrival of the launch
+      // carries the index A.step_k, so the count is one ballot and the weight is summed in a register until the end
+      // (lanes adding to the same shared-memory DOUBLE serialise in a compare-and-swap loop: that add was 56 % of the
+      // samples of a census-step launch, profiles/r02c).  Analog runs take the final-census ledger entry from the count
+      // of the last census when the block ends.
+      if (step_mode) {
+        const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
+        if (m_cen && lane == 0) atomicAdd(s_popn + A.step_k, (uint32_t)__popc(m_cen));
+        if (WEIGHTED && census_k >= 0) acc_popw += w;
+      } else if (census_k >= 0) {
+        atomicAdd(s_popn + census_k, 1u);
         if (WEIGHTED) {
-          // Lanes that add to the same shared-memory double serialise in a compare-and-swap loop, and in census-step
-          // mode every census event of the launch carries the same index, A.step_k: that one add was 56 % of the samples
-          // of a census-step launch (profiles/r02c).  There the weight is summed in a register and leaves at the end.
-          if (step_mode) { if (census_k >= 0) acc_popw += w; }
-          else {
-            if (census_k >= 0) atomicAdd(s_popw + census_k, w);
-            if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
-          }
-        } else if (m_fin && lane == 0) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)__popc(m_fin));
+          atomicAdd(s_popw + census_k, w);
+          if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
+        }
       }
       // (surface events are not counted here: segments - collisions - census events, at the end of the block)
-      if (__any_sync(MCDC_FULL, lost)) WCNT(W_LOST, (uint32_t)__popc(__ballot_sync(MCDC_FULL, lost)));
       // ---- hand the slots on: F again, C, or FREE ----
       const bool toF = alive && ev != EV_COLLISION, toC = alive && ev == EV_COLLISION, dead = act && !alive;
       const unsigned mF = __ballot_sync(MCDC_FULL, toF), mC = __ballot_sync(MCDC_FULL, toC), mD = __ballot_sync(MCDC_FULL, dead);
@@ -904,6 +904,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     if (s_popn[k] != 0u) {
       atomicAdd(A.pop_w + k, WEIGHTED ? s_popw[k] : (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]);
       atomicAdd(&sh.n_census, (unsigned long long)s_popn[k]);   // census events of the block = its population counts
+      if (!WEIGHTED && k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)s_popn[k]);   // unit weights
     }
   }
   __syncthreads();
