@@ -474,6 +474,9 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const bool odd = (ctr & 1u) != 0u;
         const double xi = u64_to_unit(odd ? blk.y : blk.x);
         if (act) { PU(U_CTR, gi) = ctr + 1u; if (!odd) PC(gi) = blk.y; }
+        // xi = (k + 1/2) 2^-52 lies in [2^-53, 1 - 2^-53]: telling the compiler so removes log's subnormal / zero / inf / NaN
+        // paths (22 instructions of ~100) without touching the arithmetic of the ordinary one
+        __builtin_assume(__double2hiint(xi) >= 0x3c900000 && __double2hiint(xi) < 0x3ff00000);
         d_coll = -log(xi);
       }
       const int cell = (int)(cl & 0xFFFFu), g = (int)(meta & 255u), pk = (int)((meta >> 8) & 4095u);
