@@ -624,9 +624,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           // a certified neighbour holds every point of this surface patch that lies strictly inside the cell's
           // forward faces (mcdc_host.cu); anything else takes the full search of A.5
           const int ax = (which < 6) ? (which >> 1) : -1;
-          const bool in_x = ax == 0 || (px ? (x < bx) : (x > bx));
-          const bool in_y = ax == 1 || (py ? (y < by) : (y > by));
-          const bool in_z = ax == 2 || (pz ? (z < bz) : (z > bz));
+          // (x < bx going up, x > bx going down: bx - x has the sign of 1 / ux and is not zero; a sentinel bx = +-inf passes)
+          const bool in_x = ax == 0 || (bx - x) * ix > 0.0;
+          const bool in_y = ax == 1 || (by - y) * iy > 0.0;
+          const bool in_z = ax == 2 || (bz - z) * iz > 0.0;
           int c2;
           if (nb != NONE16 && in_x && in_y && in_z) c2 = (int)nb;
           else {
