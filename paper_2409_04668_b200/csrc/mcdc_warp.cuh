@@ -240,7 +240,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     int phase;                                         // 0 = R, 1 = F, 2 = C
     if (nF >= 32u) phase = 1;
     else if (nC >= 32u) phase = 2;
-    else if (room >= 16u && dry == 0u) phase = 0;
+    else if (room >= (step_mode ? 32u : 16u) && dry == 0u) phase = 0;   // (bank refills come in full rounds)
     else if (nF > 0u && nF >= nC) phase = 1;
     else if (nC > 0u) phase = 2;
     else phase = 0;
