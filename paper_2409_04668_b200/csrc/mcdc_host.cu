@@ -1269,13 +1269,16 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
         pc.cap = p->cap; pc.k = k; pc.target = p->tech.pc_target ? p->tech.pc_target : (unsigned long long)sb.hs; pc.w_out = 0.0;
         // (a batch holds at most 4x its source count here unless the caller bound a larger bank: blocks past a
         // slot's count leave at once)
+        // in place: the census bank itself becomes the next live bank (survivors keep their records, removed ones are
+        // marked as holes, copies are appended behind the arrivals, whose count is frozen in bankS1.count first)
         const dim3 pgrid((p->cap + 255) / 256, ns);
         CK(cudaMemsetAsync(p->d_wfix, 0, ns * sizeof(unsigned long long), p->stream));
-        CK(cudaMemsetAsync(A.count, 0, ns * sizeof(uint32_t), p->stream));
+        CK(cudaMemcpyAsync(p->bankS1.count, Bk.count, ns * sizeof(uint32_t), cudaMemcpyDeviceToDevice, p->stream));
         k_pc_weight<<<pgrid, 256, 0, p->stream>>>(Bk, p->cap, p->d_wfix);
-        k_pc_apply<<<pgrid, 256, 0, p->stream>>>(Bk, A, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
+        k_pc_apply_inplace<<<pgrid, 256, 0, p->stream>>>(Bk, p->bankS1.count, pc, p->d_wfix, p->d_cnt, p->d_pop_w_after, p->d_pop_n_after);
         p->launches += 2;
-      } else std::swap(A, Bk);
+      }
+      std::swap(A, Bk);
     }
     CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));
   }

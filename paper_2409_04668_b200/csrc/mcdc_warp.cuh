@@ -278,6 +278,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const bool actb = (uint32_t)lane < nb;
         unsigned long long bkey = 0ull;
         uint32_t bctr = 0u, bgi = 0u;
+        bool live = false;
+        unsigned m_live = 0u;
         if (actb && gen_mode) {                          // a birth record: group and direction are sampled in the C phase
           const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
@@ -290,11 +292,19 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           if (RECORD) PU(U_HID, gi) = A.in.hid[j];
           PL(L_C, lb + nC + (uint32_t)lane) = (uint8_t)i;
           bkey = A.in.key[j]; bctr = (uint32_t)m.z; bgi = gi;
-        } else if (actb) {
-          const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - (uint32_t)lane), gi = lb + i;
+        } else if (!gen_mode) {
+          // (a record that the in-place population control removed is a hole, cell = -1: it takes no slot)
+          const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)(actb ? lane : 0);
+          const int4 m = A.in.meta[j];                   // {cell, last surface, counter, group}
+          live = actb && m.x >= 0;
+          m_live = __ballot_sync(MCDC_FULL, live);
+        }
+        if (live) {
+          const uint32_t rk = lanes_below(m_live, lane);
+          const uint32_t i = (uint32_t)PL(L_FREE, lb + nFree - 1u - rk), gi = lb + i;
           const size_t j = (size_t)bank_slot * A.bank_cap + base + (uint32_t)lane;
           const double ux = A.in.ux[j], uy = A.in.uy[j], uz = A.in.uz[j];
-          const int4 m = A.in.meta[j];                   // {cell, last surface, counter, group}
+          const int4 m = A.in.meta[j];
           PD(D_X, gi) = A.in.x[j]; PD(D_Y, gi) = A.in.y[j]; PD(D_Z, gi) = A.in.z[j]; PD(D_T, gi) = A.in.t[j];
           PD(D_UX, gi) = ux; PD(D_UY, gi) = uy; PD(D_UZ, gi) = uz;
           PD(D_IX, gi) = 1.0 / ux; PD(D_IY, gi) = 1.0 / uy; PD(D_IZ, gi) = 1.0 / uz;
@@ -303,7 +313,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           PU(U_CL, gi) = (uint32_t)m.x | ((m.y < 0 ? NONE16 : (uint32_t)m.y) << 16);
           PU(U_META, gi) = (uint32_t)m.w | ((uint32_t)A.step_k << 8) | (bank_slot << 20);
           if (RECORD) PU(U_HID, gi) = A.in.hid[j];
-          PL(L_F, lb + nF + (uint32_t)lane) = (uint8_t)i;
+          PL(L_F, lb + nF + rk) = (uint8_t)i;
           bkey = A.in.key[j]; bctr = (uint32_t)m.z; bgi = gi;
         }
         // a record that comes back with an odd counter needs the second half of its current block again
@@ -311,8 +321,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           const ulonglong2 blk = philox_block(bkey, bctr >> 1);
           if (bctr & 1u) PC(bgi) = blk.y;
         }
-        nFree -= nb;
-        if (gen_mode) nC += nb; else nF += nb;
+        if (gen_mode) { nFree -= nb; nC += nb; }
+        else { const uint32_t nl = (uint32_t)__popc(m_live); nFree -= nl; nF += nl; }
         __syncwarp();
         continue;
       }
