@@ -1134,7 +1134,10 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_p
   if (W < 32) return MCDC_ERR_NOMEM;
   p->stage_tables = staged; p->hist_threads = nt; p->pool_slots = (uint32_t)W;
   // slots a refill leaves free for fission children (mcdc_warp.cuh); the debug knob asks for pools that overflow
-  p->pool_reserve = debug_pool_slots ? 0u : MCDC_POOL_RESERVE;
+  // (weighted runs keep particles alive longer -- implicit capture -- and their pools run fuller: with 8 free slots a sixth
+  // of the weighted kernel's samples sat in the overflow queue's global loads; 16 took ic_wr from 34.2 to 28.4 ms, while
+  // the analog kernel loses 0.6 % with 16)
+  p->pool_reserve = debug_pool_slots ? 0u : (weighted ? 2u * MCDC_POOL_RESERVE : MCDC_POOL_RESERVE);
   p->pool_smem = (staged ? hot : 0) + pop_bytes + (size_t)W * nw * per_slot;
   cudaError_t e1 = warp_set_smem(staged, record, variant, score_mode(p->tab, problem_aggregate(p)), nt, (int)p->pool_smem);
   if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaFuncSetAttribute(k_warp)");
