@@ -173,3 +173,32 @@ def test_eigenvalue_mode_refuses_more_than_one_census(M):
         g.run_eigenvalue(2000, p.seed, 1, 2)
     assert e.value.code == -1
     g.close()
+
+
+def test_tallies_get_on_a_large_mesh_leaves_the_workspace_clean(M):
+    """mcdc_tallies_get computes mean / sdev of meshes of >= 2^18 bins on the device, in two spare batch accumulators of
+    the bound workspace: a run made AFTER a read must still be right (the accumulators are zero again), reads may be
+    repeated, and caller-owned result arrays (out=) are filled in place."""
+    from oracle import Oracle
+    from workloads import configs as W
+    N, B = 40_000, 4
+    p = W.config2_lduct(n_histories=N, n_batches=B)
+    assert p.n_bins >= 1 << 18
+    g = M.Problem(p)
+    g.run(N // 2, p.seed, B // 2)
+    m1, s1 = g.tallies()
+    m1b, _ = g.tallies()
+    assert np.array_equal(m1, m1b)
+    g.run(N // 2, p.seed, B // 2, first_history_id=N // 2)
+    out = (np.empty(p.n_bins), np.empty(p.n_bins))
+    m2, s2 = M.mcdc_tallies_get(g._h, p.n_bins, out=out)
+    assert m2 is out[0] and s2 is out[1]
+    o = Oracle(p)
+    o.run(N, p.seed, n_batches=B)
+    mo, so = o.tallies()
+    scale = np.abs(mo).max()
+    assert np.all(np.abs(m2.reshape(mo.shape) - mo) <= 1e-7 * np.maximum(np.abs(mo), np.abs(m2.reshape(mo.shape))) + 1e-13 * scale)
+    assert np.allclose(s2.reshape(so.shape), so, rtol=1e-6, atol=1e-12 * scale)
+    with pytest.raises(M.McdcError):
+        M.mcdc_tallies_get(g._h, p.n_bins, out=(np.empty(3), np.empty(3)))
+    g.close()
