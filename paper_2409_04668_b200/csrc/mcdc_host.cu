@@ -1115,7 +1115,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_p
 #endif
   const int nt = MCDC_WARP_THREADS;
   const int nw = nt / 32;
-  const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8, 16) : 0);
+  const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8 * POPW_COPIES, 16) : 0);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
   const size_t hot = align_up(p->tab.hot_bytes, 16);
   const size_t per_slot = warp_pool_bytes_per_slot(record, weighted);

@@ -134,6 +134,11 @@ __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool wei
   return 80 + 16 + 12 + 3 + (record ? 4 : 0) + (weighted ? 8 : 0);
 }
 
+// Copies of the census-weight array of a block (weighted variants): lane l adds to copy l & 3.  Adds of several lanes to ONE
+// shared-memory double serialise in a compare-and-swap loop (12 % of the weighted kernel's samples, profiles/r02k); four
+// copies spread the lanes of a round that reach the same census.
+#define POPW_COPIES 4
+
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
   unsigned long long n_coll, n_seg, n_census, n_children, n_lost, n_src;
@@ -182,7 +187,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
   double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16));   // WEIGHTED only
   const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16) +
-                            (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 + 15) / 16 * 16) : 0u);
+                            (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 * POPW_COPIES + 15) / 16 * 16) : 0u);
 #define PP(pr, slot) (*reinterpret_cast<double2 *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(pr) * 16u))
 #define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(k) * 8u))
 #define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + N * 80u + (slot) * 16u))
@@ -199,7 +204,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     uint4 *dst = reinterpret_cast<uint4 *>(g_smem);
     for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
   }
-  for (int k = tid; k < T.K; k += NT) { s_popn[k] = 0u; if (WEIGHTED) s_popw[k] = 0.0; }
+  for (int k = tid; k < T.K; k += NT) s_popn[k] = 0u;
+  if (WEIGHTED) for (int k = tid; k < T.K * POPW_COPIES; k += NT) s_popw[k] = 0.0;
   if (tid == 0) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
     sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
@@ -678,8 +684,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       // __match_any_sync to merge them first cost more than it saved).  Census-step mode: every arrival of the launch
       // carries the index A.step_k, so the count is one ballot and the weight is summed in a register until the end
       // (lanes adding to the same shared-memory DOUBLE serialise in a compare-and-swap loop: that add was 56 % of the
-      // samples of a census-step launch, profiles/r02c).  Analog runs take the final-census ledger entry from the count
-      // of the last census when the block ends.
+      // samples of a census-step launch, profiles/r02c).  The final-census ledger entry is what reached the last census:
+      // it is taken from that sum when the block ends.
       if (step_mode) {
         const unsigned m_cen = __ballot_sync(MCDC_FULL, census_k >= 0);
         if (m_cen && lane == 0) atomicAdd(s_popn + A.step_k, (uint32_t)__popc(m_cen));
@@ -687,8 +693,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       } else if (census_k >= 0) {
         atomicAdd(s_popn + census_k, 1u);
         if (WEIGHTED) {
-          atomicAdd(s_popw + census_k, w);
-          if (census_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], w);
+          atomicAdd(s_popw + (lane & (POPW_COPIES - 1)) * T.K + census_k, w);   // (copies: see POPW_COPIES)
         }
       }
       // (surface events are not counted here: segments - collisions - census events, at the end of the block)
@@ -904,7 +909,6 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     const double s = warp_sum(acc_popw);
     if (lane == 0 && s != 0.0) {
       atomicAdd(s_popw + A.step_k, s);
-      if (A.step_k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], s);
     }
   }
   if (lane == 0) {
@@ -916,9 +920,11 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   __syncthreads();
   for (int k = tid; k < T.K; k += NT) {
     if (s_popn[k] != 0u) {
-      atomicAdd(A.pop_w + k, WEIGHTED ? s_popw[k] : (double)s_popn[k]); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]);
+      double pw = (double)s_popn[k];
+      if (WEIGHTED) { pw = 0.0; for (int c = 0; c < POPW_COPIES; ++c) pw += s_popw[c * T.K + k]; }
+      atomicAdd(A.pop_w + k, pw); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]);
       atomicAdd(&sh.n_census, (unsigned long long)s_popn[k]);   // census events of the block = its population counts
-      if (!WEIGHTED && k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], (double)s_popn[k]);   // unit weights
+      if (k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], pw);   // what reached the last census is the final-census ledger entry
     }
   }
   __syncthreads();
