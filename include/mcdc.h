@@ -96,8 +96,9 @@ typedef struct {
   /* Test knobs of the history kernel (MCDC_SCHED_ASYNC); 0 = the library chooses.  They change which
    * code path a run takes, never its results (tests/test_gpu_paths.py holds both to the oracle):
    *  debug_pool_slots: cap on the particle slots of each warp's shared-memory pool (rounded down to
-   *    a multiple of 8, at least 32).  With 32 slots a pool is full after one refill, so every fission
-   *    child beyond the first goes through the global ring queue in HBM instead of the pool.
+   *    a multiple of 8, at least 32).  With 32 slots a pool is full after one refill and refills leave no
+   *    slot free, so fission children overflow into the global ring queue in HBM by the thousand
+   *    (mcdc_kernel_info_get counts them); with the default pools a handful per million do.
    *  debug_stage_tables: +1 stage the hot problem tables in shared memory whenever a pool of >= 32
    *    slots still fits; -1 never stage them (every table read goes through L1/L2).                  */
   uint32_t debug_pool_slots;
@@ -290,7 +291,9 @@ int mcdc_state_import(mcdc_problem *p, const double *buf, size_t n_doubles, int 
 /* Which transport kernel the LAST run of this handle launched, as text: the k_warp instantiation
  * "k_warp<STAGED,RECORD,VARIANT,SCORE,threads>", the revision of the kernel sources it was built from (first
  * 12 hex digits of their SHA-1, set by the build), the grid, the pool slots per warp and the dynamic shared
- * memory -- or "k_transport ..." for the census-stepped scheduler; empty before the first run.  Measurement
+ * memory, and the number of fission children that have gone through the global ring queue since the handle was
+ * created ("queue_children=N": evidence that a run took the overflow path) -- or "k_transport ..." for the
+ * census-stepped scheduler; empty before the first run.  Measurement
  * aid: bench.py keys the ncu-derived constants of profiles/ by this string, so a figure
  * captured from another kernel build is never printed beside this one's timing.  buf: HOST, n bytes,
  * always NUL-terminated; MCDC_ERR_ARG on NULL / n == 0.                                              */

@@ -1774,6 +1774,12 @@ extern "C" const char *mcdc_version(void) { return "0.2 sm_100a"; }
 
 extern "C" int mcdc_kernel_info_get(const mcdc_problem *p, char *buf, size_t n) {
   if (!p || !buf || n == 0) return MCDC_ERR_ARG;
-  snprintf(buf, n, "%s", p->last_kernel.c_str());
+  // + how many fission children have gone through the global ring queue since the handle was created (the producers'
+  // cursor is monotonic over launches): the evidence that a run took the overflow path
+  unsigned long long tail = 0ull;
+  if (p->d_head_tail && !p->last_kernel.empty() && p->last_kernel[2] == 'w')
+    cudaMemcpy(&tail, p->d_head_tail + 1, sizeof tail, cudaMemcpyDeviceToHost);
+  if (p->last_kernel.empty()) snprintf(buf, n, "%s", "");
+  else snprintf(buf, n, "%s queue_children=%llu", p->last_kernel.c_str(), tail);
   return MCDC_OK;
 }

@@ -59,7 +59,12 @@ def test_small_pools_send_fission_children_through_the_global_queue(M, name, N, 
     g = M.Problem(p)
     g.run(record_history_events=True, debug_pool_slots=32)
     _compare(o, g, rtol)
+    info = g.kernel_info()
+    assert " pool_slots=32 " in info and info.startswith("k_warp<1,1,0,")
     if name in ("config0", "config3"):
+        # the knob did what it is for: thousands of fission children went through the global ring queue (the default
+        # pools send about 5 in 1e5 there: 480 of 1.02e7 on the full config 3)
+        assert int(info.split("queue_children=")[1]) > max(5000, 0.03 * g.counters()["children"])
         # the knob did what it is for: with 32-slot pools the run cannot have held its children in the pools.  The
         # queue cursors are the evidence: mcdc_counters has no field for them, so run the default pool as the control
         # and require identical results -- queue or pool, the trajectories are the same
@@ -78,6 +83,7 @@ def test_unstaged_tables_instantiation_matches_the_oracle(M, name, N, B, rtol, p
     g = M.Problem(p)
     g.run(record_history_events=True, debug_stage_tables=-1, debug_pool_slots=pool)
     _compare(o, g, rtol)
+    assert g.kernel_info().startswith("k_warp<0,1,0,")     # the instantiation that reads its tables through L1 / L2
     g.close()
 
 
