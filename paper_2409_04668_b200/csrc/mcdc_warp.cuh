@@ -466,8 +466,9 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       continue;
     }
 
-    if (phase == 1) {
+    if (phase == 1) do {
       // =============== F: one segment -- distances, event choice, score, move, census / surface event ===============
+      // (a full flight round is followed by the next one without going through the phase choice again)
       const uint32_t n = min(32u, nF);
       nF -= n;
       n_seg += n;                                      // every lane of a flight round makes one segment
@@ -705,8 +706,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       if (dead) PL(L_FREE, lb + nFree + lanes_below(mD, lane)) = (uint8_t)i;
       nF += (uint32_t)__popc(mF); nC += (uint32_t)__popc(mC); nFree += (uint32_t)__popc(mD);
       __syncwarp();
-      continue;
-    }
+    } while (nF >= 32u);
+    if (phase == 1) continue;
 
     // =============== C: collisions (A.6) ===============
     {
