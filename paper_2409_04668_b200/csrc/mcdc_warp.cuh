@@ -785,14 +785,15 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
       {
         const unsigned m_cap = __ballot_sync(MCDC_FULL, captured), m_fis = __ballot_sync(MCDC_FULL, fissioned);
         if (WEIGHTED) {
-          l_cap = warp_sum(l_cap); l_fis = warp_sum(l_fis); l_prod = warp_sum(l_prod);
-          l_gain = warp_sum(l_gain); l_loss = warp_sum(l_loss);
-          if (lane == 0) {
-            if (l_cap != 0.0) atomicAdd(&sh.led[LED_CAPTURE], l_cap);
-            if (l_fis != 0.0) atomicAdd(&sh.led[LED_FISSION_ABS], l_fis);
-            if (l_prod != 0.0) atomicAdd(&sh.led[LED_PRODUCTION], l_prod);
-            if (l_gain != 0.0) atomicAdd(&sh.led[LED_VR_GAIN], l_gain);
-            if (l_loss != 0.0) atomicAdd(&sh.led[LED_VR_LOSS], l_loss);
+          // (each warp sum is 15 instructions: only the entries that some lane of this round touched are summed)
+          if (__any_sync(MCDC_FULL, l_cap != 0.0)) { l_cap = warp_sum(l_cap); if (lane == 0) atomicAdd(&sh.led[LED_CAPTURE], l_cap); }
+          if (m_fis) {
+            l_fis = warp_sum(l_fis); l_prod = warp_sum(l_prod);
+            if (lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], l_fis); if (l_prod != 0.0) atomicAdd(&sh.led[LED_PRODUCTION], l_prod); }
+          }
+          if (__any_sync(MCDC_FULL, rouletted)) {
+            l_gain = warp_sum(l_gain); l_loss = warp_sum(l_loss);
+            if (lane == 0) { if (l_gain != 0.0) atomicAdd(&sh.led[LED_VR_GAIN], l_gain); if (l_loss != 0.0) atomicAdd(&sh.led[LED_VR_LOSS], l_loss); }
           }
         } else if (lane == 0 && m_cap) atomicAdd(&sh.led[LED_CAPTURE], (double)__popc(m_cap));
         if (m_fis) {
