@@ -268,3 +268,29 @@ def test_certificates_one_bin_cells_and_async_only_workspace(M):
     i2 = g.info()
     assert i2["certified_halfspaces"] == i2["transmission_halfspaces"] > 0 and i2["one_bin_cells"] == 0
     g.close()
+
+
+def test_problem_beyond_the_history_kernels_tables_falls_back_and_still_matches(M):
+    """More census times than the compact particle word holds (4095): mcdc_problem_info says so, the asynchronous
+    scheduler request is served by the census-stepped kernel, and the results are still the oracle's."""
+    from oracle import Oracle
+    from workloads import configs as W
+    N, B = 6000, 6
+    p = W.config0_infinite_medium(n_histories=N, n_batches=B)
+    p.census_times = np.linspace(0.0, 20.0, 5001)[1:].copy()          # 5000 census steps over the same 20 s
+    g = M.Problem(p)
+    assert g.info()["warp_kernel_ok"] == 0
+    g.run(record_history_events=True)
+    assert g.kernel_info().startswith("k_transport")
+    o = Oracle(p)
+    o.run(N, p.seed, n_batches=B, record_history_events=True)
+    co, cg = o.counters(), g.counters()
+    for k in ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost", "collisions", "surf_hits",
+              "census_events", "children"):
+        assert cg[k] == co[k], (k, cg[k], co[k])
+    assert np.array_equal(o.history_events(), g.history_events())
+    (mo, _), (mg, _) = o.tallies(), g.tallies()
+    assert np.allclose(mg, mo, rtol=1e-9, atol=1e-13 * np.abs(mo).max())
+    wo, no = o.census(); wg, ng = g.census()
+    assert np.array_equal(no, ng)
+    g.close()
