@@ -294,3 +294,29 @@ def test_problem_beyond_the_history_kernels_tables_falls_back_and_still_matches(
     wo, no = o.census(); wg, ng = g.census()
     assert np.array_equal(no, ng)
     g.close()
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_a_true_void_region_is_streamed_through(M, scheduler):
+    """Sigma_t = 0 in the middle region of the slab (degenerate case of A.2: no collision distance): the history kernel
+    reads 1 / Sigma_t = +inf there instead of testing Sigma_t; counts and tallies must still be the oracle's."""
+    from oracle import Oracle
+    from workloads import configs as W
+    N, B = 60_000, 6
+    p = W.config1_slab(n_histories=N, n_batches=B)
+    for name in ("sigma_t", "sigma_c", "sigma_f", "nu", "chi"):
+        a = getattr(p, name).copy(); a[1, :] = 0.0; setattr(p, name, a)
+    s = p.sigma_s.copy(); s[1] = 0.0; p.sigma_s = s
+    o = Oracle(p); g = M.Problem(p)
+    o.run(N, p.seed, n_batches=B, record_history_events=True)
+    g.run(record_history_events=True, scheduler=scheduler)
+    co, cg = o.counters(), g.counters()
+    for k in ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost", "collisions", "surf_hits",
+              "census_events", "children"):
+        assert cg[k] == co[k], (k, cg[k], co[k])
+    assert co["collisions"] > 0 and co["lost"] == 0
+    assert np.all(o.history_events() == g.history_events(), axis=1).mean() >= 0.99999
+    (mo, _), (mg, _) = o.tallies(), g.tallies()
+    scale = np.abs(mo).max()
+    assert np.all(np.abs(mg - mo) <= 1e-9 * np.maximum(np.abs(mo), np.abs(mg)) + 1e-13 * scale)
+    g.close()
