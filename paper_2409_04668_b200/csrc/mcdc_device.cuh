@@ -66,6 +66,10 @@ struct TB {
 };
 
 __device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// fp64 add to a tally accumulator in global memory as a true reduction (REDG): atomicAdd() with an unused result compiles
+// to ATOMG with a discarded destination, which still waits for its reply before the same thread can issue the next one --
+// the DDA scorer of config 2 spent 37 % of its samples there, one L2 / DRAM round trip per tally bin (profiles/r02n)
+__device__ __forceinline__ void red_add_f64(double *p, double v) { asm volatile("red.global.add.f64 [%0], %1;" ::"l"(p), "d"(v)); }
 
 // ------------------------------------------------------------------------------------------------
 // RNG: counter-based, keyed by a 64-bit particle key; draw index = particle counter (Appendix B).

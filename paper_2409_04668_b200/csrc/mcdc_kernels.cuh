@@ -73,7 +73,7 @@ __device__ __forceinline__ void tally_add_converged(const TallySink &S, long lon
   if (S.slab != nullptr) {
     long long rel = bin - S.slab_lo;
     if (bin >= 0 && (rel < 0 || rel >= S.slab_bins)) {     // outside the step's slab (rounding-length pieces)
-      atomicAdd(S.global_x + bin, val);
+      red_add_f64(S.global_x + bin, val);
       bin = -1;
     }
     const int b = (bin >= 0) ? (int)rel : -1;
@@ -82,9 +82,9 @@ __device__ __forceinline__ void tally_add_converged(const TallySink &S, long lon
   } else if (S.aggregate) {
     double *addr = (bin >= 0) ? S.global_x + bin : nullptr;
     const bool absorbed = warp_merge_equal<unsigned long long>((unsigned long long)addr, bin >= 0, val, 3);
-    if (bin >= 0 && !absorbed) atomicAdd(addr, val);
+    if (bin >= 0 && !absorbed) red_add_f64(addr, val);
   } else if (bin >= 0) {
-    atomicAdd(S.global_x + bin, val);
+    red_add_f64(S.global_x + bin, val);
   }
 }
 
@@ -569,7 +569,7 @@ __global__ void __launch_bounds__(TRANSPORT_THREADS) k_transport(Tables T, StepP
     __syncthreads();
     for (int b = tid; b < P.slab_bins; b += TRANSPORT_THREADS) {
       double v = slab[b];
-      if (v != 0.0) atomicAdd(S.global_x + S.slab_lo + b, v);
+      if (v != 0.0) red_add_f64(S.global_x + S.slab_lo + b, v);
     }
     __syncthreads();
   }

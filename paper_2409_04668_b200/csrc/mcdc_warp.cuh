@@ -92,7 +92,7 @@ static __device__ __noinline__ void slow_score_collision(const Tables *gT, doubl
                                                   int g, double w, int mg) {
   const TB<false> tb(*gT);
   const long long cb = collision_bin(tb, x, y, z, t, g);
-  if (cb >= 0) atomicAdd(xc_slot + cb, w / tb.sig_t(mg));
+  if (cb >= 0) red_add_f64(xc_slot + cb, w / tb.sig_t(mg));
 }
 
 // A.7 for segments that may touch several tally bins (4-D DDA).  Warp-converged: every lane calls it.
@@ -591,8 +591,8 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
           const bool sc = act && one_bin && d > 0.0;
           if (SCORE == 1) {                            // one RED; the usual case indexes all accumulators with 32 bits
             if (sc) {
-              if (bins32) atomicAdd(A.x_acc + (slot * (uint32_t)T.n_bins + (uint32_t)((tbin * G + g) * (int)n_spatial + (int)cbin)), WEIGHTED ? w * d : d);
-              else atomicAdd(S.global_x + ((long long)(tbin * G + g) * n_spatial + (long long)cbin), WEIGHTED ? w * d : d);
+              if (bins32) red_add_f64(A.x_acc + (slot * (uint32_t)T.n_bins + (uint32_t)((tbin * G + g) * (int)n_spatial + (int)cbin)), WEIGHTED ? w * d : d);
+              else red_add_f64(S.global_x + ((long long)(tbin * G + g) * n_spatial + (long long)cbin), WEIGHTED ? w * d : d);
             }
           } else {
             long long bin = -1;
