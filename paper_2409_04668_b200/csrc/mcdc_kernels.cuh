@@ -68,6 +68,10 @@ __device__ __forceinline__ bool warp_merge_equal(K key, bool valid, double &val,
 }
 
 __device__ __forceinline__ void tally_add_converged(const TallySink &S, long long bin, double val) {
+  if (S.slab == nullptr && !S.aggregate) {               // plain case (kernel-uniform): one reduction per lane, no vote
+    if (bin >= 0) red_add_f64(S.global_x + bin, val);
+    return;
+  }
   unsigned valid = __ballot_sync(MCDC_FULL, bin >= 0);
   if (valid == 0u) return;
   if (S.slab != nullptr) {

@@ -142,6 +142,7 @@ __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool wei
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
   unsigned long long n_coll, n_seg, n_census, n_children, n_lost, n_src;
+  uint32_t n_leak;                   // analog runs: particles that leaked from this block (unit weights: a native 32-bit add)
   uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
 
@@ -208,7 +209,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   if (WEIGHTED) for (int k = tid; k < T.K * POPW_COPIES; k += NT) s_popw[k] = 0.0;
   if (tid == 0) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
-    sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull;
+    sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull; sh.n_leak = 0u;
   }
   if (lane < 8) sh.wcnt[wid][lane] = 0u;
   const uint32_t lb = (uint32_t)wid * W;               // first slot of this warp
@@ -626,7 +627,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
         if (bc == 1) {                                 // vacuum: leaks
           alive = false;
-          atomicAdd(&sh.led[LED_LEAK], w);
+          if (WEIGHTED) atomicAdd(&sh.led[LED_LEAK], w); else atomicAdd(&sh.n_leak, 1u);
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
           if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
           else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
@@ -932,6 +933,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   __syncthreads();
   if (tid == 0) {
     DevCounters *cnt = A.cnt;
+    if (!WEIGHTED) sh.led[LED_LEAK] += (double)sh.n_leak;
     for (int e = 0; e < LED_N; ++e)
       if (sh.led[e] != 0.0) atomicAdd(&cnt->ledger[1 + e], sh.led[e]);
     atomicAdd(&cnt->ledger[0], (double)sh.n_src);
