@@ -235,7 +235,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   if (step_mode && !A.step_source) src_exhausted = true;
   uint32_t n_seg = 0u;                                 // segments of this warp (warp-uniform)
   double acc_popw = 0.0;                               // census-step mode: weight this lane saw arrive at census A.step_k
-  enum { W_COLL = 0, W_CHILDREN, W_LOST, W_SRC };
+  enum { W_COLL = 0, W_CHILDREN, W_LOST, W_SRC, W_CAP, W_FIS };   // (W_CAP, W_FIS: analog runs, where ledger entries are counts)
 #define WCNT(k, v) do { const uint32_t v__ = (v); if (lane == 0 && v__ != 0u) sh.wcnt[wid][k] += v__; } while (0)
 
   for (;;) {
@@ -796,10 +796,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
             l_gain = warp_sum(l_gain); l_loss = warp_sum(l_loss);
             if (lane == 0) { if (l_gain != 0.0) atomicAdd(&sh.led[LED_VR_GAIN], l_gain); if (l_loss != 0.0) atomicAdd(&sh.led[LED_VR_LOSS], l_loss); }
           }
-        } else if (lane == 0 && m_cap) atomicAdd(&sh.led[LED_CAPTURE], (double)__popc(m_cap));
+        } else WCNT(W_CAP, (uint32_t)__popc(m_cap));    // unit weights: captures, absorptions and production are counts
         if (m_fis) {
           const uint32_t kids = __reduce_add_sync(MCDC_FULL, (uint32_t)n_child);
-          if (!WEIGHTED && lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], (double)__popc(m_fis)); atomicAdd(&sh.led[LED_PRODUCTION], (double)kids); }
+          if (!WEIGHTED) WCNT(W_FIS, (uint32_t)__popc(m_fis));
           WCNT(W_CHILDREN, kids);
         }
         WCNT(W_COLL, (uint32_t)__popc(__ballot_sync(MCDC_FULL, act && !born)));
@@ -918,6 +918,11 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     const uint32_t *wc = sh.wcnt[wid];
     atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_seg, (unsigned long long)n_seg);
     atomicAdd(&sh.n_children, (unsigned long long)wc[W_CHILDREN]);
+    if (!WEIGHTED) {                                     // the analog ledger, from the warp's counts
+      if (wc[W_CAP]) atomicAdd(&sh.led[LED_CAPTURE], (double)wc[W_CAP]);
+      if (wc[W_FIS]) atomicAdd(&sh.led[LED_FISSION_ABS], (double)wc[W_FIS]);
+      if (wc[W_CHILDREN]) atomicAdd(&sh.led[LED_PRODUCTION], (double)wc[W_CHILDREN]);
+    }
     atomicAdd(&sh.n_lost, (unsigned long long)wc[W_LOST]); atomicAdd(&sh.n_src, (unsigned long long)wc[W_SRC]);
   }
   __syncthreads();
