@@ -142,6 +142,7 @@ __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool wei
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
   unsigned long long n_coll, n_seg, n_census, n_children, n_lost, n_src;
+  double wled[32][LED_N];            // weighted runs: per-warp ledger sums (lane 0 of the warp adds without atomics; leaks: the warp's lanes)
   uint32_t n_leak;                   // analog runs: particles that leaked from this block (unit weights: a native 32-bit add)
   uint32_t wcnt[32][8];              // per-warp event counts (only lane 0 of the warp touches its row)
 };
@@ -212,6 +213,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull; sh.n_leak = 0u;
   }
   if (lane < 8) sh.wcnt[wid][lane] = 0u;
+  if (lane < LED_N) sh.wled[wid][lane] = 0.0;
   const uint32_t lb = (uint32_t)wid * W;               // first slot of this warp
   for (uint32_t i = lane; i < W; i += 32) PL(L_FREE, lb + i) = (uint8_t)(W - 1u - i);
   __syncthreads();
@@ -627,7 +629,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         new_cl = (cl & 0xFFFFu) | (s_star << 16);
         if (bc == 1) {                                 // vacuum: leaks
           alive = false;
-          if (WEIGHTED) atomicAdd(&sh.led[LED_LEAK], w); else atomicAdd(&sh.n_leak, 1u);
+          if (WEIGHTED) atomicAdd(&sh.wled[wid][LED_LEAK], w); else atomicAdd(&sh.n_leak, 1u);
         } else if (bc == 2) {                          // reflective: specular, stays in the cell
           if (type == ST_PLANE_X) { PD(D_UX, gi) = -ux; PD(D_IX, gi) = -ix; }
           else if (type == ST_PLANE_Y) { PD(D_UY, gi) = -uy; PD(D_IY, gi) = -iy; }
@@ -787,14 +789,14 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
         const unsigned m_cap = __ballot_sync(MCDC_FULL, captured), m_fis = __ballot_sync(MCDC_FULL, fissioned);
         if (WEIGHTED) {
           // (each warp sum is 15 instructions: only the entries that some lane of this round touched are summed)
-          if (__any_sync(MCDC_FULL, l_cap != 0.0)) { l_cap = warp_sum(l_cap); if (lane == 0) atomicAdd(&sh.led[LED_CAPTURE], l_cap); }
+          if (__any_sync(MCDC_FULL, l_cap != 0.0)) { l_cap = warp_sum(l_cap); if (lane == 0) sh.wled[wid][LED_CAPTURE] += l_cap; }
           if (m_fis) {
             l_fis = warp_sum(l_fis); l_prod = warp_sum(l_prod);
-            if (lane == 0) { atomicAdd(&sh.led[LED_FISSION_ABS], l_fis); if (l_prod != 0.0) atomicAdd(&sh.led[LED_PRODUCTION], l_prod); }
+            if (lane == 0) { sh.wled[wid][LED_FISSION_ABS] += l_fis; sh.wled[wid][LED_PRODUCTION] += l_prod; }
           }
           if (__any_sync(MCDC_FULL, rouletted)) {
             l_gain = warp_sum(l_gain); l_loss = warp_sum(l_loss);
-            if (lane == 0) { if (l_gain != 0.0) atomicAdd(&sh.led[LED_VR_GAIN], l_gain); if (l_loss != 0.0) atomicAdd(&sh.led[LED_VR_LOSS], l_loss); }
+            if (lane == 0) { sh.wled[wid][LED_VR_GAIN] += l_gain; sh.wled[wid][LED_VR_LOSS] += l_loss; }
           }
         } else WCNT(W_CAP, (uint32_t)__popc(m_cap));    // unit weights: captures, absorptions and production are counts
         if (m_fis) {
@@ -918,7 +920,10 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     const uint32_t *wc = sh.wcnt[wid];
     atomicAdd(&sh.n_coll, (unsigned long long)wc[W_COLL]); atomicAdd(&sh.n_seg, (unsigned long long)n_seg);
     atomicAdd(&sh.n_children, (unsigned long long)wc[W_CHILDREN]);
-    if (!WEIGHTED) {                                     // the analog ledger, from the warp's counts
+    if (WEIGHTED) {
+      for (int e = 0; e < LED_N; ++e)
+        if (sh.wled[wid][e] != 0.0) atomicAdd(&sh.led[e], sh.wled[wid][e]);
+    } else {                                             // the analog ledger, from the warp's counts
       if (wc[W_CAP]) atomicAdd(&sh.led[LED_CAPTURE], (double)wc[W_CAP]);
       if (wc[W_FIS]) atomicAdd(&sh.led[LED_FISSION_ABS], (double)wc[W_FIS]);
       if (wc[W_CHILDREN]) atomicAdd(&sh.led[LED_PRODUCTION], (double)wc[W_CHILDREN]);
