@@ -151,3 +151,21 @@ def test_state_export_sum_import_equals_the_single_run(M):
     assert np.array_equal(whole.tallies()[0], before)
     for h in parts + [whole, merged]:
         h.close()
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_population_control_to_a_target_beyond_the_bank_reports_overflow(M, scheduler):
+    """A control target far above what the census bank of a batch holds makes the control append more copies than fit:
+    the run must answer MCDC_ERR_BANK_OVERFLOW (device flag, no host read inside the census loop), not write past the bank."""
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=4000, n_batches=2)
+    g = M.Problem(p)
+    g.set_technique(population_control=True, pc_target=400 * 2000)
+    with pytest.raises(M.McdcError) as e:
+        g.run(scheduler=scheduler)
+    assert e.value.code == -6
+    g.set_technique(population_control=True)                # the handle is still usable
+    g.reset(); g.run(scheduler=scheduler)
+    c = g.counters()
+    assert c["histories"] == 4000 and c["lost"] == 0.0
+    g.close()
