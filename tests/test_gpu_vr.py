@@ -169,3 +169,16 @@ def test_population_control_to_a_target_beyond_the_bank_reports_overflow(M, sche
     c = g.counters()
     assert c["histories"] == 4000 and c["lost"] == 0.0
     g.close()
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_control_that_splits_every_particle_appends_copies_in_place(M, scheduler):
+    """A target of three times the batch: every arrival becomes about three particles at every census, so the in-place
+    control of the history kernel appends twice the arrivals behind them (and the next launch reads them there)."""
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=20_000, n_batches=10)
+    o, g = _pair(M, p, dict(population_control=True, pc_target=3 * 2000), scheduler=scheduler, max_histories_per_subbatch=6 * 20_000)   # (banks sized for the tripled population)
+    c = g.counters()
+    assert c["pc_added"] > 2 * c["pc_removed"] and c["pc_added"] > 20_000
+    _compare(o, g, 1e-7)
+    g.close()
