@@ -182,3 +182,16 @@ def test_control_that_splits_every_particle_appends_copies_in_place(M, scheduler
     assert c["pc_added"] > 2 * c["pc_removed"] and c["pc_added"] > 20_000
     _compare(o, g, 1e-7)
     g.close()
+
+
+@pytest.mark.timeout(900)
+def test_all_techniques_at_a_million_histories(M):
+    """Config 3 with implicit capture, roulette and population control at 1e6 histories in 100 batches: every warp of the
+    launch refills from the banks (chunked reservations, holes of the in-place control) and parks into them; integer
+    counts exact, ledger and census weights to rounding, tallies to 1e-7 (the oracle takes ~30 s on one core)."""
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=1_000_000, n_batches=100)
+    o, g = _pair(M, p, TECHS["all"], scheduler=0)
+    assert g.kernel_info().startswith("k_warp<1,1,2,1,512>")
+    _compare(o, g, 1e-7)
+    g.close()
