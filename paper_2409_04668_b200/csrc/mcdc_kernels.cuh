@@ -819,7 +819,16 @@ __global__ void __launch_bounds__(256) k_closeout(double *__restrict__ x_acc, in
   for (unsigned long long i = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; i < n_bins; i += stride) {
     double s = 0.0, q = 0.0;
     bool any = false;
-    for (int b = 0; b < n_slots; ++b) {
+    int b = 0;
+    for (; b + 4 <= n_slots; b += 4) {                   // four slots at a time: four independent loads in flight per thread
+      double v[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) v[k] = x_acc[(size_t)(b + k) * n_bins + i];
+#pragma unroll
+      for (int k = 0; k < 4; ++k)
+        if (v[k] != 0.0) { s += v[k]; q += v[k] * v[k]; x_acc[(size_t)(b + k) * n_bins + i] = 0.0; any = true; }
+    }
+    for (; b < n_slots; ++b) {
       double v = x_acc[(size_t)b * n_bins + i];
       if (v != 0.0) { s += v; q += v * v; x_acc[(size_t)b * n_bins + i] = 0.0; any = true; }
     }
