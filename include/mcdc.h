@@ -236,6 +236,46 @@ int mcdc_run_eigenvalue(mcdc_problem *p, uint64_t n_particles, uint64_t seed, ui
  * sdev[i] = batch standard error of the mean (0 with a single batch).  n_bins must equal
  * n_time_bins*G*nz*ny*nx.                                                                          */
 int mcdc_tallies_get(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
+/* mcdc_tallies_get for callers that must not allocate device memory.
+ *
+ * Who needs it.  mcdc_tallies_get turns the raw accumulators into mean / sdev on the GPU when the mesh is
+ * large, and needs 2 * n_bins doubles of device scratch for that: it borrows them from the bound workspace
+ * when that has two batch slots, and otherwise calls cudaMalloc / cudaFree.  Some hosts of this library cannot
+ * live with that second case: a process that has handed all of the GPU's memory to a pooling allocator
+ * (PyTorch's caching allocator, a per-rank budget fixed at job start), where a cudaMalloc made behind the pool's
+ * back fails or eats into what the pool was promised; and a read-out inside a timing-critical loop, where
+ * cudaMalloc and cudaFree make the host wait for everything else the device is doing.
+ *
+ * What it does.  The same A.9 statistics by the same kernel (identical results to mcdc_tallies_get), with the
+ * scratch in a fixed array that lives inside libmcdc.so's device image: 2 * MCDC_NOALLOC_MAX_BINS doubles = 16 MiB.
+ * Every GPU on which the process uses the library holds those 16 MiB from the moment the library's device
+ * code is loaded there until the process exits, whether or not this call is ever made.  The call itself
+ * makes no cudaMalloc, cudaFree or other allocating CUDA / library call: one kernel launch, two device-to-host
+ * copies on the bound stream (or the default stream if none is bound), one stream synchronisation.  A bound
+ * workspace is not needed and not touched.
+ *
+ *  mean, sdev: HOST arrays of n_bins doubles owned by the caller (pinned or pageable), layout and meaning of
+ *    mcdc_tallies_get; complete on return.
+ *  n_bins: must equal the problem's bin count (else MCDC_ERR_SIZE) and must not exceed MCDC_NOALLOC_MAX_BINS:
+ *    a larger mesh is refused with MCDC_ERR_SIZE and mcdc_last_cuda_error() then says so in words -- nothing
+ *    is launched, and nothing is silently truncated.  (Config 2's 7.2e6-bin mesh is beyond it; bind a
+ *    workspace with two slots and use mcdc_tallies_get there.)
+ *  MCDC_ERR_ARG before the first run (no histories), or if the GPU that holds the handle is not the
+ *    calling thread's current device.
+ *
+ * First call on each GPU: the library looks up the array's device address (cudaGetSymbolAddress, with that
+ * GPU current) and remembers it for the life of the process.  That look-up may make the runtime load the
+ * library's device code onto the GPU, so make the first call per GPU at start-up, before any stream capture
+ * begins anywhere in the process; later calls only launch, copy and wait.
+ *
+ * Sharing.  There is ONE array per GPU per process, shared by every handle, stream and thread.  It keeps
+ * whatever the previous call left in it; that is harmless here because each call overwrites the first n_bins
+ * entries of both halves before it copies them out, so nothing has to be cleared between calls.  But two calls
+ * whose GPU work can overlap (two host threads reading out two handles on different streams of the same
+ * GPU) write the same memory and corrupt each other's results: serialise them yourself.  Calls made one
+ * after another from one thread never overlap, since each waits for its stream before returning.        */
+#define MCDC_NOALLOC_MAX_BINS ((size_t)1 << 20)
+int mcdc_tallies_get_noalloc(const mcdc_problem *p, double *mean, double *sdev, size_t n_bins);
 /* Collision-estimator tally, the paper's one code listing (Fig. 3:
  * `add(mcdc.col_tally, part.v, loc2index(part))` inside tally_collision_event); SURVEY.md 8(f) NEXT-4;
  * reading in DESIGN.md Appendix I: at every collision the bin of the SAME mesh that holds the collision

@@ -21,8 +21,10 @@ EXPORTED_SYMBOLS = [
     "mcdc_last_cuda_error", "mcdc_version", "mcdc_technique_set", "mcdc_census_after_get",
     "mcdc_state_size", "mcdc_state_export", "mcdc_state_import", "mcdc_run_eigenvalue",
     "mcdc_collision_tally_enable", "mcdc_collision_tallies_get", "mcdc_problem_create_csg", "mcdc_kernel_info_get",
-    "mcdc_lattice_expand_size", "mcdc_lattice_expand", "mcdc_problem_create_lattice",
+    "mcdc_lattice_expand_size", "mcdc_lattice_expand", "mcdc_problem_create_lattice", "mcdc_tallies_get_noalloc",
 ]
+
+NOALLOC_MAX_BINS = 1 << 20   # MCDC_NOALLOC_MAX_BINS of include/mcdc.h
 
 _dp = C.POINTER(C.c_double)
 _ip = C.POINTER(C.c_int32)
@@ -123,6 +125,7 @@ def lib():
     L.mcdc_run.argtypes = [vp, C.c_uint64, C.c_uint64]; L.mcdc_run.restype = C.c_int
     L.mcdc_run_ex.argtypes = [vp, C.c_uint64, C.c_uint64, C.POINTER(RunOpts)]; L.mcdc_run_ex.restype = C.c_int
     L.mcdc_tallies_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_tallies_get.restype = C.c_int
+    L.mcdc_tallies_get_noalloc.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_tallies_get_noalloc.restype = C.c_int
     L.mcdc_tally_sums_get.argtypes = [vp, _dp, _dp, C.c_size_t]; L.mcdc_tally_sums_get.restype = C.c_int
     L.mcdc_counters_get.argtypes = [vp, C.POINTER(Counters)]; L.mcdc_counters_get.restype = C.c_int
     L.mcdc_census_get.argtypes = [vp, _dp, C.POINTER(C.c_uint64), C.c_size_t]; L.mcdc_census_get.restype = C.c_int
@@ -358,6 +361,27 @@ def mcdc_tallies_get(h, n_bins, out=None):
     return mean, sdev
 
 
+def mcdc_tallies_get_noalloc(h, n_bins, out=None):
+    """mcdc_tallies_get for a caller that must not allocate on the GPU (all device memory belongs to a pool, or the
+    read-out sits in a timing-critical loop): same numbers, but the device scratch is a fixed 16 MiB array inside
+    libmcdc.so, so no cudaMalloc / cudaFree happens.  Limits (include/mcdc.h): at most NOALLOC_MAX_BINS bins, else
+    McdcError(-4) whose text names the limit; one array per GPU shared by all handles, so do not run two of these
+    calls concurrently on one GPU; make the first call per GPU before any stream capture starts.  out as in
+    mcdc_tallies_get (pass pinned arrays to keep the host side allocation-free as well)."""
+    if out is None:
+        mean = np.empty(n_bins); sdev = np.empty(n_bins)
+    else:
+        mean, sdev = out
+        if mean.size != n_bins or sdev.size != n_bins or mean.dtype != np.float64 or sdev.dtype != np.float64 or \
+                not mean.flags.c_contiguous or not sdev.flags.c_contiguous:
+            raise McdcError(-4, "mcdc_tallies_get_noalloc", "out arrays must be contiguous float64 of n_bins elements")
+    rc = lib().mcdc_tallies_get_noalloc(h, _d(mean), _d(sdev), n_bins)
+    if rc in (-1, -4):   # the library leaves the reason (over the limit / wrong current device) in its error text
+        raise McdcError(rc, "mcdc_tallies_get_noalloc", lib().mcdc_last_cuda_error(h).decode())
+    _check(rc, "mcdc_tallies_get_noalloc", h)
+    return mean, sdev
+
+
 def mcdc_collision_tally_enable(h, on=True):
     _check(lib().mcdc_collision_tally_enable(h, int(bool(on))), "mcdc_collision_tally_enable", h)
 
@@ -491,6 +515,11 @@ class Problem:
 
     def tallies(self):
         m, s = mcdc_tallies_get(self._h, self.n_bins)
+        return m.reshape(self.shape), s.reshape(self.shape)
+
+    def tallies_noalloc(self):
+        """tallies() through mcdc_tallies_get_noalloc: no device allocation, at most NOALLOC_MAX_BINS bins."""
+        m, s = mcdc_tallies_get_noalloc(self._h, self.n_bins)
         return m.reshape(self.shape), s.reshape(self.shape)
 
     def enable_collision_tally(self, on=True):

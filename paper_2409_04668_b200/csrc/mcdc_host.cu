@@ -1783,3 +1783,80 @@ extern "C" int mcdc_kernel_info_get(const mcdc_problem *p, char *buf, size_t n) 
   else snprintf(buf, n, "%s queue_children=%llu", p->last_kernel.c_str(), tail);
   return MCDC_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// mcdc_tallies_get_noalloc (include/mcdc.h): the A.9 read-out of k_statistics for callers that must not
+// allocate device memory.  The 2 * n_bins doubles that batch_statistics() takes from the workspace or from
+// cudaMalloc live here in a fixed array of the library's device image instead.
+//
+// g_noalloc_scratch is that array.  In HOST code the name is only a handle for the runtime, not a device
+// address: handing `g_noalloc_scratch` itself to a kernel would make the kernel fault (or, on a GPU that can
+// reach host memory, scribble on whatever host address the stand-in happens to have).  Host code therefore
+// asks the runtime for the device address once per GPU (noalloc_scratch_address) and passes THAT to the kernel.
+// ---------------------------------------------------------------------------------------------
+#include <mutex>
+
+static __device__ __align__(256) double g_noalloc_scratch[2 * MCDC_NOALLOC_MAX_BINS];   // [0, MAX) mean, [MAX, 2 MAX) sdev
+
+namespace {
+constexpr int NOALLOC_MAX_DEVICES = 64;
+double *g_noalloc_addr[NOALLOC_MAX_DEVICES];   // device address of g_noalloc_scratch on GPU d; nullptr = not looked up yet
+std::mutex g_noalloc_mu;
+
+// Device address of the scratch array on GPU `dev`, which must be the calling thread's current device (every GPU
+// has its own copy of the array at its own address).  The first call per GPU asks the runtime; later calls read the cache.
+cudaError_t noalloc_scratch_address(int dev, double **out) {
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_addr[dev]) {
+    double *ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress((void **)&ptr, g_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (!ptr) return cudaErrorInvalidSymbol;
+    g_noalloc_addr[dev] = ptr;
+  }
+  *out = g_noalloc_addr[dev];
+  return cudaSuccess;
+}
+}  // namespace
+
+extern "C" int mcdc_tallies_get_noalloc(const mcdc_problem *cp, double *mean, double *sdev, size_t n_bins) {
+  mcdc_problem *p = const_cast<mcdc_problem *>(cp);
+  if (!p || !mean || !sdev) return MCDC_ERR_ARG;
+  if (n_bins != p->n_bins) return MCDC_ERR_SIZE;
+  if (n_bins > MCDC_NOALLOC_MAX_BINS) {
+    p->cuda_err = "mcdc_tallies_get_noalloc: the problem has " + std::to_string(n_bins) + " tally bins, the fixed scratch "
+                  "array holds MCDC_NOALLOC_MAX_BINS = " + std::to_string((size_t)MCDC_NOALLOC_MAX_BINS) +
+                  "; use mcdc_tallies_get with a two-slot workspace for this mesh";
+    return MCDC_ERR_SIZE;
+  }
+  if (p->histories == 0) return MCDC_ERR_ARG;
+  // the handle's accumulators live on the GPU that was current at mcdc_problem_create; the scratch address we need is
+  // that GPU's, and the look-up below answers for the CURRENT one -- so the two must be the same
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  cudaPointerAttributes attr;
+  CK(cudaPointerGetAttributes(&attr, p->d_sum));
+  if (attr.device != dev || dev < 0 || dev >= NOALLOC_MAX_DEVICES) {
+    p->cuda_err = "mcdc_tallies_get_noalloc: the handle lives on GPU " + std::to_string(attr.device) +
+                  " but the current device is " + std::to_string(dev);
+    return MCDC_ERR_ARG;
+  }
+  double *scratch = nullptr;
+  cudaError_t es = noalloc_scratch_address(dev, &scratch);
+  if (es != cudaSuccess) return cuda_fail(p, es, "cudaGetSymbolAddress(g_noalloc_scratch)");
+  double *d_mean = scratch, *d_sdev = scratch + MCDC_NOALLOC_MAX_BINS;
+  // k_statistics writes mean[i] and sdev[i] for every i < n_bins before anything reads them: what an earlier call
+  // left in the array is overwritten, nothing needs clearing.  Same launch shape as batch_statistics().
+  const int grid = (int)std::min<size_t>((n_bins + 255) / 256, (size_t)p->n_sm * 16);
+  k_statistics<<<grid, 256, 0, p->stream>>>(p->d_sum, p->d_sumsq, n_bins, (double)p->histories, (double)p->batches, d_mean, d_sdev);
+  cudaError_t e0 = cudaGetLastError();
+  p->launches++;
+  cudaError_t e1 = cudaMemcpyAsync(mean, d_mean, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+  cudaError_t e2 = cudaMemcpyAsync(sdev, d_sdev, n_bins * sizeof(double), cudaMemcpyDeviceToHost, p->stream);
+  cudaError_t e3 = cudaStreamSynchronize(p->stream);
+  if (e0 != cudaSuccess) return cuda_fail(p, e0, "k_statistics launch");
+  if (e1 != cudaSuccess) return cuda_fail(p, e1, "cudaMemcpyAsync(mean)");
+  if (e2 != cudaSuccess) return cuda_fail(p, e2, "cudaMemcpyAsync(sdev)");
+  if (e3 != cudaSuccess) return cuda_fail(p, e3, "k_statistics");
+  return MCDC_OK;
+}
