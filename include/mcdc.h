@@ -175,7 +175,17 @@ int mcdc_problem_create_csg(const mcdc_problem_desc *d, const int32_t *region_of
  *  mcdc_problem_create_lattice: mcdc_problem_create on *d with its geometry fields (n_surfaces, n_cells, surf_*,
  *    cell_offset, hs_*, cell_material: ignored, may be 0 / NULL) replaced by the expansion.
  * A malformed description (universe id or local surface out of range, unknown face code, empty cell, sense not
- * +-1, non-positive pitch, z_hi <= z_lo, bc out of range) gives MCDC_ERR_GEOM.                            */
+ * +-1, non-positive pitch, z_hi <= z_lo, bc out of range) gives MCDC_ERR_GEOM.
+ * Limits.  One level only: the array is two-dimensional (x, y; every element spans z_lo .. z_hi), rectangular, and a
+ * universe's cells hold materials -- a cell cannot be filled with another universe or lattice (no nesting), and
+ * there are no hexagonal lattices.  The expansion is a host-side flattening that copies a universe's surfaces and
+ * cells into every element it fills, so the flat problem has S = nx + ny + 4 + sum over elements of the universe's
+ * surfaces and C = sum over elements of its cells: memory and set-up time grow with nx * ny * |universe|.  All three
+ * calls do this arithmetic in 64 bits and refuse with MCDC_ERR_GEOM a lattice whose element count nx * ny, S, C or
+ * half-space count exceeds INT32_MAX.  Far below that, the history kernel's compact 16-bit tables hold fewer than
+ * 65 535 cells and 65 533 surfaces: a larger flat problem still runs and still gives the same results, but on the
+ * slower census-stepped kernel (mcdc_problem_info.warp_kernel_ok == 0 tells) -- a 17 x 17 lattice of pins is 578 cells,
+ * a 200 x 200 one (80 000 cells) crosses the line.                                                         */
 enum { MCDC_LAT_XLO = -1, MCDC_LAT_XHI = -2, MCDC_LAT_YLO = -3, MCDC_LAT_YHI = -4, MCDC_LAT_ZLO = -5, MCDC_LAT_ZHI = -6 };
 typedef struct {
   int32_t n_universes;

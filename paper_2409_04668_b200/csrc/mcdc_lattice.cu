@@ -35,11 +35,27 @@ bool lattice_ok(const mcdc_lattice_desc *L) {
     }
   }
   if (L->usurf_offset[U] > 0 && !L->usurf_coef) return false;
-  for (int k = 0; k < L->nx * L->ny; ++k)
+  const long long n_elem = (long long)L->nx * L->ny;                         // nx * ny overflows int from 46341 x 46341
+  if (n_elem > INT32_MAX) return false;
+  for (long long k = 0; k < n_elem; ++k)
     if (L->fill[k] < 0 || L->fill[k] >= U) return false;
   for (int f = 0; f < 6; ++f)
     if (L->bc[f] < MCDC_BC_TRANSMISSION || L->bc[f] > MCDC_BC_REFLECTIVE) return false;
   return true;
+}
+
+// Sizes of the flat geometry, in 64 bits; false when any of them does not fit the int32 fields of mcdc_problem_desc.
+// Shared by all three entry points, so that none of them expands a lattice whose sizes it could not state.
+bool flat_sizes(const mcdc_lattice_desc *L, long long &S, long long &C, long long &H) {
+  S = (long long)L->nx + 1 + (long long)L->ny + 1 + 2; C = 0; H = 0;
+  const long long n_elem = (long long)L->nx * L->ny;
+  for (long long k = 0; k < n_elem; ++k) {
+    const int u = L->fill[k];
+    S += L->usurf_offset[u + 1] - L->usurf_offset[u];
+    C += L->ucell_offset[u + 1] - L->ucell_offset[u];
+    H += L->uhs_offset[L->ucell_offset[u + 1]] - L->uhs_offset[L->ucell_offset[u]];
+  }
+  return S <= INT32_MAX && C <= INT32_MAX && H <= INT32_MAX;
 }
 
 void put_plane(Flat &F, int axis, double a, int bc) {
@@ -77,7 +93,7 @@ void expand(const mcdc_lattice_desc *L, Flat &F) {
   std::vector<int32_t> first((size_t)nx * ny);
   for (int j = 0; j < ny; ++j)
     for (int i = 0; i < nx; ++i) {
-      const int u = L->fill[j * nx + i];
+      const int u = L->fill[(size_t)j * nx + i];
       first[(size_t)j * nx + i] = (int32_t)F.bc.size();
       const double cx = L->x0 + (i + 0.5) * L->pitch_x, cy = L->y0 + (j + 0.5) * L->pitch_y;
       for (int s = L->usurf_offset[u]; s < L->usurf_offset[u + 1]; ++s) put_translated(F, L->usurf_coef + (size_t)10 * s, cx, cy, 0.0);
@@ -85,7 +101,7 @@ void expand(const mcdc_lattice_desc *L, Flat &F) {
   F.cell_off.push_back(0);
   for (int j = 0; j < ny; ++j)
     for (int i = 0; i < nx; ++i) {
-      const int u = L->fill[j * nx + i];
+      const int u = L->fill[(size_t)j * nx + i];
       const int32_t face[6] = {i, i + 1, oy + j, oy + j + 1, oz, oz + 1};
       for (int c = L->ucell_offset[u]; c < L->ucell_offset[u + 1]; ++c) {
         for (int h = L->uhs_offset[c]; h < L->uhs_offset[c + 1]; ++h) {
@@ -104,14 +120,8 @@ void expand(const mcdc_lattice_desc *L, Flat &F) {
 extern "C" int mcdc_lattice_expand_size(const mcdc_lattice_desc *lat, int32_t *n_surfaces, int32_t *n_cells, int32_t *n_halfspaces) {
   if (!n_surfaces || !n_cells || !n_halfspaces) return MCDC_ERR_ARG;
   if (!lattice_ok(lat)) return MCDC_ERR_GEOM;
-  long long S = (long long)lat->nx + 1 + lat->ny + 1 + 2, C = 0, H = 0;
-  for (int k = 0; k < lat->nx * lat->ny; ++k) {
-    const int u = lat->fill[k];
-    S += lat->usurf_offset[u + 1] - lat->usurf_offset[u];
-    C += lat->ucell_offset[u + 1] - lat->ucell_offset[u];
-    H += lat->uhs_offset[lat->ucell_offset[u + 1]] - lat->uhs_offset[lat->ucell_offset[u]];
-  }
-  if (S > INT32_MAX || C > INT32_MAX || H > INT32_MAX) return MCDC_ERR_GEOM;
+  long long S, C, H;
+  if (!flat_sizes(lat, S, C, H)) return MCDC_ERR_GEOM;
   *n_surfaces = (int32_t)S; *n_cells = (int32_t)C; *n_halfspaces = (int32_t)H;
   return MCDC_OK;
 }
@@ -120,6 +130,8 @@ extern "C" int mcdc_lattice_expand(const mcdc_lattice_desc *lat, double *surf_co
                                    int32_t *hs_surface, int32_t *hs_sense, int32_t *cell_material) {
   if (!surf_coef || !surf_bc || !cell_offset || !hs_surface || !hs_sense || !cell_material) return MCDC_ERR_ARG;
   if (!lattice_ok(lat)) return MCDC_ERR_GEOM;
+  long long S, C, H;
+  if (!flat_sizes(lat, S, C, H)) return MCDC_ERR_GEOM;
   Flat F;
   try { expand(lat, F); } catch (const std::bad_alloc &) { return MCDC_ERR_NOMEM; }
   std::copy(F.coef.begin(), F.coef.end(), surf_coef);
@@ -134,6 +146,8 @@ extern "C" int mcdc_lattice_expand(const mcdc_lattice_desc *lat, double *surf_co
 extern "C" int mcdc_problem_create_lattice(const mcdc_problem_desc *d, const mcdc_lattice_desc *lat, mcdc_problem **out) {
   if (!d || !out) return MCDC_ERR_ARG;
   if (!lattice_ok(lat)) return MCDC_ERR_GEOM;
+  long long S, C, H;
+  if (!flat_sizes(lat, S, C, H)) return MCDC_ERR_GEOM;
   Flat F;
   try { expand(lat, F); } catch (const std::bad_alloc &) { return MCDC_ERR_NOMEM; }
   mcdc_problem_desc e = *d;                              // materials, source, mesh, time grid: the caller's

@@ -53,3 +53,20 @@ def test_malformed_lattices_are_refused_by_the_library(M):
         with pytest.raises(M.McdcError) as ex:
             M.mcdc_lattice_expand(lat)
         assert ex.value.code == -3
+
+
+def test_a_lattice_whose_element_count_overflows_int32_is_refused_by_all_three_calls(M):
+    """nx * ny = 46341^2 > INT32_MAX used to wrap negative in int arithmetic: the fill check was skipped and the expansion
+    went on to size its tables from garbage.  All three entry points now share one 64-bit guard."""
+    import ctypes as C
+    from paper_2409_04668_b200 import api
+    lat = W.lattice_mixed().meta["lattice"]
+    d, keep = api._make_lattice(lat)
+    d.nx = d.ny = 46341                                   # fill is NOT that large: the guard must fire before it is read
+    n = [C.c_int32() for _ in range(3)]
+    assert M.lib().mcdc_lattice_expand_size(C.byref(d), *[C.byref(v) for v in n]) == -3
+    buf_d, buf_i = (C.c_double * 16)(), (C.c_int32 * 16)()
+    assert M.lib().mcdc_lattice_expand(C.byref(d), buf_d, buf_i, buf_i, buf_i, buf_i, buf_i) == -3
+    pd, keep2 = api._make_desc(W.lattice_mixed())
+    h = C.c_void_p()
+    assert M.lib().mcdc_problem_create_lattice(C.byref(pd), C.byref(d), C.byref(h)) == -3 and not h.value
