@@ -44,11 +44,14 @@ def ncu_constants(kernel_info, workload, technique):
         return None, "profiles/ncu_constants.json missing"
     name = kernel_info.split(" ")[0] if kernel_info else ""
     rev = next((t[4:] for t in kernel_info.split() if t.startswith("rev=")), "")
-    for e in table.get("captures", []):
-        if e.get("kernel") == name and e.get("workload") == workload and e.get("technique", "analog") == technique:
-            if e.get("rev") != rev:
-                return None, f"stale: {e.get('source')} was captured at kernel rev {e.get('rev')}, this library is rev {rev}"
+    same = [e for e in table.get("captures", [])
+            if e.get("kernel") == name and e.get("workload") == workload and e.get("technique", "analog") == technique]
+    for e in same:                       # the capture made from THIS library's revision, wherever it sits in the list
+        if e.get("rev") == rev:
             return e, e.get("source")
+    if same:
+        e = same[0]
+        return None, f"stale: {e.get('source')} was captured at kernel rev {e.get('rev')}, this library is rev {rev}"
     return None, f"no capture of {name} on {workload} ({technique}) in profiles/ncu_constants.json"
 
 

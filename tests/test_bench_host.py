@@ -38,6 +38,24 @@ def test_ncu_constants_are_keyed_by_kernel_workload_and_revision():
     assert e is None
     e, note = bench.ncu_constants("", cap["workload"], "analog")
     assert e is None
+    # a later entry of the same kernel / workload whose revision matches is found, not reported stale at the first name match
+    with open(bench.NCU_JSON) as f:
+        caps = json.load(f)["captures"]
+    older = [c for c in caps[1:] if (c["kernel"], c["workload"], c.get("technique", "analog")) ==
+             (cap["kernel"], cap["workload"], cap.get("technique", "analog")) and c["rev"] != cap["rev"]]
+    if older:
+        e, note = bench.ncu_constants(info.replace(cap["rev"], older[0]["rev"]), cap["workload"], cap.get("technique", "analog"))
+        assert e is not None and e["rev"] == older[0]["rev"] and note == older[0]["source"]
+
+
+def test_kernel_revision_covers_the_host_file_and_the_defines_and_tuned_builds_go_elsewhere():
+    from paper_2409_04668_b200 import build as b
+    assert b.kernel_rev() == b.kernel_rev([]) and len(b.kernel_rev()) == 12
+    assert b.kernel_rev(["-DMCDC_WARP_THREADS=576"]) != b.kernel_rev()
+    assert b.kernel_rev(["-DA=1", "-DB=2"]) == b.kernel_rev(["-DB=2", "-DA=1"]) != b.kernel_rev(["-DA=1"])
+    assert b.LIB_TUNED != b.LIB and b.OBJ_TUNED != b.OBJ and b.lib_path() == b.LIB
+    src = open(os.path.join(ROOT, "paper_2409_04668_b200", "build.py")).read()
+    assert '"mcdc_host.cu"]' in src.split("def kernel_rev")[1].split("def ")[0]
 
 
 def test_algorithmic_bytes_formula():
