@@ -328,9 +328,11 @@ int mcdc_problem_info_get(const mcdc_problem *p, mcdc_problem_info *info);
  * so that the caller can reduce it with any collective (ncclAllReduce on a device buffer, gloo/MPI on
  * a host buffer) and put the sum back:
  *   [0, n_bins) sum   [n_bins, 2 n_bins) sumsq   [then sum and sumsq of the collision-estimator tally, 2 n_bins
- *   more entries, while mcdc_collision_tally_enable is on]   then pop_w[K], pop_n[K], ledger[7] (source production
- *   capture fission_abs leak census_final lost), counts[7] (histories segments collisions surf_hits
- *   census_events children lost_n), vr[2] (gain, loss), pc[2] (removed, added), histories, batches.
+ *   more entries, while mcdc_collision_tally_enable is on]   then, in exactly this order, pop_w[K], pop_n[K],
+ *   ledger[9] (source production capture fission_abs leak census_final lost vr_gain vr_loss),
+ *   counts[9] (histories segments collisions surf_hits census_events children lost_n pc_removed pc_added),
+ *   histories, batches -- so with T = (2 or 4) n_bins + 2 K: vr_gain is entry T + 7, segments T + 10, pc_added
+ *   T + 17, histories (the handle's total, what mean / sdev divide by) T + 18, batches T + 19.
  * Integer entries are stored as doubles (exact below 2^53).  on_device != 0: buf is DEVICE memory
  * (copies run on the bound stream, synchronous on return); else HOST memory.  n must equal
  * mcdc_state_size.  Import REPLACES the handle's accumulators; ranks must use the same batch size. */

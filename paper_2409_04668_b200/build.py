@@ -65,14 +65,14 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
     if not force and not _stale() and not defines:
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    OBJ, LIB = (OBJ_TUNED, LIB_TUNED) if defines else (globals()["OBJ"], globals()["LIB"])
-    os.makedirs(OBJ, exist_ok=True)
+    obj_dir, lib = (OBJ_TUNED, LIB_TUNED) if defines else (OBJ, LIB)
+    os.makedirs(obj_dir, exist_ok=True)
     rev = [f'-DMCDC_KERNEL_REV="{kernel_rev(defines)}"']
 
     def compile_unit(u):
         src, obj, defs = u
         cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + list(defs) + rev + list(defines) + \
-              ["-c", os.path.join(CSRC, src), "-o", os.path.join(OBJ, obj)]
+              ["-c", os.path.join(CSRC, src), "-o", os.path.join(obj_dir, obj)]
         r = subprocess.run(cmd, cwd=CSRC, capture_output=True, text=True)
         return u, r
 
@@ -83,8 +83,8 @@ def build(force: bool = False, verbose: bool = False, defines=()) -> str:
             sys.stderr.write(r.stdout + r.stderr)
         if r.returncode != 0:
             raise subprocess.CalledProcessError(r.returncode, f"nvcc {u[0]} {' '.join(u[2])}")
-    subprocess.check_call([nvcc] + LINK_FLAGS + ["-o", LIB] + [os.path.join(OBJ, u[1]) for u in UNITS], cwd=CSRC)
-    return LIB
+    subprocess.check_call([nvcc] + LINK_FLAGS + ["-o", lib] + [os.path.join(obj_dir, u[1]) for u in UNITS], cwd=CSRC)
+    return lib
 
 
 if __name__ == "__main__":

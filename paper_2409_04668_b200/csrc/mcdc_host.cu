@@ -116,6 +116,10 @@ struct mcdc_problem {
   cudaEvent_t e_run0 = nullptr, e_run1 = nullptr, e_tr0 = nullptr, e_tr1 = nullptr;
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> ev_pairs;
   size_t ev_used = 0;
+  // census-step mode of k_warp: pinned snapshot of the live counts + overflow flag, looked at a few steps late (run_subbatch_stepwarp)
+  uint32_t *h_poll = nullptr;
+  size_t h_poll_cap = 0;
+  cudaEvent_t e_poll = nullptr;
   bool transport_attr_set = false;   // cudaFuncSetAttribute(k_transport) done for this handle's device
   std::string last_kernel;           // transport kernel instantiation + launch shape of the last run (mcdc_kernel_info_get)
   std::string cuda_err;
@@ -771,6 +775,8 @@ extern "C" void mcdc_problem_destroy(mcdc_problem *p) {
   for (auto &pr : p->ev_pairs) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
   for (cudaEvent_t e : {p->e_run0, p->e_run1, p->e_tr0, p->e_tr1})
     if (e) cudaEventDestroy(e);
+  if (p->e_poll) cudaEventDestroy(p->e_poll);
+  if (p->h_poll) cudaFreeHost(p->h_poll);
   if (p->d_ev) cudaFree(p->d_ev);
   if (p->d_xc_acc) cudaFree(p->d_xc_acc);
   if (p->d_sumc) cudaFree(p->d_sumc);
@@ -1115,7 +1121,7 @@ int plan_warp_kernel(mcdc_problem *p, bool record, int variant, uint32_t debug_p
 #endif
   const int nt = MCDC_WARP_THREADS;
   const int nw = nt / 32;
-  const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8 * POPW_COPIES, 16) : 0);
+  const size_t pop_bytes = align_up((size_t)p->K * 4, 16) + (weighted ? align_up((size_t)p->K * 8 * popw_copies(variant), 16) : 0);
   const size_t fixed = sizeof(WarpShared) + 128 + pop_bytes;
   const size_t hot = align_up(p->tab.hot_bytes, 16);
   const size_t per_slot = warp_pool_bytes_per_slot(record, weighted);
@@ -1224,6 +1230,12 @@ int run_subbatch_async(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint6
 // steps are queued back to back ("mid-run host <-> device copies" are the cost the paper itself names).
 // What the host used to read per step is decided on the device instead: grids are sized for the bank capacity and
 // blocks without work leave at once; a bank overflow sets the device flag that mcdc_run_ex checks after the run.
+// With K in the thousands that alone would queue thousands of empty launches after the population has died out (or
+// after an overflow that is reported only at the end), so past the source every STEP_POLL-th step also copies the next
+// step's live counts and the overflow flag to pinned host memory behind an event.  The host looks at a snapshot
+// STEP_POLL steps after queueing it, when it has long been made: it never waits for the head of the queue, the launches
+// still go out back to back, and at most 2 STEP_POLL steps run on nothing.
+constexpr int STEP_POLL = 16;
 int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, uint64_t first_history_id, bool record) {
   const uint32_t ns = sb.n_slots, ws_ns = p->ws_slots;
   uint32_t *counts_dev = p->counts_dev;
@@ -1252,6 +1264,13 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
   // histories does not wake every SM), every SM otherwise
   const uint64_t work_max = std::max<uint64_t>((uint64_t)sb.n_hist, (uint64_t)std::min<uint64_t>((uint64_t)p->cap * ns, (uint64_t)4 * sb.n_hist));
   const int grid = (int)std::min<uint64_t>((uint64_t)p->n_sm, std::max<uint64_t>(1, (work_max + per_block - 1) / per_block));
+  if (p->h_poll_cap < (size_t)ns + 1) {
+    if (p->h_poll) { cudaFreeHost(p->h_poll); p->h_poll = nullptr; p->h_poll_cap = 0; }
+    CK(cudaHostAlloc((void **)&p->h_poll, ((size_t)ws_ns + 1) * sizeof(uint32_t), cudaHostAllocDefault));
+    p->h_poll_cap = (size_t)ws_ns + 1;
+  }
+  if (!p->e_poll) CK(cudaEventCreateWithFlags(&p->e_poll, cudaEventDisableTiming));
+  bool poll_pending = false;
   for (int k = k_first; k < p->K; ++k) {
     const bool src = k <= k_last;
     ha.step_k = k; ha.step_source = src ? 1 : 0;
@@ -1284,6 +1303,21 @@ int run_subbatch_stepwarp(mcdc_problem *p, const SubBatch &sb, uint64_t seed, ui
       std::swap(A, Bk);
     }
     CK(cudaMemsetAsync(Bk.count, 0, ns * sizeof(uint32_t), p->stream));
+    if (k > k_last && k < p->K - 1 && (k - k_last) % STEP_POLL == 0) {
+      if (poll_pending) {                                  // the snapshot queued STEP_POLL steps ago
+        CK(cudaEventSynchronize(p->e_poll));
+        bool any_live = false;
+        for (uint32_t s = 0; s < ns; ++s) any_live = any_live || p->h_poll[s] != 0u;
+        // nothing left to transport and no source to come: every later step would be an empty launch.  Or a bank
+        // overflowed: the run is void (mcdc_run_ex reports it), no point in finishing it.  Either way the banks are
+        // left as a finished run leaves them (counts zeroed at the next run) and the close-out below still runs.
+        if (!any_live || p->h_poll[ns] != 0u) break;
+      }
+      CK(cudaMemcpyAsync(p->h_poll, A.count, ns * sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));   // A: live bank of step k + 1
+      CK(cudaMemcpyAsync(p->h_poll + ns, &p->d_cnt->overflow, sizeof(uint32_t), cudaMemcpyDeviceToHost, p->stream));
+      CK(cudaEventRecord(p->e_poll, p->stream));
+      poll_pending = true;
+    }
   }
   if (sb.closeout) {
     int cgrid = (int)std::min<size_t>((p->n_bins + 255) / 256, (size_t)p->n_sm * 8);

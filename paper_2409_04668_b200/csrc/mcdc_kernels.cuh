@@ -695,6 +695,10 @@ __global__ void __launch_bounds__(256) k_pc_apply_inplace(Bank bank, const uint3
   int4 m = make_int4(0, -1, 0, 0);
   int n = 0;
   if (have) { w = bank.w[j]; key = bank.key[j]; m = bank.meta[j]; ctr = (uint32_t)m.z; }
+  // W == 0: every arrival of this batch weighs less than 2^-40, so the fixed-point sum is zero and G.3 hands back an
+  // EMPTY bank without touching a counter (k_pc_apply: out.count stays 0).  In place that means every arrival
+  // becomes a hole; left alone, the next launch would pick all of them up as live particles.
+  if (i < n_in && W == 0ull) bank.meta[(size_t)slot * P.cap + i].x = -1;
   const double xi = draw(key, ctr);                      // the particle's own stream
   if (have) {
     n = (int)floor(w / w_t + xi);

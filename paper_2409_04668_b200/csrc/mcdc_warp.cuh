@@ -138,6 +138,9 @@ __host__ __device__ inline size_t warp_pool_bytes_per_slot(bool record, bool wei
 // shared-memory double serialise in a compare-and-swap loop (12 % of the weighted kernel's samples, profiles/r02k); four
 // copies spread the lanes of a round that reach the same census.
 #define POPW_COPIES 4
+// ... of which the census-step and generation variants (VARIANT >= 2) need only one: they sum the census weight in a
+// register per lane and add once per warp to copy 0.  With K near 4095 three unused copies cost 96 KB of the pool.
+__host__ __device__ constexpr int popw_copies(int variant) { return variant >= 2 ? 1 : POPW_COPIES; }
 
 struct WarpShared {                // block-wide totals (static shared memory)
   double led[LED_N];
@@ -189,7 +192,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   uint32_t *s_popn = reinterpret_cast<uint32_t *>(g_smem + A.smem_tables);
   double *s_popw = reinterpret_cast<double *>(g_smem + A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16));   // WEIGHTED only
   const uint32_t pool_off = A.smem_tables + (uint32_t)(((size_t)T.K * 4 + 15) / 16 * 16) +
-                            (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 * POPW_COPIES + 15) / 16 * 16) : 0u);
+                            (WEIGHTED ? (uint32_t)(((size_t)T.K * 8 * popw_copies(VARIANT) + 15) / 16 * 16) : 0u);
 #define PP(pr, slot) (*reinterpret_cast<double2 *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(pr) * 16u))
 #define PD(k, slot) (*reinterpret_cast<double *>(g_smem + pool_off + (slot) * 80u + (uint32_t)(k) * 8u))
 #define PK(slot) (*reinterpret_cast<unsigned long long *>(g_smem + pool_off + N * 80u + (slot) * 16u))
@@ -207,7 +210,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
     for (uint32_t i = tid; i < T.hot_bytes / 16u; i += NT) dst[i] = src[i];
   }
   for (int k = tid; k < T.K; k += NT) s_popn[k] = 0u;
-  if (WEIGHTED) for (int k = tid; k < T.K * POPW_COPIES; k += NT) s_popw[k] = 0.0;
+  if (WEIGHTED) for (int k = tid; k < T.K * popw_copies(VARIANT); k += NT) s_popw[k] = 0.0;
   if (tid == 0) {
     for (int e = 0; e < LED_N; ++e) sh.led[e] = 0.0;
     sh.n_coll = sh.n_seg = sh.n_census = sh.n_children = sh.n_lost = sh.n_src = 0ull; sh.n_leak = 0u;
@@ -934,7 +937,7 @@ __global__ void MCDC_WARP_BOUNDS k_warp(Tables T, HistoryArgs A) {
   for (int k = tid; k < T.K; k += NT) {
     if (s_popn[k] != 0u) {
       double pw = (double)s_popn[k];
-      if (WEIGHTED) { pw = 0.0; for (int c = 0; c < POPW_COPIES; ++c) pw += s_popw[c * T.K + k]; }
+      if (WEIGHTED) { pw = 0.0; for (int c = 0; c < popw_copies(VARIANT); ++c) pw += s_popw[c * T.K + k]; }
       atomicAdd(A.pop_w + k, pw); atomicAdd(A.pop_n + k, (unsigned long long)s_popn[k]);
       atomicAdd(&sh.n_census, (unsigned long long)s_popn[k]);   // census events of the block = its population counts
       if (k == T.K - 1) atomicAdd(&sh.led[LED_CENSUS_FINAL], pw);   // what reached the last census is the final-census ledger entry

@@ -50,7 +50,9 @@ def all_reduce_state(problem, group=None, device=None):
     n = problem.state_size()
     buf = torch.empty(n, dtype=torch.float64, device=device if device is not None else "cpu")
     problem.state_export(buf)
-    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+    # whenever a process group exists, one-rank groups included: a one-rank sum is the identity, and it is the one way to
+    # put ncclAllReduce on the exported device buffer where a second GPU does not exist (tests/test_gpu_vr.py)
+    if dist.is_available() and dist.is_initialized():
         dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
     problem.state_import(buf)
     return buf

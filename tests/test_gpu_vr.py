@@ -96,6 +96,60 @@ def test_larger_configs_with_techniques(M, name, N, B, tech, scheduler):
     g.close()
 
 
+def _vanishing_weight_problem():
+    """One-group absorber (Sigma_c / Sigma_t = 0.9, no fission) under implicit capture without roulette, first census at
+    t = 60: a history has had Poisson(60) collisions by then and weighs 0.1^collisions, below 2^-40 from the 13th on
+    (P(fewer) ~ 1e-14), so every arrival truncates to 0 in the control's 2^-40 fixed-point sum."""
+    from workloads import configs as W
+    p = W.config0_infinite_medium(n_histories=4000, n_batches=4, n_time=2, t_end=120.0)
+    p.sigma_s = np.array([[[0.1]]]); p.sigma_c = np.array([[0.9]]); p.sigma_f = np.array([[0.0]]); p.nu = np.array([[0.0]])
+    return p
+
+
+@pytest.mark.parametrize("scheduler", [0, 1])
+def test_population_control_of_a_batch_whose_weight_sums_to_zero_empties_the_bank(M, scheduler):
+    """Appendix G.3 with W = 0: the oracle's control returns an empty bank and touches no counter.  The out-of-place
+    kernel does the same by construction; the in-place one (scheduler 0: k_warp in census-step mode) has to mark every
+    arrival as a hole, else the next launch transports them on."""
+    p = _vanishing_weight_problem()
+    o, g = _pair(M, p, dict(implicit_capture=True, population_control=True), scheduler=scheduler)
+    wo, no = o.census()
+    assert no[0] == p.n_histories and no[1] == 0 and 0.0 < wo[0] < p.n_histories * 2.0 ** -40     # the case is the one meant
+    assert o.counters()["pc_removed"] == 0 and o.census_after()[1][0] == 0
+    _compare(o, g, rtol_bins=1e-9)
+    g.close()
+
+
+def test_census_step_mode_stops_queueing_once_the_population_has_died_out(M):
+    """A pure absorber with census every 20 mean free paths: no history reaches the first census (e^-20 each), and 399
+    more census steps follow.  The census-step loop looks at the live counts every 16 steps (one snapshot late) and stops:
+    same results as the oracle's full loop, a small fraction of its 400 x 3 launches."""
+    from workloads import configs as W
+    p = W.config0_infinite_medium(n_histories=4000, n_batches=4, n_time=400, t_end=8000.0)
+    p.sigma_s = np.array([[[0.0]]]); p.sigma_c = np.array([[1.0]]); p.sigma_f = np.array([[0.0]]); p.nu = np.array([[0.0]])
+    o, g = _pair(M, p, dict(population_control=True), scheduler=0)
+    assert "k_warp<" in g.kernel_info() and o.census()[1].sum() == 0
+    _compare(o, g, rtol_bins=1e-9)
+    assert g.counters()["kernel_launches"] <= 3 * 40, g.counters()["kernel_launches"]
+    g.close()
+
+
+def test_census_step_mode_keeps_a_full_pool_with_thousands_of_census_times(M):
+    """K = 4000 census times: the block's census-weight array is K doubles.  The census-step variant sums census weight in
+    registers and uses one copy of it, not the four of the weighted history kernel (which would leave ~40 pool slots per
+    warp and switch table staging off)."""
+    from workloads import configs as W
+    # (8 batches: with 2 the batch variance of a bin is the difference of two nearly equal numbers, and the sdev bar of
+    # _compare then measures summation order, not the method)
+    p = W.config0_infinite_medium(n_histories=4000, n_batches=8, n_time=4000, t_end=20.0)
+    o, g = _pair(M, p, dict(implicit_capture=True, wr_threshold=0.25, wr_survive=1.0, population_control=True), scheduler=0)
+    info = g.kernel_info()
+    slots = int(next(t for t in info.split() if t.startswith("pool_slots=")).split("=")[1])
+    assert "k_warp<" in info and slots >= 80, info
+    _compare(o, g, rtol_bins=1e-9)
+    g.close()
+
+
 def test_population_control_needs_whole_batches_per_slot(M):
     from workloads import configs as W
     p = W.config0_infinite_medium(n_histories=4000, n_batches=1)
@@ -140,6 +194,21 @@ def test_state_export_sum_import_equals_the_single_run(M):
     merged.state_import(dev[0] + dev[1])
     mw, sw = whole.tallies(); mm, sm = merged.tallies()
     assert np.allclose(mm, mw, rtol=1e-13, atol=0) and np.allclose(sm, sw, rtol=1e-9, atol=1e-18)
+    # ... and the far side of the reduction against the ORACLE's run of the whole range (not only against this library's
+    # own single run): mean / sdev at the bars of tests/test_gpu_parity.py, ledger and populations exactly
+    from oracle import Oracle
+    o = Oracle(p); o.run(N, p.seed, n_batches=B)
+    mo, so = o.tallies()
+    scale = np.abs(mo).max()
+    assert np.all(np.abs(mm - mo) <= 1e-7 * np.maximum(np.abs(mo), np.abs(mm)) + 1e-13 * scale)
+    assert np.allclose(sm, so, rtol=1e-6, atol=1e-12 * scale)
+    err = np.sqrt(so ** 2 + sm ** 2) + 1e-12 * scale
+    assert np.all(np.abs(mm - mo) <= 4.0 * err) and mm.sum() == pytest.approx(mo.sum(), rel=1e-3)
+    co, cmg = o.counters(), merged.counters()
+    for k in REAL_LEDGER + INT_COUNTS:
+        assert cmg[k] == co[k], (k, cmg[k], co[k])
+    wo, no = o.census(); wm, nm = merged.census()
+    assert np.array_equal(no, nm) and np.array_equal(wo, wm)
     cw, cm = whole.counters(), merged.counters()
     for k in ("source", "production", "capture", "fission_abs", "leak", "census_final", "lost", "histories", "segments",
               "collisions", "surf_hits", "census_events", "children", "batches"):
@@ -151,6 +220,67 @@ def test_state_export_sum_import_equals_the_single_run(M):
     assert np.array_equal(whole.tallies()[0], before)
     for h in parts + [whole, merged]:
         h.close()
+
+
+def test_exported_state_vector_has_the_layout_the_header_documents(M):
+    """include/mcdc.h: after the tallies and populations come ledger[9], counts[9], histories, batches.  Read segments,
+    vr_gain and pc_added (and their neighbours) at the documented offsets of a run in which none of them is zero."""
+    import torch
+    from workloads import configs as W
+    p = W.config0_infinite_medium(n_histories=8000, n_batches=4)
+    g = M.Problem(p); g.set_technique(**TECHS["all"]); g.run()
+    v = torch.empty(g.state_size(), dtype=torch.float64)
+    g.state_export(v)
+    v = v.numpy()
+    T = 2 * p.n_bins + 2 * p.n_census
+    assert v.size == T + 20
+    c = g.counters()
+    s, q = g.tally_sums()
+    assert np.array_equal(v[:p.n_bins], s.ravel()) and np.array_equal(v[p.n_bins:2 * p.n_bins], q.ravel())
+    w, n = g.census()
+    assert np.array_equal(v[2 * p.n_bins:2 * p.n_bins + p.n_census], w) and np.array_equal(v[T - p.n_census:T], n.astype(np.float64))
+    for i, k in enumerate(REAL_LEDGER):
+        assert v[T + i] == c[k], (k, i)
+    for i, k in enumerate(("histories", "segments", "collisions", "surf_hits", "census_events", "children", "lost_n",
+                           "pc_removed", "pc_added")):
+        assert v[T + 9 + i] == c[k], (k, i)
+    assert v[T + 7] == c["vr_gain"] > 0 and v[T + 10] == c["segments"] > 0 and v[T + 17] == c["pc_added"] > 0
+    assert v[T + 18] == p.n_histories and v[T + 19] == p.n_batches
+    g.close()
+
+
+def test_one_rank_nccl_all_reduce_of_the_exported_state_is_the_identity_and_matches_the_oracle(M):
+    """NCCL with one rank: the first time ncclAllReduce touches the device buffer that mcdc_state_export fills and
+    mcdc_state_import reads back (multi-GPU boxes do not exist in this pool).  The state must come back unchanged and
+    still be the oracle's."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from oracle import Oracle
+    from workloads import configs as W
+    p = W.config3_pin_lattice(n_histories=40_000, n_batches=8)
+    g = M.Problem(p); g.run()
+    before = torch.empty(g.state_size(), dtype=torch.float64, device="cuda"); g.state_export(before)
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", world_size=1, rank=0, device_id=torch.device("cuda:0"))
+    try:
+        assert dist.get_backend() == "nccl"
+        g.all_reduce()
+        torch.cuda.synchronize()
+    finally:
+        dist.destroy_process_group()
+    after = torch.empty_like(before); g.state_export(after)
+    assert torch.equal(before, after)
+    o = Oracle(p); o.run(p.n_histories, p.seed, n_batches=p.n_batches)
+    mo, so = o.tallies(); mg, sg = g.tallies()
+    scale = np.abs(mo).max()
+    assert np.all(np.abs(mg - mo) <= 1e-7 * np.maximum(np.abs(mo), np.abs(mg)) + 1e-13 * scale)
+    assert np.allclose(sg, so, rtol=1e-6, atol=1e-12 * scale)
+    co, cg = o.counters(), g.counters()
+    for k in REAL_LEDGER + INT_COUNTS:
+        assert cg[k] == co[k], (k, cg[k], co[k])
+    g.close()
 
 
 @pytest.mark.parametrize("scheduler", [0, 1])
