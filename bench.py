@@ -298,8 +298,18 @@ def bench_gpu(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
+    # --force-dist: the multi-rank code of this function (NCCL process group, barriers, the all-reduce of the accumulators
+    # inside the timed region, the max over ranks) run by a single rank on one GPU -- the only way to execute it where no
+    # second GPU exists.  A launcher that sets WORLD_SIZE=1 gets the same.
+    dist_on = world > 1 or args.force_dist or "WORLD_SIZE" in os.environ and "MASTER_PORT" in os.environ
+    if dist_on:
         os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        if "MASTER_PORT" not in os.environ:
+            import socket
+            with socket.socket() as sk:
+                sk.bind(("127.0.0.1", 0))
+                os.environ["MASTER_PORT"] = str(sk.getsockname()[1])
+        os.environ.setdefault("WORLD_SIZE", "1"); os.environ.setdefault("RANK", "0")
         dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
     dev = f"cuda:{local}"
     torch.cuda.set_device(dev)
@@ -317,7 +327,7 @@ def bench_gpu(args):
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if dist_on:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -339,13 +349,13 @@ def bench_gpu(args):
         g.run(n_hist, p.seed, n_b, first_history_id=first_id, **dbg)
         ms_tr += g.counters()["ms_transport"]
     c = g.counters()                                      # this rank's own counts
-    if world > 1:
+    if dist_on:
         g.all_reduce()                                    # NCCL all-reduce of sum / sumsq / ledger / populations
     ev1.record()
     barrier()
     t_wall1 = time.time()
     ms = ev0.elapsed_time(ev1)
-    if world > 1:
+    if dist_on:
         t = torch.tensor([ms, ms_tr], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms, ms_tr = float(t[0]), float(t[1])
@@ -365,7 +375,10 @@ def bench_gpu(args):
         kinfo = g.kernel_info()
         ncu, ncu_note = ncu_constants(kinfo, p.name, args.technique)
         traffic = ncu["dram_bytes_per_history"] * n_hist * args.steps / n_tr if ncu else None
-        roofline = {"bound": "hbm", "kernel": kinfo, "achieved": ach, "peak": peak, "unit": "GB/s",
+        # the label says what the figure is: SURVEY 8(d)'s algorithmic bytes over the measured copy bandwidth.  The kernel keeps
+        # particle state on the SM and its real DRAM traffic is a fraction of a percent of peak (frac_measured_dram), so it is
+        # NOT bandwidth-bound; the bound it does have is the issue rate, reported in roofline_alu.
+        roofline = {"bound": "hbm (algorithmic-bytes equivalent)", "kernel": kinfo, "achieved": ach, "peak": peak, "unit": "GB/s",
                     "frac": ach / peak, "traffic": traffic, "peak_kind": peak_kind,
                     "frac_measured_dram": (traffic * n_tr / (ms_tr * 1e-3) / 1e9 / peak) if traffic else None,
                     "ncu_source": ncu_note,
@@ -396,7 +409,7 @@ def bench_gpu(args):
                                 "only global data, the per-batch tally accumulators, are rewritten by the close-out of "
                                 "every step, so no step can reuse a previous step's cache contents",
                           "parallelism": f"history-range sharding x{world}" +
-                                         (", one NCCL all-reduce of the accumulators at the end" if world > 1 else ""),
+                                         (", one NCCL all-reduce of the accumulators at the end" if dist_on else ""),
                           "technique": args.technique},
                "segments_per_s": seg_per_s, "segments_per_history": c["segments"] / max(1, c["histories"]),
                "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "roofline_alu": roofline_alu}
@@ -419,7 +432,7 @@ def bench_gpu(args):
         M.mcdc_problem_destroy(h)
     barrier()
     dt = time.perf_counter() - t0
-    if world > 1:
+    if dist_on:
         t = torch.tensor([dt], device=dev, dtype=torch.float64)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dt = float(t[0])
@@ -439,7 +452,7 @@ def bench_gpu(args):
         out["eigenvalue"] = run_eigenvalue(M, args, dev)
     if rank == 0:
         print(json.dumps(out))
-    if world > 1:
+    if dist_on:
         dist.destroy_process_group()
 
 
@@ -532,6 +545,8 @@ def main():
     ap.add_argument("--histories", type=float, default=0)
     ap.add_argument("--batches", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--force-dist", action="store_true", help="run the multi-rank code path (NCCL group, barriers, all-reduce of "
+                    "the accumulators in the timed region) with a single rank")
     ap.add_argument("--technique", default="analog", choices=sorted(TECHNIQUES),
                     help="variance-reduction variant of the workload (DESIGN.md Appendix G); the headline is analog")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
