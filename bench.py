@@ -448,7 +448,13 @@ def bench_gpu(args):
     g.close()
     if not args.no_sweep and world == 1 and args.workload == "config3" and not args.histories and args.technique == "analog":
         out["sweep"] = run_sweep(M, args, dev, peak)
-    if args.eigenvalue and world == 1:
+    # the other workloads and the variants, so that they are the driver's numbers and not only this repository's say-so
+    # (a few seconds of GPU time, outside the headline's timed region; --no-sweep skips them with the sweep)
+    if not args.no_sweep and world == 1 and args.workload == "config3" and not args.histories and args.technique == "analog":
+        out["configs"] = run_configs(M, args, dev, peak)
+        out["variants"] = run_variants(M, args, dev)
+        out["eigenvalue"] = run_eigenvalue(M, args, dev)
+    elif args.eigenvalue and world == 1:
         out["eigenvalue"] = run_eigenvalue(M, args, dev)
     if rank == 0:
         print(json.dumps(out))
@@ -482,6 +488,89 @@ def run_eigenvalue(M, args, dev):
            "launches": int(c["kernel_launches"])}
     g.close()
     return out
+
+
+def _timed_runs(torch, g, n, seed, nb, reps):
+    """reps runs of one handle after a warm-up and a reset -> (ms per run by CUDA events around the calls, k_warp / transport
+    ms per run from the library's own events, close-out + memsets ms per run, counters)."""
+    g.run(n, seed, nb)                                    # warm-up
+    g.reset()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ms_tr = ms_dev = 0.0
+    e0.record()
+    for _ in range(reps):
+        g.run(n, seed, nb)
+        c = g.counters()
+        ms_tr += c["ms_transport"]; ms_dev += c["ms_run"]
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps, ms_tr / reps, (ms_dev - ms_tr) / reps, g.counters()
+
+
+def _e2e_once(M, torch, g, p, tech, reps):
+    """The end-to-end leg of the headline on another workload: create (host arrays) + bind + run_ex + tallies_get into pinned
+    host arrays, per step -> histories/s."""
+    ptr = (g._ws.data_ptr() + 255) // 256 * 256
+    pin = torch.empty((2, p.n_bins), dtype=torch.float64).pin_memory()
+    out_np = (pin[0].numpy(), pin[1].numpy())
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        h = M.mcdc_problem_create(p)
+        M.mcdc_workspace_bind(h, ptr, g.workspace_bytes, g.max_hist, g.max_slots, g._stream.cuda_stream)
+        if tech:
+            M.mcdc_technique_set(h, **tech)
+        M.mcdc_run_ex(h, p.n_histories, p.seed, p.n_batches)
+        M.mcdc_tallies_get(h, p.n_bins, out=out_np)
+        M.mcdc_problem_destroy(h)
+    torch.cuda.synchronize()
+    return p.n_histories * reps / (time.perf_counter() - t0)
+
+
+def run_configs(M, args, dev, peak):
+    """BASELINE configs 0, 1 and 2 at their stated sizes (config 2 stands in for the paper's one measured workload, the
+    dog-leg duct of PAPER.md:159): the figures of the headline for each, outside its timed region, same JSON line."""
+    import torch
+    from workloads import configs as W
+
+    rows = []
+    for name in ("config0", "config1", "config2"):
+        p = W.get_config(name)
+        g = M.Problem(p, device=dev)
+        ms, ms_k, ms_rest, c = _timed_runs(torch, g, p.n_histories, p.seed, p.n_batches, 3)
+        alg = algorithmic_bytes(p, c, p.n_histories * 3)
+        rows.append({"workload": p.name, "histories": p.n_histories, "n_batches": p.n_batches, "tally_bins": p.n_bins,
+                     "histories_per_s": p.n_histories / (ms * 1e-3), "segments_per_s": c["segments"] / 3 / (ms * 1e-3),
+                     "ms_per_step": ms, "ms_k_warp": ms_k, "ms_closeout_and_memsets": ms_rest,
+                     "hbm_GBps_algorithmic": alg / 3 / (ms_k * 1e-3) / 1e9, "frac_of_hbm_peak": alg / 3 / (ms_k * 1e-3) / 1e9 / peak,
+                     "kernel_info": g.kernel_info(), "e2e_histories_per_s": _e2e_once(M, torch, g, p, None, 2)})
+        g.close()
+    return rows
+
+
+def run_variants(M, args, dev):
+    """The techniques of DESIGN.md Appendix G on config 3 at the headline's size, and the general-CSG geometry: device time per
+    step by the same events as the headline.  (The k-eigenvalue mode is the 'eigenvalue' key.)"""
+    import torch
+    from workloads import configs as W
+
+    rows = []
+    cases = [("config3", name, W.get_config("config3")) for name in ("ic_wr", "pc", "all")]
+    cases.append(("csg_union", "analog", W.csg_union_geometry(n_histories=1_000_000, n_batches=100)))
+    for wl, tname, p in cases:
+        g = M.Problem(p, device=dev)
+        tech = TECHNIQUES[tname]
+        if tech:
+            g.set_technique(**tech)
+        reps = 2
+        ms, ms_k, ms_rest, c = _timed_runs(torch, g, p.n_histories, p.seed, p.n_batches, reps)
+        rows.append({"workload": p.name, "technique": tname, "histories": p.n_histories, "n_batches": p.n_batches,
+                     "histories_per_s": p.n_histories / (ms * 1e-3), "segments_per_s": c["segments"] / reps / (ms * 1e-3),
+                     "ms_per_step": ms, "ms_transport": ms_k, "launches_per_step": int(c["kernel_launches"]) // reps,
+                     "kernel_info": g.kernel_info()})
+        g.close()
+    return rows
 
 
 def run_sweep(M, args, dev, peak):
